@@ -1,0 +1,144 @@
+/*
+ * flexmoe.h -- C ABI of the B200-native FlexMoE routed-expert FFN hot path (sm_100a).
+ *
+ * What the library computes is the paper's online-clipped routed-expert FFN (arxiv/paper_2606_27866;
+ * citations are PAPER.md:<line>):
+ *
+ *   Eq. 1   FFN_e(h)      = W_down ( silu(W_gate h) (.) W_up h )
+ *   Eq. 3   W~gate = P W_gate,  W~up = P W_up,  W~down = W_down P^T        (channel ranking)
+ *   Eq. 4   FFN_e^(r)(h)  = W~down ( m(r) (.) silu(W~gate h) (.) W~up h ),  m(r) = first r_e channels
+ *   Alg. 2   y[t] = sum_{j<k} topk_w[t][j] * FFN_{e}^{(r_e)}(x[t]),  e = topk_ids[t][j]
+ *   Eq. 11-12 a budget is a table r[E] of retained widths; rho = 1 - mean_e r_e / I
+ *
+ * Conventions
+ *   - extern "C", plain pointers and sizes; no torch / C++ types.  "device" pointers are CUDA device
+ *     pointers of the current device, "host" pointers are ordinary host memory.
+ *   - bf16 tensors are raw 16-bit patterns (upper half of an IEEE fp32), row-major as stated.
+ *   - Every call returns an fxm_status; nothing throws or aborts.  *out is untouched on failure.
+ *   - The library NEVER allocates or frees device memory and never synchronises the stream: the caller
+ *     owns `packed` and `workspace` (sizes from the two *_bytes queries) and keeps them alive until
+ *     fxm_destroy().  All device work is enqueued on `stream` (a cudaStream_t passed as void*, NULL =
+ *     legacy default stream).  Asynchronous CUDA faults surface as FXM_ECUDA from a later call.
+ *   - One handle = one MoE layer.  A handle is not thread-safe.
+ *   - There is no CPU fallback: on a machine without a CUDA device every compute call returns FXM_ECUDA.
+ *
+ * Supported shapes (else FXM_ESHAPE): 1 <= E <= 256, d % 64 == 0, I % 16 == 0, 1 <= k <= min(E,16), T >= 0.
+ */
+#ifndef FLEXMOE_H_
+#define FLEXMOE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fxm_layer fxm_layer; /* opaque; host-side metadata + pointers into caller buffers */
+
+typedef enum {
+    FXM_OK = 0,
+    FXM_EINVAL = 1,     /* NULL / misaligned pointer, negative size, bad enum                              */
+    FXM_ESHAPE = 2,     /* dimensions outside the supported set above                                      */
+    FXM_EPERM = 3,      /* a row of channel_rank is not a permutation of 0..I-1                            */
+    FXM_EBUDGET = 4,    /* some r_e outside [0, I], or budget index outside the registered range           */
+    FXM_ENOTNESTED = 5, /* fxm_register_budgets(require_nested=1): r^(b+1)_e > r^(b)_e for some e          */
+    FXM_EWORKSPACE = 6, /* workspace_bytes smaller than fxm_workspace_bytes(E,d,I,T,k)                     */
+    FXM_ESTATE = 7,     /* moe_ffn before any budget was installed                                         */
+    FXM_ECUDA = 8       /* a CUDA runtime call failed (no device, launch failure, earlier async fault)     */
+} fxm_status;
+
+#define FXM_MAX_BUDGETS 15 /* tables that fxm_register_budgets can keep resident */
+
+/* implementation selector for fxm_set_impl: the tcgen05 path is the product; the SIMT path is the slow,
+ * structurally simple debug path that runs on the SAME packed layout (used to bisect the fast kernels). */
+#define FXM_IMPL_TCGEN05 0
+#define FXM_IMPL_SIMT_DEBUG 1
+
+/* ---- sizes first: the caller owns all device memory -------------------------------------------------- */
+
+/* Bytes of the packed, channel-ranked, tile-major weight blob for an [E, I, d] layer (includes the
+ * resident budget tables: (FXM_MAX_BUDGETS+1) * 256 int32, a small state block and a copy of channel_rank). */
+fxm_status fxm_packed_bytes(int E, int d, int I, size_t* bytes);
+
+/* Bytes of scratch for one moe_ffn / route call with at most T_max tokens and k experts per token:
+ * grouping indices, tile schedule, the gathered activations X_s [T_max*k + 16E, d] bf16, the SwiGLU
+ * activations H [T_max*k + 16E, ceil64(I)] bf16 and the fp32 combine accumulator [T_max, d]. */
+fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* bytes);
+
+/* ---- (1) pack: Eq. 3; layout prior art App. C.2, PAPER.md:526-540 ---------------------
+ * W_gate, W_up : device, bf16 [E][I][d]   (row c of expert e = channel c)
+ * W_down       : device, bf16 [E][d][I]   (column c = channel c)
+ * channel_rank : HOST int32 [E][I] or NULL (= identity).  channel_rank[e][p] is the ORIGINAL index of the
+ *                p-th most important channel of expert e (argsort-descending output; gather semantics).
+ *                Validated on the host before anything is enqueued (FXM_EPERM).
+ * packed       : device buffer of fxm_packed_bytes(), 1024-byte aligned.  Written by kernels on `stream`;
+ *                the three source tensors may be freed once the stream has passed this call.
+ * The packed layout is private: 16 KB tiles of 128 rows x 64 K-elements, stored
+ * pre-swizzled (128-byte swizzle) so a tile is one contiguous bulk copy into UMMA-ready shared memory;
+ * gate and up rows of the same 16 channels are adjacent, and any channel prefix of an expert is a
+ * contiguous prefix of its tiles -- a budget never moves weights. */
+fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, const void* W_up,
+                    const void* W_down, const int32_t* channel_rank, void* packed, void* stream);
+
+/* ---- (2) budgets: Eq. 11-12; runtime switching PAPER.md:230-239 --------------------
+ * Widths, not ratios.  No weight is read or written by any of these. */
+
+/* Install r_host[E] (HOST) as the current table: exactly one tiny kernel launch on `stream` (the table
+ * travels in the kernel's arguments; r_host may be reused as soon as the call returns). */
+fxm_status fxm_set_budget(fxm_layer* L, const int32_t* r_host, void* stream);
+
+/* Keep B <= FXM_MAX_BUDGETS tables r_host[B][E] (HOST) resident on the device (B tiny launches).
+ * require_nested != 0 checks r[b+1][e] <= r[b][e] for all b, e (reading R14). */
+fxm_status fxm_register_budgets(fxm_layer* L, int B, const int32_t* r_host, int require_nested, void* stream);
+
+/* Host-only, no CUDA call at all: the next fxm_moe_ffn reads registered table b. */
+fxm_status fxm_select_budget(fxm_layer* L, int b);
+
+/* k = ceil(I * num / den) in exact integer arithmetic (reading R2); -1 on bad input. */
+int32_t fxm_ratio_to_width(int I, int num, int den);
+
+/* ---- (3) forward: Alg. 2, PAPER.md:545-590 -----------------------------------------------------------
+ * x        : device bf16 [T][d]
+ * topk_ids : device int32 [T][k], each in [0, E)   (precondition; violations set a sticky device flag
+ *            readable with fxm_device_flags and the offending assignment is dropped)
+ * topk_w   : device fp32 [T][k], applied as given (the router is external and frozen)
+ * y        : device bf16 [T][d], OVERWRITTEN (Y <- 0 then accumulate); routed experts only.
+ * workspace: device, >= fxm_workspace_bytes(E,d,I,T,k), 1024-byte aligned; contents are scratch.
+ * Launches: route, gather, grouped GEMM-1(+SwiGLU), grouped GEMM-2(+scale+combine), finalize.  Grid sizes
+ * do not depend on the budget or on the routing (persistent kernels read the device-side schedule), so a
+ * call is CUDA-graph capturable.  T == 0 is a no-op. */
+fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
+                       void* y, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- parity / debug surface ---------------------------------------------------------------------------
+ * Step a2 alone (Alg. 2 l.4-6; stable by (expert id, flat index t*k+j), reading R5):
+ * counts [E], offsets [E+1] (exclusive scan, offsets[E] = T*k), perm [T*k], inv_perm [T*k]: device int32. */
+fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_t* counts, int32_t* offsets,
+                     int32_t* perm, int32_t* inv_perm, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Inverse of pack for a prefix: writes the first r ranked channels of expert e as plain row-major bf16
+ * Wg [r][d], Wu [r][d], Wd [d][r] (device).  Test surface and the offline-clipping export. */
+fxm_status fxm_unpack_prefix(fxm_layer* L, int e, int r, void* Wg, void* Wu, void* Wd, void* stream);
+
+/* Copy the internal SwiGLU activations of the LAST moe_ffn on this workspace into row-major bf16
+ * H_out [T*k][I] in sorted (perm) order; columns >= r_e are 0.  Debug only. */
+fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k, void* workspace, void* H_out,
+                            void* stream);
+
+fxm_status fxm_set_impl(fxm_layer* L, int impl);          /* FXM_IMPL_* ; default FXM_IMPL_TCGEN05 */
+/* Token-tile width of the grouped GEMMs: 128, 256, or 0 = choose from T*k/E (default).  Tuning knob only. */
+fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
+/* Synchronises `stream`, then returns the sticky device flag word (bit0: expert id out of range,
+ * bit1: a pipeline wait timed out -- a bug) in *flags and clears it. */
+fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream);
+/* Number of kernels one fxm_moe_ffn enqueues (bench.py's gpu_launches). */
+int fxm_launches_per_ffn(const fxm_layer* L);
+
+const char* fxm_status_string(fxm_status s);
+void fxm_destroy(fxm_layer* L); /* frees host metadata only */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FLEXMOE_H_ */

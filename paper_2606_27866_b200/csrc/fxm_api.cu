@@ -1,0 +1,275 @@
+// fxm_api.cu -- the C ABI of include/flexmoe.h: argument validation, host metadata, launch sequencing.
+// No arithmetic of the method lives here; every step of the path runs in the kernels of this directory.
+#include "../../include/flexmoe.h"
+#include "fxm_internal.cuh"
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+using namespace fxm;
+
+struct fxm_layer {
+    Dims D;
+    uint8_t* packed;         // caller's buffer: [gate/up tiles][down tiles][tables][state][channel_rank copy]
+    int* tables;             // [MAX_TABLES][TABLE_STRIDE] int32
+    DevState* state;
+    int n_registered;
+    int current;             // index of the table the next moe_ffn reads; -1 = none installed
+    int impl;
+    int num_sms;
+    int tile_n_override;     // 0 = choose from T*k/E
+    std::vector<int> host_tables;   // mirror of the resident tables (validation / introspection only)
+};
+
+static bool make_dims(int E, int d, int I, Dims* D) {
+    if (E < 1 || E > MAX_E || d < 64 || d % 64 != 0 || I < 16 || I % 16 != 0) return false;
+    D->E = E; D->d = d; D->I = I;
+    D->Ip = (I + CB - 1) / CB * CB;
+    D->nCB = D->Ip / CB;
+    D->nKB1 = d / KB;
+    D->nDB = (d + WT_ROWS - 1) / WT_ROWS;
+    return true;
+}
+
+static size_t tables_offset(const Dims& D) { return align_up(gu_bytes(D) + dn_bytes(D), 1024); }
+static size_t state_offset(const Dims& D) { return tables_offset(D) + sizeof(int) * MAX_TABLES * TABLE_STRIDE; }
+static size_t rank_offset(const Dims& D) { return align_up(state_offset(D) + sizeof(DevState), 1024); }
+static size_t packed_total(const Dims& D) { return align_up(rank_offset(D) + sizeof(int) * (size_t)D.E * D.I, 1024); }
+
+static int choose_tile_n(const fxm_layer* L, int T, int k) {
+    if (L->tile_n_override == 128 || L->tile_n_override == 256) return L->tile_n_override;
+    // mean rows per expert > 192: 256-token tiles halve the weight re-reads; below that 128 wastes less
+    return ((long long)T * k > 192LL * L->D.E) ? 256 : 128;
+}
+
+extern "C" {
+
+const char* fxm_status_string(fxm_status s) {
+    switch (s) {
+        case FXM_OK: return "FXM_OK";
+        case FXM_EINVAL: return "FXM_EINVAL: bad pointer, size or enum";
+        case FXM_ESHAPE: return "FXM_ESHAPE: unsupported dimensions";
+        case FXM_EPERM: return "FXM_EPERM: channel_rank row is not a permutation";
+        case FXM_EBUDGET: return "FXM_EBUDGET: width outside [0, I] or unknown budget index";
+        case FXM_ENOTNESTED: return "FXM_ENOTNESTED: budget tables are not nested";
+        case FXM_EWORKSPACE: return "FXM_EWORKSPACE: workspace too small";
+        case FXM_ESTATE: return "FXM_ESTATE: no budget installed";
+        case FXM_ECUDA: return "FXM_ECUDA: CUDA runtime failure";
+    }
+    return "FXM_?";
+}
+
+fxm_status fxm_packed_bytes(int E, int d, int I, size_t* bytes) {
+    Dims D;
+    if (!bytes) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    *bytes = packed_total(D);
+    return FXM_OK;
+}
+
+fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* bytes) {
+    Dims D;
+    if (!bytes || T_max < 0) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    if (k < 1 || k > MAX_K || k > E) return FXM_ESHAPE;
+    if ((long long)T_max * k > (1LL << 30)) return FXM_ESHAPE;
+    *bytes = map_workspace(D, T_max, k, nullptr).bytes;
+    return FXM_OK;
+}
+
+int32_t fxm_ratio_to_width(int I, int num, int den) {
+    if (I < 0 || den <= 0 || num < 0 || num > den) return -1;
+    return (int32_t)(((int64_t)I * num + den - 1) / den);
+}
+
+fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down,
+                    const int32_t* channel_rank, void* packed, void* stream) {
+    Dims D;
+    if (!out || !W_gate || !W_up || !W_down || !packed) return FXM_EINVAL;
+    if (((uintptr_t)packed & 1023u) || ((uintptr_t)W_gate & 15u) || ((uintptr_t)W_up & 15u) || ((uintptr_t)W_down & 1u))
+        return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    if (channel_rank) {                                           // validated on the host: offline, once
+        std::vector<uint8_t> seen((size_t)I);
+        for (int e = 0; e < E; ++e) {
+            std::fill(seen.begin(), seen.end(), 0);
+            for (int p = 0; p < I; ++p) {
+                const int c = channel_rank[(size_t)e * I + p];
+                if (c < 0 || c >= I || seen[c]) return FXM_EPERM;
+                seen[c] = 1;
+            }
+        }
+    }
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return FXM_ECUDA;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return FXM_ECUDA;
+    if (init_sm100_kernels() != cudaSuccess) return FXM_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint8_t* pk = (uint8_t*)packed;
+    int* tables = (int*)(pk + tables_offset(D));
+    DevState* state = (DevState*)(pk + state_offset(D));
+    int* rank_dev = channel_rank ? (int*)(pk + rank_offset(D)) : nullptr;
+    if (cudaMemsetAsync(tables, 0, sizeof(int) * MAX_TABLES * TABLE_STRIDE + sizeof(DevState), st) != cudaSuccess)
+        return FXM_ECUDA;
+    if (rank_dev && cudaMemcpyAsync(rank_dev, channel_rank, sizeof(int) * (size_t)E * I, cudaMemcpyHostToDevice, st) !=
+                        cudaSuccess)
+        return FXM_ECUDA;
+    if (launch_pack(D, (const __nv_bfloat16*)W_gate, (const __nv_bfloat16*)W_up, (const __nv_bfloat16*)W_down, rank_dev,
+                    pk, st) != cudaSuccess)
+        return FXM_ECUDA;
+    fxm_layer* L = new (std::nothrow) fxm_layer();
+    if (!L) return FXM_EINVAL;
+    L->D = D; L->packed = pk; L->tables = tables; L->state = state;
+    L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
+    L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
+    *out = L;
+    return FXM_OK;
+}
+
+void fxm_destroy(fxm_layer* L) { delete L; }
+
+static fxm_status check_table(const fxm_layer* L, const int32_t* r) {
+    for (int e = 0; e < L->D.E; ++e)
+        if (r[e] < 0 || r[e] > L->D.I) return FXM_EBUDGET;
+    return FXM_OK;
+}
+
+fxm_status fxm_set_budget(fxm_layer* L, const int32_t* r_host, void* stream) {
+    if (!L || !r_host) return FXM_EINVAL;
+    fxm_status s = check_table(L, r_host);
+    if (s != FXM_OK) return s;
+    const int slot = MAX_TABLES - 1;                              // the slot fxm_register_budgets never uses
+    if (launch_set_table(L->tables + (size_t)slot * TABLE_STRIDE, r_host, L->D.E, (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    std::copy(r_host, r_host + L->D.E, L->host_tables.begin() + (size_t)slot * TABLE_STRIDE);
+    L->current = slot;
+    return FXM_OK;
+}
+
+fxm_status fxm_register_budgets(fxm_layer* L, int B, const int32_t* r_host, int require_nested, void* stream) {
+    if (!L || !r_host || B < 1 || B > FXM_MAX_BUDGETS) return FXM_EINVAL;
+    const int E = L->D.E;
+    for (int b = 0; b < B; ++b) {
+        fxm_status s = check_table(L, r_host + (size_t)b * E);
+        if (s != FXM_OK) return s;
+        if (require_nested && b > 0)
+            for (int e = 0; e < E; ++e)
+                if (r_host[(size_t)b * E + e] > r_host[(size_t)(b - 1) * E + e]) return FXM_ENOTNESTED;
+    }
+    for (int b = 0; b < B; ++b) {
+        if (launch_set_table(L->tables + (size_t)b * TABLE_STRIDE, r_host + (size_t)b * E, E, (cudaStream_t)stream) !=
+            cudaSuccess)
+            return FXM_ECUDA;
+        std::copy(r_host + (size_t)b * E, r_host + (size_t)(b + 1) * E, L->host_tables.begin() + (size_t)b * TABLE_STRIDE);
+    }
+    L->n_registered = B;
+    return FXM_OK;
+}
+
+fxm_status fxm_select_budget(fxm_layer* L, int b) {
+    if (!L) return FXM_EINVAL;
+    if (b < 0 || b >= L->n_registered) return FXM_EBUDGET;
+    L->current = b;                                               // host-only: the next launch reads another 1 KB table
+    return FXM_OK;
+}
+
+fxm_status fxm_set_impl(fxm_layer* L, int impl) {
+    if (!L || (impl != FXM_IMPL_TCGEN05 && impl != FXM_IMPL_SIMT_DEBUG)) return FXM_EINVAL;
+    L->impl = impl;
+    return FXM_OK;
+}
+
+fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n) {
+    if (!L || (tile_n != 0 && tile_n != 128 && tile_n != 256)) return FXM_EINVAL;
+    L->tile_n_override = tile_n;
+    return FXM_OK;
+}
+
+int fxm_launches_per_ffn(const fxm_layer* L) { (void)L; return 5; }
+
+static fxm_status check_call(const fxm_layer* L, int T, int k, const void* ws, size_t ws_bytes) {
+    if (!L || T < 0 || !ws || ((uintptr_t)ws & 1023u)) return FXM_EINVAL;
+    if (k < 1 || k > MAX_K || k > L->D.E || (long long)T * k > (1LL << 30)) return FXM_ESHAPE;
+    if (ws_bytes < map_workspace(L->D, T, k, nullptr).bytes) return FXM_EWORKSPACE;
+    return FXM_OK;
+}
+
+fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_t* counts, int32_t* offsets,
+                     int32_t* perm, int32_t* inv_perm, void* workspace, size_t workspace_bytes, void* stream) {
+    fxm_status s = check_call(L, T, k, workspace, workspace_bytes);
+    if (s != FXM_OK) return s;
+    if (!counts || !offsets || (T > 0 && (!topk_ids || !perm || !inv_perm))) return FXM_EINVAL;
+    const Workspace ws = map_workspace(L->D, T, k, workspace);
+    const int* table = L->current >= 0 ? L->tables + (size_t)L->current * TABLE_STRIDE : nullptr;
+    if (launch_route(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), counts, offsets, perm, inv_perm, ws, L->state,
+                     (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k, void* y,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    fxm_status s = check_call(L, T, k, workspace, workspace_bytes);
+    if (s != FXM_OK) return s;
+    if (T == 0) return FXM_OK;
+    if (!x || !topk_ids || !topk_w || !y || ((uintptr_t)x & 15u) || ((uintptr_t)y & 7u)) return FXM_EINVAL;
+    if (L->current < 0) return FXM_ESTATE;
+    const Dims& D = L->D;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Workspace ws = map_workspace(D, T, k, workspace);
+    const int* table = L->tables + (size_t)L->current * TABLE_STRIDE;
+    const int tile_n = choose_tile_n(L, T, k);
+    // a2 + a3: grouping and the tile schedule for the CURRENT table
+    if (launch_route(D, topk_ids, T, k, table, tile_n, ws.counts, ws.offsets, ws.perm, ws.inv_perm, ws, L->state, st) !=
+        cudaSuccess)
+        return FXM_ECUDA;
+    // gather x rows into sorted swizzled panels; zero the combine accumulator
+    if (launch_prep(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+    if (L->impl == FXM_IMPL_TCGEN05) {
+        if (launch_gemm1_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
+        if (launch_gemm2_sm100(D, L->packed, table, topk_w, k, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess)
+            return FXM_ECUDA;
+    } else {
+        if (launch_gemm1_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
+        if (launch_gemm2_simt(D, L->packed, table, topk_w, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+    }
+    if (launch_finalize(D, T, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_unpack_prefix(fxm_layer* L, int e, int r, void* Wg, void* Wu, void* Wd, void* stream) {
+    if (!L || e < 0 || e >= L->D.E) return FXM_EINVAL;
+    if (r < 0 || r > L->D.I) return FXM_EBUDGET;
+    if (r == 0) return FXM_OK;
+    if (!Wg || !Wu || !Wd) return FXM_EINVAL;
+    if (launch_unpack_prefix(L->D, L->packed, e, r, (__nv_bfloat16*)Wg, (__nv_bfloat16*)Wu, (__nv_bfloat16*)Wd,
+                             (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k, void* workspace, void* H_out,
+                            void* stream) {
+    if (!L || !workspace || !H_out || !topk_ids || T < 0) return FXM_EINVAL;
+    if (L->current < 0) return FXM_ESTATE;
+    if (T == 0) return FXM_OK;
+    const Workspace ws = map_workspace(L->D, T, k, workspace);
+    if (launch_read_h(L->D, T, k, topk_ids, L->tables + (size_t)L->current * TABLE_STRIDE, ws, (__nv_bfloat16*)H_out,
+                      (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream) {
+    if (!L || !flags) return FXM_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t v = 0;
+    if (cudaMemcpyAsync(&v, &L->state->flags, sizeof(v), cudaMemcpyDeviceToHost, st) != cudaSuccess) return FXM_ECUDA;
+    if (cudaMemsetAsync(&L->state->flags, 0, sizeof(v), st) != cudaSuccess) return FXM_ECUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return FXM_ECUDA;
+    *flags = v;
+    return FXM_OK;
+}
+
+}  // extern "C"

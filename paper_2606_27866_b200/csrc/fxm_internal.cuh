@@ -1,0 +1,154 @@
+// fxm_internal.cuh -- shared declarations of the CUDA path (layout math, workspace map, launchers).
+// Nothing here is shared with oracle/ (the CPU oracle has its own plain row-major view of the problem).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stddef.h>
+
+namespace fxm {
+
+// ------------------------------------------------------------------------------------------------
+// Tile geometry.  Every operand of both grouped GEMMs is stored as "SW128 K-major" tiles:
+// rows of 64 bf16 (128 bytes), the 16-byte chunk index of a row XOR-ed with (row & 7) -- exactly what
+// tcgen05.mma expects in shared memory for LayoutType SWIZZLE_128B, so a tile is moved with ONE
+// contiguous cp.async.bulk and never re-arranged on chip.
+// ------------------------------------------------------------------------------------------------
+constexpr int KB = 64;                 // K elements per tile row (128 bytes)
+constexpr int ROW_BYTES = 128;
+constexpr int WT_ROWS = 128;           // weight tile rows = UMMA M
+constexpr int WT_BYTES = WT_ROWS * ROW_BYTES;   // 16 KB
+constexpr int CB = 64;                 // channels per gate/up tile (64 gate rows + 64 up rows)
+constexpr int ROW_ALIGN = 16;          // padded-row alignment of an expert segment (UMMA N granularity)
+constexpr int MAX_E = 256;
+constexpr int MAX_K = 16;
+constexpr int TABLE_STRIDE = 256;      // int32 per resident budget table
+constexpr int MAX_TABLES = 16;         // FXM_MAX_BUDGETS registered + 1 "set_budget" slot
+
+// byte offset of element (row, col) inside a swizzled tile whose rows are 128 B; row is the row index
+// relative to a base that is a multiple of 8 rows.
+__host__ __device__ inline uint32_t sw128_off(uint32_t row, uint32_t col) {
+    return row * ROW_BYTES + ((((col >> 3) ^ row) & 7u) << 4) + ((col & 7u) << 1);
+}
+// byte offset of 16-byte chunk `ch` (0..7) of `row`
+__host__ __device__ inline uint32_t sw128_chunk(uint32_t row, uint32_t ch) {
+    return row * ROW_BYTES + (((ch ^ row) & 7u) << 4);
+}
+
+struct Dims {
+    int E, d, I;
+    int Ip;      // ceil64(I)
+    int nCB;     // Ip / 64  channel blocks
+    int nKB1;    // d / 64   K blocks of GEMM-1
+    int nDB;     // ceil(d / 128) row blocks of the down projection
+};
+
+// packed blob: [gate/up tiles][down tiles][tables][state]
+//   gate/up tile (e, cb, kb):  rows pr=0..127: g16 = pr/32, w = pr%32; w<16 -> gate channel cb*64+g16*16+w,
+//                              else up channel cb*64+g16*16+(w-16); cols = x features kb*64 .. +63
+//   down tile (e, kb2, db):    rows = output features db*128 .. +127, cols = channels kb2*64 .. +63
+__host__ __device__ inline size_t gu_tile_index(const Dims& D, int e, int cb, int kb) {
+    return ((size_t)e * D.nCB + cb) * D.nKB1 + kb;
+}
+__host__ __device__ inline size_t dn_tile_index(const Dims& D, int e, int kb2, int db) {
+    return ((size_t)e * D.nCB + kb2) * D.nDB + db;
+}
+__host__ __device__ inline size_t gu_bytes(const Dims& D) { return (size_t)D.E * D.nCB * D.nKB1 * WT_BYTES; }
+__host__ __device__ inline size_t dn_bytes(const Dims& D) { return (size_t)D.E * D.nCB * D.nDB * WT_BYTES; }
+
+struct DevState {           // lives at the tail of the packed blob
+    uint32_t flags;         // bit0: expert id out of range; bit1: pipeline wait timed out
+    uint32_t pad[63];
+};
+
+// ------------------------------------------------------------------------------------------------
+// Workspace map (all offsets 1024-byte aligned).  P = padded-row capacity for this call.
+// ------------------------------------------------------------------------------------------------
+struct Sched {              // written by the route kernel, read by everything after it
+    int ntt;                // number of token tiles (experts with n_e == 0 or r_e == 0 get none: pruned work is never issued)
+    int W1;                 // GEMM-1 work items  = sum_j ceil(r_e(j) / 64)
+    int W2;                 // GEMM-2 work items  = ntt * nDB
+    int P_used;             // padded rows in use
+    int A;                  // T * k
+    int pad[11];
+};
+
+struct Workspace {
+    int* counts;            // [E]
+    int* offsets;           // [E+1]
+    int* poff;              // [E+1] padded-row offset of each expert segment (multiple of 16)
+    Sched* sched;
+    int* perm;              // [A]
+    int* inv_perm;          // [A]
+    int* row_flat;          // [P]  flat assignment index f = t*k+j of each padded row, -1 for padding
+    int4* tt;               // [NT] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}
+    int4* items1;           // [NT*nCB] GEMM-1 work items {expert, first padded row, valid rows, channel block}
+    uint8_t* Xs;            // [nKB1][P][128 B]  gathered activations, swizzled panels
+    uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
+    float* yacc;            // [T][d]
+    int P;                  // padded-row capacity (multiple of 16)
+    int NT;                 // token-tile capacity
+    size_t bytes;           // total
+};
+
+constexpr int TILE_N_MAX = 256;   // largest token tile any kernel uses (schedule capacity is sized for the smallest)
+constexpr int TILE_N_MIN = 128;
+
+__host__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+__host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base) {
+    Workspace w{};
+    const size_t A = (size_t)T * k;
+    const int P = (int)align_up(A + (size_t)(ROW_ALIGN - 1) * D.E, ROW_ALIGN) + ROW_ALIGN;
+    const int NT = (int)(A / TILE_N_MIN) + D.E + 1;
+    size_t o = 0;
+    auto take = [&](size_t n) { size_t r = o; o = align_up(o + n, 1024); return r; };
+    uint8_t* b = (uint8_t*)base;
+    w.counts = (int*)(b + take(sizeof(int) * MAX_E));
+    w.offsets = (int*)(b + take(sizeof(int) * (MAX_E + 1)));
+    w.poff = (int*)(b + take(sizeof(int) * (MAX_E + 1)));
+    w.sched = (Sched*)(b + take(sizeof(Sched)));
+    w.perm = (int*)(b + take(sizeof(int) * (A + 1)));
+    w.inv_perm = (int*)(b + take(sizeof(int) * (A + 1)));
+    w.row_flat = (int*)(b + take(sizeof(int) * (size_t)P));
+    w.tt = (int4*)(b + take(sizeof(int4) * (size_t)NT));
+    w.items1 = (int4*)(b + take(sizeof(int4) * (size_t)NT * D.nCB));
+    w.Xs = b + take((size_t)D.nKB1 * P * ROW_BYTES);
+    w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
+    w.yacc = (float*)(b + take(sizeof(float) * (size_t)T * D.d));
+    w.P = P;
+    w.NT = NT;
+    w.bytes = o;
+    return w;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Launchers (each enqueues on `st` and returns cudaGetLastError()).
+// ------------------------------------------------------------------------------------------------
+cudaError_t launch_pack(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
+                        const int* rank_dev /*[E][I] or null*/, uint8_t* packed, cudaStream_t st);
+cudaError_t launch_unpack_prefix(const Dims& D, const uint8_t* packed, int e, int r, __nv_bfloat16* Wg,
+                                 __nv_bfloat16* Wu, __nv_bfloat16* Wd, cudaStream_t st);
+cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStream_t st);
+cudaError_t launch_route(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n,
+                         int* counts, int* offsets, int* perm, int* inv_perm, const Workspace& ws,
+                         DevState* state, cudaStream_t st);   // also writes ws.poff/row_flat/tt/items1/sched
+cudaError_t launch_prep(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st);
+cudaError_t launch_finalize(const Dims& D, int T, const Workspace& ws, __nv_bfloat16* y, cudaStream_t st);
+cudaError_t launch_read_h(const Dims& D, int T, int k, const int* ids, const int* r_table, const Workspace& ws,
+                          __nv_bfloat16* H_out, cudaStream_t st);
+
+// SIMT debug path (same layouts, no tensor cores, no async copies)
+cudaError_t launch_gemm1_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                              cudaStream_t st);
+cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const float* topk_w, int k,
+                              const Workspace& ws, cudaStream_t st);
+
+// tcgen05 / TMEM / bulk-copy path
+cudaError_t launch_gemm1_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                               DevState* state, int tile_n, int num_sms, cudaStream_t st);
+cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const float* topk_w, int k,
+                               const Workspace& ws, DevState* state, int tile_n, int num_sms, cudaStream_t st);
+cudaError_t init_sm100_kernels();   // cudaFuncSetAttribute for the dynamic shared memory sizes
+
+}  // namespace fxm

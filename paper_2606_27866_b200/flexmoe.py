@@ -1,0 +1,268 @@
+"""Thin Python binding of the C ABI in include/flexmoe.h (same names, argument marshalling only).
+
+torch is used for device memory and streams; every step of the path runs in the CUDA kernels of
+csrc/.  There is no CPU fallback: if libflexmoe.so is missing or no CUDA device is present the calls
+raise.  This module never imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "csrc")
+_SO = os.path.join(_HERE, "libflexmoe.so")
+_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_sm100.cu"]
+_HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_HERE, "..", "include", "flexmoe.h")]
+
+IMPL_TCGEN05 = 0
+IMPL_SIMT_DEBUG = 1
+MAX_BUDGETS = 15
+
+_STATUS = ["FXM_OK", "FXM_EINVAL", "FXM_ESHAPE", "FXM_EPERM", "FXM_EBUDGET", "FXM_ENOTNESTED",
+           "FXM_EWORKSPACE", "FXM_ESTATE", "FXM_ECUDA"]
+
+
+class FxmError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        self.name = _STATUS[code] if 0 <= code < len(_STATUS) else f"FXM_{code}"
+        super().__init__(f"{where}: {self.name}")
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """nvcc-compile csrc/*.cu for sm_100a into paper_2606_27866_b200/libflexmoe.so (in-tree)."""
+    srcs = [os.path.join(_CSRC, s) for s in _SOURCES]
+    deps = srcs + _HEADERS
+    if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(p) for p in deps):
+        return _SO
+    cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+           "-Xcompiler", "-fPIC", "-shared", "-o", _SO] + srcs
+    if verbose:
+        cmd.insert(1, "-Xptxas=-v")
+    subprocess.check_call(cmd)
+    return _SO
+
+
+_lib = None
+
+
+def lib():
+    """Load the shared library (building it first if nvcc is available and it is stale/missing)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        build()
+    L = ctypes.CDLL(_SO)
+    vp, i32, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+    L.fxm_packed_bytes.argtypes = [i32, i32, i32, ctypes.POINTER(sz)]
+    L.fxm_workspace_bytes.argtypes = [i32, i32, i32, i32, i32, ctypes.POINTER(sz)]
+    L.fxm_pack.argtypes = [ctypes.POINTER(vp), i32, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.fxm_set_budget.argtypes = [vp, vp, vp]
+    L.fxm_register_budgets.argtypes = [vp, i32, vp, i32, vp]
+    L.fxm_select_budget.argtypes = [vp, i32]
+    L.fxm_ratio_to_width.argtypes = [i32, i32, i32]
+    L.fxm_ratio_to_width.restype = ctypes.c_int32
+    L.fxm_moe_ffn.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_route.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
+    L.fxm_unpack_prefix.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+    L.fxm_debug_read_h.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+    L.fxm_set_impl.argtypes = [vp, i32]
+    L.fxm_set_tile_n.argtypes = [vp, i32]
+    L.fxm_device_flags.argtypes = [vp, ctypes.POINTER(ctypes.c_uint32), vp]
+    L.fxm_launches_per_ffn.argtypes = [vp]
+    L.fxm_status_string.argtypes = [i32]
+    L.fxm_status_string.restype = ctypes.c_char_p
+    L.fxm_destroy.argtypes = [vp]
+    L.fxm_destroy.restype = None
+    _lib = L
+    return L
+
+
+EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
+           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_route", "fxm_unpack_prefix",
+           "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_device_flags", "fxm_launches_per_ffn",
+           "fxm_status_string", "fxm_destroy"]
+
+
+def _chk(code: int, where: str):
+    if code != 0:
+        raise FxmError(code, where)
+
+
+def packed_bytes(E: int, d: int, I: int) -> int:
+    n = ctypes.c_size_t()
+    _chk(lib().fxm_packed_bytes(E, d, I, ctypes.byref(n)), "fxm_packed_bytes")
+    return n.value
+
+
+def workspace_bytes(E: int, d: int, I: int, T_max: int, k: int) -> int:
+    n = ctypes.c_size_t()
+    _chk(lib().fxm_workspace_bytes(E, d, I, T_max, k, ctypes.byref(n)), "fxm_workspace_bytes")
+    return n.value
+
+
+def ratio_to_width(I: int, num: int, den: int) -> int:
+    return int(lib().fxm_ratio_to_width(I, num, den))
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _i32_host(a):
+    import numpy as np
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+class Layer:
+    """One packed MoE layer.  Owns (via torch) the packed weight blob and a workspace."""
+
+    def __init__(self, handle, E, d, I, packed):
+        self._h = handle
+        self.E, self.d, self.I = E, d, I
+        self.packed = packed            # torch.uint8 tensor; must outlive the handle
+        self._ws = None
+        self._ws_key = None
+
+    # -- (1) pack ---------------------------------------------------------------------------------
+    @staticmethod
+    def pack(W_gate, W_up, W_down, channel_rank=None, stream=None) -> "Layer":
+        """W_gate/W_up [E,I,d], W_down [E,d,I]: CUDA bf16 tensors; channel_rank [E,I] int32 (host) or None."""
+        import torch
+        assert W_gate.is_cuda and W_gate.dtype == torch.bfloat16 and W_gate.is_contiguous()
+        assert W_up.is_cuda and W_up.dtype == torch.bfloat16 and W_up.is_contiguous()
+        assert W_down.is_cuda and W_down.dtype == torch.bfloat16 and W_down.is_contiguous()
+        E, I, d = W_gate.shape
+        assert tuple(W_up.shape) == (E, I, d) and tuple(W_down.shape) == (E, d, I)
+        nbytes = packed_bytes(E, d, I)
+        packed = torch.empty(nbytes + 1024, dtype=torch.uint8, device=W_gate.device)
+        off = (-packed.data_ptr()) % 1024
+        packed = packed[off:off + nbytes]
+        rk = None
+        rk_ptr = None
+        if channel_rank is not None:
+            rk = _i32_host(channel_rank)
+            assert rk.shape == (E, I)
+            rk_ptr = ctypes.c_void_p(rk.ctypes.data)
+        h = ctypes.c_void_p()
+        _chk(lib().fxm_pack(ctypes.byref(h), E, d, I, W_gate.data_ptr(), W_up.data_ptr(), W_down.data_ptr(), rk_ptr,
+                            packed.data_ptr(), _stream_ptr(stream)), "fxm_pack")
+        return Layer(h, E, d, I, packed)
+
+    def __del__(self):
+        try:
+            if self._h:
+                lib().fxm_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    # -- (2) budgets ------------------------------------------------------------------------------
+    def set_budget(self, r, stream=None):
+        r = _i32_host(r)
+        assert r.shape == (self.E,)
+        _chk(lib().fxm_set_budget(self._h, r.ctypes.data, _stream_ptr(stream)), "fxm_set_budget")
+
+    def register_budgets(self, tables, require_nested=True, stream=None):
+        t = _i32_host(tables)
+        assert t.ndim == 2 and t.shape[1] == self.E
+        _chk(lib().fxm_register_budgets(self._h, t.shape[0], t.ctypes.data, int(bool(require_nested)),
+                                        _stream_ptr(stream)), "fxm_register_budgets")
+
+    def select_budget(self, b: int):
+        _chk(lib().fxm_select_budget(self._h, int(b)), "fxm_select_budget")
+
+    def set_impl(self, impl: int):
+        _chk(lib().fxm_set_impl(self._h, int(impl)), "fxm_set_impl")
+
+    def set_tile_n(self, n: int):
+        _chk(lib().fxm_set_tile_n(self._h, int(n)), "fxm_set_tile_n")
+
+    # -- workspace ----------------------------------------------------------------------------------
+    def workspace(self, T: int, k: int):
+        """A cached 1024-aligned torch buffer large enough for (T, k)."""
+        import torch
+        need = workspace_bytes(self.E, self.d, self.I, T, k)
+        if self._ws is None or self._ws.numel() < need:
+            raw = torch.empty(need + 1024, dtype=torch.uint8, device=self.packed.device)
+            off = (-raw.data_ptr()) % 1024
+            self._ws = raw[off:off + need]
+        return self._ws
+
+    # -- (3) forward --------------------------------------------------------------------------------
+    def moe_ffn(self, x, topk_ids, topk_w, out=None, workspace=None, stream=None):
+        """x [T,d] bf16, topk_ids [T,k] int32, topk_w [T,k] fp32 (CUDA, contiguous) -> y [T,d] bf16."""
+        import torch
+        T, d = x.shape
+        k = topk_ids.shape[1]
+        assert d == self.d and x.dtype == torch.bfloat16 and x.is_cuda and x.is_contiguous()
+        assert topk_ids.dtype == torch.int32 and topk_ids.is_contiguous() and tuple(topk_ids.shape) == (T, k)
+        assert topk_w.dtype == torch.float32 and topk_w.is_contiguous() and tuple(topk_w.shape) == (T, k)
+        y = torch.empty((T, d), dtype=torch.bfloat16, device=x.device) if out is None else out
+        ws = self.workspace(T, k) if workspace is None else workspace
+        _chk(lib().fxm_moe_ffn(self._h, x.data_ptr(), topk_ids.data_ptr(), topk_w.data_ptr(), T, k, y.data_ptr(),
+                               ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_moe_ffn")
+        return y
+
+    # -- parity / debug surface -----------------------------------------------------------------------
+    def route(self, topk_ids, stream=None):
+        import torch
+        T, k = topk_ids.shape
+        assert topk_ids.dtype == torch.int32 and topk_ids.is_cuda and topk_ids.is_contiguous()
+        dev = topk_ids.device
+        counts = torch.empty(self.E, dtype=torch.int32, device=dev)
+        offsets = torch.empty(self.E + 1, dtype=torch.int32, device=dev)
+        perm = torch.empty(max(T * k, 1), dtype=torch.int32, device=dev)
+        inv = torch.empty(max(T * k, 1), dtype=torch.int32, device=dev)
+        ws = self.workspace(T, k)
+        _chk(lib().fxm_route(self._h, topk_ids.data_ptr(), T, k, counts.data_ptr(), offsets.data_ptr(), perm.data_ptr(),
+                             inv.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_route")
+        return counts, offsets, perm[:T * k], inv[:T * k]
+
+    def unpack_prefix(self, e: int, r: int, stream=None):
+        import torch
+        dev = self.packed.device
+        Wg = torch.empty((r, self.d), dtype=torch.bfloat16, device=dev)
+        Wu = torch.empty((r, self.d), dtype=torch.bfloat16, device=dev)
+        Wd = torch.empty((self.d, r), dtype=torch.bfloat16, device=dev)
+        _chk(lib().fxm_unpack_prefix(self._h, e, r, Wg.data_ptr(), Wu.data_ptr(), Wd.data_ptr(), _stream_ptr(stream)),
+             "fxm_unpack_prefix")
+        return Wg, Wu, Wd
+
+    def debug_read_h(self, topk_ids, stream=None):
+        import torch
+        T, k = topk_ids.shape
+        H = torch.zeros((T * k, self.I), dtype=torch.bfloat16, device=self.packed.device)
+        ws = self.workspace(T, k)
+        _chk(lib().fxm_debug_read_h(self._h, topk_ids.data_ptr(), T, k, ws.data_ptr(), H.data_ptr(), _stream_ptr(stream)),
+             "fxm_debug_read_h")
+        return H
+
+    def device_flags(self, stream=None) -> int:
+        f = ctypes.c_uint32()
+        _chk(lib().fxm_device_flags(self._h, ctypes.byref(f), _stream_ptr(stream)), "fxm_device_flags")
+        return f.value
+
+    def launches_per_ffn(self) -> int:
+        return int(lib().fxm_launches_per_ffn(self._h))
+
+
+# --------------------------------------------------------------------------------------- torch helpers
+def bf16_from_bits(bits, device="cuda"):
+    """numpy uint16 bf16 bit patterns -> torch.bfloat16 tensor on `device` (no arithmetic)."""
+    import numpy as np
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(bits).view(np.int16))
+    return t.to(device).view(torch.bfloat16)
+
+
+def bf16_to_bits(t):
+    """torch.bfloat16 tensor -> numpy uint16 bit patterns."""
+    import numpy as np
+    import torch
+    return t.detach().contiguous().view(torch.int16).cpu().numpy().view(np.uint16)

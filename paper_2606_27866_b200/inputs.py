@@ -9,8 +9,8 @@ configs C1..C5 are BASELINE.json `configs` in order.  The paper's own workloads
 PAPER.md:165, 220) are not available; these inputs take their SHAPES only.
 
 bf16 tensors are carried as numpy uint16 bit patterns (numpy has no bf16).
-Draw order per config (one numpy Generator, seed given): x, W_gate, W_up, W_down,
-channel_rank, router logits, budget tables.
+Streams per config: weights (W_gate, W_up, W_down, channel_rank in that order) from
+default_rng([seed, 1]); x, router logits, then budget tables from default_rng([seed, 2, T]).
 """
 from __future__ import annotations
 
@@ -236,17 +236,30 @@ def table_fig6_like(shape: Shape, rng: np.random.Generator) -> np.ndarray:
 # --------------------------------------------------------------------------- named configs
 
 
+_LAYER_CACHE: dict = {}
+
+
+def layer_for(name: str, seed: int = 0) -> Layer:
+    """The weights of a named config: one independent generator stream default_rng([seed, 1]), so the layer does
+    not depend on T and can be cached across the T values of a config (C4 is 3.5 GB of bf16)."""
+    key = (name.upper(), seed)
+    if key not in _LAYER_CACHE:
+        _LAYER_CACHE.clear()                    # keep at most one big layer alive
+        _LAYER_CACHE[key] = make_layer(SHAPES[key[0]], np.random.default_rng([seed, 1]))
+    return _LAYER_CACHE[key]
+
+
 def config(name: str, T: int | None = None, seed: int = 0, layer: bool = True):
-    """Returns (Layer|None, Batch, rng) for a named config, following the common draw order.
-    `layer=False` skips the weight draw (used when only routing inputs are needed); the
-    generator stream then differs, which is fine for index-only tests."""
+    """Returns (Layer|None, Batch, rng) for a named config.  Streams: weights + channel_rank from
+    default_rng([seed, 1]) (see layer_for); x then router logits from default_rng([seed, 2, T]); the returned
+    rng is that second stream, from which the caller draws budget tables."""
     name = name.upper()
     sh = SHAPES[name]
-    rng = np.random.default_rng(seed)
     default_T = {"C1": 64, "C2": 4096, "C3": 8192, "C4": 8192, "C5": 4096}[name]
     T = default_T if T is None else T
+    lay = layer_for(name, seed) if layer else None
+    rng = np.random.default_rng([seed, 2, T])
     x = make_x(T, sh.d, rng)
-    lay = make_layer(sh, rng) if layer else None
     if name == "C3":
         lg = make_logits(T, sh.E, rng, 1.0, 1.5)
     else:

@@ -1,0 +1,106 @@
+"""CPU-side checks of the boundary: the C-ABI library builds/loads, exports every symbol include/flexmoe.h
+declares, and its host-only entry points (sizes, ratio->width, status strings) behave.  No compute calls."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_27866_b200 import flexmoe as fx
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "flexmoe.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(fxm_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = fx.lib()
+    names = declared_symbols()
+    assert len(names) >= 15
+    for n in names:
+        assert hasattr(L, n), f"{n} declared in include/flexmoe.h but not exported"
+    assert sorted(fx.EXPORTS) == names, "binding and header disagree on the entry points"
+
+
+def test_sizes_match_the_layout_formulas():
+    # C2: 3*E*I*d*2 bytes of weights (I, d already tile multiples) + tables/state/rank
+    E, d, I = 60, 2048, 1408
+    w = 3 * E * I * d * 2
+    n = fx.packed_bytes(E, d, I)
+    assert w <= n <= w + 64 * 1024 + 4 * E * I + 4096
+    # padded dims: I=80 -> 128 channels, d=192 -> 256 down rows
+    n2 = fx.packed_bytes(3, 192, 80)
+    assert n2 >= 3 * (128 * 192 * 2 * 2 + 256 * 128 * 2)
+    ws1 = fx.workspace_bytes(E, d, I, 4096, 4)
+    ws2 = fx.workspace_bytes(E, d, I, 16, 4)
+    assert ws1 > ws2 > 0
+    A, P = 4096 * 4, 4096 * 4 + 16 * E
+    assert ws1 >= P * d * 2 + P * I * 2 + 4096 * d * 4           # Xs + H + yacc
+    assert ws1 <= 1.2 * (P * d * 2 + P * I * 2 + 4096 * d * 4) + (1 << 20)
+
+
+@pytest.mark.parametrize("args,code", [((0, 64, 16), "FXM_ESHAPE"), ((257, 64, 16), "FXM_ESHAPE"),
+                                       ((4, 100, 16), "FXM_ESHAPE"), ((4, 64, 24), "FXM_ESHAPE")])
+def test_bad_shapes(args, code):
+    with pytest.raises(fx.FxmError) as ei:
+        fx.packed_bytes(*args)
+    assert ei.value.name == code
+
+
+def test_workspace_rejects_bad_k():
+    for k in (0, 17, 9):
+        with pytest.raises(fx.FxmError):
+            fx.workspace_bytes(8, 64, 16, 10, k)
+
+
+def test_ratio_to_width_is_integer_ceil_and_matches_oracle():
+    """k = ceil(r * d_ff) in exact integers (reading R2): 0.7 * 10 -> 7, not 8."""
+    assert fx.ratio_to_width(10, 7, 10) == 7
+    assert fx.ratio_to_width(14336, 1, 10) == 1434
+    rng = np.random.default_rng(0)
+    for _ in range(200):
+        I = int(rng.integers(1, 20000))
+        den = int(rng.integers(1, 64))
+        num = int(rng.integers(0, den + 1))
+        assert fx.ratio_to_width(I, num, den) == oracle.ratio_to_width(I, num, den) == -(-I * num // den)
+    assert fx.ratio_to_width(10, 3, 0) == -1 and fx.ratio_to_width(10, 5, 4) == -1
+
+
+def test_status_strings():
+    L = fx.lib()
+    for i in range(9):
+        assert L.fxm_status_string(i).decode().startswith("FXM_")
+
+
+def test_null_arguments_do_not_crash():
+    L = fx.lib()
+    assert L.fxm_packed_bytes(8, 64, 16, None) == 1
+    assert L.fxm_set_budget(None, None, None) == 1
+    assert L.fxm_select_budget(None, 0) == 1
+    h = ctypes.c_void_p()
+    assert L.fxm_pack(ctypes.byref(h), 8, 64, 16, None, None, None, None, None, None) == 1
+    assert not h.value
+    L.fxm_destroy(None)
+
+
+def test_product_never_imports_the_oracle():
+    """The CUDA path must not route through oracle/ (and the oracle must not import the product)."""
+    pkg = os.path.join(ROOT, "paper_2606_27866_b200")
+    for dp, _, fs in os.walk(pkg):
+        for f in fs:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dp, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert not re.search(r"#\s*include[^\n]*oracle", txt), f
+                assert "liboracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2606_27866_b200" not in txt and "from paper_2606_27866_b200" not in txt
+            assert "flexmoe.h" not in txt and "fxm_internal" not in txt

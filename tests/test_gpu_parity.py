@@ -1,0 +1,260 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the CPU oracle, element by element,
+on the same seeded inputs.  Indices bit-exact; FFN output within north_star's tolerance (gpu_util.TOL_*).
+Run on the B200 box:  python -m pytest tests -m gpu -x -q"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_27866_b200 import inputs as gen
+
+pytestmark = pytest.mark.gpu
+
+
+def _fx():
+    from paper_2606_27866_b200 import flexmoe as fx
+    return fx
+
+
+def _small_layer(seed, d, E, k, I, w_std=0.05):
+    sh = gen.Shape("t", d, E, k, I)
+    rng = np.random.default_rng(seed)
+    return sh, gen.make_layer(sh, rng, w_std=w_std), rng
+
+
+# ------------------------------------------------------------------------------------------------ pack
+@pytest.mark.parametrize("d,E,I", [(64, 2, 16), (256, 8, 512), (192, 3, 80), (128, 5, 1408)])
+def test_pack_unpack_roundtrip_bitexact(d, E, I):
+    """Eq. 3: unpack_prefix(pack(W, rank), r) == oracle.pack(W, rank)[:r] bit for bit."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, rng = _small_layer(1, d, E, min(2, E), I)
+    L = gu.pack_layer(lay)
+    Gt, Ut, Dt = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
+    for e in range(E):
+        for r in sorted({I, 0, 16, I // 2 // 16 * 16 + 16 if I > 32 else 16}):
+            r = min(r, I)
+            Wg, Wu, Wd = L.unpack_prefix(e, r)
+            torch.cuda.synchronize()
+            assert np.array_equal(fx.bf16_to_bits(Wg), Gt[e, :r]) if r else True
+            assert np.array_equal(fx.bf16_to_bits(Wu), Ut[e, :r]) if r else True
+            assert np.array_equal(fx.bf16_to_bits(Wd), Dt[e, :, :r]) if r else True
+
+
+def test_pack_rejects_non_permutation():
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, rng = _small_layer(2, 64, 2, 1, 32)
+    lay.channel_rank[1, 3] = lay.channel_rank[1, 4]
+    with pytest.raises(fx.FxmError) as ei:
+        gu.pack_layer(lay)
+    assert ei.value.name == "FXM_EPERM"
+
+
+# ----------------------------------------------------------------------------------------------- route
+@pytest.mark.parametrize("T,k,E,seed", [(0, 2, 8, 0), (1, 1, 4, 1), (1, 4, 60, 2), (64, 2, 8, 0), (16, 4, 60, 3),
+                                        (37, 3, 7, 4), (1000, 6, 64, 5), (4096, 4, 60, 6), (8192, 8, 64, 7),
+                                        (8192, 6, 64, 8), (333, 16, 256, 9)])
+def test_route_bitexact(T, k, E, seed):
+    """Alg. 2 l.4-6, reading R5: stable grouping; all four index arrays bit-exact."""
+    import torch
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(seed, 64, E, k, 32)
+    L = gu.pack_layer(lay, identity=True)
+    bias = 1.5 if seed == 8 else 0.0                      # C3-style skew: some experts empty, some huge
+    ids, _ = gen.route(gen.make_logits(T, E, rng, 1.0, bias), k)
+    c, o, p, ip = [t.cpu().numpy() for t in L.route(torch.from_numpy(ids).cuda().reshape(T, k))]
+    rc, ro, rp, rip = oracle.route(ids.reshape(T, k), E)
+    assert np.array_equal(c, rc) and np.array_equal(o, ro)
+    assert np.array_equal(p, rp) and np.array_equal(ip, rip)
+    assert L.device_flags() == 0
+
+
+def test_route_duplicate_and_single_expert():
+    """Degenerate routings: every assignment to one expert; duplicate ids inside a token (reading R13)."""
+    import torch
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(0, 64, 8, 2, 32)
+    L = gu.pack_layer(lay, identity=True)
+    for ids in (np.full((300, 2), 5, np.int32), np.repeat(rng.integers(0, 8, (129, 1)), 2, 1).astype(np.int32)):
+        got = [t.cpu().numpy() for t in L.route(torch.from_numpy(ids).cuda())]
+        ref = oracle.route(ids, 8)
+        for g, r in zip(got, ref):
+            assert np.array_equal(g, r)
+
+
+# ------------------------------------------------------------------------------------------ FFN, small
+def _c1():
+    lay, b, rng = gen.config("C1")
+    return gen.SHAPES["C1"], lay, b, rng
+
+
+@pytest.mark.parametrize("impl", [1, 0])
+@pytest.mark.parametrize("table", ["full", "c1", "all128", "ragged", "zeros_some"])
+def test_c1_tiny_all_budgets(impl, table):
+    """C1 (BASELINE.json configs[0]): d=256, E=8, top-2, I=512, T=64, every element vs the oracle."""
+    import gpu_util as gu
+    sh, lay, b, rng = _c1()
+    r = {"full": np.full(sh.E, sh.I), "c1": gen.table_c1(sh, rng), "all128": np.full(sh.E, 128),
+         "ragged": np.array([512, 16, 100 // 16 * 16 + 4 * 0 + 48, 336, 64, 80, 496, 272]),
+         "zeros_some": np.array([0, 512, 0, 256, 64, 0, 128, 384])}[table].astype(np.int32)
+    L = gu.pack_layer(lay)
+    y = gu.run_ffn(L, b, r, impl=impl)
+    gu.check_close(y, gu.oracle_ffn(lay, b, r), f"C1 {table} impl={impl}")
+
+
+@pytest.mark.parametrize("impl", [1, 0])
+def test_widths_not_multiple_of_64_and_padded_dims(impl):
+    """I % 64 != 0 (padded channel block), d % 128 == 64 (padded down rows), r_e any multiple of 1."""
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(3, 192, 6, 3, 80, w_std=0.1)
+    b = gen.make_batch(sh, 50, rng)
+    L = gu.pack_layer(lay)
+    for r in ([80] * 6, [1, 7, 33, 64, 65, 79], [0, 0, 0, 0, 0, 5]):
+        r = np.array(r, np.int32)
+        gu.check_close(gu.run_ffn(L, b, r, impl=impl), gu.oracle_ffn(lay, b, r), f"r={r.tolist()} impl={impl}")
+
+
+@pytest.mark.parametrize("tile_n", [128, 256])
+def test_multi_tile_ragged_segments(tile_n):
+    """Expert segments that span several token tiles plus a ragged tail, heavy skew, empty experts."""
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(4, 128, 6, 2, 192, w_std=0.08)
+    T = 900
+    lg = gen.make_logits(T, sh.E, rng, 1.0, 2.0)
+    lg[:, 4] = -1e9                                        # expert 4 never routed
+    ids, w = gen.route(lg, sh.k)
+    b = gen.Batch(gen.make_x(T, sh.d, rng), ids, w)
+    r = np.array([192, 128, 64, 176, 192, 16], np.int32)
+    L = gu.pack_layer(lay)
+    gu.check_close(gu.run_ffn(L, b, r, tile_n=tile_n), gu.oracle_ffn(lay, b, r), f"tile_n={tile_n}")
+
+
+def test_h_intermediate_matches_definition():
+    """Step a4 alone: H = silu(G) (.) U in sorted order, channels >= r_e exactly 0 (pad-zero rule)."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    r = gen.table_c1(sh, rng)
+    L = gu.pack_layer(lay)
+    gu.run_ffn(L, b, r)
+    ids = torch.from_numpy(b.topk_ids).cuda()
+    H = gen.bf16_bits_to_f32(fx.bf16_to_bits(L.debug_read_h(ids))).astype(np.float64)
+    Gt, Ut, _ = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
+    x = gen.bf16_bits_to_f32(b.x).astype(np.float64)
+    _, _, perm, _ = oracle.route(b.topk_ids, sh.E)
+    for s in range(0, perm.size, 7):
+        f = perm[s]
+        t, e = f // sh.k, b.topk_ids.ravel()[f]
+        g = gen.bf16_bits_to_f32(Gt[e]).astype(np.float64) @ x[t]
+        u = gen.bf16_bits_to_f32(Ut[e]).astype(np.float64) @ x[t]
+        h = g / (1 + np.exp(-g)) * u
+        h[r[e]:] = 0
+        assert np.all(H[s, r[e]:] == 0)
+        assert np.abs(H[s] - h).max() <= 2.0 ** -7 * max(np.abs(h).max(), 1e-6)
+
+
+def test_budget_switch_select_and_nested_check():
+    """a1: registered tables + host-only select; nestedness check (reading R14)."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    tabs = np.array([[512] * 8, [512, 384, 512, 256, 512, 128, 512, 64], [256, 128, 192, 64, 512, 64, 128, 0]], np.int32)
+    L = gu.pack_layer(lay)
+    with pytest.raises(fx.FxmError) as ei:
+        L.register_budgets(tabs[::-1].copy(), require_nested=True)
+    assert ei.value.name == "FXM_ENOTNESTED"
+    L.register_budgets(tabs, require_nested=True)
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    before = L.packed.clone()
+    for bi in (2, 0, 1, 2, 1):
+        L.select_budget(bi)
+        y = gen.bf16_bits_to_f32(fx.bf16_to_bits(L.moe_ffn(x, ids, w))).astype(np.float64)
+        gu.check_close(y, gu.oracle_ffn(lay, b, tabs[bi]), f"budget {bi}")
+    E, d, I = sh.E, sh.d, sh.I
+    nw = 3 * E * ((I + 63) // 64 * 64) * d * 2
+    assert torch.equal(before[:nw], L.packed[:nw]), "a budget switch must not touch the weights"
+    with pytest.raises(fx.FxmError):
+        L.select_budget(3)
+
+
+def test_errors_and_state():
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    L = gu.pack_layer(lay)
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    with pytest.raises(fx.FxmError) as ei:
+        L.moe_ffn(x, ids, w)
+    assert ei.value.name == "FXM_ESTATE"
+    with pytest.raises(fx.FxmError) as ei:
+        L.set_budget(np.full(sh.E, sh.I + 1, np.int32))
+    assert ei.value.name == "FXM_EBUDGET"
+    L.set_budget(np.full(sh.E, sh.I, np.int32))
+    small_ws = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    off = (-small_ws.data_ptr()) % 1024
+    with pytest.raises(fx.FxmError) as ei:
+        L.moe_ffn(x, ids, w, workspace=small_ws[off:off + 2048])
+    assert ei.value.name == "FXM_EWORKSPACE"
+    bad = ids.clone()
+    bad[3, 1] = 99
+    L.moe_ffn(x, bad, w)
+    torch.cuda.synchronize()
+    assert L.device_flags() & 1
+    # T = 0 is a no-op
+    L.moe_ffn(x[:0], ids[:0], w[:0])
+
+
+# ------------------------------------------------------------------------------- FFN, paper-shaped sizes
+def _rows_sample(T, n, seed):
+    return np.sort(np.random.default_rng(seed).choice(T, size=min(n, T), replace=False)).astype(np.int32)
+
+
+@pytest.mark.parametrize("T", [1, 16, 4096])
+@pytest.mark.parametrize("r", [704, 1408])
+def test_c2_qwen15_shaped(T, r):
+    """C2 (BASELINE.json configs[1], the bench workload): d=2048, E=60, top-4, I=1408, uniform r_e.
+    T<=16: every row; T=4096: grouping indices in full + 96 sampled rows (rows of y are independent)."""
+    import torch
+    import gpu_util as gu
+    lay, b, rng = gen.config("C2", T=T)
+    sh = gen.SHAPES["C2"]
+    rt = gen.table_uniform(sh, r)
+    L = gu.pack_layer(lay)
+    y = gu.run_ffn(L, b, rt)
+    rows = None if T <= 16 else _rows_sample(T, 96, 11)
+    ref = gu.oracle_ffn(lay, b, rt, rows=rows)
+    gu.check_close(y if rows is None else y[rows], ref, f"C2 T={T} r={r}")
+    got = [t.cpu().numpy() for t in L.route(torch.from_numpy(b.topk_ids).cuda())]
+    for g, rr in zip(got, oracle.route(b.topk_ids, sh.E)):
+        assert np.array_equal(g, rr)
+
+
+def test_c3_deepseek_shaped_skewed_heterogeneous():
+    """C3: d=2048, E=64, top-6, I=1408, T=8192, skewed load (mu_e + eps reading), per-expert r_e with mean 60 %."""
+    import gpu_util as gu
+    lay, b, rng = gen.config("C3")
+    sh = gen.SHAPES["C3"]
+    r = gen.table_mean_ratio(sh, rng, 0.6)
+    L = gu.pack_layer(lay)
+    y = gu.run_ffn(L, b, r)
+    rows = _rows_sample(8192, 64, 12)
+    gu.check_close(y[rows], gu.oracle_ffn(lay, b, r, rows=rows), "C3")
+
+
+@pytest.mark.parametrize("T", [1, 64, 8192])
+def test_c4_qwen2_57b_shaped_budget_sweep(T):
+    """C4: d=3584, E=64, top-8, I=2560; nested heterogeneous tables at 0/25/40/50/75 % pruned."""
+    import gpu_util as gu
+    lay, b, rng = gen.config("C4", T=T)
+    sh = gen.SHAPES["C4"]
+    tabs = gen.tables_nested_descent(sh, rng)
+    L = gu.pack_layer(lay)
+    rows = None if T == 1 else _rows_sample(T, 24, 13)
+    for bi in (0, 2, 4):
+        y = gu.run_ffn(L, b, tabs[bi])
+        ref = gu.oracle_ffn(lay, b, tabs[bi], rows=rows)
+        gu.check_close(y if rows is None else y[rows], ref, f"C4 T={T} budget {bi}")
