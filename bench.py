@@ -1,0 +1,568 @@
+#!/usr/bin/env python
+"""bench.py -- routed-expert FFN tokens/s and % of roofline on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]              our arm (C-ABI library, CUDA kernels)
+    python bench.py --impl reference [--steps K] [--warmup W]        the CPU oracle, timed on the host cores
+    python bench.py --sweep [--sweep-configs C2,C3,C4,C5]            every config x T x budget -> gpurun_out/sweep.json
+
+A "step" is one fxm_moe_ffn call (route -> gather -> grouped GEMM-1+SwiGLU -> grouped GEMM-2+combine ->
+finalize) over one batch of synthetic tokens.  Default workload = BASELINE.json
+configs[1]: the Qwen1.5-MoE-A2.7B-shaped layer (d=2048, E=60, top-4, I=1408), T=4096, uniform r_e=704 (50 %
+pruned).  N>1 = independent replicas of the layer, tokens sharded across ranks (weak scaling, no data-path
+collective).  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "routed_expert_ffn_tokens_per_s"
+UNIT = "tokens/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "bf16_tflops": float(d["bf16_tflops"]),
+                "bf16_tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                "source": "measured (MEASURED_PEAKS.json)"}
+    except Exception:
+        return dict(FALLBACK_PEAKS, source="fallback (B200_PROFILING.md)")
+
+
+# ------------------------------------------------------------------------------------------ work model
+def work_model(ids: np.ndarray, r: np.ndarray, d: int, T: int, k: int):
+    """Algorithmic work of one call: S = sum_e n_e r_e,
+    R_act = sum over experts with n_e>0 of r_e.  FLOPs = 6 d S (gate 2 + up 2 + down 2 per token-channel-d);
+    bytes = each retained weight of an active expert once (6 d R_act) + x + y (4 T d) + ids/weights (8 A)."""
+    n = np.bincount(ids.ravel(), minlength=r.size).astype(np.int64)
+    S = int((n * r.astype(np.int64)).sum())
+    R_act = int(r.astype(np.int64)[n > 0].sum())
+    A = T * k
+    return {
+        "S": S, "R_act": R_act,
+        "flops": 6.0 * d * S, "bytes": 6.0 * d * R_act + 4.0 * T * d + 8.0 * A,
+        "gemm1_flops": 4.0 * d * S, "gemm1_bytes": 4.0 * d * R_act + 2.0 * A * d + 2.0 * S,
+        "gemm2_flops": 2.0 * d * S, "gemm2_bytes": 2.0 * d * R_act + 2.0 * S + 4.0 * T * d,
+    }
+
+
+def roof_time_s(flops, nbytes, peaks, tf_key="bf16_tflops"):
+    t_tc = flops / (peaks[tf_key] * 1e12)
+    t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
+    return (t_tc, "tensor") if t_tc >= t_hbm else (t_hbm, "hbm")
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Polls NVML (SM clock, power, clock-event reasons) from a thread while a timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int):
+        self.samples = []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        self._h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._h = None
+
+    def _poll(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                mhz = int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                try:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                except Exception:
+                    rs = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                pw = nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0
+                self.samples.append((time.perf_counter(), mhz, rs, pw))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def start(self):
+        if self._h is not None:
+            self._thr = threading.Thread(target=self._poll, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self, windows):
+        """windows: list of (t0, t1) perf_counter intervals during which the GPU was under load."""
+        if self._h is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"], "samples": 0}
+        sel = [s for s in self.samples if any(a <= s[0] <= b for a, b in windows)]
+        if not sel:          # region shorter than one poll: take the samples closest to it
+            mid = sum(a + b for a, b in windows) / (2 * len(windows))
+            sel = sorted(self.samples, key=lambda s: abs(s[0] - mid))[:3]
+        bits = 0
+        for s in sel:
+            bits |= s[2]
+        reasons = [n for b, n in self.REASONS.items() if bits & b]
+        return {"sm_mhz": float(np.median([s[1] for s in sel])) if sel else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(sel),
+                "power_w_max": round(max(s[3] for s in sel), 1) if sel else None}
+
+
+# ------------------------------------------------------------------------------------------ workload
+DEFAULTS = {"config": "C2", "T": 4096, "r": 704}
+
+
+def make_table(gen, sh, spec, rng):
+    """spec: an int width (uniform), 'full', 'hetero:<b>' (C4 nested-descent table b), 'mean60' (C3) or 'c1'."""
+    if isinstance(spec, int) or str(spec).isdigit():
+        return gen.table_uniform(sh, int(spec))
+    if spec == "full":
+        return gen.table_uniform(sh, sh.I)
+    if spec == "c1":
+        return gen.table_c1(sh, rng)
+    if spec == "mean60":
+        return gen.table_mean_ratio(sh, rng, 0.6)
+    if str(spec).startswith("hetero:"):
+        return gen.tables_nested_descent(sh, rng)[int(spec.split(":")[1])]
+    raise SystemExit(f"unknown table spec {spec!r}")
+
+
+def host_batches(gen, cfg, T, n, seed0):
+    """n seeded batches (x, ids, w) of a named config; batch i uses seed seed0+i."""
+    out = []
+    for i in range(n):
+        _, b, rng = gen.config(cfg, T=T, seed=seed0 + i, layer=False)
+        out.append((b, rng))
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_27866_b200 import flexmoe as fx
+    from paper_2606_27866_b200 import inputs as gen
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    fx.lib()                                        # fails loudly if libflexmoe.so is missing and cannot be built
+
+    cfg, T = args.config.upper(), args.T
+    sh = gen.SHAPES[cfg]
+    peaks = load_peaks()
+    NB = args.batches
+    lay = gen.layer_for(cfg, 0)                      # same weights on every rank (replicas)
+    hb = host_batches(gen, cfg, T, NB, 1000 * rank)  # each rank its own tokens
+    r = make_table(gen, sh, args.r, hb[0][1])
+    L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate), fx.bf16_from_bits(lay.W_up), fx.bf16_from_bits(lay.W_down),
+                      lay.channel_rank)
+    L.set_budget(r)
+    torch.cuda.synchronize()
+    dev = [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
+           for b, _ in hb]
+    y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up (untimed)
+    for i in range(args.warmup):
+        L.moe_ffn(*dev[i % NB], out=y)
+    barrier()
+    flags = L.device_flags()
+    assert flags == 0, f"device flags {flags:#x}"
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    # ---- timed region 1: K steps, inputs resident in HBM, per-kernel events recorded inside it
+    barrier()
+    L.profile_begin(args.steps)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    w0 = time.perf_counter()
+    e0.record(stream)
+    for i in range(args.steps):
+        L.moe_ffn(*dev[i % NB], out=y)
+    e1.record(stream)
+    barrier()
+    w1 = time.perf_counter()
+    ms_total = e0.elapsed_time(e1)
+    kern_ms, n_prof = L.profile_end()
+
+    # ---- timed region 2: end to end through fxm_moe_ffn_host (pinned host buffers, H2D + D2H inside)
+    hx = [(fx.bf16_from_bits(b.x, "cpu").pin_memory(), torch.from_numpy(b.topk_ids).pin_memory(),
+           torch.from_numpy(b.topk_w).pin_memory()) for b, _ in hb]
+    hy = torch.empty((T, sh.d), dtype=torch.bfloat16).pin_memory()
+    for i in range(max(3, min(args.warmup, 5))):
+        L.moe_ffn_host(*hx[i % NB], hy)
+    barrier()
+    w2 = time.perf_counter()
+    e0.record(stream)
+    for i in range(args.steps):
+        L.moe_ffn_host(*hx[i % NB], hy)
+    e1.record(stream)
+    barrier()
+    w3 = time.perf_counter()
+    ms_e2e = e0.elapsed_time(e1)
+    sampler.stop()
+    clocks = sampler.summary([(w0, w1), (w2, w3)])
+
+    if world > 1:
+        t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_e2e = float(t[0]), float(t[1])
+
+    tokens = world * T * args.steps
+    value = tokens / (ms_total * 1e-3)
+    e2e_value = tokens / (ms_e2e * 1e-3)
+    wm = [work_model(b.topk_ids, r, sh.d, T, sh.k) for b, _ in hb]
+    sel = [wm[i % NB] for i in range(args.steps)]
+    mean = lambda key: float(np.mean([w[key] for w in sel]))
+
+    # ---- roofline of the dominant kernel (largest share of the step) and of the whole step
+    per_launch_ms = {kname: v / max(n_prof, 1) for kname, v in kern_ms.items()}
+    dom = max(per_launch_ms, key=per_launch_ms.get)
+    kflops = {"gemm1_swiglu": mean("gemm1_flops"), "gemm2_combine": mean("gemm2_flops")}.get(dom, 0.0)
+    kbytes = {"gemm1_swiglu": mean("gemm1_bytes"), "gemm2_combine": mean("gemm2_bytes")}.get(dom, mean("bytes"))
+    t_roof, bound = roof_time_s(kflops, kbytes, peaks)
+    dur = per_launch_ms[dom] * 1e-3
+    if bound == "tensor":
+        achieved, peak, unit = kflops / dur / 1e12, peaks["bf16_tflops"], "TFLOP/s"
+    else:
+        achieved, peak, unit = kbytes / dur / 1e9, peaks["hbm_gbs"], "GB/s"
+    roofline = {"bound": bound, "achieved": round(achieved, 2), "peak": peak, "unit": unit,
+                "frac": round(achieved / peak, 4), "traffic": args.traffic, "kernel": dom,
+                "kernel_ms": round(per_launch_ms[dom], 5), "peak_source": peaks["source"] + ", burst figure",
+                "frac_of_sustained": round(achieved / peaks["bf16_tflops_sustained"], 4) if bound == "tensor" else None,
+                "algorithmic": {"flops": kflops, "bytes": kbytes}}
+    step_roof, step_bound = roof_time_s(mean("flops"), mean("bytes"), peaks)
+    step_s = ms_total * 1e-3 / args.steps
+    roofline_step = {"bound": step_bound, "t_roof_us": round(step_roof * 1e6, 2), "t_step_us": round(step_s * 1e6, 2),
+                     "frac": round(step_roof / step_s, 4), "tflops": round(mean("flops") / step_s / 1e12, 2),
+                     "gbs": round(mean("bytes") / step_s / 1e9, 1),
+                     "kernel_ms_per_step": {kname: round(v, 5) for kname, v in per_launch_ms.items()}}
+
+    out = {
+        "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": round(ms_total / args.steps, 5), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": f"{cfg} {sh.name}: d={sh.d} E={sh.E} top-{sh.k} I={sh.I} T={T} per GPU, r={args.r} "
+                               f"(rho={1 - float(r.mean()) / sh.I:.3f})",
+                   "l2": f"inputs larger than L2: {6 * sh.d * int(r.sum()) / 1e6:.0f} MB of retained weights streamed "
+                         f"per step, {NB} rotating token batches",
+                   "parallelism": f"replicas x{world}, tokens sharded, no data-path collective"},
+        "e2e": {"value": round(e2e_value, 1), "unit": UNIT,
+                "h2d_bytes_per_step": int(T * sh.d * 2 + 2 * T * sh.k * 4), "d2h_bytes_per_step": int(T * sh.d * 2),
+                "ms_per_step": round(ms_e2e / args.steps, 5), "api": "fxm_moe_ffn_host (pinned host buffers)"},
+        "gpu_launches": int(L.launches_per_ffn() * args.steps),
+        "clocks": clocks, "roofline": roofline, "roofline_step": roofline_step,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"], out["parity_sample"] = cpu_baseline(gen, fx, lay, hb[0][0], r, L, dev[0], y, args.cpu_seconds)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle legs
+def _oracle_sample_rows(T, n, seed=7):
+    return np.sort(np.random.default_rng(seed).choice(T, size=min(n, T), replace=False)).astype(np.int32)
+
+
+def _time_oracle(oracle, b, packed, r, rows):
+    t0 = time.perf_counter()
+    ref = oracle.moe_ffn(b.x, *packed, r, b.topk_ids, b.topk_w, rows=rows)
+    return time.perf_counter() - t0, ref
+
+
+def cpu_baseline(gen, fx, lay, b, r, L, dev0, y, seconds):
+    """The oracle as it stands (oracle/oracle.c, fp64, OpenMP over tokens) timed on this box's host cores on a
+    bounded token sample of the SAME workload; the same rows of the GPU output are compared with it."""
+    import torch
+    import oracle
+    cores = oracle.threads()
+    T = b.x.shape[0]
+    packed = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
+    n0 = min(T, cores)
+    t_cal, _ = _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n0))
+    n = int(min(T, max(n0, (seconds / max(t_cal, 1e-6)) * n0)))
+    n = max(cores, n // cores * cores) if T >= cores else T
+    rows = _oracle_sample_rows(T, n)
+    dt, ref = _time_oracle(oracle, b, packed, r, rows)
+    L.moe_ffn(*dev0, out=y)
+    torch.cuda.synchronize()
+    yv = gen.bf16_bits_to_f32(fx.bf16_to_bits(y[torch.from_numpy(rows.astype(np.int64)).cuda()])).astype(np.float64)
+    scale = float(np.abs(ref).max())
+    parity = {"rows": int(rows.size), "max_err_over_max_ref": float(np.abs(yv - ref).max() / scale),
+              "rel_l2": float(np.linalg.norm(yv - ref) / np.linalg.norm(ref)), "tol": {"max": 1e-2, "l2": 5e-3}}
+    return ({"value": round(rows.size / dt, 2), "unit": UNIT, "cores": cores, "kind": "oracle",
+             "sample": f"{rows.size} of {T} tokens (seeded random rows, full k and r_e), {dt:.1f} s wall, fp64, "
+                       f"OpenMP over tokens"}, parity)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the same config/metric; each step = a bounded token sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2606_27866_b200 import inputs as gen
+    cfg, T = args.config.upper(), args.T
+    sh = gen.SHAPES[cfg]
+    lay, b, rng = gen.config(cfg, T=T, seed=0)
+    r = make_table(gen, sh, args.r, rng)
+    cores = oracle.threads()
+    packed = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
+    n0 = min(T, cores)
+    t_cal, _ = _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n0))
+    budget_s = args.cpu_seconds * 6.0                      # whole run (warm-up + steps) ~ 1.5 min by default
+    per_step = budget_s / (args.steps + args.warmup)
+    n = int(min(T, max(n0, per_step / max(t_cal, 1e-6) * n0)))
+    n = max(cores, n // cores * cores) if T >= cores else T
+    for i in range(args.warmup):
+        _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n, seed=100 + i))
+    total = 0.0
+    for i in range(args.steps):
+        dt, _ = _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n, seed=200 + i))
+        total += dt
+    value = n * args.steps / total
+    sample = f"{n} of {T} tokens per step (seeded random rows), fp64, OpenMP over tokens"
+    out = {"impl": "reference", "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(total / args.steps * 1e3, 3),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"{cfg} {sh.name}: d={sh.d} E={sh.E} top-{sh.k} I={sh.I} T={T}, r={args.r} "
+                                  f"(rho={1 - float(r.mean()) / sh.I:.3f})", "l2": "n/a (CPU)",
+                      "parallelism": "host cores, rank 0 only"},
+           "cpu_baseline": {"value": round(value, 2), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": round(value, 2), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ sweep (not the bench line)
+def _time_calls(torch, L, dev, y, iters, warm, flush_buf):
+    """Per-call device time (CUDA events around every call on the current stream).  With flush_buf, a buffer
+    larger than L2 is rewritten before every call so weights never come from L2 (decode points)."""
+    st = torch.cuda.current_stream()
+    for i in range(warm):
+        L.moe_ffn(*dev[i % len(dev)], out=y)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    L.profile_begin(iters)
+    for i in range(iters):
+        if flush_buf is not None:
+            flush_buf.add_(1)
+        ev[i][0].record(st)
+        L.moe_ffn(*dev[i % len(dev)], out=y)
+        ev[i][1].record(st)
+    torch.cuda.synchronize()
+    kern, n = L.profile_end()
+    ms = np.array([a.elapsed_time(b) for a, b in ev])
+    return ms, {kname: v / n for kname, v in kern.items()}
+
+
+SWEEP = {
+    "C2": {"T": [1, 16, 4096], "tables": [("r=704 (50%)", 704), ("r=1408 (0%)", "full")]},
+    "C3": {"T": [8192], "tables": [("mean 40% pruned, heterogeneous", "mean60"), ("0%", "full")]},
+    "C4": {"T": [1, 64, 8192], "tables": [("0%", 2560), ("25%", 1920), ("40%", 1536), ("50%", 1280), ("75%", 640),
+                                          ("H 0%", "hetero:0"), ("H 25%", "hetero:1"), ("H 40%", "hetero:2"),
+                                          ("H 50%", "hetero:3"), ("H 75%", "hetero:4")]},
+}
+
+
+def run_sweep(args):
+    import torch
+    from paper_2606_27866_b200 import flexmoe as fx
+    from paper_2606_27866_b200 import inputs as gen
+    torch.cuda.set_device(0)
+    peaks = load_peaks()
+    flush_buf = torch.zeros(512 << 20, dtype=torch.uint8, device="cuda")
+    rows = []
+    for cfg in [c.strip().upper() for c in args.sweep_configs.split(",") if c.strip()]:
+        if cfg not in SWEEP:
+            continue
+        sh = gen.SHAPES[cfg]
+        lay = gen.layer_for(cfg, 0)
+        L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate), fx.bf16_from_bits(lay.W_up), fx.bf16_from_bits(lay.W_down),
+                          lay.channel_rank)
+        torch.cuda.synchronize()
+        for T in SWEEP[cfg]["T"]:
+            NB = 8
+            hb = host_batches(gen, cfg, T, NB, 0)
+            dev = [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
+                   for b, _ in hb]
+            y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
+            for label, spec in SWEEP[cfg]["tables"]:
+                r = make_table(gen, sh, spec, np.random.default_rng([0, 3]))
+                L.set_budget(r)
+                iters = 200 if T <= 64 else (60 if cfg != "C4" else 24)
+                ms, kern = _time_calls(torch, L, dev, y, iters, 5, flush_buf if T <= 64 else None)
+                wm = [work_model(b.topk_ids, r, sh.d, T, sh.k) for b, _ in hb]
+                fl = float(np.mean([w["flops"] for w in wm]))
+                by = float(np.mean([w["bytes"] for w in wm]))
+                t_roof, bound = roof_time_s(fl, by, peaks)
+                med = float(np.median(ms)) * 1e-3
+                rows.append({"config": cfg, "T": T, "budget": label, "rho": round(1 - float(r.mean()) / sh.I, 4),
+                             "ms_median": round(med * 1e3, 5), "ms_p10": round(float(np.percentile(ms, 10)), 5),
+                             "ms_p90": round(float(np.percentile(ms, 90)), 5), "tokens_per_s": round(T / med, 1),
+                             "tflops": round(fl / med / 1e12, 2), "gbs": round(by / med / 1e9, 1), "bound": bound,
+                             "t_roof_us": round(t_roof * 1e6, 2), "roofline_frac": round(t_roof / med, 4),
+                             "l2": "flushed before every call" if T <= 64 else "weights > L2",
+                             "kernel_ms": {kname: round(v, 5) for kname, v in kern.items()}})
+                print(json.dumps(rows[-1]), flush=True)
+            assert L.device_flags() == 0
+        del L
+        torch.cuda.empty_cache()
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "sweep.json"), "w") as f:
+        json.dump({"peaks": peaks, "rows": rows}, f, indent=1)
+
+
+# ------------------------------------------------------------------------------------------ C5: online budget switching
+def run_switch(args):
+    """BASELINE.json configs[4]: C4-shaped layer, `--switch-steps` interleaved decode (T=32) / prefill (T=4096)
+    steps, a different registered nested table every step (fxm_select_budget: host-only)."""
+    import torch
+    from paper_2606_27866_b200 import flexmoe as fx
+    from paper_2606_27866_b200 import inputs as gen
+    torch.cuda.set_device(0)
+    sh = gen.SHAPES["C5"]
+    lay = gen.layer_for("C5", 0)
+    L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate), fx.bf16_from_bits(lay.W_up), fx.bf16_from_bits(lay.W_down),
+                      lay.channel_rank)
+    tabs = gen.tables_nested_descent(sh, np.random.default_rng([0, 3]))
+    L.register_budgets(tabs, require_nested=True)
+    pools = {}
+    for T in (32, 4096):
+        hb = host_batches(gen, "C5", T, 16, 0)
+        pools[T] = [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
+                    for b, _ in hb]
+    ys = {T: torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda") for T in pools}
+    L.workspace(4096, sh.k)
+    rng = np.random.default_rng(5)
+    seq, prev = [], -1
+    for _ in range(args.switch_steps):
+        b = int(rng.integers(len(tabs)))
+        while b == prev:
+            b = int(rng.integers(len(tabs)))
+        seq.append(b)
+        prev = b
+    st = torch.cuda.current_stream()
+
+    def loop(switching):
+        host_sel = 0.0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(st)
+        for i, b in enumerate(seq):
+            T = 32 if i % 2 == 0 else 4096
+            if switching:
+                t0 = time.perf_counter()
+                L.select_budget(b)
+                host_sel += time.perf_counter() - t0
+            L.moe_ffn(*pools[T][(i // 2) % 16], out=ys[T])
+        e1.record(st)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3, host_sel
+
+    L.select_budget(2)
+    loop(False)                                            # warm-up
+    frozen = {}
+    for b in range(len(tabs)):                             # the frozen-budget loops the switching loop is compared with
+        L.select_budget(b)
+        frozen[b] = loop(False)[0]
+    t_sw, host_sel = loop(True)
+    expect = float(np.mean([frozen[b] for b in seq]))      # mean of frozen-loop times weighted by how often b is used
+    # fxm_set_budget (one tiny launch carrying the table in its arguments): stream time per switch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0.record(st)
+    for b in seq:
+        L.set_budget(tabs[b])
+    e1.record(st)
+    t_host_set = (time.perf_counter() - t0) / len(seq)
+    torch.cuda.synchronize()
+    t_dev_set = e0.elapsed_time(e1) * 1e-3 / len(seq)
+    tokens = sum(32 if i % 2 == 0 else 4096 for i in range(len(seq)))
+    out = {"workload": f"C5: C4-shaped layer, {len(seq)} interleaved T=32 / T=4096 steps, 5 nested tables "
+                       f"(rho={[round(1 - float(t.mean()) / sh.I, 3) for t in tabs]}), table switched every step",
+           "sustained_tokens_per_s_switching": round(tokens / t_sw, 1),
+           "loop_s_switching": round(t_sw, 5), "loop_s_expected_from_frozen_loops": round(expect, 5),
+           "switch_cost_us_per_step_device": round((t_sw - expect) / len(seq) * 1e6, 3),
+           "select_budget_host_us": round(host_sel / len(seq) * 1e6, 3),
+           "set_budget_host_us": round(t_host_set * 1e6, 3), "set_budget_stream_us": round(t_dev_set * 1e6, 3),
+           "frozen_loop_s": {str(b): round(v, 5) for b, v in frozen.items()},
+           "weights_touched_by_switch_bytes": 0, "table_bytes": int(sh.E * 4)}
+    assert L.device_flags() == 0
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "switch.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default=DEFAULTS["config"])
+    ap.add_argument("--T", type=int, default=DEFAULTS["T"])
+    ap.add_argument("--r", default=str(DEFAULTS["r"]), help="uniform width, 'full', 'hetero:<b>', 'mean60', 'c1'")
+    ap.add_argument("--batches", type=int, default=8, help="rotating pre-generated token batches")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture (else null)")
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--sweep-configs", default="C2,C3,C4")
+    ap.add_argument("--switch", action="store_true")
+    ap.add_argument("--switch-steps", type=int, default=1000)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    if args.switch:
+        return run_switch(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -111,6 +111,25 @@ int32_t fxm_ratio_to_width(int I, int num, int den);
 fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
                        void* y, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Same forward with HOST buffers (pinned memory recommended so the copies are asynchronous): enqueues on
+ * `stream` the host->device copies of x [T][d] bf16, topk_ids [T][k] int32 and topk_w [T][k] fp32 into a
+ * staging area at the tail of `workspace`, the five kernels of fxm_moe_ffn, and the device->host copy of
+ * y [T][d] bf16.  workspace >= fxm_workspace_bytes_host(E,d,I,T,k).  Does not synchronise: y_host is valid
+ * once `stream` has passed this call.  This is the end-to-end entry point bench.py times as `e2e`. */
+fxm_status fxm_workspace_bytes_host(int E, int d, int I, int T_max, int k, size_t* bytes);
+fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
+                            int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- measurement surface -------------------------------------------------------------------------------
+ * Per-kernel device times of fxm_moe_ffn: between fxm_profile_begin and fxm_profile_end every
+ * fxm_moe_ffn call (at most max_calls of them, <= 4096) records a CUDA event on its stream before each of its
+ * FXM_N_KERNELS launches and after the last.  fxm_profile_end synchronises those events and writes, per kernel
+ * (order: route, gather, GEMM-1+SwiGLU, GEMM-2+combine, finalize), the SUM of its durations in milliseconds over
+ * the *calls recorded; events are host objects, no device memory is allocated. */
+#define FXM_N_KERNELS 5
+fxm_status fxm_profile_begin(fxm_layer* L, int max_calls);
+fxm_status fxm_profile_end(fxm_layer* L, float* ms_sum /* [FXM_N_KERNELS] */, int* calls);
+
 /* ---- parity / debug surface ---------------------------------------------------------------------------
  * Step a2 alone (Alg. 2 l.4-6; stable by (expert id, flat index t*k+j), reading R5):
  * counts [E], offsets [E+1] (exclusive scan, offsets[E] = T*k), perm [T*k], inv_perm [T*k]: device int32. */

@@ -20,7 +20,15 @@ struct fxm_layer {
     int num_sms;
     int tile_n_override;     // 0 = choose from T*k/E
     std::vector<int> host_tables;   // mirror of the resident tables (validation / introspection only)
+    std::vector<cudaEvent_t> prof_events;   // fxm_profile_begin: (FXM_N_KERNELS + 1) events per recorded call
+    int prof_capacity;       // calls that can still be recorded
+    int prof_calls;          // calls recorded so far
 };
+
+static size_t host_stage_bytes(const Dims& D, int T, int k) {
+    // device staging of the host-buffer entry point: x, y (bf16 [T][d]), ids (int32 [T][k]), w (fp32 [T][k])
+    return 2 * align_up((size_t)T * D.d * 2, 1024) + 2 * align_up((size_t)T * k * 4, 1024);
+}
 
 static bool make_dims(int E, int d, int I, Dims* D) {
     if (E < 1 || E > MAX_E || d < 64 || d % 64 != 0 || I < 16 || I % 16 != 0) return false;
@@ -78,6 +86,16 @@ fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* by
     return FXM_OK;
 }
 
+fxm_status fxm_workspace_bytes_host(int E, int d, int I, int T_max, int k, size_t* bytes) {
+    size_t inner = 0;
+    fxm_status s = fxm_workspace_bytes(E, d, I, T_max, k, &inner);
+    if (s != FXM_OK) return s;
+    Dims D;
+    make_dims(E, d, I, &D);
+    *bytes = inner + host_stage_bytes(D, T_max, k);
+    return FXM_OK;
+}
+
 int32_t fxm_ratio_to_width(int I, int num, int den) {
     if (I < 0 || den <= 0 || num < 0 || num > den) return -1;
     return (int32_t)(((int64_t)I * num + den - 1) / den);
@@ -123,11 +141,16 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
     L->D = D; L->packed = pk; L->tables = tables; L->state = state;
     L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
     L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
+    L->prof_capacity = 0; L->prof_calls = 0;
     *out = L;
     return FXM_OK;
 }
 
-void fxm_destroy(fxm_layer* L) { delete L; }
+void fxm_destroy(fxm_layer* L) {
+    if (!L) return;
+    for (cudaEvent_t ev : L->prof_events) cudaEventDestroy(ev);
+    delete L;
+}
 
 static fxm_status check_table(const fxm_layer* L, const int32_t* r) {
     for (int e = 0; e < L->D.E; ++e)
@@ -186,7 +209,39 @@ fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n) {
     return FXM_OK;
 }
 
-int fxm_launches_per_ffn(const fxm_layer* L) { (void)L; return 5; }
+int fxm_launches_per_ffn(const fxm_layer* L) { (void)L; return FXM_N_KERNELS; }
+
+fxm_status fxm_profile_begin(fxm_layer* L, int max_calls) {
+    if (!L || max_calls < 1 || max_calls > 4096) return FXM_EINVAL;
+    for (cudaEvent_t ev : L->prof_events) cudaEventDestroy(ev);
+    L->prof_events.assign((size_t)max_calls * (FXM_N_KERNELS + 1), nullptr);
+    for (cudaEvent_t& ev : L->prof_events)
+        if (cudaEventCreate(&ev) != cudaSuccess) return FXM_ECUDA;
+    L->prof_capacity = max_calls;
+    L->prof_calls = 0;
+    return FXM_OK;
+}
+
+fxm_status fxm_profile_end(fxm_layer* L, float* ms_sum, int* calls) {
+    if (!L || !ms_sum || !calls) return FXM_EINVAL;
+    for (int j = 0; j < FXM_N_KERNELS; ++j) ms_sum[j] = 0.f;
+    fxm_status rc = FXM_OK;
+    for (int c = 0; c < L->prof_calls && rc == FXM_OK; ++c) {
+        cudaEvent_t* ev = &L->prof_events[(size_t)c * (FXM_N_KERNELS + 1)];
+        if (cudaEventSynchronize(ev[FXM_N_KERNELS]) != cudaSuccess) { rc = FXM_ECUDA; break; }
+        for (int j = 0; j < FXM_N_KERNELS; ++j) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, ev[j], ev[j + 1]) != cudaSuccess) { rc = FXM_ECUDA; break; }
+            ms_sum[j] += ms;
+        }
+    }
+    *calls = L->prof_calls;
+    for (cudaEvent_t ev : L->prof_events) cudaEventDestroy(ev);
+    L->prof_events.clear();
+    L->prof_capacity = 0;
+    L->prof_calls = 0;
+    return rc;
+}
 
 static fxm_status check_call(const fxm_layer* L, int T, int k, const void* ws, size_t ws_bytes) {
     if (!L || T < 0 || !ws || ((uintptr_t)ws & 1023u)) return FXM_EINVAL;
@@ -220,21 +275,61 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
     const Workspace ws = map_workspace(D, T, k, workspace);
     const int* table = L->tables + (size_t)L->current * TABLE_STRIDE;
     const int tile_n = choose_tile_n(L, T, k);
+    cudaEvent_t* ev = nullptr;                                    // per-kernel timing, only between profile_begin/end
+    if (L->prof_capacity > 0) {
+        ev = &L->prof_events[(size_t)L->prof_calls * (FXM_N_KERNELS + 1)];
+        ++L->prof_calls;
+        --L->prof_capacity;
+    }
+#define FXM_MARK(j) if (ev && cudaEventRecord(ev[j], st) != cudaSuccess) return FXM_ECUDA;
     // a2 + a3: grouping and the tile schedule for the CURRENT table
+    FXM_MARK(0)
     if (launch_route(D, topk_ids, T, k, table, tile_n, ws.counts, ws.offsets, ws.perm, ws.inv_perm, ws, L->state, st) !=
         cudaSuccess)
         return FXM_ECUDA;
     // gather x rows into sorted swizzled panels; zero the combine accumulator
+    FXM_MARK(1)
     if (launch_prep(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+    FXM_MARK(2)
     if (L->impl == FXM_IMPL_TCGEN05) {
         if (launch_gemm1_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
+        FXM_MARK(3)
         if (launch_gemm2_sm100(D, L->packed, table, topk_w, k, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess)
             return FXM_ECUDA;
     } else {
         if (launch_gemm1_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
+        FXM_MARK(3)
         if (launch_gemm2_simt(D, L->packed, table, topk_w, k, ws, st) != cudaSuccess) return FXM_ECUDA;
     }
+    FXM_MARK(4)
     if (launch_finalize(D, T, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
+    FXM_MARK(5)
+#undef FXM_MARK
+    return FXM_OK;
+}
+
+fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
+                            int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!L || T < 0 || !workspace || ((uintptr_t)workspace & 1023u)) return FXM_EINVAL;
+    if (k < 1 || k > MAX_K || k > L->D.E || (long long)T * k > (1LL << 30)) return FXM_ESHAPE;
+    const size_t inner = map_workspace(L->D, T, k, nullptr).bytes;
+    if (workspace_bytes < inner + host_stage_bytes(L->D, T, k)) return FXM_EWORKSPACE;
+    if (T == 0) return FXM_OK;
+    if (!x_host || !topk_ids_host || !topk_w_host || !y_host) return FXM_EINVAL;
+    if (L->current < 0) return FXM_ESTATE;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t xb = (size_t)T * L->D.d * 2, ab = (size_t)T * k * 4;
+    uint8_t* p = (uint8_t*)workspace + inner;
+    uint8_t* xd = p;  p += align_up(xb, 1024);
+    uint8_t* yd = p;  p += align_up(xb, 1024);
+    uint8_t* idd = p; p += align_up(ab, 1024);
+    uint8_t* wd = p;
+    if (cudaMemcpyAsync(xd, x_host, xb, cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
+    if (cudaMemcpyAsync(idd, topk_ids_host, ab, cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
+    if (cudaMemcpyAsync(wd, topk_w_host, ab, cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
+    fxm_status s = fxm_moe_ffn(L, xd, (const int32_t*)idd, (const float*)wd, T, k, yd, workspace, inner, stream);
+    if (s != FXM_OK) return s;
+    if (cudaMemcpyAsync(y_host, yd, xb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return FXM_ECUDA;
     return FXM_OK;
 }
 

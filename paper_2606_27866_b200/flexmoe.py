@@ -66,6 +66,10 @@ def lib():
     L.fxm_ratio_to_width.argtypes = [i32, i32, i32]
     L.fxm_ratio_to_width.restype = ctypes.c_int32
     L.fxm_moe_ffn.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_workspace_bytes_host.argtypes = [i32, i32, i32, i32, i32, ctypes.POINTER(sz)]
+    L.fxm_moe_ffn_host.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_profile_begin.argtypes = [vp, i32]
+    L.fxm_profile_end.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i32)]
     L.fxm_route.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
     L.fxm_unpack_prefix.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     L.fxm_debug_read_h.argtypes = [vp, vp, i32, i32, vp, vp, vp]
@@ -82,7 +86,8 @@ def lib():
 
 
 EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
-           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_route", "fxm_unpack_prefix",
+           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_workspace_bytes_host", "fxm_moe_ffn_host",
+           "fxm_profile_begin", "fxm_profile_end", "fxm_route", "fxm_unpack_prefix",
            "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_device_flags", "fxm_launches_per_ffn",
            "fxm_status_string", "fxm_destroy"]
 
@@ -102,6 +107,16 @@ def workspace_bytes(E: int, d: int, I: int, T_max: int, k: int) -> int:
     n = ctypes.c_size_t()
     _chk(lib().fxm_workspace_bytes(E, d, I, T_max, k, ctypes.byref(n)), "fxm_workspace_bytes")
     return n.value
+
+
+def workspace_bytes_host(E: int, d: int, I: int, T_max: int, k: int) -> int:
+    n = ctypes.c_size_t()
+    _chk(lib().fxm_workspace_bytes_host(E, d, I, T_max, k, ctypes.byref(n)), "fxm_workspace_bytes_host")
+    return n.value
+
+
+N_KERNELS = 5
+KERNEL_NAMES = ("route", "gather", "gemm1_swiglu", "gemm2_combine", "finalize")
 
 
 def ratio_to_width(I: int, num: int, den: int) -> int:
@@ -208,6 +223,43 @@ class Layer:
         _chk(lib().fxm_moe_ffn(self._h, x.data_ptr(), topk_ids.data_ptr(), topk_w.data_ptr(), T, k, y.data_ptr(),
                                ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_moe_ffn")
         return y
+
+    def workspace_host(self, T: int, k: int):
+        import torch
+        need = workspace_bytes_host(self.E, self.d, self.I, T, k)
+        if getattr(self, "_wsh", None) is None or self._wsh.numel() < need:
+            raw = torch.empty(need + 1024, dtype=torch.uint8, device=self.packed.device)
+            off = (-raw.data_ptr()) % 1024
+            self._wsh = raw[off:off + need]
+        return self._wsh
+
+    def moe_ffn_host(self, x_host, ids_host, w_host, y_host, stream=None):
+        """Host-buffer forward (fxm_moe_ffn_host): x_host/y_host [T,d] bf16, ids_host [T,k] int32, w_host [T,k]
+        fp32 CPU tensors (pinned recommended).  Asynchronous; y_host is valid after the stream is synchronised."""
+        import torch
+        T, d = x_host.shape
+        k = ids_host.shape[1]
+        for t in (x_host, ids_host, w_host, y_host):
+            assert not t.is_cuda and t.is_contiguous()
+        assert d == self.d and x_host.dtype == torch.bfloat16 and y_host.dtype == torch.bfloat16
+        assert tuple(y_host.shape) == (T, d) and ids_host.dtype == torch.int32 and w_host.dtype == torch.float32
+        assert tuple(ids_host.shape) == (T, k) and tuple(w_host.shape) == (T, k)
+        ws = self.workspace_host(T, k)
+        _chk(lib().fxm_moe_ffn_host(self._h, x_host.data_ptr(), ids_host.data_ptr(), w_host.data_ptr(), T, k,
+                                    y_host.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
+             "fxm_moe_ffn_host")
+        return y_host
+
+    # -- measurement surface ----------------------------------------------------------------------------
+    def profile_begin(self, max_calls: int):
+        _chk(lib().fxm_profile_begin(self._h, int(max_calls)), "fxm_profile_begin")
+
+    def profile_end(self):
+        """-> (dict kernel name -> summed ms over the recorded calls, number of calls)."""
+        ms = (ctypes.c_float * N_KERNELS)()
+        n = ctypes.c_int()
+        _chk(lib().fxm_profile_end(self._h, ms, ctypes.byref(n)), "fxm_profile_end")
+        return {KERNEL_NAMES[j]: float(ms[j]) for j in range(N_KERNELS)}, n.value
 
     # -- parity / debug surface -----------------------------------------------------------------------
     def route(self, topk_ids, stream=None):
