@@ -257,8 +257,11 @@ fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_
     if (!counts || !offsets || (T > 0 && (!topk_ids || !perm || !inv_perm))) return FXM_EINVAL;
     const Workspace ws = map_workspace(L->D, T, k, workspace);
     const int* table = L->current >= 0 ? L->tables + (size_t)L->current * TABLE_STRIDE : nullptr;
-    if (launch_route(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), counts, offsets, perm, inv_perm, ws, L->state,
-                     (cudaStream_t)stream) != cudaSuccess)
+    if (launch_route_plan(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), counts, offsets, ws, L->state,
+                          (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    if (launch_scatter_gather(L->D, topk_ids, T, k, table, counts, offsets, perm, inv_perm, nullptr, ws,
+                              (cudaStream_t)stream) != cudaSuccess)
         return FXM_ECUDA;
     return FXM_OK;
 }
@@ -284,25 +287,25 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
 #define FXM_MARK(j) if (ev && cudaEventRecord(ev[j], st) != cudaSuccess) return FXM_ECUDA;
     // a2 + a3: grouping and the tile schedule for the CURRENT table
     FXM_MARK(0)
-    if (launch_route(D, topk_ids, T, k, table, tile_n, ws.counts, ws.offsets, ws.perm, ws.inv_perm, ws, L->state, st) !=
-        cudaSuccess)
+    if (launch_route_plan(D, topk_ids, T, k, table, tile_n, ws.counts, ws.offsets, ws, L->state, st) != cudaSuccess)
         return FXM_ECUDA;
-    // gather x rows into sorted swizzled panels; zero the combine accumulator
+    // stable scatter of the indices + gather of the x rows into sorted swizzled panels
     FXM_MARK(1)
-    if (launch_prep(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+    if (launch_scatter_gather(D, topk_ids, T, k, table, ws.counts, ws.offsets, ws.perm, ws.inv_perm,
+                              (const __nv_bfloat16*)x, ws, st) != cudaSuccess)
+        return FXM_ECUDA;
     FXM_MARK(2)
     if (L->impl == FXM_IMPL_TCGEN05) {
         if (launch_gemm1_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
         FXM_MARK(3)
-        if (launch_gemm2_sm100(D, L->packed, table, topk_w, k, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess)
-            return FXM_ECUDA;
+        if (launch_gemm2_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
     } else {
         if (launch_gemm1_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
         FXM_MARK(3)
-        if (launch_gemm2_simt(D, L->packed, table, topk_w, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+        if (launch_gemm2_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
     }
     FXM_MARK(4)
-    if (launch_finalize(D, T, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
+    if (launch_combine(D, T, k, topk_w, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
     FXM_MARK(5)
 #undef FXM_MARK
     return FXM_OK;

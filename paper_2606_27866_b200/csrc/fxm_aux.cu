@@ -1,7 +1,6 @@
 // fxm_aux.cu -- the bandwidth-only kernels around the two grouped GEMMs:
-//   pack / unpack_prefix (Eq. 3), set_table (Eq. 11), prep (gather x rows into
-//   the sorted, padded, swizzled panels + zero the combine accumulator; Alg. 2 l.4-7),
-//   finalize (one rounding of y to bf16), read_h (debug).
+//   pack / unpack_prefix (Eq. 3), set_table (Eq. 11), combine (router-weighted sum of
+//   each token's k expert outputs, one rounding of y to bf16; Alg. 2 l.19-20), read_h (debug).
 #include "fxm_internal.cuh"
 
 namespace fxm {
@@ -113,58 +112,58 @@ cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStrea
     return cudaGetLastError();
 }
 
-// ----------------------------------------------------------------------------------------------- prep
-// One warp per padded row p: copy x[token(p)] (d bf16) into the swizzled panels Xs[kb][p][.]; padding rows
-// become zeros so no garbage ever reaches a tensor core.  The same grid zeroes the fp32 accumulator.
-__global__ void k_prep(Dims D, const uint4* __restrict__ x, int T, int k, const int* __restrict__ row_flat,
-                       const Sched* __restrict__ sched, uint8_t* __restrict__ Xs, int P, float4* __restrict__ yacc) {
-    const int lane = threadIdx.x & 31;
-    const int warps_per_block = blockDim.x >> 5;
-    const int gw = blockIdx.x * warps_per_block + (threadIdx.x >> 5);
-    const int nw = gridDim.x * warps_per_block;
-    const int P_used = sched->P_used;
-    const int chunks_per_row = D.d >> 3;                       // 16-byte chunks in an x row
-    for (int p = gw; p < P_used; p += nw) {
-        const int f = row_flat[p];
-        const uint4* src = f >= 0 ? x + (size_t)(f / k) * chunks_per_row : nullptr;
-        for (int c = lane; c < chunks_per_row; c += 32) {
-            const uint4 v = src ? src[c] : make_uint4(0, 0, 0, 0);
-            const int kb = c >> 3, ch = c & 7;
-            *(uint4*)(Xs + ((size_t)kb * P + p) * ROW_BYTES + (((ch ^ p) & 7) << 4)) = v;
+// -------------------------------------------------------------------------------------------- combine
+// Alg. 2 l.19-20: Y[token] += alpha * Z_down, done as a GATHER so that no atomics are needed and
+// the sum runs in slot order j = 0..k-1 in fp32 with exactly one rounding of y (readings R8, R11):
+//   y[t][i] = sum_j topk_w[t][j] * O[i/128][prow[t*k+j]][i%128]
+// One block per token; a thread owns 8 consecutive output features (16 bytes of each O row).
+__global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __restrict__ prow,
+                                                 const float* __restrict__ topk_w, const uint8_t* __restrict__ O,
+                                                 int P, uint4* __restrict__ y) {
+    __shared__ int s_p[MAX_K];
+    __shared__ float s_w[MAX_K];
+    const int t = blockIdx.x;
+    if (threadIdx.x < k) {
+        s_p[threadIdx.x] = prow[(size_t)t * k + threadIdx.x];
+        s_w[threadIdx.x] = topk_w[(size_t)t * k + threadIdx.x];
+    }
+    __syncthreads();
+    const int chunks = D.d >> 3;
+    for (int c = threadIdx.x; c < chunks; c += blockDim.x) {
+        const uint8_t* col = O + (size_t)(c >> 4) * P * O_ROW_BYTES + ((c & 15) << 4);
+        float acc[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = 0.f;
+        for (int j0 = 0; j0 < k; j0 += 4) {
+            uint4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int p = j0 + u < k ? s_p[j0 + u] : -1;
+                v[u] = p >= 0 ? __ldg((const uint4*)(col + (size_t)p * O_ROW_BYTES)) : make_uint4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (j0 + u >= k) break;
+                const float wj = s_w[j0 + u];
+                const uint32_t h[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    acc[2 * q] += wj * __uint_as_float(h[q] << 16);
+                    acc[2 * q + 1] += wj * __uint_as_float(h[q] & 0xFFFF0000u);
+                }
+            }
         }
-    }
-    const size_t n4 = (size_t)T * D.d / 4;
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
-        yacc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-}
-
-cudaError_t launch_prep(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st) {
-    const int threads = 256;
-    size_t want = ((size_t)T * k + 7) / 8;
-    const size_t zero_blocks = ((size_t)T * D.d / 4 + threads * 4 - 1) / (threads * 4);
-    if (zero_blocks > want) want = zero_blocks;
-    int blocks = (int)(want < 148 * 8 ? want : 148 * 8);
-    if (blocks < 1) blocks = 1;
-    k_prep<<<blocks, threads, 0, st>>>(D, (const uint4*)x, T, k, ws.row_flat, ws.sched, ws.Xs, ws.P, (float4*)ws.yacc);
-    return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------------------------------- finalize
-__global__ void k_finalize(const float4* __restrict__ yacc, uint2* __restrict__ y, size_t n4) {
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
-        const float4 v = yacc[i];
-        __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
-        uint2 o;
-        o.x = *(uint32_t*)&a;
-        o.y = *(uint32_t*)&b;
-        y[i] = o;
+        uint4 o;
+        __nv_bfloat162 b0 = __floats2bfloat162_rn(acc[0], acc[1]), b1 = __floats2bfloat162_rn(acc[2], acc[3]);
+        __nv_bfloat162 b2 = __floats2bfloat162_rn(acc[4], acc[5]), b3 = __floats2bfloat162_rn(acc[6], acc[7]);
+        o.x = *(uint32_t*)&b0; o.y = *(uint32_t*)&b1; o.z = *(uint32_t*)&b2; o.w = *(uint32_t*)&b3;
+        y[(size_t)t * chunks + c] = o;
     }
 }
-cudaError_t launch_finalize(const Dims& D, int T, const Workspace& ws, __nv_bfloat16* y, cudaStream_t st) {
-    const size_t n4 = (size_t)T * D.d / 4;
-    if (n4 == 0) return cudaSuccess;
-    const int blocks = (int)((n4 + 255) / 256 < 148 * 16 ? (n4 + 255) / 256 : 148 * 16);
-    k_finalize<<<blocks, 256, 0, st>>>((const float4*)ws.yacc, (uint2*)y, n4);
+cudaError_t launch_combine(const Dims& D, int T, int k, const float* topk_w, const Workspace& ws, __nv_bfloat16* y,
+                           cudaStream_t st) {
+    if (T == 0) return cudaSuccess;
+    k_combine<<<T, 128, 0, st>>>(D, k, ws.prow, topk_w, ws.O, ws.P, (uint4*)y);
     return cudaGetLastError();
 }
 

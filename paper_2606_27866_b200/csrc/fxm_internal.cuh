@@ -56,9 +56,10 @@ __host__ __device__ inline size_t dn_tile_index(const Dims& D, int e, int kb2, i
 __host__ __device__ inline size_t gu_bytes(const Dims& D) { return (size_t)D.E * D.nCB * D.nKB1 * WT_BYTES; }
 __host__ __device__ inline size_t dn_bytes(const Dims& D) { return (size_t)D.E * D.nCB * D.nDB * WT_BYTES; }
 
-struct DevState {           // lives at the tail of the packed blob
+struct DevState {           // lives at the tail of the packed blob (zeroed by pack)
     uint32_t flags;         // bit0: expert id out of range; bit1: pipeline wait timed out
-    uint32_t pad[63];
+    uint32_t ticket;        // route: blocks that have published their histogram (reset by the last one)
+    uint32_t pad[62];
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -81,11 +82,15 @@ struct Workspace {
     int* perm;              // [A]
     int* inv_perm;          // [A]
     int* row_flat;          // [P]  flat assignment index f = t*k+j of each padded row, -1 for padding
+    int* prow;              // [A]  padded row of each flat assignment; -1 = dropped or expert of width 0
+    int* bhist;             // [RB][E] per-route-block expert histogram, then exclusive base over blocks
     int4* tt;               // [NT] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}
     int4* items1;           // [NT*nCB] GEMM-1 work items {expert, first padded row, valid rows, channel block}
     uint8_t* Xs;            // [nKB1][P][128 B]  gathered activations, swizzled panels
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
-    float* yacc;            // [T][d]
+    uint8_t* O;             // [nDB][P][256 B]  expert outputs, bf16, 128 output features per panel row
+    int RB;                 // route blocks
+    int chunk;              // flat assignments per route block
     int P;                  // padded-row capacity (multiple of 16)
     int NT;                 // token-tile capacity
     size_t bytes;           // total
@@ -96,11 +101,21 @@ constexpr int TILE_N_MIN = 128;
 
 __host__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+constexpr int O_ROW_BYTES = 256;  // one row of an O panel: 128 output features, bf16
+constexpr int RT_THREADS = 256;   // route kernels: 8 warps per block
+// flat assignments per route block: 128 while that gives <= 512 blocks, then whatever keeps 512 blocks
+__host__ inline int route_chunk(long long A) {
+    if (A <= 128LL * 512) return 128;
+    return (int)(((A + 511) / 512 + 127) / 128 * 128);
+}
+
 __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base) {
     Workspace w{};
     const size_t A = (size_t)T * k;
     const int P = (int)align_up(A + (size_t)(ROW_ALIGN - 1) * D.E, ROW_ALIGN) + ROW_ALIGN;
     const int NT = (int)(A / TILE_N_MIN) + D.E + 1;
+    const int chunk = route_chunk((long long)A);
+    const int RB = (int)((A + chunk - 1) / chunk) > 0 ? (int)((A + chunk - 1) / chunk) : 1;
     size_t o = 0;
     auto take = [&](size_t n) { size_t r = o; o = align_up(o + n, 1024); return r; };
     uint8_t* b = (uint8_t*)base;
@@ -111,11 +126,15 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.perm = (int*)(b + take(sizeof(int) * (A + 1)));
     w.inv_perm = (int*)(b + take(sizeof(int) * (A + 1)));
     w.row_flat = (int*)(b + take(sizeof(int) * (size_t)P));
+    w.prow = (int*)(b + take(sizeof(int) * (A + 1)));
+    w.bhist = (int*)(b + take(sizeof(int) * (size_t)RB * D.E));
     w.tt = (int4*)(b + take(sizeof(int4) * (size_t)NT));
     w.items1 = (int4*)(b + take(sizeof(int4) * (size_t)NT * D.nCB));
     w.Xs = b + take((size_t)D.nKB1 * P * ROW_BYTES);
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
-    w.yacc = (float*)(b + take(sizeof(float) * (size_t)T * D.d));
+    w.O = b + take((size_t)D.nDB * P * O_ROW_BYTES);
+    w.RB = RB;
+    w.chunk = chunk;
     w.P = P;
     w.NT = NT;
     w.bytes = o;
@@ -130,25 +149,30 @@ cudaError_t launch_pack(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloa
 cudaError_t launch_unpack_prefix(const Dims& D, const uint8_t* packed, int e, int r, __nv_bfloat16* Wg,
                                  __nv_bfloat16* Wu, __nv_bfloat16* Wd, cudaStream_t st);
 cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStream_t st);
-cudaError_t launch_route(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n,
-                         int* counts, int* offsets, int* perm, int* inv_perm, const Workspace& ws,
-                         DevState* state, cudaStream_t st);   // also writes ws.poff/row_flat/tt/items1/sched
-cudaError_t launch_prep(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st);
-cudaError_t launch_finalize(const Dims& D, int T, const Workspace& ws, __nv_bfloat16* y, cudaStream_t st);
+// a2/a3 part 1: per-block histograms; the last block to finish scans them and writes counts/offsets/poff/tt/items1/sched
+cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n,
+                              int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st);
+// a2 part 2: stable scatter (perm/inv_perm/row_flat/prow) and, when x != null, the gather of x rows into ws.Xs
+cudaError_t launch_scatter_gather(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
+                                  const int* offsets, int* perm, int* inv_perm, const __nv_bfloat16* x,
+                                  const Workspace& ws, cudaStream_t st);
+// y[t] = sum_j topk_w[t][j] * O[row of (t,j)]   (fp32 sum in slot order, one rounding)
+cudaError_t launch_combine(const Dims& D, int T, int k, const float* topk_w, const Workspace& ws, __nv_bfloat16* y,
+                           cudaStream_t st);
 cudaError_t launch_read_h(const Dims& D, int T, int k, const int* ids, const int* r_table, const Workspace& ws,
                           __nv_bfloat16* H_out, cudaStream_t st);
 
 // SIMT debug path (same layouts, no tensor cores, no async copies)
 cudaError_t launch_gemm1_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
                               cudaStream_t st);
-cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const float* topk_w, int k,
-                              const Workspace& ws, cudaStream_t st);
+cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                              cudaStream_t st);
 
 // tcgen05 / TMEM / bulk-copy path
 cudaError_t launch_gemm1_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
                                DevState* state, int tile_n, int num_sms, cudaStream_t st);
-cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const float* topk_w, int k,
-                               const Workspace& ws, DevState* state, int tile_n, int num_sms, cudaStream_t st);
+cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                               DevState* state, int tile_n, int num_sms, cudaStream_t st);
 cudaError_t init_sm100_kernels();   // cudaFuncSetAttribute for the dynamic shared memory sizes
 
 }  // namespace fxm

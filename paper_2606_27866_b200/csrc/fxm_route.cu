@@ -1,21 +1,26 @@
-// fxm_route.cu -- step a2/a3: router-output grouping (stable per-expert counting sort, bit-exact indices)
-// and the device-side tile schedule that skips pruned work.
+// fxm_route.cu -- step a2/a3: router-output grouping (stable per-expert counting sort, bit-exact indices),
+// the device-side tile schedule that skips pruned work, and the gather of token rows into sorted panels.
 //   Alg. 2 l.4-6: "(pi, eid) <- Sort(eid)", read as the STABLE sort by (expert id, flat
 //   index f = t*k+j) so that exactly one permutation is correct (reading R5).
 //   Alg. 2 l.2-3, 8-11: BucketByRetI / AlignUp / view lists are replaced by a tile list
 //   computed here from counts[] and the CURRENT width table r[]: only tiles with channel index < r_e and
 //   token row < n_e exist.
+//   Alg. 2 l.7: X[pi] -- the gather of routed token rows -- is fused into the scatter pass.
 //
-// One CTA of 32 warps.  Warp w owns the contiguous slice [w*chunk, (w+1)*chunk) of the flat assignment
-// array, so "earlier warp, earlier step, lower lane" is exactly "lower flat index": ranks are assigned with
-// __match_any_sync inside a step, a running per-warp counter across steps, and an exclusive scan over warps
-// -- no atomics, hence a deterministic, stable result.
+// Two launches, no atomics decide any position (hence deterministic and stable):
+//   k_route_plan     grid = RB blocks.  Block b histograms the flat assignments [b*chunk, (b+1)*chunk) per
+//                    expert.  The LAST block to publish (ticket counter) turns the RB x E histogram into
+//                    exclusive bases over blocks and writes counts, offsets, padded offsets, the token tiles
+//                    and the GEMM-1 work items for the current width table.
+//   k_scatter_gather grid = RB blocks.  Block b ranks its assignments: base over blocks + base over the
+//                    warps of the block + __match_any_sync rank inside a 32-wide step ("earlier block, earlier
+//                    warp, earlier step, lower lane" == "lower flat index"), writes perm / inv_perm / row_flat
+//                    / prow, then copies the x rows of ITS assignments into the swizzled K-major panels Xs.
 #include "fxm_internal.cuh"
 
 namespace fxm {
 
-constexpr int RT_WARPS = 32;
-constexpr int RT_BATCH = 8;       // independent id loads in flight per lane
+constexpr int RT_WARPS = RT_THREADS / 32;
 
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 #pragma unroll
@@ -26,57 +31,70 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     return v;
 }
 
-__global__ void __launch_bounds__(RT_WARPS * 32, 1)
-k_route(Dims D, const int* __restrict__ ids, int A, const int* __restrict__ r_table, int tile_n,
-        int* __restrict__ counts, int* __restrict__ offsets, int* __restrict__ perm, int* __restrict__ inv_perm,
-        int* __restrict__ poff, int* __restrict__ row_flat, int4* __restrict__ tt, int4* __restrict__ items1,
-        Sched* __restrict__ sched, DevState* __restrict__ state) {
-    __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, then per-warp running base
+// per-warp histogram of the block's chunk; warp w owns the contiguous sub-range [wlo, whi)
+__device__ __forceinline__ bool block_histogram(const int* __restrict__ ids, int E, int wlo, int whi, int lane,
+                                                int* __restrict__ wh /* this warp's [MAX_E] row */) {
+    bool bad = false;
+    for (int base = wlo; base < whi; base += 32) {
+        const int f = base + lane;
+        int id = f < whi ? ids[f] : -1;
+        if (f < whi && (id < 0 || id >= E)) { bad = true; id = -1; }
+        const unsigned m = __match_any_sync(0xffffffffu, id);
+        if (id >= 0 && lane == __ffs(m) - 1) wh[id] += __popc(m);
+        __syncwarp();
+    }
+    return bad;
+}
+
+__global__ void __launch_bounds__(RT_THREADS)
+k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table, int tile_n,
+             int* __restrict__ counts, int* __restrict__ offsets, int* __restrict__ bhist, int* __restrict__ poff,
+             int4* __restrict__ tt, int4* __restrict__ items1, Sched* __restrict__ sched,
+             DevState* __restrict__ state) {
+    __shared__ int whist[RT_WARPS][MAX_E];
     __shared__ int s_cnt[MAX_E], s_off[MAX_E + 1], s_poff[MAX_E + 1];
-    __shared__ int s_ntt;
+    __shared__ int s_ntt, s_last;
     const int E = D.E;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    for (int i = tid; i < RT_WARPS * MAX_E; i += blockDim.x) (&whist[0][0])[i] = 0;
+    for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
     __syncthreads();
-
-    int chunk = (A + RT_WARPS - 1) / RT_WARPS;
-    chunk = (chunk + 31) & ~31;
-    const int lo = min(A, w * chunk), hi = min(A, lo + chunk);
-    bool bad = false;
-
-    // ---- pass 1: per-warp histogram
-    for (int base = lo; base < hi; base += 32 * RT_BATCH) {
-        int idv[RT_BATCH];
+    const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
+    const int sub = chunk / RT_WARPS;
+    const int wlo = min(hi, lo + w * sub), whi = min(hi, wlo + sub);
+    if (block_histogram(ids, E, wlo, whi, lane, whist[w])) atomicOr(&state->flags, 1u);
+    __syncthreads();
+    for (int e = tid; e < E; e += RT_THREADS) {
+        int c = 0;
 #pragma unroll
-        for (int b = 0; b < RT_BATCH; ++b) {
-            const int f = base + b * 32 + lane;
-            idv[b] = f < hi ? ids[f] : -1;
-        }
-#pragma unroll
-        for (int b = 0; b < RT_BATCH; ++b) {
-            if (base + b * 32 >= hi) break;                 // warp-uniform
-            int id = idv[b];
-            const bool in_range = base + b * 32 + lane < hi;
-            if (in_range && (id < 0 || id >= E)) { bad = true; id = -1; }
-            const unsigned m = __match_any_sync(0xffffffffu, id);
-            if (id >= 0 && lane == __ffs(m) - 1) whist[w][id] += __popc(m);
-            __syncwarp();
-        }
+        for (int ww = 0; ww < RT_WARPS; ++ww) c += whist[ww][e];
+        bhist[(size_t)blockIdx.x * E + e] = c;
     }
-    if (bad) atomicOr(&state->flags, 1u);
+    __threadfence();
     __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(&state->ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
 
-    // ---- exclusive scan over warps (per expert)
-    if (tid < E) {
+    // ---- last block: exclusive scan over blocks (per expert; loads of one b are coalesced over e)
+    const int RB = gridDim.x;
+    for (int e = tid; e < E; e += RT_THREADS) {
         int run = 0;
-#pragma unroll 4
-        for (int ww = 0; ww < RT_WARPS; ++ww) {
-            const int c = whist[ww][tid];
-            whist[ww][tid] = run;
+        int b = 0;
+        for (; b + 8 <= RB; b += 8) {
+            int c[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) c[u] = __ldcg(bhist + (size_t)(b + u) * E + e);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { bhist[(size_t)(b + u) * E + e] = run; run += c[u]; }
+        }
+        for (; b < RB; ++b) {
+            const int c = __ldcg(bhist + (size_t)b * E + e);
+            bhist[(size_t)b * E + e] = run;
             run += c;
         }
-        s_cnt[tid] = run;
-        counts[tid] = run;
+        s_cnt[e] = run;
+        counts[e] = run;
     }
     __syncthreads();
 
@@ -114,55 +132,125 @@ k_route(Dims D, const int* __restrict__ ids, int A, const int* __restrict__ r_ta
             sched->W2 = c_tiles * D.nDB;
             sched->P_used = c_poff;
             sched->A = A;
+            state->ticket = 0;                               // ready for the next call on this layer
         }
     }
     __syncthreads();
-    if (tid <= E) { offsets[tid] = s_off[tid]; poff[tid] = s_poff[tid]; }
-    if (tid < E)                                              // padding rows of each segment
-        for (int p = s_poff[tid] + s_cnt[tid]; p < s_poff[tid + 1]; ++p) row_flat[p] = -1;
+    for (int e = tid; e <= E; e += RT_THREADS) { offsets[e] = s_off[e]; poff[e] = s_poff[e]; }
     // GEMM-1 work items: one per (token tile, RETAINED channel block) -- pruned blocks are never listed
-    for (int j = tid; j < s_ntt; j += blockDim.x) {
+    for (int j = tid; j < s_ntt; j += RT_THREADS) {
         const int4 t = tt[j];
         const int nb = ((r_table ? r_table[t.x] : D.I) + CB - 1) / CB;
         for (int cb = 0; cb < nb; ++cb) items1[t.w + cb] = make_int4(t.x, t.y, t.z, cb);
     }
+}
 
-    // ---- pass 2: stable scatter
-    for (int base = lo; base < hi; base += 32 * RT_BATCH) {
-        int idv[RT_BATCH];
+// copy one x row (d bf16) into the swizzled panels Xs[kb][p][.]; src == nullptr writes zeros
+__device__ __forceinline__ void put_row(const uint4* __restrict__ src, uint8_t* __restrict__ Xs, int P, int p,
+                                        int chunks_per_row, int lane) {
+    for (int c0 = lane; c0 < chunks_per_row; c0 += 128) {
+        uint4 v[4];
 #pragma unroll
-        for (int b = 0; b < RT_BATCH; ++b) {
-            const int f = base + b * 32 + lane;
-            idv[b] = f < hi ? ids[f] : -1;
+        for (int u = 0; u < 4; ++u) {
+            const int c = c0 + 32 * u;
+            v[u] = (src && c < chunks_per_row) ? __ldg(src + c) : make_uint4(0, 0, 0, 0);
         }
 #pragma unroll
-        for (int b = 0; b < RT_BATCH; ++b) {
-            if (base + b * 32 >= hi) break;
-            const int f = base + b * 32 + lane;
-            int id = idv[b];
-            if (id < 0 || id >= E) id = -1;
-            const unsigned m = __match_any_sync(0xffffffffu, id);
-            if (id >= 0) {
-                const int rank = whist[w][id] + __popc(m & ((1u << lane) - 1u));
-                const int pos = s_off[id] + rank;
-                perm[pos] = f;
-                inv_perm[f] = pos;
-                row_flat[s_poff[id] + rank] = f;
-            } else if (f < hi) {
-                inv_perm[f] = -1;                            // dropped (precondition violation)
-            }
-            __syncwarp();
-            if (id >= 0 && lane == __ffs(m) - 1) whist[w][id] += __popc(m);
-            __syncwarp();
+        for (int u = 0; u < 4; ++u) {
+            const int c = c0 + 32 * u;
+            if (c < chunks_per_row)
+                *(uint4*)(Xs + ((size_t)(c >> 3) * P + p) * ROW_BYTES + ((((c & 7) ^ p) & 7) << 4)) = v[u];
         }
     }
 }
 
-cudaError_t launch_route(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int* counts,
-                         int* offsets, int* perm, int* inv_perm, const Workspace& ws, DevState* state,
-                         cudaStream_t st) {
-    k_route<<<1, RT_WARPS * 32, 0, st>>>(D, ids, T * k, r_table, tile_n, counts, offsets, perm, inv_perm, ws.poff,
-                                         ws.row_flat, ws.tt, ws.items1, ws.sched, state);
+__global__ void __launch_bounds__(RT_THREADS)
+k_scatter_gather(Dims D, const int* __restrict__ ids, int A, int chunk, int k, const int* __restrict__ r_table,
+                 const int* __restrict__ counts, const int* __restrict__ offsets, const int* __restrict__ poff,
+                 const int* __restrict__ bbase, int* __restrict__ perm, int* __restrict__ inv_perm,
+                 int* __restrict__ row_flat, int* __restrict__ prow, const uint4* __restrict__ x,
+                 uint8_t* __restrict__ Xs, int P, int RB) {
+    __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, then per-warp running base
+    const int E = D.E;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int chunks_per_row = D.d >> 3;
+    if ((int)blockIdx.x >= RB) {
+        // ---- extra blocks: padding rows of the expert segments get zero activations and no assignment
+        for (int e = blockIdx.x - RB; e < E; e += gridDim.x - RB) {
+            const int p0 = poff[e] + counts[e], p1 = poff[e + 1];
+            for (int p = p0 + w; p < p1; p += RT_WARPS) {
+                if (lane == 0) row_flat[p] = -1;
+                if (x) put_row(nullptr, Xs, P, p, chunks_per_row, lane);
+            }
+        }
+        return;
+    }
+    for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
+    __syncthreads();
+    const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
+    const int sub = chunk / RT_WARPS;
+    const int wlo = min(hi, lo + w * sub), whi = min(hi, wlo + sub);
+    block_histogram(ids, E, wlo, whi, lane, whist[w]);
+    __syncthreads();
+    for (int e = tid; e < E; e += RT_THREADS) {      // exclusive scan over the warps of this block, on top of the block base
+        int run = bbase[(size_t)blockIdx.x * E + e];
+#pragma unroll
+        for (int ww = 0; ww < RT_WARPS; ++ww) {
+            const int c = whist[ww][e];
+            whist[ww][e] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+
+    // ---- stable scatter
+    for (int base = wlo; base < whi; base += 32) {
+        const int f = base + lane;
+        int id = f < whi ? ids[f] : -1;
+        if (id < 0 || id >= E) id = -1;
+        const unsigned m = __match_any_sync(0xffffffffu, id);
+        if (id >= 0) {
+            const int rank = whist[w][id] + __popc(m & ((1u << lane) - 1u));
+            const int pos = offsets[id] + rank;
+            const int pr = poff[id] + rank;
+            perm[pos] = f;
+            inv_perm[f] = pos;
+            row_flat[pr] = f;
+            prow[f] = (!r_table || r_table[id] > 0) ? pr : -1;   // width-0 experts get no tiles: nothing to read back
+        } else if (f < whi) {
+            inv_perm[f] = -1;                                // dropped (precondition violation, flagged by the plan kernel)
+            prow[f] = -1;
+        }
+        __syncwarp();
+        if (id >= 0 && lane == __ffs(m) - 1) whist[w][id] += __popc(m);
+        __syncwarp();
+    }
+
+    if (!x) return;
+    __syncthreads();                                        // prow[] of this block's chunk is complete
+
+    // ---- gather: one warp per assignment of this block
+    for (int f = lo + w; f < hi; f += RT_WARPS) {
+        const int p = prow[f];
+        if (p < 0) continue;                                 // warp-uniform
+        put_row(x + (size_t)(f / k) * chunks_per_row, Xs, P, p, chunks_per_row, lane);
+    }
+}
+
+cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int* counts,
+                              int* offsets, const Workspace& ws, DevState* state, cudaStream_t st) {
+    k_route_plan<<<ws.RB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, r_table, tile_n, counts, offsets, ws.bhist,
+                                               ws.poff, ws.tt, ws.items1, ws.sched, state);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_gather(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
+                                  const int* offsets, int* perm, int* inv_perm, const __nv_bfloat16* x,
+                                  const Workspace& ws, cudaStream_t st) {
+    const int PB = D.E < 148 ? D.E : 148;                    // extra blocks that only zero the padding rows
+    k_scatter_gather<<<ws.RB + PB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, k, r_table, counts, offsets, ws.poff,
+                                                        ws.bhist, perm, inv_perm, ws.row_flat, ws.prow,
+                                                        (const uint4*)x, ws.Xs, ws.P, ws.RB);
     return cudaGetLastError();
 }
 

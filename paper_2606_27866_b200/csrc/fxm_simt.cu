@@ -5,7 +5,7 @@
 // is never selected unless the caller asks for it with fxm_set_impl().
 //   a4: G = X_e W~gate[0:r_e]^T, U = X_e W~up[0:r_e]^T, H = silu(G) (.) U, channels >= r_e forced to 0
 //       (Eq. 4; Alg. 2 l.12-16)
-//   a5: y[t] += topk_w[t][j] * (H_e[:, 0:r_e] W~down[:, 0:r_e]^T)   (Alg. 2 l.18-20)
+//   a5: O[row] = H_e[:, 0:r_e] W~down[:, 0:r_e]^T (Alg. 2 l.18); scale + sum over k in k_combine
 #include "fxm_internal.cuh"
 
 namespace fxm {
@@ -71,8 +71,7 @@ __global__ void __launch_bounds__(128) k_gemm1_simt(Dims D, const uint8_t* __res
 __global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, const uint8_t* __restrict__ packed,
                                                     const int* __restrict__ r_table, const int4* __restrict__ tt,
                                                     const Sched* __restrict__ sched, const uint8_t* __restrict__ H,
-                                                    const int* __restrict__ row_flat, const float* __restrict__ topk_w,
-                                                    int k, float* __restrict__ yacc, int P) {
+                                                    uint8_t* __restrict__ O, int P) {
     const int W2 = sched->W2;
     const uint8_t* dn = packed + gu_bytes(D);
     for (int wi = blockIdx.x; wi < W2; wi += gridDim.x) {
@@ -100,10 +99,9 @@ __global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, const uint8_t* __res
             }
 #pragma unroll
             for (int q = 0; q < SIMT_TOK; ++q) {
-                if (t0 + q < nvalid && i < D.d) {
-                    const int f = row_flat[row0 + t0 + q];
-                    atomicAdd(yacc + (size_t)(f / k) * D.d + i, topk_w[f] * acc[q]);
-                }
+                if (t0 + q < nvalid && i < D.d)
+                    *(__nv_bfloat16*)(O + ((size_t)db * P + row0 + t0 + q) * O_ROW_BYTES + pr * 2) =
+                        __float2bfloat16_rn(acc[q]);
             }
         }
     }
@@ -114,10 +112,9 @@ cudaError_t launch_gemm1_simt(const Dims& D, const uint8_t* packed, const int* r
     k_gemm1_simt<<<148 * 16, 128, 0, st>>>(D, packed, r_table, ws.tt, ws.sched, ws.Xs, ws.H, ws.P);
     return cudaGetLastError();
 }
-cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const float* topk_w, int k,
-                              const Workspace& ws, cudaStream_t st) {
-    k_gemm2_simt<<<148 * 16, 128, 0, st>>>(D, packed, r_table, ws.tt, ws.sched, ws.H, ws.row_flat, topk_w, k, ws.yacc,
-                                           ws.P);
+cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                              cudaStream_t st) {
+    k_gemm2_simt<<<148 * 16, 128, 0, st>>>(D, packed, r_table, ws.tt, ws.sched, ws.H, ws.O, ws.P);
     return cudaGetLastError();
 }
 

@@ -8,8 +8,11 @@
 //       >= r_e forced to 0 (the paper's pad-zero rule), one rounding to bf16, tile written to
 //       the H panel with one bulk store.
 //   a5  GEMM-2 + scale + combine (Alg. 2 l.18-20):
-//         D[128 out features, N tokens] = Wd_tile[128, r_e] . H_tile[N, r_e]^T ;  yacc[tok][i] += w * D[i][tok]
-//       K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.
+//         D[128 out features, N tokens] = Wd_tile[128, r_e] . H_tile[N, r_e]^T
+//       K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.  The epilogue transposes the
+//       accumulator through shared memory into rows of 128 output features (bf16) and writes the tile to the
+//       O panel with one bulk store; the router-weight scale and the sum over a token's k experts are a gather
+//       in k_combine (no atomics, slot order, fp32, one rounding).
 //   a6  decode-sized T uses the same kernels: N shrinks to 16 and the kernel becomes a weight streamer
 //       (16 KB bulk copies back to back, MMA cost negligible).
 //
@@ -130,18 +133,15 @@ struct GemmArgs {
     const Sched* sched;
     const uint8_t* Bsrc;       // Xs (GEMM-1) or H (GEMM-2) panels
     uint8_t* H;                // GEMM-1 output panels
-    const int* row_flat;       // GEMM-2
-    const float* topk_w;       // GEMM-2
-    float* yacc;               // GEMM-2
+    uint8_t* O;                // GEMM-2 output panels
     DevState* state;
     int P;                     // panel row capacity
-    int k;
 };
 
-template <int TN, int STAGES>
+template <int MODE, int TN, int STAGES>
 struct SmemPlan {
     static constexpr int STAGE_BYTES = WT_BYTES + TN * ROW_BYTES;
-    static constexpr int STAGING_BYTES = TN * ROW_BYTES;            // GEMM-1: H tile; GEMM-2: token ids + weights
+    static constexpr int STAGING_BYTES = TN * (MODE == 1 ? ROW_BYTES : O_ROW_BYTES);   // H tile / O tile
     static constexpr int BAR_OFF = STAGES * STAGE_BYTES + STAGING_BYTES;
     static constexpr int TOTAL = BAR_OFF + 256 + 1024;              // + barriers + alignment slack
 };
@@ -149,7 +149,7 @@ struct SmemPlan {
 template <int MODE, int TN, int STAGES>
 __global__ void __launch_bounds__(192, 1) k_gemm_sm100(const GemmArgs a) {
     extern __shared__ uint8_t smem_raw[];
-    using Plan = SmemPlan<TN, STAGES>;
+    using Plan = SmemPlan<MODE, TN, STAGES>;
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
     const uint32_t bar_base = smem_base + Plan::BAR_OFF;
@@ -251,17 +251,6 @@ __global__ void __launch_bounds__(192, 1) k_gemm_sm100(const GemmArgs a) {
             const int n = (nvalid + 15) & ~15;
             const int r = a.r_table[e];
             const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)as * TN;
-            if (MODE == 2) {
-                // token index and router weight of each column of this tile
-                int* s_tok = (int*)staging;
-                float* s_w = (float*)(staging + TN * 4);
-                for (int t = et; t < n; t += 128) {
-                    const int f = t < nvalid ? a.row_flat[row0 + t] : -1;
-                    s_tok[t] = f >= 0 ? f / a.k : -1;
-                    s_w[t] = f >= 0 ? a.topk_w[f] : 0.f;
-                }
-                epi_bar_sync();
-            }
             mbar_wait(tfull_bar(as), aphase, a.state);
             tc_fence_after();
             if (MODE == 1) {
@@ -297,28 +286,30 @@ __global__ void __launch_bounds__(192, 1) k_gemm_sm100(const GemmArgs a) {
                 }
                 epi_bar_sync();
             } else {
-                const int i = (wi % D.nDB) * WT_ROWS + q * 32 + lane;   // output feature of this lane
-                const int* s_tok = (const int*)staging;
-                const float* s_w = (const float*)(staging + TN * 4);
+                const int db = wi % D.nDB;
+                uint8_t* mine = staging + (q * 32 + lane) * 2;       // this lane's output feature inside an O row
                 for (int c0 = 0; c0 < n; c0 += 16) {
                     uint32_t v[16];
                     tmem_ld16(taddr + c0, v);
                     tmem_ld_wait();
-                    if (i < D.d) {
 #pragma unroll
-                        for (int jj = 0; jj < 16; ++jj) {
-                            const int tok = s_tok[c0 + jj];
-                            if (tok >= 0) atomicAdd(a.yacc + (size_t)tok * D.d + i, s_w[c0 + jj] * __uint_as_float(v[jj]));
-                        }
-                    }
+                    for (int jj = 0; jj < 16; ++jj)                 // 32 lanes -> 64 contiguous bytes of row c0+jj
+                        *(__nv_bfloat16*)(mine + (c0 + jj) * O_ROW_BYTES) = __float2bfloat16_rn(__uint_as_float(v[jj]));
                 }
                 tc_fence_before();
                 mbar_arrive(tempty_bar(as));
-                epi_bar_sync();                                // s_tok / s_w are rewritten by the next tile
+                fence_proxy_async_smem();
+                epi_bar_sync();
+                if (et == 0) {
+                    bulk_s2g(a.O + ((size_t)db * a.P + row0) * O_ROW_BYTES, staging_s, (uint32_t)n * O_ROW_BYTES);
+                    bulk_commit();
+                    bulk_wait_read0();
+                }
+                epi_bar_sync();
             }
             if (++as == 2) { as = 0; aphase ^= 1u; }
         }
-        if (MODE == 1 && et == 0) bulk_wait0();
+        if (et == 0) bulk_wait0();
     }
 
     tc_fence_before();
@@ -332,7 +323,7 @@ __global__ void __launch_bounds__(192, 1) k_gemm_sm100(const GemmArgs a) {
 // ---------------------------------------------------------------------------------------------- launchers
 template <int MODE, int TN, int STAGES>
 static cudaError_t launch_t(const GemmArgs& a, int num_sms, cudaStream_t st) {
-    using Plan = SmemPlan<TN, STAGES>;
+    using Plan = SmemPlan<MODE, TN, STAGES>;
     k_gemm_sm100<MODE, TN, STAGES><<<num_sms, 192, Plan::TOTAL, st>>>(a);
     return cudaGetLastError();
 }
@@ -341,12 +332,12 @@ cudaError_t init_sm100_kernels() {
     cudaError_t e;
 #define FXM_SET(MODE, TN, ST)                                                                                     \
     e = cudaFuncSetAttribute(k_gemm_sm100<MODE, TN, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize,             \
-                             SmemPlan<TN, ST>::TOTAL);                                                            \
+                             SmemPlan<MODE, TN, ST>::TOTAL);                                                            \
     if (e != cudaSuccess) return e;
     FXM_SET(1, 128, 5)
     FXM_SET(2, 128, 5)
     FXM_SET(1, 256, 4)
-    FXM_SET(2, 256, 4)
+    FXM_SET(2, 256, 3)
 #undef FXM_SET
     return cudaSuccess;
 }
@@ -359,12 +350,12 @@ cudaError_t launch_gemm1_sm100(const Dims& D, const uint8_t* packed, const int* 
     return tile_n == 256 ? launch_t<1, 256, 4>(a, num_sms, st) : launch_t<1, 128, 5>(a, num_sms, st);
 }
 
-cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const float* topk_w, int k,
-                               const Workspace& ws, DevState* state, int tile_n, int num_sms, cudaStream_t st) {
+cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                               DevState* state, int tile_n, int num_sms, cudaStream_t st) {
     GemmArgs a{};
     a.D = D; a.packed = packed; a.r_table = r_table; a.items = ws.tt; a.sched = ws.sched; a.Bsrc = ws.H;
-    a.row_flat = ws.row_flat; a.topk_w = topk_w; a.yacc = ws.yacc; a.state = state; a.P = ws.P; a.k = k;
-    return tile_n == 256 ? launch_t<2, 256, 4>(a, num_sms, st) : launch_t<2, 128, 5>(a, num_sms, st);
+    a.O = ws.O; a.state = state; a.P = ws.P;
+    return tile_n == 256 ? launch_t<2, 256, 3>(a, num_sms, st) : launch_t<2, 128, 5>(a, num_sms, st);
 }
 
 }  // namespace fxm
