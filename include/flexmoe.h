@@ -50,10 +50,12 @@ typedef enum {
 
 #define FXM_MAX_BUDGETS 15 /* tables that fxm_register_budgets can keep resident */
 
-/* implementation selector for fxm_set_impl: the tcgen05 path is the product; the SIMT path is the slow,
- * structurally simple debug path that runs on the SAME packed layout (used to bisect the fast kernels). */
+/* implementation selector for fxm_set_impl: the CTA-pair tcgen05 path (cta_group::2) is the product; the
+ * single-CTA tcgen05 path and the slow, structurally simple SIMT path run on the SAME packed layout and
+ * exist to bisect the fast kernels. */
 #define FXM_IMPL_TCGEN05 0
 #define FXM_IMPL_SIMT_DEBUG 1
+#define FXM_IMPL_TCGEN05_1CTA 2
 
 /* ---- sizes first: the caller owns all device memory -------------------------------------------------- */
 

@@ -46,10 +46,12 @@ static size_t rank_offset(const Dims& D) { return align_up(state_offset(D) + siz
 static size_t packed_total(const Dims& D) { return align_up(rank_offset(D) + sizeof(int) * (size_t)D.E * D.I, 1024); }
 
 static int choose_tile_n(const fxm_layer* L, int T, int k) {
+    if (L->impl == FXM_IMPL_TCGEN05) return PAIR_TILE_N;         // CTA-pair kernels: one or two 256-token sub-tiles
     if (L->tile_n_override == 128 || L->tile_n_override == 256) return L->tile_n_override;
     // mean rows per expert > 192: 256-token tiles halve the weight re-reads; below that 128 wastes less
     return ((long long)T * k > 192LL * L->D.E) ? 256 : 128;
 }
+static int plan_grp(const fxm_layer* L) { return L->impl == FXM_IMPL_TCGEN05 ? 2 : 1; }
 
 extern "C" {
 
@@ -122,7 +124,7 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return FXM_ECUDA;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return FXM_ECUDA;
-    if (init_sm100_kernels() != cudaSuccess) return FXM_ECUDA;
+    if (init_sm100_kernels() != cudaSuccess || init_pair_kernels() != cudaSuccess) return FXM_ECUDA;
     cudaStream_t st = (cudaStream_t)stream;
     uint8_t* pk = (uint8_t*)packed;
     int* tables = (int*)(pk + tables_offset(D));
@@ -198,7 +200,7 @@ fxm_status fxm_select_budget(fxm_layer* L, int b) {
 }
 
 fxm_status fxm_set_impl(fxm_layer* L, int impl) {
-    if (!L || (impl != FXM_IMPL_TCGEN05 && impl != FXM_IMPL_SIMT_DEBUG)) return FXM_EINVAL;
+    if (!L || (impl != FXM_IMPL_TCGEN05 && impl != FXM_IMPL_SIMT_DEBUG && impl != FXM_IMPL_TCGEN05_1CTA)) return FXM_EINVAL;
     L->impl = impl;
     return FXM_OK;
 }
@@ -257,7 +259,7 @@ fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_
     if (!counts || !offsets || (T > 0 && (!topk_ids || !perm || !inv_perm))) return FXM_EINVAL;
     const Workspace ws = map_workspace(L->D, T, k, workspace);
     const int* table = L->current >= 0 ? L->tables + (size_t)L->current * TABLE_STRIDE : nullptr;
-    if (launch_route_plan(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), counts, offsets, ws, L->state,
+    if (launch_route_plan(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), plan_grp(L), counts, offsets, ws, L->state,
                           (cudaStream_t)stream) != cudaSuccess)
         return FXM_ECUDA;
     if (launch_scatter_gather(L->D, topk_ids, T, k, table, counts, offsets, perm, inv_perm, nullptr, ws,
@@ -287,7 +289,7 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
 #define FXM_MARK(j) if (ev && cudaEventRecord(ev[j], st) != cudaSuccess) return FXM_ECUDA;
     // a2 + a3: grouping and the tile schedule for the CURRENT table
     FXM_MARK(0)
-    if (launch_route_plan(D, topk_ids, T, k, table, tile_n, ws.counts, ws.offsets, ws, L->state, st) != cudaSuccess)
+    if (launch_route_plan(D, topk_ids, T, k, table, tile_n, plan_grp(L), ws.counts, ws.offsets, ws, L->state, st) != cudaSuccess)
         return FXM_ECUDA;
     // stable scatter of the indices + gather of the x rows into sorted swizzled panels
     FXM_MARK(1)
@@ -296,6 +298,10 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
         return FXM_ECUDA;
     FXM_MARK(2)
     if (L->impl == FXM_IMPL_TCGEN05) {
+        if (launch_gemm1_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
+        FXM_MARK(3)
+        if (launch_gemm2_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
+    } else if (L->impl == FXM_IMPL_TCGEN05_1CTA) {
         if (launch_gemm1_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
         FXM_MARK(3)
         if (launch_gemm2_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;

@@ -115,7 +115,7 @@ cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStrea
 // -------------------------------------------------------------------------------------------- combine
 // Alg. 2 l.19-20: Y[token] += alpha * Z_down, done as a GATHER so that no atomics are needed and
 // the sum runs in slot order j = 0..k-1 in fp32 with exactly one rounding of y (readings R8, R11):
-//   y[t][i] = sum_j topk_w[t][j] * O[i/128][prow[t*k+j]][i%128]
+//   y[t][i] = sum_j topk_w[t][j] * O[prow[t*k+j]][i]
 // One block per token; a thread owns 8 consecutive output features (16 bytes of each O row).
 __global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __restrict__ prow,
                                                  const float* __restrict__ topk_w, const uint8_t* __restrict__ O,
@@ -129,8 +129,10 @@ __global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __res
     }
     __syncthreads();
     const int chunks = D.d >> 3;
+    const size_t orow = (size_t)D.nDB * WT_ROWS * 2;              // bytes per O row
+    (void)P;
     for (int c = threadIdx.x; c < chunks; c += blockDim.x) {
-        const uint8_t* col = O + (size_t)(c >> 4) * P * O_ROW_BYTES + ((c & 15) << 4);
+        const uint8_t* col = O + ((size_t)c << 4);
         float acc[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[q] = 0.f;
@@ -139,7 +141,7 @@ __global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __res
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const int p = j0 + u < k ? s_p[j0 + u] : -1;
-                v[u] = p >= 0 ? __ldg((const uint4*)(col + (size_t)p * O_ROW_BYTES)) : make_uint4(0, 0, 0, 0);
+                v[u] = p >= 0 ? __ldg((const uint4*)(col + (size_t)p * orow)) : make_uint4(0, 0, 0, 0);
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {

@@ -88,7 +88,7 @@ struct Workspace {
     int4* items1;           // [NT*nCB] GEMM-1 work items {expert, first padded row, valid rows, channel block}
     uint8_t* Xs;            // [nKB1][P][128 B]  gathered activations, swizzled panels
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
-    uint8_t* O;             // [nDB][P][256 B]  expert outputs, bf16, 128 output features per panel row
+    uint8_t* O;             // [P][nDB*128]  expert outputs per padded row, bf16, row-major
     int RB;                 // route blocks
     int chunk;              // flat assignments per route block
     int P;                  // padded-row capacity (multiple of 16)
@@ -101,7 +101,6 @@ constexpr int TILE_N_MIN = 128;
 
 __host__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-constexpr int O_ROW_BYTES = 256;  // one row of an O panel: 128 output features, bf16
 constexpr int RT_THREADS = 256;   // route kernels: 8 warps per block
 // flat assignments per route block: 128 while that gives <= 512 blocks, then whatever keeps 512 blocks
 __host__ inline int route_chunk(long long A) {
@@ -132,7 +131,7 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.items1 = (int4*)(b + take(sizeof(int4) * (size_t)NT * D.nCB));
     w.Xs = b + take((size_t)D.nKB1 * P * ROW_BYTES);
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
-    w.O = b + take((size_t)D.nDB * P * O_ROW_BYTES);
+    w.O = b + take((size_t)P * D.nDB * WT_ROWS * 2);
     w.RB = RB;
     w.chunk = chunk;
     w.P = P;
@@ -150,7 +149,8 @@ cudaError_t launch_unpack_prefix(const Dims& D, const uint8_t* packed, int e, in
                                  __nv_bfloat16* Wu, __nv_bfloat16* Wd, cudaStream_t st);
 cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStream_t st);
 // a2/a3 part 1: per-block histograms; the last block to finish scans them and writes counts/offsets/poff/tt/items1/sched
-cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n,
+// tile_n = max rows of a token tile; grp = weight blocks per work item (1: single-CTA kernels, 2: CTA-pair kernels)
+cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int grp,
                               int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st);
 // a2 part 2: stable scatter (perm/inv_perm/row_flat/prow) and, when x != null, the gather of x rows into ws.Xs
 cudaError_t launch_scatter_gather(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
@@ -174,5 +174,13 @@ cudaError_t launch_gemm1_sm100(const Dims& D, const uint8_t* packed, const int* 
 cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
                                DevState* state, int tile_n, int num_sms, cudaStream_t st);
 cudaError_t init_sm100_kernels();   // cudaFuncSetAttribute for the dynamic shared memory sizes
+
+// CTA-pair path (cta_group::2, token tiles up to 512 rows); the schedule must have been planned with grp = 2
+constexpr int PAIR_TILE_N = 512;
+cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                              DevState* state, int num_sms, cudaStream_t st);
+cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+                              DevState* state, int num_sms, cudaStream_t st);
+cudaError_t init_pair_kernels();
 
 }  // namespace fxm

@@ -47,7 +47,7 @@ __device__ __forceinline__ bool block_histogram(const int* __restrict__ ids, int
 }
 
 __global__ void __launch_bounds__(RT_THREADS)
-k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table, int tile_n,
+k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table, int tile_n, int grp,
              int* __restrict__ counts, int* __restrict__ offsets, int* __restrict__ bhist, int* __restrict__ poff,
              int4* __restrict__ tt, int4* __restrict__ items1, Sched* __restrict__ sched,
              DevState* __restrict__ state) {
@@ -106,8 +106,8 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
             const int n = e < E ? s_cnt[e] : 0;
             const int r = e < E ? (r_table ? r_table[e] : D.I) : 0;   // no table yet (fxm_route only): full width
             const int np = (n + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
-            const int nt = (n > 0 && r > 0) ? (n + tile_n - 1) / tile_n : 0;   // pruned-away / idle experts: no tiles
-            const int nb = (r + CB - 1) / CB;
+            const int nt = (n > 0 && r > 0) ? (np + tile_n - 1) / tile_n : 0;   // pruned-away / idle experts: no tiles
+            const int nb = ((r + CB - 1) / CB + grp - 1) / grp;                 // GEMM-1 items per token tile
             const int i_off = warp_incl_scan(n, lane), i_poff = warp_incl_scan(np, lane);
             const int i_tiles = warp_incl_scan(nt, lane), i_work = warp_incl_scan(nt * nb, lane);
             if (e < E) {
@@ -115,8 +115,10 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
                 s_poff[e] = c_poff + i_poff - np;
                 int j = c_tiles + i_tiles - nt, wk = c_work + i_work - nt * nb;
                 const int p0 = c_poff + i_poff - np;
-                for (int row = 0; row < n && nt > 0; row += tile_n, ++j, wk += nb)
-                    tt[j] = make_int4(e, p0 + row, min(tile_n, n - row), wk);
+                // balanced split of the padded segment into nt tiles of <= tile_n rows, each a multiple of 16 rows
+                const int per = nt > 0 ? ((np + nt - 1) / nt + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN : 0;
+                for (int row = 0; row < np && nt > 0; row += per, ++j, wk += nb)
+                    tt[j] = make_int4(e, p0 + row, min(per, n - row), wk);      // .z = valid rows of the tile (>= 1)
             }
             c_off += __shfl_sync(0xffffffffu, i_off, 31);
             c_poff += __shfl_sync(0xffffffffu, i_poff, 31);
@@ -129,7 +131,7 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
             s_ntt = c_tiles;
             sched->ntt = c_tiles;
             sched->W1 = c_work;
-            sched->W2 = c_tiles * D.nDB;
+            sched->W2 = c_tiles * ((D.nDB + grp - 1) / grp);
             sched->P_used = c_poff;
             sched->A = A;
             state->ticket = 0;                               // ready for the next call on this layer
@@ -140,7 +142,7 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
     // GEMM-1 work items: one per (token tile, RETAINED channel block) -- pruned blocks are never listed
     for (int j = tid; j < s_ntt; j += RT_THREADS) {
         const int4 t = tt[j];
-        const int nb = ((r_table ? r_table[t.x] : D.I) + CB - 1) / CB;
+        const int nb = (((r_table ? r_table[t.x] : D.I) + CB - 1) / CB + grp - 1) / grp;
         for (int cb = 0; cb < nb; ++cb) items1[t.w + cb] = make_int4(t.x, t.y, t.z, cb);
     }
 }
@@ -237,9 +239,9 @@ k_scatter_gather(Dims D, const int* __restrict__ ids, int A, int chunk, int k, c
     }
 }
 
-cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int* counts,
-                              int* offsets, const Workspace& ws, DevState* state, cudaStream_t st) {
-    k_route_plan<<<ws.RB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, r_table, tile_n, counts, offsets, ws.bhist,
+cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int grp,
+                              int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st) {
+    k_route_plan<<<ws.RB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, r_table, tile_n, grp, counts, offsets, ws.bhist,
                                                ws.poff, ws.tt, ws.items1, ws.sched, state);
     return cudaGetLastError();
 }

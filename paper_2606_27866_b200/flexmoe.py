@@ -13,11 +13,12 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libflexmoe.so")
-_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_sm100.cu"]
-_HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_HERE, "..", "include", "flexmoe.h")]
+_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_sm100.cu", "fxm_pair.cu"]
+_HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_CSRC, "fxm_ptx.cuh"), os.path.join(_HERE, "..", "include", "flexmoe.h")]
 
 IMPL_TCGEN05 = 0
 IMPL_SIMT_DEBUG = 1
+IMPL_TCGEN05_1CTA = 2
 MAX_BUDGETS = 15
 
 _STATUS = ["FXM_OK", "FXM_EINVAL", "FXM_ESHAPE", "FXM_EPERM", "FXM_EBUDGET", "FXM_ENOTNESTED",

@@ -41,8 +41,8 @@ def test_sizes_match_the_layout_formulas():
     ws2 = fx.workspace_bytes(E, d, I, 16, 4)
     assert ws1 > ws2 > 0
     A, P = 4096 * 4, 4096 * 4 + 16 * E
-    assert ws1 >= P * d * 2 + P * I * 2 + 4096 * d * 4           # Xs + H + yacc
-    assert ws1 <= 1.2 * (P * d * 2 + P * I * 2 + 4096 * d * 4) + (1 << 20)
+    assert ws1 >= P * d * 2 + P * I * 2 + P * d * 2              # Xs + H + O (bf16 expert outputs per padded row)
+    assert ws1 <= 1.2 * (P * d * 2 + P * I * 2 + P * d * 2) + (1 << 20)
 
 
 @pytest.mark.parametrize("args,code", [((0, 64, 16), "FXM_ESHAPE"), ((257, 64, 16), "FXM_ESHAPE"),

@@ -89,7 +89,7 @@ def _c1():
     return gen.SHAPES["C1"], lay, b, rng
 
 
-@pytest.mark.parametrize("impl", [1, 0])
+@pytest.mark.parametrize("impl", [1, 2, 0])
 @pytest.mark.parametrize("table", ["full", "c1", "all128", "ragged", "zeros_some"])
 def test_c1_tiny_all_budgets(impl, table):
     """C1 (BASELINE.json configs[0]): d=256, E=8, top-2, I=512, T=64, every element vs the oracle."""
@@ -103,7 +103,7 @@ def test_c1_tiny_all_budgets(impl, table):
     gu.check_close(y, gu.oracle_ffn(lay, b, r), f"C1 {table} impl={impl}")
 
 
-@pytest.mark.parametrize("impl", [1, 0])
+@pytest.mark.parametrize("impl", [1, 2, 0])
 def test_widths_not_multiple_of_64_and_padded_dims(impl):
     """I % 64 != 0 (padded channel block), d % 128 == 64 (padded down rows), r_e any multiple of 1."""
     import gpu_util as gu
@@ -115,9 +115,10 @@ def test_widths_not_multiple_of_64_and_padded_dims(impl):
         gu.check_close(gu.run_ffn(L, b, r, impl=impl), gu.oracle_ffn(lay, b, r), f"r={r.tolist()} impl={impl}")
 
 
-@pytest.mark.parametrize("tile_n", [128, 256])
-def test_multi_tile_ragged_segments(tile_n):
-    """Expert segments that span several token tiles plus a ragged tail, heavy skew, empty experts."""
+@pytest.mark.parametrize("impl,tile_n", [(2, 128), (2, 256), (0, 0)])
+def test_multi_tile_ragged_segments(impl, tile_n):
+    """Expert segments that span several token tiles plus a ragged tail, heavy skew, empty experts.
+    impl 0 = CTA-pair kernels (token tiles up to 512 rows = two sub-tiles), impl 2 = single-CTA kernels."""
     import gpu_util as gu
     sh, lay, rng = _small_layer(4, 128, 6, 2, 192, w_std=0.08)
     T = 900
@@ -127,7 +128,24 @@ def test_multi_tile_ragged_segments(tile_n):
     b = gen.Batch(gen.make_x(T, sh.d, rng), ids, w)
     r = np.array([192, 128, 64, 176, 192, 16], np.int32)
     L = gu.pack_layer(lay)
-    gu.check_close(gu.run_ffn(L, b, r, tile_n=tile_n), gu.oracle_ffn(lay, b, r), f"tile_n={tile_n}")
+    gu.check_close(gu.run_ffn(L, b, r, impl=impl, tile_n=tile_n), gu.oracle_ffn(lay, b, r), f"impl={impl} tile_n={tile_n}")
+
+
+@pytest.mark.parametrize("T", [130, 273, 300, 520, 1100])
+def test_pair_subtile_boundaries(T):
+    """CTA-pair path: one expert receives every token, so its segment is T rows: <=256 (one sub-tile), 257..512
+    (two sub-tiles sharing the weight operand), >512 (several token tiles); odd retained-block counts give the
+    second CTA of a pair a pruned block that must be skipped."""
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(5, 192, 3, 2, 320, w_std=0.08)
+    ids = np.tile(np.array([[1, 2]], np.int32), (T, 1))
+    ids[::7, 1] = 0
+    w = rng.random((T, 2)).astype(np.float32)
+    b = gen.Batch(gen.make_x(T, sh.d, rng), ids, w)
+    L = gu.pack_layer(lay)
+    for r in ([320, 320, 320], [192, 64, 304], [16, 130, 65]):
+        r = np.array(r, np.int32)
+        gu.check_close(gu.run_ffn(L, b, r), gu.oracle_ffn(lay, b, r), f"T={T} r={r.tolist()}")
 
 
 def test_h_intermediate_matches_definition():
