@@ -254,8 +254,8 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (largest share of the step) and of the whole step
     per_launch_ms = {kname: v / max(n_prof, 1) for kname, v in kern_ms.items()}
     dom = max(per_launch_ms, key=per_launch_ms.get)
-    kflops = {"gemm1_swiglu": mean("gemm1_flops"), "gemm2_combine": mean("gemm2_flops")}.get(dom, 0.0)
-    kbytes = {"gemm1_swiglu": mean("gemm1_bytes"), "gemm2_combine": mean("gemm2_bytes")}.get(dom, mean("bytes"))
+    kflops = {"gemm1_swiglu": mean("gemm1_flops"), "gemm2": mean("gemm2_flops")}.get(dom, 0.0)
+    kbytes = {"gemm1_swiglu": mean("gemm1_bytes"), "gemm2": mean("gemm2_bytes")}.get(dom, mean("bytes"))
     t_roof, bound = roof_time_s(kflops, kbytes, peaks)
     dur = per_launch_ms[dom] * 1e-3
     if bound == "tensor":

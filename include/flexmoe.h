@@ -65,7 +65,7 @@ fxm_status fxm_packed_bytes(int E, int d, int I, size_t* bytes);
 
 /* Bytes of scratch for one moe_ffn / route call with at most T_max tokens and k experts per token:
  * grouping indices, tile schedule, the gathered activations X_s [T_max*k + 16E, d] bf16, the SwiGLU
- * activations H [T_max*k + 16E, ceil64(I)] bf16 and the fp32 combine accumulator [T_max, d]. */
+ * activations H [T_max*k + 16E, ceil64(I)] bf16 and the expert outputs O [T_max*k + 16E, ceil128(d)] bf16. */
 fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* bytes);
 
 /* ---- (1) pack: Eq. 3; layout prior art App. C.2, PAPER.md:526-540 ---------------------
@@ -107,7 +107,7 @@ int32_t fxm_ratio_to_width(int I, int num, int den);
  * topk_w   : device fp32 [T][k], applied as given (the router is external and frozen)
  * y        : device bf16 [T][d], OVERWRITTEN (Y <- 0 then accumulate); routed experts only.
  * workspace: device, >= fxm_workspace_bytes(E,d,I,T,k), 1024-byte aligned; contents are scratch.
- * Launches: route, gather, grouped GEMM-1(+SwiGLU), grouped GEMM-2(+scale+combine), finalize.  Grid sizes
+ * Launches: route plan, scatter, gather, grouped GEMM-1(+SwiGLU), grouped GEMM-2, combine (scale + sum).  Grid sizes
  * do not depend on the budget or on the routing (persistent kernels read the device-side schedule), so a
  * call is CUDA-graph capturable.  T == 0 is a no-op. */
 fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
@@ -126,9 +126,9 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
  * Per-kernel device times of fxm_moe_ffn: between fxm_profile_begin and fxm_profile_end every
  * fxm_moe_ffn call (at most max_calls of them, <= 4096) records a CUDA event on its stream before each of its
  * FXM_N_KERNELS launches and after the last.  fxm_profile_end synchronises those events and writes, per kernel
- * (order: route, gather, GEMM-1+SwiGLU, GEMM-2+combine, finalize), the SUM of its durations in milliseconds over
+ * (order: route plan, scatter, gather, GEMM-1+SwiGLU, GEMM-2, combine), the SUM of its durations in milliseconds over
  * the *calls recorded; events are host objects, no device memory is allocated. */
-#define FXM_N_KERNELS 5
+#define FXM_N_KERNELS 6
 fxm_status fxm_profile_begin(fxm_layer* L, int max_calls);
 fxm_status fxm_profile_end(fxm_layer* L, float* ms_sum /* [FXM_N_KERNELS] */, int* calls);
 

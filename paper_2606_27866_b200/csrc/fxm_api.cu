@@ -262,8 +262,8 @@ fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_
     if (launch_route_plan(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), plan_grp(L), counts, offsets, ws, L->state,
                           (cudaStream_t)stream) != cudaSuccess)
         return FXM_ECUDA;
-    if (launch_scatter_gather(L->D, topk_ids, T, k, table, counts, offsets, perm, inv_perm, nullptr, ws,
-                              (cudaStream_t)stream) != cudaSuccess)
+    if (launch_scatter(L->D, topk_ids, T, k, table, counts, offsets, perm, inv_perm, ws, (cudaStream_t)stream) !=
+        cudaSuccess)
         return FXM_ECUDA;
     return FXM_OK;
 }
@@ -291,28 +291,30 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
     FXM_MARK(0)
     if (launch_route_plan(D, topk_ids, T, k, table, tile_n, plan_grp(L), ws.counts, ws.offsets, ws, L->state, st) != cudaSuccess)
         return FXM_ECUDA;
-    // stable scatter of the indices + gather of the x rows into sorted swizzled panels
+    // stable scatter of the indices
     FXM_MARK(1)
-    if (launch_scatter_gather(D, topk_ids, T, k, table, ws.counts, ws.offsets, ws.perm, ws.inv_perm,
-                              (const __nv_bfloat16*)x, ws, st) != cudaSuccess)
+    if (launch_scatter(D, topk_ids, T, k, table, ws.counts, ws.offsets, ws.perm, ws.inv_perm, ws, st) != cudaSuccess)
         return FXM_ECUDA;
+    // gather of the x rows into sorted swizzled panels
     FXM_MARK(2)
+    if (launch_gather(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+    FXM_MARK(3)
     if (L->impl == FXM_IMPL_TCGEN05) {
         if (launch_gemm1_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
-        FXM_MARK(3)
+        FXM_MARK(4)
         if (launch_gemm2_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
     } else if (L->impl == FXM_IMPL_TCGEN05_1CTA) {
         if (launch_gemm1_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
-        FXM_MARK(3)
+        FXM_MARK(4)
         if (launch_gemm2_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
     } else {
         if (launch_gemm1_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
-        FXM_MARK(3)
+        FXM_MARK(4)
         if (launch_gemm2_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
     }
-    FXM_MARK(4)
-    if (launch_combine(D, T, k, topk_w, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
     FXM_MARK(5)
+    if (launch_combine(D, T, k, topk_w, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
+    FXM_MARK(6)
 #undef FXM_MARK
     return FXM_OK;
 }

@@ -102,10 +102,10 @@ constexpr int TILE_N_MIN = 128;
 __host__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 constexpr int RT_THREADS = 256;   // route kernels: 8 warps per block
-// flat assignments per route block: 128 while that gives <= 512 blocks, then whatever keeps 512 blocks
+// flat assignments per route block: a multiple of 256 that keeps the grid at <= 128 blocks
 __host__ inline int route_chunk(long long A) {
-    if (A <= 128LL * 512) return 128;
-    return (int)(((A + 511) / 512 + 127) / 128 * 128);
+    const long long per = (A + 127) / 128;
+    return (int)((per + 255) / 256 * 256 > 0 ? (per + 255) / 256 * 256 : 256);
 }
 
 __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base) {
@@ -152,10 +152,11 @@ cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStrea
 // tile_n = max rows of a token tile; grp = weight blocks per work item (1: single-CTA kernels, 2: CTA-pair kernels)
 cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int grp,
                               int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st);
-// a2 part 2: stable scatter (perm/inv_perm/row_flat/prow) and, when x != null, the gather of x rows into ws.Xs
-cudaError_t launch_scatter_gather(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
-                                  const int* offsets, int* perm, int* inv_perm, const __nv_bfloat16* x,
-                                  const Workspace& ws, cudaStream_t st);
+// a2 part 2: stable scatter (perm / inv_perm / row_flat / prow)
+cudaError_t launch_scatter(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
+                           const int* offsets, int* perm, int* inv_perm, const Workspace& ws, cudaStream_t st);
+// gather of the x rows into the sorted, padded, swizzled panels ws.Xs
+cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st);
 // y[t] = sum_j topk_w[t][j] * O[row of (t,j)]   (fp32 sum in slot order, one rounding)
 cudaError_t launch_combine(const Dims& D, int T, int k, const float* topk_w, const Workspace& ws, __nv_bfloat16* y,
                            cudaStream_t st);

@@ -3,33 +3,40 @@
 //   a4  GEMM-1 + SwiGLU (Eq. 4; Alg. 2 l.12-16), swap-AB:
 //         D[256 packed weight rows, N tokens] = Wgu[256, d] . Xs[N, d]^T,   UMMA M = 256 over the pair:
 //         CTA r of the pair owns channel block cb = 2*cbp + r (64 gate + 64 up rows, lanes 0..127 of ITS TMEM).
+//         Epilogue: h = silu(g) * u (gate lane l, up lane l+16: one shuffle), channels >= r_e forced to 0 (the
+//         paper's pad-zero rule), one rounding to bf16, stored straight into the swizzled H panel.
 //   a5  GEMM-2 (Alg. 2 l.18):
 //         D[256 out features, N tokens] = Wd[256, r_e] . H[N, r_e]^T,  CTA r owns feature block db = 2*dbp + r;
-//         K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.
+//         K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.  Epilogue: one rounding to
+//         bf16, O[row][feature]; the router-weight scale and the sum over k experts are the gather in k_combine.
 //
 // Token tiles are up to 512 rows: a tile is one or two SUB-TILES of <= 256 tokens (UMMA N <= 256) that share the
-// weight operand -- each weight byte is pulled from HBM/L2 into shared memory once per (expert, token tile), so a
+// weight operand -- each weight byte is pulled from HBM into shared memory once per (expert, token tile), so a
 // ragged expert (e.g. 273 tokens = 256 + 32 padded) does not re-read its weights for the tail.  Sub-tile s lives
 // in TMEM columns [256 s, 256 s + N_s); sub-tiles are handed to the epilogue round-robin over the two halves, so
 // tiles of <= 256 tokens are double-buffered (the epilogue of one overlaps the MMAs of the next).
 //
-// Per CTA and pipeline stage: A = one 16 KB weight tile, B0/B1 = this CTA's HALF of each sub-tile's token rows
-// (the pair MMA reads N/2 rows from each CTA's shared memory).  Everything is moved by contiguous cp.async.bulk
-// copies of pre-swizzled SW128 K-major data; no tensor map is needed.
+// Two operand rings per CTA, because the operands have different latencies: the WEIGHT ring is deep (8 x 16 KB:
+// weights have no reuse inside a token tile and come from HBM, ~2-3 us away under load), the TOKEN ring is
+// shallow (3 x 32 KB: this CTA's half of each sub-tile's rows, re-read by every weight block, so they come from
+// L2).  Everything is moved by contiguous cp.async.bulk copies of pre-swizzled SW128 K-major data.
 //
-// Warp roles (192 threads per CTA):  warp 0 = bulk-copy producer (both CTAs), warp 1 = MMA issuer in the leader
-// CTA / RELAY in the peer CTA (forwards "my operands have landed" to the leader's barrier, since a plain bulk copy
-// can only signal a barrier of its own CTA), warps 2-5 = epilogue (each CTA drains its own TMEM lanes).
-// Barriers: full[s] (local, tx bytes), pfull[s] (leader, 1 remote arrive), empty[s] (both CTAs, multicast commit),
-// tfull[h] (both CTAs, multicast commit), tempty[h] (leader, one arrive per CTA).
+// Warp roles (384 threads per CTA): warp 0 = weight producer, warp 2 = token producer, warp 1 = MMA issuer in the
+// leader CTA / RELAY in the peer CTA (forwards "my operands of this k-block have landed" to the leader's barrier,
+// since a plain bulk copy can only signal a barrier of its own CTA), warps 4-11 = epilogue (each CTA drains its
+// own TMEM lanes; two warps per lane quadrant, each taking half of the columns).
+// Barriers: fullA/fullB (local, tx bytes), pfull (leader, 1 remote arrive per k-block), emptyA/emptyB (both CTAs,
+// multicast commit), tfull[h] (both CTAs, multicast commit), tempty[h] (leader, one arrive per CTA).
 #include "fxm_ptx.cuh"
 
 namespace fxm {
 
 constexpr int PAIR_NSUB = 256;                  // tokens per sub-tile (UMMA N max)
 constexpr int PAIR_BHALF = PAIR_NSUB / 2 * ROW_BYTES;   // 16 KB: one CTA's half of a sub-tile's B operand
-constexpr int PAIR_STAGE = WT_BYTES + 2 * PAIR_BHALF;   // 48 KB
-constexpr int PAIR_STAGES = 4;
+constexpr int PAIR_BSLOT = 2 * PAIR_BHALF;      // 32 KB
+constexpr int PAIR_NA = 8;                      // weight ring depth
+constexpr int PAIR_NB = 3;                      // token ring depth
+constexpr int PAIR_THREADS = 384;
 
 struct PairArgs {
     Dims D;
@@ -44,12 +51,10 @@ struct PairArgs {
     int P;
 };
 
-template <int MODE>
-struct PairSmem {
-    static constexpr int STAGING = MODE == 1 ? PAIR_NSUB * ROW_BYTES : 0;     // H sub-tile (GEMM-2 stores straight from registers)
-    static constexpr int BAR_OFF = PAIR_STAGES * PAIR_STAGE + STAGING;
-    static constexpr int TOTAL = BAR_OFF + 256 + 1024;
-};
+constexpr int PAIR_A_OFF = 0;
+constexpr int PAIR_B_OFF = PAIR_NA * WT_BYTES;
+constexpr int PAIR_BAR_OFF = PAIR_B_OFF + PAIR_NB * PAIR_BSLOT;
+constexpr int PAIR_SMEM = PAIR_BAR_OFF + 512 + 1024;      // + barriers + alignment slack
 
 // ------------------------------------------------------------------------------------------ cluster PTX
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -145,27 +150,31 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
     return it;
 }
 
+__device__ __forceinline__ void epi_bar_sync256() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+
 template <int MODE>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(const PairArgs a) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_gemm_pair(const PairArgs a) {
     extern __shared__ uint8_t smem_raw[];
-    using Plan = PairSmem<MODE>;
-    constexpr int ST = PAIR_STAGES;
+    constexpr int NA = PAIR_NA, NB = PAIR_NB;
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    const uint32_t bar_base = smem_base + Plan::BAR_OFF;
-    auto full_bar = [&](int s) { return bar_base + 8u * s; };
-    auto pfull_bar = [&](int s) { return bar_base + 8u * (ST + s); };
-    auto empty_bar = [&](int s) { return bar_base + 8u * (2 * ST + s); };
-    auto tfull_bar = [&](int h) { return bar_base + 8u * (3 * ST + h); };
-    auto tempty_bar = [&](int h) { return bar_base + 8u * (3 * ST + 2 + h); };
-    volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + Plan::BAR_OFF + 8 * (3 * ST + 4));
+    const uint32_t bar_base = smem_base + PAIR_BAR_OFF;
+    auto fullA = [&](int s) { return bar_base + 8u * s; };
+    auto emptyA = [&](int s) { return bar_base + 8u * (NA + s); };
+    auto pfull = [&](int s) { return bar_base + 8u * (2 * NA + s); };
+    auto fullB = [&](int s) { return bar_base + 8u * (3 * NA + s); };
+    auto emptyB = [&](int s) { return bar_base + 8u * (3 * NA + NB + s); };
+    auto tfull_bar = [&](int h) { return bar_base + 8u * (3 * NA + 2 * NB + h); };
+    auto tempty_bar = [&](int h) { return bar_base + 8u * (3 * NA + 2 * NB + 2 + h); };
+    volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + PAIR_BAR_OFF + 8 * (3 * NA + 2 * NB + 4));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const Dims& D = a.D;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < ST; ++s) { mbar_init(full_bar(s), 1); mbar_init(pfull_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < NA; ++s) { mbar_init(fullA(s), 1); mbar_init(emptyA(s), 1); mbar_init(pfull(s), 1); }
+        for (int s = 0; s < NB; ++s) { mbar_init(fullB(s), 1); mbar_init(emptyB(s), 1); }
         for (int h = 0; h < 2; ++h) { mbar_init(tfull_bar(h), 1); mbar_init(tempty_bar(h), 2); }
         fence_barrier_init();
     }
@@ -181,10 +190,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(
     const uint8_t* dn = a.packed + gu_bytes(D);
 
     if (warp == 0) {
-        // ===================================================== producer (both CTAs): this CTA's A tile and B halves
+        // ===================================================== weight producer (both CTAs): this CTA's 16 KB A tiles
         if (lane == 0) {
-            int stage = 0;
-            uint32_t phase = 0;
+            int sa = 0;
+            uint32_t pa = 0;
             for (int wi = wi0; wi < W; wi += wstep) {
                 const PairItem it = pair_item<MODE>(a, wi, rank);
                 const uint8_t* asrc;
@@ -196,27 +205,40 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(
                     asrc = dn + dn_tile_index(D, it.e, 0, it.blk) * WT_BYTES;
                     astride = (size_t)D.nDB * WT_BYTES;
                 }
+                for (int kb = 0; kb < it.nk; ++kb) {
+                    mbar_wait(emptyA(sa), pa ^ 1u, a.state);
+                    mbar_expect_tx(fullA(sa), WT_BYTES);
+                    bulk_g2s(smem_base + PAIR_A_OFF + sa * WT_BYTES, asrc + kb * astride, WT_BYTES, fullA(sa));
+                    if (++sa == NA) { sa = 0; pa ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 2) {
+        // ===================================================== token producer (both CTAs): this CTA's half of each sub-tile
+        if (lane == 0) {
+            int sb = 0;
+            uint32_t pb = 0;
+            const size_t bstride = (size_t)a.P * ROW_BYTES;
+            for (int wi = wi0; wi < W; wi += wstep) {
+                const PairItem it = pair_item<MODE>(a, wi, rank);
                 const uint32_t h0 = (uint32_t)it.n0 >> 1, h1 = (uint32_t)it.n1 >> 1;      // rows of each sub-tile this CTA holds
                 const uint8_t* b0 = a.Bsrc + (size_t)(it.row0 + rank * h0) * ROW_BYTES;
                 const uint8_t* b1 = a.Bsrc + (size_t)(it.row0 + PAIR_NSUB + rank * h1) * ROW_BYTES;
-                const size_t bstride = (size_t)a.P * ROW_BYTES;
-                const uint32_t tx = WT_BYTES + (h0 + h1) * ROW_BYTES;
                 for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
-                    const uint32_t sa = smem_base + stage * PAIR_STAGE;
-                    mbar_expect_tx(full_bar(stage), tx);
-                    bulk_g2s(sa, asrc + kb * astride, WT_BYTES, full_bar(stage));
-                    bulk_g2s(sa + WT_BYTES, b0 + kb * bstride, h0 * ROW_BYTES, full_bar(stage));
-                    if (h1) bulk_g2s(sa + WT_BYTES + PAIR_BHALF, b1 + kb * bstride, h1 * ROW_BYTES, full_bar(stage));
-                    if (++stage == ST) { stage = 0; phase ^= 1u; }
+                    mbar_wait(emptyB(sb), pb ^ 1u, a.state);
+                    const uint32_t sbase = smem_base + PAIR_B_OFF + sb * PAIR_BSLOT;
+                    mbar_expect_tx(fullB(sb), (h0 + h1) * ROW_BYTES);
+                    bulk_g2s(sbase, b0 + kb * bstride, h0 * ROW_BYTES, fullB(sb));
+                    if (h1) bulk_g2s(sbase + PAIR_BHALF, b1 + kb * bstride, h1 * ROW_BYTES, fullB(sb));
+                    if (++sb == NB) { sb = 0; pb ^= 1u; }
                 }
             }
         }
     } else if (warp == 1) {
         if (lane == 0 && rank == 0) {
             // ================================================= MMA issuer (leader CTA): one thread issues for the pair
-            int stage = 0;
-            uint32_t phase = 0, sc = 0;
+            int sa = 0, sb = 0;
+            uint32_t pa = 0, pb = 0, sc = 0;
             for (int wi = wi0; wi < W; wi += wstep) {
                 const PairItem it = pair_item<MODE>(a, wi, rank);
                 const uint32_t hA = sc & 1u, hB = (sc + 1u) & 1u;
@@ -226,12 +248,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(
                 const uint32_t d0 = tmem_base + hA * PAIR_NSUB, d1 = tmem_base + hB * PAIR_NSUB;
                 const uint32_t id0 = make_idesc2((uint32_t)it.n0), id1 = make_idesc2((uint32_t)(it.n1 ? it.n1 : 16));
                 for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(full_bar(stage), phase, a.state);
-                    mbar_wait(pfull_bar(stage), phase, a.state);
+                    mbar_wait(fullA(sa), pa, a.state);
+                    mbar_wait(fullB(sb), pb, a.state);
+                    mbar_wait(pfull(sa), pa, a.state);          // the peer CTA's halves of this k-block
                     tc_fence_after();
-                    const uint32_t sa = smem_base + stage * PAIR_STAGE;
-                    const uint64_t adesc = make_desc_sw128(sa);
-                    const uint64_t bd0 = make_desc_sw128(sa + WT_BYTES), bd1 = make_desc_sw128(sa + WT_BYTES + PAIR_BHALF);
+                    const uint32_t sB = smem_base + PAIR_B_OFF + sb * PAIR_BSLOT;
+                    const uint64_t adesc = make_desc_sw128(smem_base + PAIR_A_OFF + sa * WT_BYTES);
+                    const uint64_t bd0 = make_desc_sw128(sB), bd1 = make_desc_sw128(sB + PAIR_BHALF);
 #pragma unroll
                     for (int kk = 0; kk < KB / 16; ++kk)
                         umma2_bf16(d0, adesc + 2u * kk, bd0 + 2u * kk, id0, (uint32_t)((kb | kk) != 0));
@@ -240,32 +263,35 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(
                         for (int kk = 0; kk < KB / 16; ++kk)
                             umma2_bf16(d1, adesc + 2u * kk, bd1 + 2u * kk, id1, (uint32_t)((kb | kk) != 0));
                     }
-                    umma2_commit_mc(empty_bar(stage));          // frees this stage in BOTH CTAs when the MMAs retire
-                    if (++stage == ST) { stage = 0; phase ^= 1u; }
+                    umma2_commit_mc(emptyA(sa));                // frees the slots in BOTH CTAs when these MMAs retire
+                    umma2_commit_mc(emptyB(sb));
+                    if (++sa == NA) { sa = 0; pa ^= 1u; }
+                    if (++sb == NB) { sb = 0; pb ^= 1u; }
                 }
                 umma2_commit_mc(tfull_bar(hA));
                 if (it.n1) umma2_commit_mc(tfull_bar(hB));
                 sc += it.n1 ? 2u : 1u;
             }
         } else if (lane == 0) {
-            // ================================================= relay (peer CTA): my operands of stage s have landed
-            int stage = 0;
-            uint32_t phase = 0;
+            // ================================================= relay (peer CTA): my operands of this k-block have landed
+            int sa = 0, sb = 0;
+            uint32_t pa = 0, pb = 0;
             for (int wi = wi0; wi < W; wi += wstep) {
                 const PairItem it = pair_item<MODE>(a, wi, rank);
                 for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(full_bar(stage), phase, a.state);
-                    mbar_arrive_remote(pfull_bar(stage), 0);
-                    if (++stage == ST) { stage = 0; phase ^= 1u; }
+                    mbar_wait(fullA(sa), pa, a.state);
+                    mbar_wait(fullB(sb), pb, a.state);
+                    mbar_arrive_remote(pfull(sa), 0);
+                    if (++sa == NA) { sa = 0; pa ^= 1u; }
+                    if (++sb == NB) { sb = 0; pb ^= 1u; }
                 }
             }
         }
-    } else {
-        // ===================================================== epilogue warps 2..5 (both CTAs, own TMEM lanes)
-        const int q = warp & 3;
-        const int et = threadIdx.x - 64;
-        uint8_t* staging = smem_gen + ST * PAIR_STAGE;
-        const uint32_t staging_s = smem_base + ST * PAIR_STAGE;
+    } else if (warp >= 4) {
+        // ===================================================== epilogue warps 4..11 (both CTAs, own TMEM lanes)
+        const int q = warp & 3;                                // TMEM lane quadrant this warp may read
+        const int grp = (warp - 4) >> 2;                       // which half of the columns
+        const int et = threadIdx.x - 128;
         const int dpad = D.nDB * WT_ROWS;
         uint32_t sc = 0;
         for (int wi = wi0; wi < W; wi += wstep) {
@@ -274,67 +300,69 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(
             for (int s = 0; s < nsub; ++s, ++sc) {
                 const uint32_t h = sc & 1u;
                 const int n = s ? it.n1 : it.n0;
+                const int split = ((n >> 4) + 1) / 2 * 16;    // columns [0, split) -> group 0, [split, n) -> group 1
+                const int cbeg = grp ? split : 0, cend = grp ? n : split;
                 const int rowS = it.row0 + s * PAIR_NSUB;
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + h * PAIR_NSUB;
                 mbar_wait(tfull_bar(h), (sc >> 1) & 1u, a.state);
                 tc_fence_after();
-                if (MODE == 1) {
-                    if (it.valid) {
+                if (it.valid && cbeg < cend) {
+                    // two register buffers: the TMEM load of the next 16 columns is in flight while these are processed
+                    uint32_t va[16], vb[16];
+                    if (MODE == 1) {
                         const int ch = q * 16 + (lane & 15);
                         const bool keep = it.blk * CB + ch < it.r;       // tail mask of the last retained block (pad-zero rule)
                         const int odd = lane >> 4;
-                        for (int c0 = 0; c0 < n; c0 += 16) {
-                            uint32_t v[16];
-                            tmem_ld16(taddr + c0, v);
-                            tmem_ld_wait();
+                        uint8_t* hrow = a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES;
+                        auto swiglu16 = [&](const uint32_t (&v)[16], int c0) {
 #pragma unroll
                             for (int m = 0; m < 8; ++m) {
                                 const float mine0 = __uint_as_float(v[2 * m]), mine1 = __uint_as_float(v[2 * m + 1]);
-                                const float send = odd ? mine0 : mine1;
+                                const float send = odd ? mine0 : mine1;                    // what the twin lane needs
                                 const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
-                                const float g = odd ? recv : mine0;
-                                const float u = odd ? mine1 : recv;
+                                const float g = odd ? recv : mine0;                        // gate lives in lanes 0-15
+                                const float u = odd ? mine1 : recv;                        // up lives in lanes 16-31
                                 float hv = __fdividef(g, 1.f + __expf(-g)) * u;
                                 if (!keep) hv = 0.f;
-                                const uint32_t t = c0 + 2 * m + odd;
-                                *(__nv_bfloat16*)(staging + sw128_off(t, ch)) = __float2bfloat16_rn(hv);
+                                const uint32_t t = c0 + 2 * m + odd;                       // 16 lanes -> one full 32-byte sector
+                                *(__nv_bfloat16*)(hrow + sw128_off(t, ch)) = __float2bfloat16_rn(hv);
                             }
+                        };
+                        tmem_ld16(taddr + cbeg, va);
+                        for (int c0 = cbeg; c0 < cend; c0 += 32) {
+                            tmem_ld_wait();
+                            if (c0 + 16 < cend) tmem_ld16(taddr + c0 + 16, vb);
+                            swiglu16(va, c0);
+                            tmem_ld_wait();
+                            if (c0 + 32 < cend) tmem_ld16(taddr + c0 + 32, va);
+                            if (c0 + 16 < cend) swiglu16(vb, c0 + 16);
                         }
-                    }
-                    tc_fence_before();
-                    fence_proxy_async_smem();
-                    epi_bar_sync();
-                    if (et == 0) {
-                        if (rank == 0) mbar_arrive(tempty_bar(h)); else mbar_arrive_remote(tempty_bar(h), 0);
-                        if (it.valid) {
-                            bulk_s2g(a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES, staging_s, (uint32_t)n * ROW_BYTES);
-                            bulk_commit();
-                            bulk_wait_read0();
-                        }
-                    }
-                    epi_bar_sync();
-                } else {
-                    if (it.valid) {
+                    } else {
                         // lane = output feature; 16 token columns per load; 32 lanes -> 64 contiguous bytes of one O row
                         uint8_t* dst = a.O + ((size_t)rowS * dpad + it.blk * WT_ROWS + q * 32 + lane) * 2;
-                        for (int c0 = 0; c0 < n; c0 += 16) {
-                            uint32_t v[16];
-                            tmem_ld16(taddr + c0, v);
-                            tmem_ld_wait();
+                        auto store16 = [&](const uint32_t (&v)[16], int c0) {
 #pragma unroll
                             for (int jj = 0; jj < 16; ++jj)
                                 *(__nv_bfloat16*)(dst + (size_t)(c0 + jj) * dpad * 2) = __float2bfloat16_rn(__uint_as_float(v[jj]));
+                        };
+                        tmem_ld16(taddr + cbeg, va);
+                        for (int c0 = cbeg; c0 < cend; c0 += 32) {
+                            tmem_ld_wait();
+                            if (c0 + 16 < cend) tmem_ld16(taddr + c0 + 16, vb);
+                            store16(va, c0);
+                            tmem_ld_wait();
+                            if (c0 + 32 < cend) tmem_ld16(taddr + c0 + 32, va);
+                            if (c0 + 16 < cend) store16(vb, c0 + 16);
                         }
                     }
-                    tc_fence_before();
-                    epi_bar_sync();
-                    if (et == 0) {
-                        if (rank == 0) mbar_arrive(tempty_bar(h)); else mbar_arrive_remote(tempty_bar(h), 0);
-                    }
+                }
+                tc_fence_before();
+                epi_bar_sync256();                             // all 8 warps have drained this half of TMEM
+                if (et == 0) {
+                    if (rank == 0) mbar_arrive(tempty_bar(h)); else mbar_arrive_remote(tempty_bar(h), 0);
                 }
             }
         }
-        if (MODE == 1 && et == 0) bulk_wait0();
     }
 
     tc_fence_before();
@@ -349,14 +377,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(192, 1) k_gemm_pair(
 // ---------------------------------------------------------------------------------------------- launchers
 template <int MODE>
 static cudaError_t launch_pair_t(const PairArgs& a, int num_sms, cudaStream_t st) {
-    k_gemm_pair<MODE><<<num_sms / 2 * 2, 192, PairSmem<MODE>::TOTAL, st>>>(a);   // cluster dims are compiled in
+    k_gemm_pair<MODE><<<num_sms / 2 * 2, PAIR_THREADS, PAIR_SMEM, st>>>(a);   // cluster dims are compiled in
     return cudaGetLastError();
 }
 
 cudaError_t init_pair_kernels() {
-    cudaError_t e = cudaFuncSetAttribute(k_gemm_pair<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem<1>::TOTAL);
+    cudaError_t e = cudaFuncSetAttribute(k_gemm_pair<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, PAIR_SMEM);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_gemm_pair<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PairSmem<2>::TOTAL);
+    return cudaFuncSetAttribute(k_gemm_pair<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PAIR_SMEM);
 }
 
 cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,

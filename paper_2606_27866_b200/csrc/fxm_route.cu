@@ -5,17 +5,18 @@
 //   Alg. 2 l.2-3, 8-11: BucketByRetI / AlignUp / view lists are replaced by a tile list
 //   computed here from counts[] and the CURRENT width table r[]: only tiles with channel index < r_e and
 //   token row < n_e exist.
-//   Alg. 2 l.7: X[pi] -- the gather of routed token rows -- is fused into the scatter pass.
+//   Alg. 2 l.7: X[pi] -- the gather of routed token rows into sorted panels.
 //
-// Two launches, no atomics decide any position (hence deterministic and stable):
+// Three launches, no atomics decide any position (hence deterministic and stable):
 //   k_route_plan     grid = RB blocks.  Block b histograms the flat assignments [b*chunk, (b+1)*chunk) per
 //                    expert.  The LAST block to publish (ticket counter) turns the RB x E histogram into
 //                    exclusive bases over blocks and writes counts, offsets, padded offsets, the token tiles
 //                    and the GEMM-1 work items for the current width table.
-//   k_scatter_gather grid = RB blocks.  Block b ranks its assignments: base over blocks + base over the
+//   k_scatter        grid = RB blocks.  Block b ranks its assignments: base over blocks + base over the
 //                    warps of the block + __match_any_sync rank inside a 32-wide step ("earlier block, earlier
 //                    warp, earlier step, lower lane" == "lower flat index"), writes perm / inv_perm / row_flat
-//                    / prow, then copies the x rows of ITS assignments into the swizzled K-major panels Xs.
+//                    / prow.
+//   k_gather         full grid, one warp per padded row: x rows -> swizzled K-major panels Xs.
 #include "fxm_internal.cuh"
 
 namespace fxm {
@@ -76,25 +77,50 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
     if (!s_last) return;
     __threadfence();
 
-    // ---- last block: exclusive scan over blocks (per expert; loads of one b are coalesced over e)
+    // ---- last block: exclusive scan over blocks, per expert.  Thread (e, s) owns rows [s*L, (s+1)*L) of column e:
+    //      pass 1 sums them, the S segment sums are scanned through shared memory, pass 2 writes the prefixes.
     const int RB = gridDim.x;
-    for (int e = tid; e < E; e += RT_THREADS) {
-        int run = 0;
-        int b = 0;
-        for (; b + 8 <= RB; b += 8) {
+    const int S = RT_THREADS / E > 0 ? RT_THREADS / E : 1;     // E <= 256 = RT_THREADS
+    const int L = (RB + S - 1) / S;
+    int* seg = &whist[0][0];                                     // [S][E] <= 256 ints, histogram rows are dead now
+    const int e0 = tid % E, s0 = tid / E;
+    const int b_lo = min(RB, s0 * L), b_hi = s0 < S ? min(RB, b_lo + L) : b_lo;
+    {
+        int sum = 0;
+        int b = b_lo;
+        for (; b + 8 <= b_hi; b += 8) {
             int c[8];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) c[u] = __ldcg(bhist + (size_t)(b + u) * E + e);
+            for (int u = 0; u < 8; ++u) c[u] = __ldcg(bhist + (size_t)(b + u) * E + e0);
 #pragma unroll
-            for (int u = 0; u < 8; ++u) { bhist[(size_t)(b + u) * E + e] = run; run += c[u]; }
+            for (int u = 0; u < 8; ++u) sum += c[u];
         }
-        for (; b < RB; ++b) {
-            const int c = __ldcg(bhist + (size_t)b * E + e);
-            bhist[(size_t)b * E + e] = run;
+        for (; b < b_hi; ++b) sum += __ldcg(bhist + (size_t)b * E + e0);
+        __syncthreads();                                         // everyone is done reading whist
+        if (s0 < S) seg[s0 * E + e0] = sum;
+    }
+    __syncthreads();
+    {
+        int run = 0;
+        for (int ss = 0; ss < s0 && ss < S; ++ss) run += seg[ss * E + e0];
+        if (s0 == S - 1) {                                       // the last segment also knows the column total
+            const int tot = run + seg[s0 * E + e0];
+            s_cnt[e0] = tot;
+            counts[e0] = tot;
+        }
+        int b = b_lo;
+        for (; b + 8 <= b_hi; b += 8) {
+            int c[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) c[u] = __ldcg(bhist + (size_t)(b + u) * E + e0);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { bhist[(size_t)(b + u) * E + e0] = run; run += c[u]; }
+        }
+        for (; b < b_hi; ++b) {
+            const int c = __ldcg(bhist + (size_t)b * E + e0);
+            bhist[(size_t)b * E + e0] = run;
             run += c;
         }
-        s_cnt[e] = run;
-        counts[e] = run;
     }
     __syncthreads();
 
@@ -167,26 +193,13 @@ __device__ __forceinline__ void put_row(const uint4* __restrict__ src, uint8_t* 
 }
 
 __global__ void __launch_bounds__(RT_THREADS)
-k_scatter_gather(Dims D, const int* __restrict__ ids, int A, int chunk, int k, const int* __restrict__ r_table,
-                 const int* __restrict__ counts, const int* __restrict__ offsets, const int* __restrict__ poff,
-                 const int* __restrict__ bbase, int* __restrict__ perm, int* __restrict__ inv_perm,
-                 int* __restrict__ row_flat, int* __restrict__ prow, const uint4* __restrict__ x,
-                 uint8_t* __restrict__ Xs, int P, int RB) {
+k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table,
+          const int* __restrict__ counts, const int* __restrict__ offsets, const int* __restrict__ poff,
+          const int* __restrict__ bbase, int* __restrict__ perm, int* __restrict__ inv_perm,
+          int* __restrict__ row_flat, int* __restrict__ prow) {
     __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, then per-warp running base
     const int E = D.E;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int chunks_per_row = D.d >> 3;
-    if ((int)blockIdx.x >= RB) {
-        // ---- extra blocks: padding rows of the expert segments get zero activations and no assignment
-        for (int e = blockIdx.x - RB; e < E; e += gridDim.x - RB) {
-            const int p0 = poff[e] + counts[e], p1 = poff[e + 1];
-            for (int p = p0 + w; p < p1; p += RT_WARPS) {
-                if (lane == 0) row_flat[p] = -1;
-                if (x) put_row(nullptr, Xs, P, p, chunks_per_row, lane);
-            }
-        }
-        return;
-    }
     for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
     __syncthreads();
     const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
@@ -228,14 +241,23 @@ k_scatter_gather(Dims D, const int* __restrict__ ids, int A, int chunk, int k, c
         __syncwarp();
     }
 
-    if (!x) return;
-    __syncthreads();                                        // prow[] of this block's chunk is complete
+    // ---- padding rows of the expert segments carry no assignment
+    for (int e = blockIdx.x * RT_THREADS + tid; e < E; e += gridDim.x * RT_THREADS)
+        for (int p = poff[e] + counts[e]; p < poff[e + 1]; ++p) row_flat[p] = -1;
+}
 
-    // ---- gather: one warp per assignment of this block
-    for (int f = lo + w; f < hi; f += RT_WARPS) {
-        const int p = prow[f];
-        if (p < 0) continue;                                 // warp-uniform
-        put_row(x + (size_t)(f / k) * chunks_per_row, Xs, P, p, chunks_per_row, lane);
+// Alg. 2 l.7, X[pi]: one warp per padded row p copies x[token(p)] into the swizzled panels; padding
+// rows become zeros so no garbage ever reaches a tensor core.
+__global__ void __launch_bounds__(256)
+k_gather(Dims D, const uint4* __restrict__ x, int k, const int* __restrict__ row_flat, const Sched* __restrict__ sched,
+         uint8_t* __restrict__ Xs, int P) {
+    const int lane = threadIdx.x & 31;
+    const int gw = blockIdx.x * 8 + (threadIdx.x >> 5), nw = gridDim.x * 8;
+    const int P_used = sched->P_used;
+    const int chunks_per_row = D.d >> 3;
+    for (int p = gw; p < P_used; p += nw) {
+        const int f = row_flat[p];
+        put_row(f >= 0 ? x + (size_t)(f / k) * chunks_per_row : nullptr, Xs, P, p, chunks_per_row, lane);
     }
 }
 
@@ -246,13 +268,19 @@ cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const
     return cudaGetLastError();
 }
 
-cudaError_t launch_scatter_gather(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
-                                  const int* offsets, int* perm, int* inv_perm, const __nv_bfloat16* x,
-                                  const Workspace& ws, cudaStream_t st) {
-    const int PB = D.E < 148 ? D.E : 148;                    // extra blocks that only zero the padding rows
-    k_scatter_gather<<<ws.RB + PB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, k, r_table, counts, offsets, ws.poff,
-                                                        ws.bhist, perm, inv_perm, ws.row_flat, ws.prow,
-                                                        (const uint4*)x, ws.Xs, ws.P, ws.RB);
+cudaError_t launch_scatter(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
+                           const int* offsets, int* perm, int* inv_perm, const Workspace& ws, cudaStream_t st) {
+    k_scatter<<<ws.RB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, r_table, counts, offsets, ws.poff, ws.bhist, perm,
+                                            inv_perm, ws.row_flat, ws.prow);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st) {
+    const long long rows = (long long)T * k + (long long)D.E * (ROW_ALIGN - 1);
+    long long blocks = (rows + 7) / 8;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks < 1) blocks = 1;
+    k_gather<<<(int)blocks, 256, 0, st>>>(D, (const uint4*)x, k, ws.row_flat, ws.sched, ws.Xs, ws.P);
     return cudaGetLastError();
 }
 

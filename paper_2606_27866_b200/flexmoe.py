@@ -116,8 +116,8 @@ def workspace_bytes_host(E: int, d: int, I: int, T_max: int, k: int) -> int:
     return n.value
 
 
-N_KERNELS = 5
-KERNEL_NAMES = ("route", "gather", "gemm1_swiglu", "gemm2_combine", "finalize")
+N_KERNELS = 6
+KERNEL_NAMES = ("route_plan", "scatter", "gather", "gemm1_swiglu", "gemm2", "combine")
 
 
 def ratio_to_width(I: int, num: int, den: int) -> int:
