@@ -107,7 +107,8 @@ int32_t fxm_ratio_to_width(int I, int num, int den);
  * topk_w   : device fp32 [T][k], applied as given (the router is external and frozen)
  * y        : device bf16 [T][d], OVERWRITTEN (Y <- 0 then accumulate); routed experts only.
  * workspace: device, >= fxm_workspace_bytes(E,d,I,T,k), 1024-byte aligned; contents are scratch.
- * Launches: route plan, scatter, gather, grouped GEMM-1(+SwiGLU), grouped GEMM-2, combine (scale + sum).  Grid sizes
+ * Launches: route plan, scatter, gather, grouped GEMM-1(+SwiGLU), grouped GEMM-2, combine (scale + sum) -- or, for
+ * decode-sized calls (fxm_set_decode), ONE fused launch that streams the retained weights once.  Grid sizes
  * do not depend on the budget or on the routing (persistent kernels read the device-side schedule), so a
  * call is CUDA-graph capturable.  T == 0 is a no-op. */
 fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
@@ -126,9 +127,9 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
  * Per-kernel device times of fxm_moe_ffn: between fxm_profile_begin and fxm_profile_end every
  * fxm_moe_ffn call (at most max_calls of them, <= 4096) records a CUDA event on its stream before each of its
  * FXM_N_KERNELS launches and after the last.  fxm_profile_end synchronises those events and writes, per kernel
- * (order: route plan, scatter, gather, GEMM-1+SwiGLU, GEMM-2, combine), the SUM of its durations in milliseconds over
+ * (order: route plan, scatter, gather, GEMM-1+SwiGLU, GEMM-2, combine, fused decode kernel), the SUM of its durations in milliseconds over
  * the *calls recorded; events are host objects, no device memory is allocated. */
-#define FXM_N_KERNELS 6
+#define FXM_N_KERNELS 7
 fxm_status fxm_profile_begin(fxm_layer* L, int max_calls);
 fxm_status fxm_profile_end(fxm_layer* L, float* ms_sum /* [FXM_N_KERNELS] */, int* calls);
 
@@ -150,10 +151,17 @@ fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k,
 fxm_status fxm_set_impl(fxm_layer* L, int impl);          /* FXM_IMPL_* ; default FXM_IMPL_TCGEN05 */
 /* Token-tile width of the grouped GEMMs: 128, 256, or 0 = choose from T*k/E (default).  Tuning knob only. */
 fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
+/* Step a6: calls with T*k <= max_assignments (<= 1024; 0 = never) run as ONE launch of the fused
+ * weight-streaming decode kernel instead of the six launches above; prefetch_tiles = how many 16 KB weight tiles
+ * its L2 prefetch cursor runs ahead of the shared-memory ring (0..256).  Tuning knob only: results agree within
+ * the stated tolerance either way.  Needs d <= 3840, else the general path is used regardless. */
+#define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 768
+#define FXM_DECODE_DEFAULT_PREFETCH 8
+fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles);
 /* Synchronises `stream`, then returns the sticky device flag word (bit0: expert id out of range,
  * bit1: a pipeline wait timed out -- a bug) in *flags and clears it. */
 fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream);
-/* Number of kernels one fxm_moe_ffn enqueues (bench.py's gpu_launches). */
+/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode) or 6 (bench.py's gpu_launches). */
 int fxm_launches_per_ffn(const fxm_layer* L);
 
 const char* fxm_status_string(fxm_status s);

@@ -19,6 +19,9 @@ struct fxm_layer {
     int impl;
     int num_sms;
     int tile_n_override;     // 0 = choose from T*k/E
+    int dec_max_A;           // the fused decode kernel takes calls with T*k <= dec_max_A (0 = never)
+    int dec_pf;              // its L2 prefetch distance in 16 KB tiles
+    int last_launches;       // kernels enqueued by the last fxm_moe_ffn
     std::vector<int> host_tables;   // mirror of the resident tables (validation / introspection only)
     std::vector<cudaEvent_t> prof_events;   // fxm_profile_begin: (FXM_N_KERNELS + 1) events per recorded call
     int prof_capacity;       // calls that can still be recorded
@@ -52,6 +55,11 @@ static int choose_tile_n(const fxm_layer* L, int T, int k) {
     return ((long long)T * k > 192LL * L->D.E) ? 256 : 128;
 }
 static int plan_grp(const fxm_layer* L) { return L->impl == FXM_IMPL_TCGEN05 ? 2 : 1; }
+// a6: decode-sized calls (a handful of tokens per expert) go to the single-launch weight-streaming kernel
+static bool use_decode(const fxm_layer* L, int T, int k) {
+    const long long A = (long long)T * k;
+    return L->impl == FXM_IMPL_TCGEN05 && A <= L->dec_max_A && A <= DEC_MAX_A && decode_supported(L->D);
+}
 
 extern "C" {
 
@@ -124,7 +132,8 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return FXM_ECUDA;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return FXM_ECUDA;
-    if (init_sm100_kernels() != cudaSuccess || init_pair_kernels() != cudaSuccess) return FXM_ECUDA;
+    if (init_sm100_kernels() != cudaSuccess || init_pair_kernels() != cudaSuccess || init_decode_kernel() != cudaSuccess)
+        return FXM_ECUDA;
     cudaStream_t st = (cudaStream_t)stream;
     uint8_t* pk = (uint8_t*)packed;
     int* tables = (int*)(pk + tables_offset(D));
@@ -144,6 +153,7 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
     L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
     L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
     L->prof_capacity = 0; L->prof_calls = 0;
+    L->dec_max_A = FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS; L->dec_pf = FXM_DECODE_DEFAULT_PREFETCH; L->last_launches = 0;
     *out = L;
     return FXM_OK;
 }
@@ -211,7 +221,14 @@ fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n) {
     return FXM_OK;
 }
 
-int fxm_launches_per_ffn(const fxm_layer* L) { (void)L; return FXM_N_KERNELS; }
+fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles) {
+    if (!L || max_assignments < 0 || prefetch_tiles < 0 || prefetch_tiles > 256) return FXM_EINVAL;
+    L->dec_max_A = max_assignments > DEC_MAX_A ? DEC_MAX_A : max_assignments;
+    L->dec_pf = prefetch_tiles;
+    return FXM_OK;
+}
+
+int fxm_launches_per_ffn(const fxm_layer* L) { return L ? L->last_launches : 0; }
 
 fxm_status fxm_profile_begin(fxm_layer* L, int max_calls) {
     if (!L || max_calls < 1 || max_calls > 4096) return FXM_EINVAL;
@@ -287,6 +304,16 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
         --L->prof_capacity;
     }
 #define FXM_MARK(j) if (ev && cudaEventRecord(ev[j], st) != cudaSuccess) return FXM_ECUDA;
+    if (use_decode(L, T, k)) {
+        // a6: one launch does a2..a5 (in-kernel grouping, weight streaming, SwiGLU, scale + combine)
+        for (int j = 0; j < FXM_N_KERNELS; ++j) FXM_MARK(j)
+        if (launch_decode(D, L->packed, table, (const __nv_bfloat16*)x, topk_ids, topk_w, T, k, ws.yacc,
+                          (__nv_bfloat16*)y, L->state, L->num_sms, L->dec_pf, st) != cudaSuccess)
+            return FXM_ECUDA;
+        FXM_MARK(FXM_N_KERNELS)
+        L->last_launches = 1;
+        return FXM_OK;
+    }
     // a2 + a3: grouping and the tile schedule for the CURRENT table
     FXM_MARK(0)
     if (launch_route_plan(D, topk_ids, T, k, table, tile_n, plan_grp(L), ws.counts, ws.offsets, ws, L->state, st) != cudaSuccess)
@@ -315,7 +342,9 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
     FXM_MARK(5)
     if (launch_combine(D, T, k, topk_w, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
     FXM_MARK(6)
+    FXM_MARK(7)
 #undef FXM_MARK
+    L->last_launches = 6;
     return FXM_OK;
 }
 

@@ -24,6 +24,7 @@ constexpr int MAX_E = 256;
 constexpr int MAX_K = 16;
 constexpr int TABLE_STRIDE = 256;      // int32 per resident budget table
 constexpr int MAX_TABLES = 16;         // FXM_MAX_BUDGETS registered + 1 "set_budget" slot
+constexpr int DEC_MAX_A = 1024;        // most assignments T*k the fused decode kernel takes (int16 indices, smem routing)
 
 // byte offset of element (row, col) inside a swizzled tile whose rows are 128 B; row is the row index
 // relative to a base that is a multiple of 8 rows.
@@ -59,7 +60,9 @@ __host__ __device__ inline size_t dn_bytes(const Dims& D) { return (size_t)D.E *
 struct DevState {           // lives at the tail of the packed blob (zeroed by pack)
     uint32_t flags;         // bit0: expert id out of range; bit1: pipeline wait timed out
     uint32_t ticket;        // route: blocks that have published their histogram (reset by the last one)
-    uint32_t pad[62];
+    uint32_t bar_count[2];  // decode kernel: arrivals at grid barrier 0 / 1 (reset by the last arriver)
+    uint32_t bar_gen[2];    // decode kernel: generation of grid barrier 0 / 1 (sense reversal; never reset)
+    uint32_t pad[58];
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -89,6 +92,7 @@ struct Workspace {
     uint8_t* Xs;            // [nKB1][P][128 B]  gathered activations, swizzled panels
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
     uint8_t* O;             // [P][nDB*128]  expert outputs per padded row, bf16, row-major
+    float* yacc;            // [T][d] fp32 accumulator of the fused decode kernel (only when T*k <= DEC_MAX_A)
     int RB;                 // route blocks
     int chunk;              // flat assignments per route block
     int P;                  // padded-row capacity (multiple of 16)
@@ -132,6 +136,7 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.Xs = b + take((size_t)D.nKB1 * P * ROW_BYTES);
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
     w.O = b + take((size_t)P * D.nDB * WT_ROWS * 2);
+    w.yacc = (float*)(b + take(A <= (size_t)DEC_MAX_A ? (size_t)T * D.d * sizeof(float) : 0));
     w.RB = RB;
     w.chunk = chunk;
     w.P = P;
@@ -183,5 +188,12 @@ cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r
 cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
                               DevState* state, int num_sms, cudaStream_t st);
 cudaError_t init_pair_kernels();
+
+// fused single-launch decode kernel (fxm_decode.cu): T*k <= DEC_MAX_A, d <= 3840
+bool decode_supported(const Dims& D);
+cudaError_t init_decode_kernel();
+cudaError_t launch_decode(const Dims& D, const uint8_t* packed, const int* r_table, const __nv_bfloat16* x,
+                          const int* ids, const float* topk_w, int T, int k, float* yacc, __nv_bfloat16* y,
+                          DevState* state, int num_sms, int pf, cudaStream_t st);
 
 }  // namespace fxm

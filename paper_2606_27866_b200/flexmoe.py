@@ -13,7 +13,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libflexmoe.so")
-_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_sm100.cu", "fxm_pair.cu"]
+_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_sm100.cu", "fxm_pair.cu", "fxm_decode.cu"]
 _HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_CSRC, "fxm_ptx.cuh"), os.path.join(_HERE, "..", "include", "flexmoe.h")]
 
 IMPL_TCGEN05 = 0
@@ -76,6 +76,7 @@ def lib():
     L.fxm_debug_read_h.argtypes = [vp, vp, i32, i32, vp, vp, vp]
     L.fxm_set_impl.argtypes = [vp, i32]
     L.fxm_set_tile_n.argtypes = [vp, i32]
+    L.fxm_set_decode.argtypes = [vp, i32, i32]
     L.fxm_device_flags.argtypes = [vp, ctypes.POINTER(ctypes.c_uint32), vp]
     L.fxm_launches_per_ffn.argtypes = [vp]
     L.fxm_status_string.argtypes = [i32]
@@ -89,7 +90,7 @@ def lib():
 EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
            "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_workspace_bytes_host", "fxm_moe_ffn_host",
            "fxm_profile_begin", "fxm_profile_end", "fxm_route", "fxm_unpack_prefix",
-           "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_device_flags", "fxm_launches_per_ffn",
+           "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_set_decode", "fxm_device_flags", "fxm_launches_per_ffn",
            "fxm_status_string", "fxm_destroy"]
 
 
@@ -116,8 +117,10 @@ def workspace_bytes_host(E: int, d: int, I: int, T_max: int, k: int) -> int:
     return n.value
 
 
-N_KERNELS = 6
-KERNEL_NAMES = ("route_plan", "scatter", "gather", "gemm1_swiglu", "gemm2", "combine")
+N_KERNELS = 7
+KERNEL_NAMES = ("route_plan", "scatter", "gather", "gemm1_swiglu", "gemm2", "combine", "decode_fused")
+DECODE_DEFAULT_MAX_ASSIGNMENTS = 768
+DECODE_DEFAULT_PREFETCH = 8
 
 
 def ratio_to_width(I: int, num: int, den: int) -> int:
@@ -198,6 +201,9 @@ class Layer:
 
     def set_tile_n(self, n: int):
         _chk(lib().fxm_set_tile_n(self._h, int(n)), "fxm_set_tile_n")
+
+    def set_decode(self, max_assignments: int = DECODE_DEFAULT_MAX_ASSIGNMENTS, prefetch_tiles: int = DECODE_DEFAULT_PREFETCH):
+        _chk(lib().fxm_set_decode(self._h, int(max_assignments), int(prefetch_tiles)), "fxm_set_decode")
 
     # -- workspace ----------------------------------------------------------------------------------
     def workspace(self, T: int, k: int):

@@ -23,10 +23,16 @@ def pack_layer(lay, identity=False):
     return L
 
 
-def run_ffn(L, batch, r, impl=fx.IMPL_TCGEN05, tile_n=0):
+def run_ffn(L, batch, r, impl=fx.IMPL_TCGEN05, tile_n=0, decode=None):
+    """decode: None = the library's default choice, False = never the fused decode kernel (general six-launch
+    path even for tiny T), True = the fused decode kernel whenever T*k <= 1024."""
     import torch
     L.set_impl(impl)
     L.set_tile_n(tile_n)
+    if decode is None:
+        L.set_decode()
+    else:
+        L.set_decode(1024 if decode else 0)
     L.set_budget(r)
     x = to_dev(batch.x)
     ids = torch.from_numpy(batch.topk_ids).cuda()

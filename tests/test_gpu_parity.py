@@ -89,7 +89,21 @@ def _c1():
     return gen.SHAPES["C1"], lay, b, rng
 
 
-@pytest.mark.parametrize("impl", [1, 2, 0])
+# impl: 1 = SIMT debug, 2 = single-CTA tcgen05, 0 = CTA-pair tcgen05 (general path forced), "dec" = fused decode kernel
+IMPLS = [1, 2, 0, "dec"]
+
+
+def _run(gu, L, b, r, impl, **kw):
+    if impl == "dec":
+        y = gu.run_ffn(L, b, r, impl=0, decode=True, **kw)
+        assert L.launches_per_ffn() == 1, "the fused decode kernel was not taken"
+        return y
+    y = gu.run_ffn(L, b, r, impl=impl, decode=False, **kw)
+    assert L.launches_per_ffn() == 6
+    return y
+
+
+@pytest.mark.parametrize("impl", IMPLS)
 @pytest.mark.parametrize("table", ["full", "c1", "all128", "ragged", "zeros_some"])
 def test_c1_tiny_all_budgets(impl, table):
     """C1 (BASELINE.json configs[0]): d=256, E=8, top-2, I=512, T=64, every element vs the oracle."""
@@ -99,11 +113,11 @@ def test_c1_tiny_all_budgets(impl, table):
          "ragged": np.array([512, 16, 100 // 16 * 16 + 4 * 0 + 48, 336, 64, 80, 496, 272]),
          "zeros_some": np.array([0, 512, 0, 256, 64, 0, 128, 384])}[table].astype(np.int32)
     L = gu.pack_layer(lay)
-    y = gu.run_ffn(L, b, r, impl=impl)
+    y = _run(gu, L, b, r, impl)
     gu.check_close(y, gu.oracle_ffn(lay, b, r), f"C1 {table} impl={impl}")
 
 
-@pytest.mark.parametrize("impl", [1, 2, 0])
+@pytest.mark.parametrize("impl", IMPLS)
 def test_widths_not_multiple_of_64_and_padded_dims(impl):
     """I % 64 != 0 (padded channel block), d % 128 == 64 (padded down rows), r_e any multiple of 1."""
     import gpu_util as gu
@@ -112,7 +126,7 @@ def test_widths_not_multiple_of_64_and_padded_dims(impl):
     L = gu.pack_layer(lay)
     for r in ([80] * 6, [1, 7, 33, 64, 65, 79], [0, 0, 0, 0, 0, 5]):
         r = np.array(r, np.int32)
-        gu.check_close(gu.run_ffn(L, b, r, impl=impl), gu.oracle_ffn(lay, b, r), f"r={r.tolist()} impl={impl}")
+        gu.check_close(_run(gu, L, b, r, impl), gu.oracle_ffn(lay, b, r), f"r={r.tolist()} impl={impl}")
 
 
 @pytest.mark.parametrize("impl,tile_n", [(2, 128), (2, 256), (0, 0)])
@@ -145,7 +159,75 @@ def test_pair_subtile_boundaries(T):
     L = gu.pack_layer(lay)
     for r in ([320, 320, 320], [192, 64, 304], [16, 130, 65]):
         r = np.array(r, np.int32)
-        gu.check_close(gu.run_ffn(L, b, r), gu.oracle_ffn(lay, b, r), f"T={T} r={r.tolist()}")
+        gu.check_close(gu.run_ffn(L, b, r, decode=False), gu.oracle_ffn(lay, b, r), f"T={T} r={r.tolist()}")
+
+
+# ------------------------------------------------------------------------------------- fused decode kernel (a6)
+@pytest.mark.parametrize("T,k,E,bias", [(1, 1, 4, 0.0), (3, 2, 5, 0.0), (40, 4, 6, 2.0), (200, 2, 6, 2.5), (64, 16, 16, 0.0),
+                                        (128, 8, 256, 1.0), (1024, 1, 7, 1.0)])
+def test_decode_groups_runs_and_skew(T, k, E, bias):
+    """a6: experts with more than 16 tokens (several token groups re-streaming the weights), experts with none,
+    width-0 experts, ragged widths, A up to the kernel's limit of 1024 assignments; every element vs the oracle."""
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(21 + T, 192, E, k, 208, w_std=0.08)
+    lg = gen.make_logits(T, E, rng, 1.0, bias)
+    if E > 3:
+        lg[:, 2] = -1e9                                    # expert 2 never routed
+    ids, w = gen.route(lg, k)
+    b = gen.Batch(gen.make_x(T, sh.d, rng), ids, w)
+    L = gu.pack_layer(lay)
+    r = rng.integers(0, 208 // 16 + 1, size=E).astype(np.int32) * 16
+    r[0] = 208
+    r[E - 1] = 0
+    for rt in (np.full(E, 208, np.int32), r, (r // 3).astype(np.int32)):
+        y = gu.run_ffn(L, b, rt, decode=True)
+        assert L.launches_per_ffn() == 1
+        gu.check_close(y, gu.oracle_ffn(lay, b, rt), f"decode T={T} k={k} E={E} r={rt.tolist()[:8]}")
+
+
+def test_decode_repeated_calls_and_interleaving_with_general_path():
+    """The grid barriers of the decode kernel are sense-reversing counters that live across calls: many calls in a
+    row (no host sync), alternating with general-path calls and with budget switches, must all be right."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    tabs = np.array([[512] * 8, [512, 384, 512, 256, 512, 128, 512, 64], [256, 128, 192, 64, 512, 64, 128, 0]], np.int32)
+    L = gu.pack_layer(lay)
+    L.register_budgets(tabs, require_nested=True)
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    refs = [gu.oracle_ffn(lay, b, t) for t in tabs]
+    outs = []
+    for i in range(24):
+        bi = (i * 7) % 3
+        L.select_budget(bi)
+        L.set_decode(0 if i % 5 == 4 else 1024)
+        outs.append((bi, L.moe_ffn(x, ids, w)))
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
+    for bi, y in outs:
+        gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), refs[bi], f"call with budget {bi}")
+
+
+def test_decode_out_of_range_id_is_flagged_and_dropped():
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    r = np.full(sh.E, sh.I, np.int32)
+    L = gu.pack_layer(lay)
+    L.set_budget(r)
+    L.set_decode(1024)
+    ids = b.topk_ids.copy()
+    ids[3, 1] = 99
+    w = b.topk_w.copy()
+    y = L.moe_ffn(gu.to_dev(b.x), torch.from_numpy(ids).cuda(), torch.from_numpy(w).cuda())
+    torch.cuda.synchronize()
+    assert L.device_flags() & 1
+    w[3, 1] = 0.0                                          # dropping the assignment == giving it weight 0
+    ids[3, 1] = 0
+    ref = oracle.moe_ffn(b.x, *gu.oracle_packed(lay), r, ids, w)
+    gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), ref, "dropped assignment")
 
 
 def test_h_intermediate_matches_definition():
@@ -156,7 +238,7 @@ def test_h_intermediate_matches_definition():
     sh, lay, b, rng = _c1()
     r = gen.table_c1(sh, rng)
     L = gu.pack_layer(lay)
-    gu.run_ffn(L, b, r)
+    gu.run_ffn(L, b, r, decode=False)                       # the H panels exist only on the general path
     ids = torch.from_numpy(b.topk_ids).cuda()
     H = gen.bf16_bits_to_f32(fx.bf16_to_bits(L.debug_read_h(ids))).astype(np.float64)
     Gt, Ut, _ = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
@@ -231,9 +313,9 @@ def _rows_sample(T, n, seed):
     return np.sort(np.random.default_rng(seed).choice(T, size=min(n, T), replace=False)).astype(np.int32)
 
 
-@pytest.mark.parametrize("T", [1, 16, 4096])
+@pytest.mark.parametrize("T,decode", [(1, True), (16, True), (1, False), (16, False), (4096, None)])
 @pytest.mark.parametrize("r", [704, 1408])
-def test_c2_qwen15_shaped(T, r):
+def test_c2_qwen15_shaped(T, r, decode):
     """C2 (BASELINE.json configs[1], the bench workload): d=2048, E=60, top-4, I=1408, uniform r_e.
     T<=16: every row; T=4096: grouping indices in full + 96 sampled rows (rows of y are independent)."""
     import torch
@@ -242,7 +324,8 @@ def test_c2_qwen15_shaped(T, r):
     sh = gen.SHAPES["C2"]
     rt = gen.table_uniform(sh, r)
     L = gu.pack_layer(lay)
-    y = gu.run_ffn(L, b, rt)
+    y = gu.run_ffn(L, b, rt, decode=decode)
+    assert L.launches_per_ffn() == (1 if decode else 6)
     rows = None if T <= 16 else _rows_sample(T, 96, 11)
     ref = gu.oracle_ffn(lay, b, rt, rows=rows)
     gu.check_close(y if rows is None else y[rows], ref, f"C2 T={T} r={r}")
@@ -263,8 +346,8 @@ def test_c3_deepseek_shaped_skewed_heterogeneous():
     gu.check_close(y[rows], gu.oracle_ffn(lay, b, r, rows=rows), "C3")
 
 
-@pytest.mark.parametrize("T", [1, 64, 8192])
-def test_c4_qwen2_57b_shaped_budget_sweep(T):
+@pytest.mark.parametrize("T,decode", [(1, None), (64, None), (64, False), (8192, None)])
+def test_c4_qwen2_57b_shaped_budget_sweep(T, decode):
     """C4: d=3584, E=64, top-8, I=2560; nested heterogeneous tables at 0/25/40/50/75 % pruned."""
     import gpu_util as gu
     lay, b, rng = gen.config("C4", T=T)
@@ -273,6 +356,7 @@ def test_c4_qwen2_57b_shaped_budget_sweep(T):
     L = gu.pack_layer(lay)
     rows = None if T == 1 else _rows_sample(T, 24, 13)
     for bi in (0, 2, 4):
-        y = gu.run_ffn(L, b, tabs[bi])
+        y = gu.run_ffn(L, b, tabs[bi], decode=decode)
+        assert L.launches_per_ffn() == (6 if (decode is False or T > 64) else 1)
         ref = gu.oracle_ffn(lay, b, tabs[bi], rows=rows)
         gu.check_close(y if rows is None else y[rows], ref, f"C4 T={T} budget {bi}")
