@@ -129,10 +129,9 @@ __global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __res
     }
     __syncthreads();
     const int chunks = D.d >> 3;
-    const size_t orow = (size_t)D.nDB * WT_ROWS * 2;              // bytes per O row
-    (void)P;
+    const size_t orow = 2 * WT_ROWS;                              // bytes per row of an O panel
     for (int c = threadIdx.x; c < chunks; c += blockDim.x) {
-        const uint8_t* col = O + ((size_t)c << 4);
+        const uint8_t* col = O + (size_t)(c >> 4) * P * orow + ((size_t)(c & 15) << 4);   // panel c/16, 16-byte chunk c%16
         float acc[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[q] = 0.f;

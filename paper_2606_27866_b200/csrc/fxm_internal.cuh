@@ -36,6 +36,11 @@ __host__ __device__ inline uint32_t sw128_chunk(uint32_t row, uint32_t ch) {
     return row * ROW_BYTES + (((ch ^ row) & 7u) << 4);
 }
 
+// byte offset of output feature i of padded row p in the O panels
+__host__ __device__ inline size_t o_off(int P, int p, int i) {
+    return ((size_t)(i >> 7) * P + p) * (2 * WT_ROWS) + (size_t)(i & 127) * 2;
+}
+
 struct Dims {
     int E, d, I;
     int Ip;      // ceil64(I)
@@ -74,7 +79,8 @@ struct Sched {              // written by the route kernel, read by everything a
     int W2;                 // GEMM-2 work items  = ntt * nDB
     int P_used;             // padded rows in use
     int A;                  // T * k
-    int pad[11];
+    int max_n;              // rows of the widest token tile (multiple of 16; 16 if there is none)
+    int pad[10];
 };
 
 struct Workspace {
@@ -91,7 +97,7 @@ struct Workspace {
     int4* items1;           // [NT*nCB] GEMM-1 work items {expert, first padded row, valid rows, channel block}
     uint8_t* Xs;            // [nKB1][P][128 B]  gathered activations, swizzled panels
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
-    uint8_t* O;             // [P][nDB*128]  expert outputs per padded row, bf16, row-major
+    uint8_t* O;             // [nDB][P][256 B]  expert outputs, bf16: panel db holds features db*128..+127 of every padded row
     float* yacc;            // [T][d] fp32 accumulator of the fused decode kernel (only when T*k <= DEC_MAX_A)
     int RB;                 // route blocks
     int chunk;              // flat assignments per route block

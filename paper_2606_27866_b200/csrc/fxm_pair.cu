@@ -4,39 +4,44 @@
 //         D[256 packed weight rows, N tokens] = Wgu[256, d] . Xs[N, d]^T,   UMMA M = 256 over the pair:
 //         CTA r of the pair owns channel block cb = 2*cbp + r (64 gate + 64 up rows, lanes 0..127 of ITS TMEM).
 //         Epilogue: h = silu(g) * u (gate lane l, up lane l+16: one shuffle), channels >= r_e forced to 0 (the
-//         paper's pad-zero rule), one rounding to bf16, stored straight into the swizzled H panel.
+//         paper's pad-zero rule), one rounding to bf16 -> the swizzled H panel.
 //   a5  GEMM-2 (Alg. 2 l.18):
 //         D[256 out features, N tokens] = Wd[256, r_e] . H[N, r_e]^T,  CTA r owns feature block db = 2*dbp + r;
 //         K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.  Epilogue: one rounding to
-//         bf16, O[row][feature]; the router-weight scale and the sum over k experts are the gather in k_combine.
+//         bf16 -> the O panel; the router-weight scale and the sum over k experts are the gather in k_combine.
 //
-// Token tiles are up to 512 rows: a tile is one or two SUB-TILES of <= 256 tokens (UMMA N <= 256) that share the
-// weight operand -- each weight byte is pulled from HBM into shared memory once per (expert, token tile), so a
-// ragged expert (e.g. 273 tokens = 256 + 32 padded) does not re-read its weights for the tail.  Sub-tile s lives
-// in TMEM columns [256 s, 256 s + N_s); sub-tiles are handed to the epilogue round-robin over the two halves, so
-// tiles of <= 256 tokens are double-buffered (the epilogue of one overlaps the MMAs of the next).
+// Token tiles are up to 512 rows: a tile is one or two SUB-TILES of <= 256 tokens (UMMA N <= 256, balanced split)
+// that share the weight operand -- each weight byte is pulled into shared memory once per (expert, token tile).
 //
-// Two operand rings per CTA, because the operands have different latencies: the WEIGHT ring is deep (8 x 16 KB:
-// weights have no reuse inside a token tile and come from HBM, ~2-3 us away under load), the TOKEN ring is
-// shallow (3 x 32 KB: this CTA's half of each sub-tile's rows, re-read by every weight block, so they come from
-// L2).  Everything is moved by contiguous cp.async.bulk copies of pre-swizzled SW128 K-major data.
+// Pipeline (what the in-kernel timeline of the previous version showed: the MMA thread was ISSUE-bound -- three
+// barrier waits, two commits and a register->uniform-register "waterfall" per instruction, because it ran in a
+// divergent `lane == 0` branch -- and the epilogue was serialised with the main loop):
+//   * every role runs WARP-UNIFORM: all 32 lanes walk the loops and poll the barriers, one elected lane issues the
+//     asynchronous instruction, so descriptors and addresses live in uniform registers;
+//   * ONE ring of stages, each stage = this CTA's 16 KB weight tile + its half of the token rows of one k-block;
+//     the stage size follows the largest token tile of the call (Sched::max_n), so small tiles get a deep ring;
+//   * ONE wait per k-block for the MMA warp: the leader's full barrier counts its own producer's arrive(+tx) AND the
+//     peer CTA's relay ("my half has landed"); ONE multicast commit frees the stage in both CTAs;
+//   * TMEM is a circular column allocator: a sub-tile takes N contiguous columns, so the MMAs of the next item start
+//     as soon as the columns they need are drained (tiles of <= 256 tokens are fully double-buffered);
+//   * the epilogue stages its output in shared memory in the final layout and writes it with bulk stores (the H / O
+//     panels make a CTA's output of a sub-tile one contiguous range);
+//   * an L2 prefetch cursor runs ahead of the weight loads so the ring refills at L2 latency.
 //
-// Warp roles (384 threads per CTA): warp 0 = weight producer, warp 2 = token producer, warp 1 = MMA issuer in the
-// leader CTA / RELAY in the peer CTA (forwards "my operands of this k-block have landed" to the leader's barrier,
-// since a plain bulk copy can only signal a barrier of its own CTA), warps 4-11 = epilogue (each CTA drains its
-// own TMEM lanes; two warps per lane quadrant, each taking half of the columns).
-// Barriers: fullA/fullB (local, tx bytes), pfull (leader, 1 remote arrive per k-block), emptyA/emptyB (both CTAs,
-// multicast commit), tfull[h] (both CTAs, multicast commit), tempty[h] (leader, one arrive per CTA).
+// Warp roles (384 threads per CTA): warp 0 = producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA),
+// warps 4-11 = epilogue (each CTA drains its own TMEM lanes; two warps per lane quadrant).
 #include "fxm_ptx.cuh"
 
 namespace fxm {
 
-constexpr int PAIR_NSUB = 256;                  // tokens per sub-tile (UMMA N max)
-constexpr int PAIR_BHALF = PAIR_NSUB / 2 * ROW_BYTES;   // 16 KB: one CTA's half of a sub-tile's B operand
-constexpr int PAIR_BSLOT = 2 * PAIR_BHALF;      // 32 KB
-constexpr int PAIR_NA = 8;                      // weight ring depth
-constexpr int PAIR_NB = 3;                      // token ring depth
+constexpr int PAIR_NSUB = 256;                  // most tokens per sub-tile (UMMA N max)
 constexpr int PAIR_THREADS = 384;
+constexpr int PAIR_MAX_STAGES = 8;
+constexpr int PAIR_STAGING = 2 * 16384;         // two 16 KB epilogue staging buffers
+constexpr int PAIR_SMEM = 232448;               // 227 KB: everything a CTA can have
+constexpr int PAIR_RING_BYTES = PAIR_SMEM - 1024 /*alignment slack*/ - PAIR_STAGING - 1024 /*barriers*/;
+constexpr int PAIR_TQ = 8;                      // TMEM sub-tile barrier ring
+constexpr int PAIR_PF = 12;                     // weight tiles the L2 prefetch cursor runs ahead
 
 struct PairArgs {
     Dims D;
@@ -46,15 +51,10 @@ struct PairArgs {
     const Sched* sched;
     const uint8_t* Bsrc;       // Xs (GEMM-1) or H (GEMM-2) panels
     uint8_t* H;                // GEMM-1 output panels
-    uint8_t* O;                // GEMM-2 output rows [P][dpad] bf16
+    uint8_t* O;                // GEMM-2 output panels [nDB][P][256 B]
     DevState* state;
     int P;
 };
-
-constexpr int PAIR_A_OFF = 0;
-constexpr int PAIR_B_OFF = PAIR_NA * WT_BYTES;
-constexpr int PAIR_BAR_OFF = PAIR_B_OFF + PAIR_NB * PAIR_BSLOT;
-constexpr int PAIR_SMEM = PAIR_BAR_OFF + 512 + 1024;      // + barriers + alignment slack
 
 // ------------------------------------------------------------------------------------------ cluster PTX
 __device__ __forceinline__ uint32_t cluster_ctarank() {
@@ -75,6 +75,16 @@ __device__ __forceinline__ uint32_t cluster_count_x() {
 __device__ __forceinline__ void cluster_sync_all() {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// one lane of a converged warp
+__device__ __forceinline__ bool elect_one() {
+    uint32_t p;
+    asm volatile(
+        "{\n\t.reg .pred q;\n\t"
+        "elect.sync _|q, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(p));
+    return p != 0;
 }
 // arrive on the mbarrier at the same shared-memory offset in CTA `rank` of the cluster.  Default semantics
 // (release at CTA scope): the signals forwarded this way order asynchronous-proxy traffic (bulk copies into shared
@@ -114,8 +124,10 @@ __device__ __forceinline__ void umma2_commit_mc(uint32_t bar) {
 __device__ __forceinline__ uint32_t make_idesc2(uint32_t n) {     // M = 256 (pair), N = n
     return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((256u >> 4) << 24);
 }
+__device__ __forceinline__ void epi_bar_sync256() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ int shfl0(int v) { return __shfl_sync(0xffffffffu, v, 0); }   // also tells the compiler: warp-uniform
 
-// ------------------------------------------------------------------------------------------------ kernel
+// ------------------------------------------------------------------------------------------------ items
 struct PairItem {
     int e, row0, n0, n1, blk, nk, r;
     bool valid;               // false: this CTA's weight block lies beyond the retained width (odd block count)
@@ -138,7 +150,8 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
     it.e = q.x;
     it.row0 = q.y;
     const int n = (q.z + 15) & ~15;
-    it.n0 = n < PAIR_NSUB ? n : PAIR_NSUB;
+    // one sub-tile up to 256 tokens, else two balanced ones (both multiples of 16)
+    it.n0 = n <= PAIR_NSUB ? n : (((n >> 4) + 1) >> 1) << 4;
     it.n1 = n - it.n0;
     it.r = a.r_table[it.e];
     const int nb = (it.r + CB - 1) / CB;
@@ -150,32 +163,74 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
     return it;
 }
 
-__device__ __forceinline__ void epi_bar_sync256() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+// Circular TMEM column allocator, replayed identically by the MMA warp and by every epilogue thread: sub-tile
+// number q (in issue order) takes w contiguous columns at the returned offset.  `need` = how many sub-tiles must
+// have been drained before the MMAs of q may write (sub-tiles are drained in order): the newest earlier sub-tile
+// whose columns overlap, and q - PAIR_TQ because the barrier ring has PAIR_TQ entries.
+struct TmemRing {
+    uint32_t head, seq;
+    uint32_t lo[PAIR_TQ], hi[PAIR_TQ];
+    __device__ __forceinline__ void init() { head = 0; seq = 0; }
+    __device__ __forceinline__ uint32_t record(uint32_t c, uint32_t w) {      // -> sub-tiles that must be drained first
+        uint32_t nd = seq >= (uint32_t)PAIR_TQ ? seq - PAIR_TQ + 1 : 0;
+#pragma unroll
+        for (uint32_t i = 1; i < (uint32_t)PAIR_TQ; ++i) {
+            if (i <= seq) {
+                const uint32_t s = seq - i;
+                if (lo[s % PAIR_TQ] < c + w && hi[s % PAIR_TQ] > c && s + 1 > nd) nd = s + 1;
+            }
+        }
+        lo[seq % PAIR_TQ] = c;
+        hi[seq % PAIR_TQ] = c + w;
+        ++seq;
+        return nd;
+    }
+    // the one or two sub-tiles of an item (n0 + n1 <= 512); they never overlap each other
+    __device__ __forceinline__ void alloc_item(uint32_t n0, uint32_t n1, uint32_t& c0, uint32_t& c1, uint32_t& need) {
+        if (head + n0 > 512u) head = 0;
+        c0 = head;
+        c1 = 0;
+        if (n1) {
+            if (c0 + n0 + n1 <= 512u) c1 = c0 + n0;
+            else if (n1 <= c0) c1 = 0;
+            else { c0 = 0; c1 = n0; }
+        }
+        head = n1 ? c1 + n1 : c0 + n0;
+        need = record(c0, n0);
+        if (n1) need = max(need, record(c1, n1));              // disjoint from [c0, c0 + n0) by construction
+    }
+};
 
+// ------------------------------------------------------------------------------------------------ kernel
 template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_gemm_pair(const PairArgs a) {
     extern __shared__ uint8_t smem_raw[];
-    constexpr int NA = PAIR_NA, NB = PAIR_NB;
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    const uint32_t bar_base = smem_base + PAIR_BAR_OFF;
-    auto fullA = [&](int s) { return bar_base + 8u * s; };
-    auto emptyA = [&](int s) { return bar_base + 8u * (NA + s); };
-    auto pfull = [&](int s) { return bar_base + 8u * (2 * NA + s); };
-    auto fullB = [&](int s) { return bar_base + 8u * (3 * NA + s); };
-    auto emptyB = [&](int s) { return bar_base + 8u * (3 * NA + NB + s); };
-    auto tfull_bar = [&](int h) { return bar_base + 8u * (3 * NA + 2 * NB + h); };
-    auto tempty_bar = [&](int h) { return bar_base + 8u * (3 * NA + 2 * NB + 2 + h); };
-    volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + PAIR_BAR_OFF + 8 * (3 * NA + 2 * NB + 4));
+    const uint32_t stg_base = smem_base + PAIR_RING_BYTES;                    // epilogue staging, 2 x 16 KB
+    uint8_t* stg_gen = smem_gen + PAIR_RING_BYTES;
+    const uint32_t bar_base = stg_base + PAIR_STAGING;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (PAIR_MAX_STAGES + s); };
+    auto tfull_bar = [&](uint32_t q) { return bar_base + 8u * (2 * PAIR_MAX_STAGES + (q % PAIR_TQ)); };
+    auto tempty_bar = [&](uint32_t q) { return bar_base + 8u * (2 * PAIR_MAX_STAGES + PAIR_TQ + (q % PAIR_TQ)); };
+    volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + PAIR_RING_BYTES + PAIR_STAGING + 8 * (2 * PAIR_MAX_STAGES + 2 * PAIR_TQ));
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = shfl0(threadIdx.x >> 5), lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const Dims& D = a.D;
 
+    // ring geometry of this call: a stage holds one 16 KB weight tile and this CTA's half of the widest token tile
+    const int max_n = a.sched->max_n;
+    const uint32_t stage_bytes = WT_BYTES + (((uint32_t)max_n * (ROW_BYTES / 2) + 1023u) & ~1023u);
+    const int NS = min(PAIR_MAX_STAGES, (int)(PAIR_RING_BYTES / stage_bytes));
+
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NA; ++s) { mbar_init(fullA(s), 1); mbar_init(emptyA(s), 1); mbar_init(pfull(s), 1); }
-        for (int s = 0; s < NB; ++s) { mbar_init(fullB(s), 1); mbar_init(emptyB(s), 1); }
-        for (int h = 0; h < 2; ++h) { mbar_init(tfull_bar(h), 1); mbar_init(tempty_bar(h), 2); }
+        for (int s = 0; s < PAIR_MAX_STAGES; ++s) {
+            mbar_init(full_bar(s), rank == 0 ? 2 : 1);            // leader: own producer + the peer's relay
+            mbar_init(empty_bar(s), 1);
+        }
+        for (int q = 0; q < PAIR_TQ; ++q) { mbar_init(tfull_bar(q), 1); mbar_init(tempty_bar(q), 2); }
         fence_barrier_init();
     }
     if (warp == 1) tmem_alloc2(smem_u32((const void*)tmem_slot), 512);
@@ -188,73 +243,94 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
     const int W = MODE == 1 ? a.sched->W1 : a.sched->W2;
     const int wi0 = (int)cluster_id_x(), wstep = (int)cluster_count_x();
     const uint8_t* dn = a.packed + gu_bytes(D);
+    auto a_src = [&](const PairItem& it, size_t& stride) -> const uint8_t* {
+        if (MODE == 1) { stride = WT_BYTES; return a.packed + gu_tile_index(D, it.e, it.blk, 0) * WT_BYTES; }
+        stride = (size_t)D.nDB * WT_BYTES;
+        return dn + dn_tile_index(D, it.e, 0, it.blk) * WT_BYTES;
+    };
 
     if (warp == 0) {
-        // ===================================================== weight producer (both CTAs): this CTA's 16 KB A tiles
-        if (lane == 0) {
-            int sa = 0;
-            uint32_t pa = 0;
-            for (int wi = wi0; wi < W; wi += wstep) {
-                const PairItem it = pair_item<MODE>(a, wi, rank);
-                const uint8_t* asrc;
-                size_t astride;
-                if (MODE == 1) {
-                    asrc = a.packed + gu_tile_index(D, it.e, it.blk, 0) * WT_BYTES;
-                    astride = WT_BYTES;
-                } else {
-                    asrc = dn + dn_tile_index(D, it.e, 0, it.blk) * WT_BYTES;
-                    astride = (size_t)D.nDB * WT_BYTES;
+        // ===================================================== producer (both CTAs): weight tile + token half per k-block
+        const bool leader_lane = elect_one();
+        int s = 0;
+        uint32_t ph = 0;
+        const size_t bstride = (size_t)a.P * ROW_BYTES;
+        // L2 prefetch cursor over the same weight-tile sequence, PAIR_PF tiles ahead
+        int pf_wi = wi0, pf_kb = 0, pf_nk = 0;
+        const uint8_t* pf_src = nullptr;
+        size_t pf_stride = 0;
+        auto pf_load_item = [&]() {
+            if (pf_wi < W) {
+                const PairItem pit = pair_item<MODE>(a, pf_wi, rank);
+                pf_src = a_src(pit, pf_stride);
+                pf_nk = pit.nk;
+            }
+        };
+        auto pf_step = [&]() {
+            if (pf_wi >= W) return;
+            if (leader_lane) bulk_prefetch_l2(pf_src + pf_kb * pf_stride, WT_BYTES);
+            if (++pf_kb == pf_nk) { pf_kb = 0; pf_wi += wstep; pf_load_item(); }
+        };
+        pf_load_item();
+        for (int i = 0; i < PAIR_PF; ++i) pf_step();
+        for (int wi = wi0; wi < W; wi += wstep) {
+            const PairItem it = pair_item<MODE>(a, wi, rank);
+            size_t astride;
+            const uint8_t* asrc = a_src(it, astride);
+            const uint32_t h0 = (uint32_t)it.n0 >> 1, h1 = (uint32_t)it.n1 >> 1;      // rows of each sub-tile this CTA holds
+            const uint8_t* b0 = a.Bsrc + (size_t)(it.row0 + rank * h0) * ROW_BYTES;
+            const uint8_t* b1 = a.Bsrc + (size_t)(it.row0 + it.n0 + rank * h1) * ROW_BYTES;
+            const uint32_t tx = WT_BYTES + (h0 + h1) * ROW_BYTES;
+            for (int kb = 0; kb < it.nk; ++kb) {
+                mbar_wait(empty_bar(s), ph ^ 1u, a.state);
+                if (leader_lane) {
+                    const uint32_t sb = smem_base + s * stage_bytes;
+                    mbar_expect_tx(full_bar(s), tx);
+                    bulk_g2s(sb, asrc + kb * astride, WT_BYTES, full_bar(s));
+                    bulk_g2s(sb + WT_BYTES, b0 + kb * bstride, h0 * ROW_BYTES, full_bar(s));
+                    if (h1) bulk_g2s(sb + WT_BYTES + h0 * ROW_BYTES, b1 + kb * bstride, h1 * ROW_BYTES, full_bar(s));
                 }
-                for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(emptyA(sa), pa ^ 1u, a.state);
-                    mbar_expect_tx(fullA(sa), WT_BYTES);
-                    bulk_g2s(smem_base + PAIR_A_OFF + sa * WT_BYTES, asrc + kb * astride, WT_BYTES, fullA(sa));
-                    if (++sa == NA) { sa = 0; pa ^= 1u; }
-                }
+                pf_step();
+                if (++s == NS) { s = 0; ph ^= 1u; }
             }
         }
-    } else if (warp == 2) {
-        // ===================================================== token producer (both CTAs): this CTA's half of each sub-tile
-        if (lane == 0) {
-            int sb = 0;
-            uint32_t pb = 0;
-            const size_t bstride = (size_t)a.P * ROW_BYTES;
-            for (int wi = wi0; wi < W; wi += wstep) {
-                const PairItem it = pair_item<MODE>(a, wi, rank);
-                const uint32_t h0 = (uint32_t)it.n0 >> 1, h1 = (uint32_t)it.n1 >> 1;      // rows of each sub-tile this CTA holds
-                const uint8_t* b0 = a.Bsrc + (size_t)(it.row0 + rank * h0) * ROW_BYTES;
-                const uint8_t* b1 = a.Bsrc + (size_t)(it.row0 + PAIR_NSUB + rank * h1) * ROW_BYTES;
-                for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(emptyB(sb), pb ^ 1u, a.state);
-                    const uint32_t sbase = smem_base + PAIR_B_OFF + sb * PAIR_BSLOT;
-                    mbar_expect_tx(fullB(sb), (h0 + h1) * ROW_BYTES);
-                    bulk_g2s(sbase, b0 + kb * bstride, h0 * ROW_BYTES, fullB(sb));
-                    if (h1) bulk_g2s(sbase + PAIR_BHALF, b1 + kb * bstride, h1 * ROW_BYTES, fullB(sb));
-                    if (++sb == NB) { sb = 0; pb ^= 1u; }
-                }
+    } else if (warp == 1 && rank != 0) {
+        // ===================================================== relay (peer CTA): "my half of this k-block has landed"
+        const bool leader_lane = elect_one();
+        int s = 0;
+        uint32_t ph = 0;
+        for (int wi = wi0; wi < W; wi += wstep) {
+            const PairItem it = pair_item<MODE>(a, wi, rank);
+            for (int kb = 0; kb < it.nk; ++kb) {
+                mbar_wait(full_bar(s), ph, a.state);
+                if (leader_lane) mbar_arrive_remote(full_bar(s), 0);
+                if (++s == NS) { s = 0; ph ^= 1u; }
             }
         }
     } else if (warp == 1) {
-        if (lane == 0 && rank == 0) {
-            // ================================================= MMA issuer (leader CTA): one thread issues for the pair
-            int sa = 0, sb = 0;
-            uint32_t pa = 0, pb = 0, sc = 0;
-            for (int wi = wi0; wi < W; wi += wstep) {
-                const PairItem it = pair_item<MODE>(a, wi, rank);
-                const uint32_t hA = sc & 1u, hB = (sc + 1u) & 1u;
-                mbar_wait(tempty_bar(hA), ((sc >> 1) & 1u) ^ 1u, a.state);
-                if (it.n1) mbar_wait(tempty_bar(hB), (((sc + 1u) >> 1) & 1u) ^ 1u, a.state);
+        // ===================================================== MMA issuer (leader CTA): one elected lane issues for the pair
+        const bool leader_lane = elect_one();
+        TmemRing ring;
+        ring.init();
+        int s = 0;
+        uint32_t ph = 0, drained = 0;
+        for (int wi = wi0; wi < W; wi += wstep) {
+            const PairItem it = pair_item<MODE>(a, wi, rank);
+            uint32_t c0, c1, need;
+            const uint32_t q0 = ring.seq;
+            ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, c0, c1, need);
+            for (; drained < need; ++drained) mbar_wait(tempty_bar(drained), (drained / PAIR_TQ) & 1u, a.state);
+            tc_fence_after();
+            const uint32_t d0 = tmem_base + c0, d1 = tmem_base + c1;
+            const uint32_t id0 = make_idesc2((uint32_t)it.n0), id1 = make_idesc2((uint32_t)(it.n1 ? it.n1 : 16));
+            const uint32_t boff1 = WT_BYTES + ((uint32_t)it.n0 >> 1) * ROW_BYTES;
+            for (int kb = 0; kb < it.nk; ++kb) {
+                mbar_wait(full_bar(s), ph, a.state);                 // both halves of this k-block (own producer + relay)
                 tc_fence_after();
-                const uint32_t d0 = tmem_base + hA * PAIR_NSUB, d1 = tmem_base + hB * PAIR_NSUB;
-                const uint32_t id0 = make_idesc2((uint32_t)it.n0), id1 = make_idesc2((uint32_t)(it.n1 ? it.n1 : 16));
-                for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(fullA(sa), pa, a.state);
-                    mbar_wait(fullB(sb), pb, a.state);
-                    mbar_wait(pfull(sa), pa, a.state);          // the peer CTA's halves of this k-block
-                    tc_fence_after();
-                    const uint32_t sB = smem_base + PAIR_B_OFF + sb * PAIR_BSLOT;
-                    const uint64_t adesc = make_desc_sw128(smem_base + PAIR_A_OFF + sa * WT_BYTES);
-                    const uint64_t bd0 = make_desc_sw128(sB), bd1 = make_desc_sw128(sB + PAIR_BHALF);
+                if (leader_lane) {
+                    const uint32_t sb = smem_base + s * stage_bytes;
+                    const uint64_t adesc = make_desc_sw128(sb);
+                    const uint64_t bd0 = make_desc_sw128(sb + WT_BYTES), bd1 = make_desc_sw128(sb + boff1);
 #pragma unroll
                     for (int kk = 0; kk < KB / 16; ++kk)
                         umma2_bf16(d0, adesc + 2u * kk, bd0 + 2u * kk, id0, (uint32_t)((kb | kk) != 0));
@@ -263,106 +339,116 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
                         for (int kk = 0; kk < KB / 16; ++kk)
                             umma2_bf16(d1, adesc + 2u * kk, bd1 + 2u * kk, id1, (uint32_t)((kb | kk) != 0));
                     }
-                    umma2_commit_mc(emptyA(sa));                // frees the slots in BOTH CTAs when these MMAs retire
-                    umma2_commit_mc(emptyB(sb));
-                    if (++sa == NA) { sa = 0; pa ^= 1u; }
-                    if (++sb == NB) { sb = 0; pb ^= 1u; }
+                    umma2_commit_mc(empty_bar(s));                    // frees the stage in BOTH CTAs when these MMAs retire
                 }
-                umma2_commit_mc(tfull_bar(hA));
-                if (it.n1) umma2_commit_mc(tfull_bar(hB));
-                sc += it.n1 ? 2u : 1u;
+                __syncwarp();
+                if (++s == NS) { s = 0; ph ^= 1u; }
             }
-        } else if (lane == 0) {
-            // ================================================= relay (peer CTA): my operands of this k-block have landed
-            int sa = 0, sb = 0;
-            uint32_t pa = 0, pb = 0;
-            for (int wi = wi0; wi < W; wi += wstep) {
-                const PairItem it = pair_item<MODE>(a, wi, rank);
-                for (int kb = 0; kb < it.nk; ++kb) {
-                    mbar_wait(fullA(sa), pa, a.state);
-                    mbar_wait(fullB(sb), pb, a.state);
-                    mbar_arrive_remote(pfull(sa), 0);
-                    if (++sa == NA) { sa = 0; pa ^= 1u; }
-                    if (++sb == NB) { sb = 0; pb ^= 1u; }
-                }
+            if (leader_lane) {
+                umma2_commit_mc(tfull_bar(q0));
+                if (it.n1) umma2_commit_mc(tfull_bar(q0 + 1));
             }
+            __syncwarp();
         }
     } else if (warp >= 4) {
         // ===================================================== epilogue warps 4..11 (both CTAs, own TMEM lanes)
+        // A sub-tile is drained in CHUNKS of CH token columns: TMEM -> registers -> (SwiGLU | round) -> a 16 KB staging
+        // buffer in the FINAL global layout -> one bulk store per chunk.  Two staging buffers alternate.
+        constexpr int CH = MODE == 1 ? 128 : 64;                // tokens per chunk: 128 x 128 B (H rows) or 64 x 256 B (O rows)
+        constexpr int ROWB = MODE == 1 ? ROW_BYTES : 2 * WT_ROWS;   // bytes per token row of this CTA's output
         const int q = warp & 3;                                // TMEM lane quadrant this warp may read
-        const int grp = (warp - 4) >> 2;                       // which half of the columns
+        const int grp = (warp - 4) >> 2;                       // which half of a chunk's 16-column groups
         const int et = threadIdx.x - 128;
-        const int dpad = D.nDB * WT_ROWS;
-        uint32_t sc = 0;
+        TmemRing ring;
+        ring.init();
+        uint32_t nchunk = 0;
         for (int wi = wi0; wi < W; wi += wstep) {
             const PairItem it = pair_item<MODE>(a, wi, rank);
             const int nsub = it.n1 ? 2 : 1;
-            for (int s = 0; s < nsub; ++s, ++sc) {
-                const uint32_t h = sc & 1u;
-                const int n = s ? it.n1 : it.n0;
-                const int split = ((n >> 4) + 1) / 2 * 16;    // columns [0, split) -> group 0, [split, n) -> group 1
-                const int cbeg = grp ? split : 0, cend = grp ? n : split;
-                const int rowS = it.row0 + s * PAIR_NSUB;
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + h * PAIR_NSUB;
-                mbar_wait(tfull_bar(h), (sc >> 1) & 1u, a.state);
+            uint32_t cc0, cc1, need_unused;
+            const uint32_t sq0 = ring.seq;
+            ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, cc0, cc1, need_unused);
+            for (int sidx = 0; sidx < nsub; ++sidx) {
+                const int n = sidx ? it.n1 : it.n0;
+                const uint32_t col0 = sidx ? cc1 : cc0;
+                const uint32_t sq = sq0 + sidx;
+                const int rowS = it.row0 + (sidx ? it.n0 : 0);
+                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + col0;
+                mbar_wait(tfull_bar(sq), (sq / PAIR_TQ) & 1u, a.state);
                 tc_fence_after();
-                if (it.valid && cbeg < cend) {
-                    // two register buffers: the TMEM load of the next 16 columns is in flight while these are processed
-                    uint32_t va[16], vb[16];
-                    if (MODE == 1) {
-                        const int ch = q * 16 + (lane & 15);
-                        const bool keep = it.blk * CB + ch < it.r;       // tail mask of the last retained block (pad-zero rule)
-                        const int odd = lane >> 4;
-                        uint8_t* hrow = a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES;
-                        auto swiglu16 = [&](const uint32_t (&v)[16], int c0) {
+                for (int ch0 = 0; ch0 < n; ch0 += CH, ++nchunk) {
+                    const int rows = min(CH, n - ch0);
+                    uint8_t* stg = stg_gen + (nchunk & 1u) * 16384u;
+                    const int ngrp = rows >> 4;                          // 16-column groups in this chunk
+                    const int gbeg = grp ? (ngrp + 1) >> 1 : 0, gend = grp ? ngrp : (ngrp + 1) >> 1;
+                    if (it.valid && gbeg < gend) {
+                        uint32_t va[16], vb[16];
+                        if (MODE == 1) {
+                            const int chn = q * 16 + (lane & 15);
+                            const bool keep = it.blk * CB + chn < it.r;       // tail mask of the last retained block (pad-zero rule)
+                            const int odd = lane >> 4;
+                            auto swiglu16 = [&](const uint32_t (&v)[16], int t0) {
 #pragma unroll
-                            for (int m = 0; m < 8; ++m) {
-                                const float mine0 = __uint_as_float(v[2 * m]), mine1 = __uint_as_float(v[2 * m + 1]);
-                                const float send = odd ? mine0 : mine1;                    // what the twin lane needs
-                                const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
-                                const float g = odd ? recv : mine0;                        // gate lives in lanes 0-15
-                                const float u = odd ? mine1 : recv;                        // up lives in lanes 16-31
-                                float hv = __fdividef(g, 1.f + __expf(-g)) * u;
-                                if (!keep) hv = 0.f;
-                                const uint32_t t = c0 + 2 * m + odd;                       // 16 lanes -> one full 32-byte sector
-                                *(__nv_bfloat16*)(hrow + sw128_off(t, ch)) = __float2bfloat16_rn(hv);
+                                for (int m = 0; m < 8; ++m) {
+                                    const float mine0 = __uint_as_float(v[2 * m]), mine1 = __uint_as_float(v[2 * m + 1]);
+                                    const float send = odd ? mine0 : mine1;                    // what the twin lane needs
+                                    const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
+                                    const float g = odd ? recv : mine0;                        // gate lives in lanes 0-15
+                                    const float u = odd ? mine1 : recv;                        // up lives in lanes 16-31
+                                    float hv = __fdividef(g, 1.f + __expf(-g)) * u;
+                                    if (!keep) hv = 0.f;
+                                    const uint32_t t = t0 + 2 * m + odd;                       // token row inside the chunk
+                                    *(__nv_bfloat16*)(stg + sw128_off(t, chn)) = __float2bfloat16_rn(hv);
+                                }
+                            };
+                            tmem_ld16(taddr + ch0 + gbeg * 16, va);
+                            for (int g = gbeg; g < gend; g += 2) {
+                                tmem_ld_wait();
+                                if (g + 1 < gend) tmem_ld16(taddr + ch0 + (g + 1) * 16, vb);
+                                swiglu16(va, g * 16);
+                                tmem_ld_wait();
+                                if (g + 2 < gend) tmem_ld16(taddr + ch0 + (g + 2) * 16, va);
+                                if (g + 1 < gend) swiglu16(vb, (g + 1) * 16);
                             }
-                        };
-                        tmem_ld16(taddr + cbeg, va);
-                        for (int c0 = cbeg; c0 < cend; c0 += 32) {
-                            tmem_ld_wait();
-                            if (c0 + 16 < cend) tmem_ld16(taddr + c0 + 16, vb);
-                            swiglu16(va, c0);
-                            tmem_ld_wait();
-                            if (c0 + 32 < cend) tmem_ld16(taddr + c0 + 32, va);
-                            if (c0 + 16 < cend) swiglu16(vb, c0 + 16);
-                        }
-                    } else {
-                        // lane = output feature; 16 token columns per load; 32 lanes -> 64 contiguous bytes of one O row
-                        uint8_t* dst = a.O + ((size_t)rowS * dpad + it.blk * WT_ROWS + q * 32 + lane) * 2;
-                        auto store16 = [&](const uint32_t (&v)[16], int c0) {
+                        } else {
+                            // lane = output feature; 16 token columns per load; 32 lanes -> 64 contiguous bytes of one O row
+                            uint8_t* dst = stg + (q * 32 + lane) * 2;
+                            auto store16 = [&](const uint32_t (&v)[16], int t0) {
 #pragma unroll
-                            for (int jj = 0; jj < 16; ++jj)
-                                *(__nv_bfloat16*)(dst + (size_t)(c0 + jj) * dpad * 2) = __float2bfloat16_rn(__uint_as_float(v[jj]));
-                        };
-                        tmem_ld16(taddr + cbeg, va);
-                        for (int c0 = cbeg; c0 < cend; c0 += 32) {
-                            tmem_ld_wait();
-                            if (c0 + 16 < cend) tmem_ld16(taddr + c0 + 16, vb);
-                            store16(va, c0);
-                            tmem_ld_wait();
-                            if (c0 + 32 < cend) tmem_ld16(taddr + c0 + 32, va);
-                            if (c0 + 16 < cend) store16(vb, c0 + 16);
+                                for (int jj = 0; jj < 16; ++jj)
+                                    *(__nv_bfloat16*)(dst + (t0 + jj) * ROWB) = __float2bfloat16_rn(__uint_as_float(v[jj]));
+                            };
+                            tmem_ld16(taddr + ch0 + gbeg * 16, va);
+                            for (int g = gbeg; g < gend; g += 2) {
+                                tmem_ld_wait();
+                                if (g + 1 < gend) tmem_ld16(taddr + ch0 + (g + 1) * 16, vb);
+                                store16(va, g * 16);
+                                tmem_ld_wait();
+                                if (g + 2 < gend) tmem_ld16(taddr + ch0 + (g + 2) * 16, va);
+                                if (g + 1 < gend) store16(vb, (g + 1) * 16);
+                            }
+                        }
+                    }
+                    const bool last = ch0 + CH >= n;
+                    fence_proxy_async_smem();                      // staging writes -> visible to the bulk-copy engine
+                    if (last) tc_fence_before();
+                    if (et == 0) bulk_wait_read0();                // the previous chunk's store has left the OTHER buffer
+                    epi_bar_sync256();
+                    if (et == 0) {
+                        if (it.valid) {
+                            uint8_t* gdst = MODE == 1 ? a.H + ((size_t)it.blk * a.P + rowS + ch0) * ROW_BYTES
+                                                      : a.O + ((size_t)it.blk * a.P + rowS + ch0) * ROWB;
+                            bulk_s2g(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROWB);
+                            bulk_commit();
+                        }
+                        if (last) {                                // all 8 warps have drained this sub-tile's columns
+                            if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
                         }
                     }
                 }
-                tc_fence_before();
-                epi_bar_sync256();                             // all 8 warps have drained this half of TMEM
-                if (et == 0) {
-                    if (rank == 0) mbar_arrive(tempty_bar(h)); else mbar_arrive_remote(tempty_bar(h), 0);
-                }
             }
         }
+        if (et == 0) bulk_wait0();
     }
 
     tc_fence_before();

@@ -32,6 +32,9 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     return v;
 }
 
+// balanced split of np padded rows into nt tiles: rows per tile, a multiple of 16
+__device__ __forceinline__ int per_rows(int np, int nt) { return ((np + nt - 1) / nt + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN; }
+
 // per-warp histogram of the block's chunk; warp w owns the contiguous sub-range [wlo, whi)
 __device__ __forceinline__ bool block_histogram(const int* __restrict__ ids, int E, int wlo, int whi, int lane,
                                                 int* __restrict__ wh /* this warp's [MAX_E] row */) {
@@ -126,7 +129,7 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
 
     // ---- warp 0: scans over experts -> offsets, padded offsets, token tiles, work prefixes
     if (w == 0) {
-        int c_off = 0, c_poff = 0, c_tiles = 0, c_work = 0;
+        int c_off = 0, c_poff = 0, c_tiles = 0, c_work = 0, c_max = ROW_ALIGN;
         for (int base = 0; base < E; base += 32) {
             const int e = base + lane;
             const int n = e < E ? s_cnt[e] : 0;
@@ -142,9 +145,15 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
                 int j = c_tiles + i_tiles - nt, wk = c_work + i_work - nt * nb;
                 const int p0 = c_poff + i_poff - np;
                 // balanced split of the padded segment into nt tiles of <= tile_n rows, each a multiple of 16 rows
-                const int per = nt > 0 ? ((np + nt - 1) / nt + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN : 0;
+                const int per = nt > 0 ? per_rows(np, nt) : 0;
                 for (int row = 0; row < np && nt > 0; row += per, ++j, wk += nb)
                     tt[j] = make_int4(e, p0 + row, min(per, n - row), wk);      // .z = valid rows of the tile (>= 1)
+            }
+            {
+                int mx = nt > 0 ? min(per_rows(np, nt), np) : 0;          // rows of this expert's widest tile
+#pragma unroll
+                for (int o = 16; o; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+                c_max = max(c_max, mx);
             }
             c_off += __shfl_sync(0xffffffffu, i_off, 31);
             c_poff += __shfl_sync(0xffffffffu, i_poff, 31);
@@ -160,6 +169,7 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
             sched->W2 = c_tiles * ((D.nDB + grp - 1) / grp);
             sched->P_used = c_poff;
             sched->A = A;
+            sched->max_n = c_max;
             state->ticket = 0;                               // ready for the next call on this layer
         }
     }

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, const uint8_t* __res
 #pragma unroll
             for (int q = 0; q < SIMT_TOK; ++q) {
                 if (t0 + q < nvalid && i < D.d)
-                    *(__nv_bfloat16*)(O + ((size_t)(row0 + t0 + q) * D.nDB * WT_ROWS + i) * 2) = __float2bfloat16_rn(acc[q]);
+                    *(__nv_bfloat16*)(O + o_off(P, row0 + t0 + q, i)) = __float2bfloat16_rn(acc[q]);
             }
         }
     }

@@ -191,15 +191,14 @@ __global__ void __launch_bounds__(192, 1) k_gemm_sm100(const GemmArgs a) {
                 epi_bar_sync();
             } else {
                 // lane = output feature; 16 token columns per load; 32 lanes -> 64 contiguous bytes of one O row
-                const int dpad = D.nDB * WT_ROWS;
-                uint8_t* dst = a.O + ((size_t)row0 * dpad + (wi % D.nDB) * WT_ROWS + q * 32 + lane) * 2;
+                uint8_t* dst = a.O + o_off(a.P, row0, (wi % D.nDB) * WT_ROWS + q * 32 + lane);
                 for (int c0 = 0; c0 < n; c0 += 16) {
                     uint32_t v[16];
                     tmem_ld16(taddr + c0, v);
                     tmem_ld_wait();
 #pragma unroll
                     for (int jj = 0; jj < 16; ++jj)
-                        *(__nv_bfloat16*)(dst + (size_t)(c0 + jj) * dpad * 2) = __float2bfloat16_rn(__uint_as_float(v[jj]));
+                        *(__nv_bfloat16*)(dst + (size_t)(c0 + jj) * (2 * WT_ROWS)) = __float2bfloat16_rn(__uint_as_float(v[jj]));
                 }
                 tc_fence_before();
                 mbar_arrive(tempty_bar(as));

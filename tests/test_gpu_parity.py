@@ -145,7 +145,7 @@ def test_multi_tile_ragged_segments(impl, tile_n):
     gu.check_close(gu.run_ffn(L, b, r, impl=impl, tile_n=tile_n), gu.oracle_ffn(lay, b, r), f"impl={impl} tile_n={tile_n}")
 
 
-@pytest.mark.parametrize("T", [130, 273, 300, 520, 1100])
+@pytest.mark.parametrize("T", [130, 273, 300, 512, 520, 1024, 1100, 2048, 4001])
 def test_pair_subtile_boundaries(T):
     """CTA-pair path: one expert receives every token, so its segment is T rows: <=256 (one sub-tile), 257..512
     (two sub-tiles sharing the weight operand), >512 (several token tiles); odd retained-block counts give the
