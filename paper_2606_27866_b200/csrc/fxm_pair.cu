@@ -28,14 +28,15 @@
 //     panels make a CTA's output of a sub-tile one contiguous range);
 //   * an L2 prefetch cursor runs ahead of the weight loads so the ring refills at L2 latency.
 //
-// Warp roles (384 threads per CTA): warp 0 = producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA),
-// warps 4-11 = epilogue (each CTA drains its own TMEM lanes; two warps per lane quadrant).
+// Warp roles (640 threads per CTA): warp 0 = producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA),
+// warps 4-19 = epilogue (each CTA drains its own TMEM lanes; four warps per lane quadrant).
 #include "fxm_ptx.cuh"
 
 namespace fxm {
 
 constexpr int PAIR_NSUB = 256;                  // most tokens per sub-tile (UMMA N max)
-constexpr int PAIR_THREADS = 384;
+constexpr int PAIR_EPI_WARPS = 16;              // epilogue warps: 4 per TMEM lane quadrant (the SwiGLU epilogue is issue-bound)
+constexpr int PAIR_THREADS = 128 + 32 * PAIR_EPI_WARPS;
 constexpr int PAIR_MAX_STAGES = 8;
 constexpr int PAIR_STAGING = 2 * 16384;         // two 16 KB epilogue staging buffers
 constexpr int PAIR_SMEM = 232448;               // 227 KB: everything a CTA can have
@@ -124,8 +125,22 @@ __device__ __forceinline__ void umma2_commit_mc(uint32_t bar) {
 __device__ __forceinline__ uint32_t make_idesc2(uint32_t n) {     // M = 256 (pair), N = n
     return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((256u >> 4) << 24);
 }
-__device__ __forceinline__ void epi_bar_sync256() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+__device__ __forceinline__ void epi_bar_sync_all() { asm volatile("bar.sync 1, %0;" ::"n"(32 * PAIR_EPI_WARPS) : "memory"); }
 __device__ __forceinline__ int shfl0(int v) { return __shfl_sync(0xffffffffu, v, 0); }   // also tells the compiler: warp-uniform
+
+// ------------------------------------------------------------------------------------------------ timeline
+// -DFXM_TRACE: the leader CTA of every cluster records clock64() stamps of its first 16 items (tuning aid; the
+// product build has none of this).  Fields: 0 item start (MMA warp), 1 accumulator columns free, 2 main loop done,
+// 3 cycles spent waiting for full stages, 4 epilogue sees the first sub-tile, 5 epilogue done, 6 producer cycles
+// spent waiting for empty stages, 7 tokens, 8 k-blocks.
+#ifdef FXM_TRACE
+__device__ long long g_trace[2][74][16][10];
+#define FXM_TR(mode, j, f, v) do { if ((j) < 16 && cluster_id_x() < 74u) g_trace[(mode) - 1][cluster_id_x()][(j)][(f)] = (long long)(v); } while (0)
+#define FXM_CLK() clock64()
+#else
+#define FXM_TR(mode, j, f, v) do { } while (0)
+#define FXM_CLK() 0ll
+#endif
 
 // ------------------------------------------------------------------------------------------------ items
 struct PairItem {
@@ -255,7 +270,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
         int s = 0;
         uint32_t ph = 0;
         const size_t bstride = (size_t)a.P * ROW_BYTES;
-        // L2 prefetch cursor over the same weight-tile sequence, PAIR_PF tiles ahead
+        // L2 prefetch cursor over the same weight-tile sequence, PAIR_PF tiles ahead (prefetching the token halves as
+        // well was measured and did not help: they are shared by the clusters of an expert and mostly hit L2)
         int pf_wi = wi0, pf_kb = 0, pf_nk = 0;
         const uint8_t* pf_src = nullptr;
         size_t pf_stride = 0;
@@ -273,8 +289,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
         };
         pf_load_item();
         for (int i = 0; i < PAIR_PF; ++i) pf_step();
-        for (int wi = wi0; wi < W; wi += wstep) {
+        int tj = 0;
+        for (int wi = wi0; wi < W; wi += wstep, ++tj) {
             const PairItem it = pair_item<MODE>(a, wi, rank);
+            long long tw = 0;
             size_t astride;
             const uint8_t* asrc = a_src(it, astride);
             const uint32_t h0 = (uint32_t)it.n0 >> 1, h1 = (uint32_t)it.n1 >> 1;      // rows of each sub-tile this CTA holds
@@ -282,7 +300,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
             const uint8_t* b1 = a.Bsrc + (size_t)(it.row0 + it.n0 + rank * h1) * ROW_BYTES;
             const uint32_t tx = WT_BYTES + (h0 + h1) * ROW_BYTES;
             for (int kb = 0; kb < it.nk; ++kb) {
+                const long long tw0 = FXM_CLK();
                 mbar_wait(empty_bar(s), ph ^ 1u, a.state);
+                tw += FXM_CLK() - tw0;
                 if (leader_lane) {
                     const uint32_t sb = smem_base + s * stage_bytes;
                     mbar_expect_tx(full_bar(s), tx);
@@ -293,6 +313,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
                 pf_step();
                 if (++s == NS) { s = 0; ph ^= 1u; }
             }
+            if (rank == 0 && leader_lane) FXM_TR(MODE, tj, 6, tw);
         }
     } else if (warp == 1 && rank != 0) {
         // ===================================================== relay (peer CTA): "my half of this k-block has landed"
@@ -314,18 +335,24 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
         ring.init();
         int s = 0;
         uint32_t ph = 0, drained = 0;
-        for (int wi = wi0; wi < W; wi += wstep) {
+        int tj = 0;
+        for (int wi = wi0; wi < W; wi += wstep, ++tj) {
             const PairItem it = pair_item<MODE>(a, wi, rank);
+            [[maybe_unused]] const long long t_start = FXM_CLK();
+            long long tw = 0;
             uint32_t c0, c1, need;
             const uint32_t q0 = ring.seq;
             ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, c0, c1, need);
             for (; drained < need; ++drained) mbar_wait(tempty_bar(drained), (drained / PAIR_TQ) & 1u, a.state);
             tc_fence_after();
+            [[maybe_unused]] const long long t_acc = FXM_CLK();
             const uint32_t d0 = tmem_base + c0, d1 = tmem_base + c1;
             const uint32_t id0 = make_idesc2((uint32_t)it.n0), id1 = make_idesc2((uint32_t)(it.n1 ? it.n1 : 16));
             const uint32_t boff1 = WT_BYTES + ((uint32_t)it.n0 >> 1) * ROW_BYTES;
             for (int kb = 0; kb < it.nk; ++kb) {
+                const long long tw0 = FXM_CLK();
                 mbar_wait(full_bar(s), ph, a.state);                 // both halves of this k-block (own producer + relay)
+                tw += FXM_CLK() - tw0;
                 tc_fence_after();
                 if (leader_lane) {
                     const uint32_t sb = smem_base + s * stage_bytes;
@@ -347,22 +374,26 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
             if (leader_lane) {
                 umma2_commit_mc(tfull_bar(q0));
                 if (it.n1) umma2_commit_mc(tfull_bar(q0 + 1));
+                FXM_TR(MODE, tj, 0, t_start); FXM_TR(MODE, tj, 1, t_acc); FXM_TR(MODE, tj, 2, FXM_CLK()); FXM_TR(MODE, tj, 3, tw);
+                FXM_TR(MODE, tj, 7, it.n0 + it.n1); FXM_TR(MODE, tj, 8, it.nk);
             }
             __syncwarp();
         }
     } else if (warp >= 4) {
-        // ===================================================== epilogue warps 4..11 (both CTAs, own TMEM lanes)
+        // ===================================================== epilogue warps 4..19 (both CTAs, own TMEM lanes)
         // A sub-tile is drained in CHUNKS of CH token columns: TMEM -> registers -> (SwiGLU | round) -> a 16 KB staging
         // buffer in the FINAL global layout -> one bulk store per chunk.  Two staging buffers alternate.
         constexpr int CH = MODE == 1 ? 128 : 64;                // tokens per chunk: 128 x 128 B (H rows) or 64 x 256 B (O rows)
         constexpr int ROWB = MODE == 1 ? ROW_BYTES : 2 * WT_ROWS;   // bytes per token row of this CTA's output
         const int q = warp & 3;                                // TMEM lane quadrant this warp may read
-        const int grp = (warp - 4) >> 2;                       // which half of a chunk's 16-column groups
+        constexpr int NWQ = PAIR_EPI_WARPS / 4;                // warps per lane quadrant
+        const int wq = (warp - 4) >> 2;                        // which share of a chunk's 16-column groups
         const int et = threadIdx.x - 128;
         TmemRing ring;
         ring.init();
         uint32_t nchunk = 0;
-        for (int wi = wi0; wi < W; wi += wstep) {
+        int tj = 0;
+        for (int wi = wi0; wi < W; wi += wstep, ++tj) {
             const PairItem it = pair_item<MODE>(a, wi, rank);
             const int nsub = it.n1 ? 2 : 1;
             uint32_t cc0, cc1, need_unused;
@@ -375,12 +406,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
                 const int rowS = it.row0 + (sidx ? it.n0 : 0);
                 const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + col0;
                 mbar_wait(tfull_bar(sq), (sq / PAIR_TQ) & 1u, a.state);
+                if (et == 0 && rank == 0 && sidx == 0) FXM_TR(MODE, tj, 4, FXM_CLK());
                 tc_fence_after();
                 for (int ch0 = 0; ch0 < n; ch0 += CH, ++nchunk) {
                     const int rows = min(CH, n - ch0);
                     uint8_t* stg = stg_gen + (nchunk & 1u) * 16384u;
                     const int ngrp = rows >> 4;                          // 16-column groups in this chunk
-                    const int gbeg = grp ? (ngrp + 1) >> 1 : 0, gend = grp ? ngrp : (ngrp + 1) >> 1;
+                    const int gbeg = ngrp * wq / NWQ, gend = ngrp * (wq + 1) / NWQ;
                     if (it.valid && gbeg < gend) {
                         uint32_t va[16], vb[16];
                         if (MODE == 1) {
@@ -433,7 +465,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
                     fence_proxy_async_smem();                      // staging writes -> visible to the bulk-copy engine
                     if (last) tc_fence_before();
                     if (et == 0) bulk_wait_read0();                // the previous chunk's store has left the OTHER buffer
-                    epi_bar_sync256();
+                    epi_bar_sync_all();
                     if (et == 0) {
                         if (it.valid) {
                             uint8_t* gdst = MODE == 1 ? a.H + ((size_t)it.blk * a.P + rowS + ch0) * ROW_BYTES
@@ -441,8 +473,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
                             bulk_s2g(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROWB);
                             bulk_commit();
                         }
-                        if (last) {                                // all 8 warps have drained this sub-tile's columns
+                        if (last) {                                // all epilogue warps have drained this sub-tile's columns
                             if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
+                            if (rank == 0 && sidx == nsub - 1) FXM_TR(MODE, tj, 5, FXM_CLK());
                         }
                     }
                 }
@@ -490,3 +523,7 @@ cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r
 }
 
 }  // namespace fxm
+
+#ifdef FXM_TRACE
+extern "C" int fxm_trace_read(void* dst) { return (int)cudaMemcpyFromSymbol(dst, fxm::g_trace, sizeof(fxm::g_trace)); }
+#endif
