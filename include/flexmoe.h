@@ -156,7 +156,7 @@ fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
  * its L2 prefetch cursor runs ahead of the shared-memory ring (0..256).  Tuning knob only: results agree within
  * the stated tolerance either way.  Needs d <= 3840, else the general path is used regardless. */
 #define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 768
-#define FXM_DECODE_DEFAULT_PREFETCH 8
+#define FXM_DECODE_DEFAULT_PREFETCH 0
 fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles);
 /* Synchronises `stream`, then returns the sticky device flag word (bit0: expert id out of range,
  * bit1: a pipeline wait timed out -- a bug) in *flags and clears it. */

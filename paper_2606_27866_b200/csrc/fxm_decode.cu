@@ -67,6 +67,7 @@ struct DecAux {
 struct DecTmp {
     int16_t ids[DEC_MAX_A];
     int cnt[MAX_E], off[MAX_E + 1], ibase[MAX_E + 1], gbase[MAX_E + 1];
+    int wh[DEC_THREADS / 32][MAX_E];   // per-warp expert histogram, then the warp's running base
     int first_run;
 };
 
@@ -74,26 +75,47 @@ __host__ __device__ inline int dec_fixed_smem(const Dims& D) {
     return 1024 + D.nKB1 * DEC_XE_KB_BYTES + 2 * DEC_XE_KB_BYTES + (int)((sizeof(DecAux) + 1023) / 1024 * 1024);
 }
 
+// one lane of a converged warp.  The asynchronous instructions (bulk copies, tcgen05.mma / commit) take their operands
+// from uniform registers: they are issued by ONE elected lane inside loops that all 32 lanes walk, so the compiler keeps
+// addresses and descriptors uniform (a `lane == 0` branch costs a register->uniform waterfall per instruction).
+__device__ __forceinline__ bool dec_elect_one() {
+    uint32_t p;
+    asm volatile(
+        "{\n\t.reg .pred q;\n\t"
+        "elect.sync _|q, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(p));
+    return p != 0;
+}
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
     uint32_t v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-// one thread per CTA, after the CTA's own work has been made visible with __threadfence()
+// Grid barrier, one thread per CTA (all CTAs are co-resident: cooperative launch).  Two levels, because 148 atomics on ONE
+// address serialise in L2 (measured: 10-20 us per barrier): CTA b arrives on sub-counter b % 8, the last arriver of a
+// sub-counter arrives on the top counter, the last of those bumps the generation word that everyone polls (it lives in
+// another 128-byte line than the counters).  Every counter is reset by its last arriver before the generation moves.
 __device__ __forceinline__ void grid_arrive(DevState* st, int i, uint32_t G) {
     __threadfence();
-    const uint32_t old = atomicAdd(&st->bar_count[i], 1u);
-    if (old == G - 1u) {
-        st->bar_count[i] = 0u;
+    const uint32_t grp = blockIdx.x & 7u;
+    const uint32_t gsize = (G - grp + 7u) >> 3;                       // CTAs with this residue
+    if (atomicAdd(&st->bar_sub[i][grp], 1u) == gsize - 1u) {
+        st->bar_sub[i][grp] = 0u;
         __threadfence();
-        atomicAdd(&st->bar_gen[i], 1u);
+        const uint32_t ngrp = G < 8u ? G : 8u;
+        if (atomicAdd(&st->bar_count[i], 1u) == ngrp - 1u) {
+            st->bar_count[i] = 0u;
+            __threadfence();
+            atomicAdd(&st->bar_gen[i], 1u);
+        }
     }
 }
 __device__ __forceinline__ void grid_wait(DevState* st, int i, uint32_t gen0) {
     const long long t0 = clock64();
     uint32_t spins = 0;
     while (ld_acquire_u32(&st->bar_gen[i]) == gen0) {
-        __nanosleep(64);
+        __nanosleep(1000);                                         // 148 pollers: keep the L2 slice of the barrier words quiet
         if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) {
             atomicOr(&st->flags, 2u);
             __threadfence_system();
@@ -117,45 +139,59 @@ struct ItemCur {
     }
 };
 
-// the sequence of weight tiles in issue order: G(0), G(1), D(0), G(2), D(1), ..., G(n-1), D(n-2), D(n-1)
-struct TileStream {
+// the weight stream in issue order, one PART at a time: G(0), G(1), D(0), G(2), D(1), ..., G(n-1), D(n-2), D(n-1).
+// A part is a contiguous range of 16 KB tiles: G(i) = the d/64 gate/up tiles of item i, D(i) = its ceil(d/128) down tiles.
+struct PartStream {
     const DecAux* ax;
     const uint8_t* gu;
     const uint8_t* dn;
     Dims D;
     ItemCur g, d;
     int i;            // step: the G part of item i, then the D part of item i-1
-    int part;         // 0 = G, 1 = D
-    int j;            // tile inside the part
+    int sub;          // 0 = G(i) comes next, 1 = D(i-1) comes next
     __device__ __forceinline__ void init(const DecAux* a, const DecArgs& args) {
         ax = a; D = args.D; gu = args.packed; dn = args.packed + gu_bytes(args.D);
         g.init(a); d.init(a);
-        i = 0; part = 0; j = 0;
-        if (a->n_items == 0) i = 1;            // nothing at all: done() is true
+        i = 0; sub = 0;
     }
-    __device__ __forceinline__ bool done() const { return i > ax->n_items; }
-    __device__ __forceinline__ const uint8_t* addr() const {
-        if (part == 0) return gu + (gu_tile_index(D, g.e(ax), g.cb, 0) + j) * WT_BYTES;
-        return dn + (dn_tile_index(D, d.e(ax), d.cb, 0) + j) * WT_BYTES;
-    }
-    __device__ __forceinline__ void next() {
-        ++j;
-        if (part == 0) {
-            if (j < D.nKB1) return;
-            j = 0;
-            g.next(ax);
-            if (i >= 1) { part = 1; return; }
-            ++i;                                // after G(0) comes G(1) (or D(0) if there is only one item)
-            if (i >= ax->n_items) part = 1;
-            return;
+    __device__ __forceinline__ bool next(const uint8_t*& base, int& count) {
+        const int n = ax->n_items;
+        while (n > 0 && i <= n) {
+            if (sub == 0) {
+                sub = 1;
+                if (i < n) {
+                    base = gu + gu_tile_index(D, g.e(ax), g.cb, 0) * WT_BYTES;
+                    count = D.nKB1;
+                    g.next(ax);
+                    return true;
+                }
+            }
+            sub = 0;
+            const int ii = i++;
+            if (ii >= 1) {
+                base = dn + dn_tile_index(D, d.e(ax), d.cb, 0) * WT_BYTES;
+                count = D.nDB;
+                d.next(ax);
+                return true;
+            }
         }
-        if (j < D.nDB) return;
-        j = 0;
-        d.next(ax);
-        ++i;
-        part = i < ax->n_items ? 0 : 1;
+        return false;
     }
 };
+
+// -DFXM_TRACE: per-CTA globaltimer stamps (ns): 0 entry, 1 prologue done, 2 roles done (this CTA's last reduction issued),
+// 3 grid barrier #1 passed, 4 exit.  Tuning aid only.
+#ifdef FXM_TRACE
+__device__ unsigned long long g_dtrace[148][8];
+__device__ __forceinline__ unsigned long long dec_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define DEC_TR(f) do { if (threadIdx.x == 0 && blockIdx.x < 148) g_dtrace[blockIdx.x][f] = dec_now(); } while (0)
+#else
+#define DEC_TR(f) do { } while (0)
+#endif
 
 __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -183,6 +219,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int E = D.E, A = a.A, k = a.k;
+    DEC_TR(0);
     const uint32_t G = gridDim.x;
 
     // ------------------------------------------------------------------------------------------ prologue
@@ -218,11 +255,31 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     if (tid == 0) grid_arrive(a.state, 0, G);
     const uint32_t tmem_base = ax->tmem_slot;
 
-    // counts: thread e scans the assignments (A <= 1024, broadcast reads)
-    if (tid < E) {
-        int c = 0;
-        for (int f = 0; f < A; ++f) c += (tp->ids[f] == tid);
-        tp->cnt[tid] = c;
+    // counts (Alg. 2 l.4-6, stable counting sort as in fxm_route.cu): warp w owns the contiguous chunk [w*chunk, (w+1)*chunk)
+    // of the flat assignments; per 32-wide step the lowest lane of every group of equal ids adds the group size to
+    // the warp's histogram row
+    constexpr int NW = DEC_THREADS / 32;
+    const int chunk = ((A + NW - 1) / NW + 31) & ~31;
+    const int wlo = min(A, warp * chunk), whi = min(A, wlo + chunk);
+    for (int i = tid; i < NW * MAX_E; i += DEC_THREADS) (&tp->wh[0][0])[i] = 0;
+    __syncthreads();
+    for (int base = wlo; base < whi; base += 32) {
+        const int f = base + lane;
+        const int id = f < whi ? (int)tp->ids[f] : -1;
+        const unsigned m = __match_any_sync(0xffffffffu, id);
+        if (id >= 0 && lane == __ffs(m) - 1) tp->wh[warp][id] += __popc(m);
+        __syncwarp();
+    }
+    __syncthreads();
+    if (tid < E) {                                                  // exclusive scan over the warps, per expert
+        int run = 0;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) {
+            const int c = tp->wh[w][tid];
+            tp->wh[w][tid] = run;
+            run += c;
+        }
+        tp->cnt[tid] = run;
     }
     __syncthreads();
     // warp 0: exclusive scans over experts: sorted offsets, item base, run base
@@ -258,11 +315,18 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     __syncthreads();
     const int W = ax->W;
     const int lo = (int)((long long)blockIdx.x * W / (long long)G), hi = (int)((long long)(blockIdx.x + 1) * W / (long long)G);
+    // stable positions (ascending flat index inside an expert, reading R5): expert offset + earlier warps + earlier
+    // steps of this warp + lower lanes of this step
+    for (int base = wlo; base < whi; base += 32) {
+        const int f = base + lane;
+        const int id = f < whi ? (int)tp->ids[f] : -1;
+        const unsigned m = __match_any_sync(0xffffffffu, id);
+        if (id >= 0) ax->perm[tp->off[id] + tp->wh[warp][id] + __popc(m & ((1u << lane) - 1u))] = (int16_t)f;
+        __syncwarp();
+        if (id >= 0 && lane == __ffs(m) - 1) tp->wh[warp][id] += __popc(m);
+        __syncwarp();
+    }
     if (tid < E) {
-        // stable positions (ascending flat index inside an expert), reading R5
-        int pos = tp->off[tid];
-        for (int f = 0; f < A; ++f)
-            if (tp->ids[f] == tid) ax->perm[pos++] = (int16_t)f;
         // the run that contains item `lo`
         const int r = ax->r[tid];
         const int nb = (r + CB - 1) / CB;
@@ -291,28 +355,48 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     fence_proxy_async_smem();
     __syncthreads();
     const int n_items = ax->n_items, n_runs = ax->n_runs;
+    DEC_TR(1);
 
     if (warp == 0) {
         // ===================================================== weight producer + L2 prefetch cursor
-        if (lane == 0 && n_items > 0) {
-            TileStream ld, pf;
+        // per tile: wait for the slot, arm the barrier, one 16 KB bulk copy; optionally one 16 KB L2 prefetch `pf` tiles
+        // further down the same stream (a second cursor).  Measured on B200: the prefetch competes with the ring's own
+        // loads for the SM's outstanding requests and every distance > 0 is slower (C4 T=64 0 %: 558 us at 0, 580 at 8,
+        // 978 at 64), so the default distance is 0.
+        if (n_items > 0) {
+            const bool el = dec_elect_one();
+            PartStream ld, pf;
             ld.init(ax, a);
             pf.init(ax, a);
-            for (int p = 0; p < a.pf && !pf.done(); ++p) { bulk_prefetch_l2(pf.addr(), WT_BYTES); pf.next(); }
+            const uint8_t* pb = nullptr;
+            int pc = 0, pj = 0;
+            bool pf_live = pf.next(pb, pc);
+            auto pf_step = [&]() {
+                if (!pf_live) return;
+                if (el) bulk_prefetch_l2(pb + (size_t)pj * WT_BYTES, WT_BYTES);
+                if (++pj == pc) { pj = 0; pf_live = pf.next(pb, pc); }
+            };
+            for (int p = 0; p < a.pf; ++p) pf_step();
             int stage = 0;
             uint32_t phase = 0;
-            while (!ld.done()) {
-                if (!pf.done()) { bulk_prefetch_l2(pf.addr(), WT_BYTES); pf.next(); }
-                mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
-                mbar_expect_tx(full_bar(stage), WT_BYTES);
-                bulk_g2s(ring_s + stage * WT_BYTES, ld.addr(), WT_BYTES, full_bar(stage));
-                ld.next();
-                if (++stage == NS) { stage = 0; phase ^= 1u; }
+            const uint8_t* base = nullptr;
+            int count = 0;
+            while (ld.next(base, count)) {
+                for (int j = 0; j < count; ++j) {
+                    if (a.pf > 0) pf_step();
+                    mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
+                    if (el) {
+                        mbar_expect_tx(full_bar(stage), WT_BYTES);
+                        bulk_g2s(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage));
+                    }
+                    if (++stage == NS) { stage = 0; phase ^= 1u; }
+                }
             }
         }
     } else if (warp == 1) {
         // ===================================================== MMA issuer
-        if (lane == 0 && n_items > 0) {
+        if (n_items > 0) {
+            const bool el = dec_elect_one();
             ItemCur g, d;
             g.init(ax); d.init(ax);
             int stage = 0;
@@ -328,16 +412,22 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     for (int kb = 0; kb < D.nKB1; ++kb) {
                         mbar_wait(full_bar(stage), phase, a.state);
                         tc_fence_after();
-                        const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
-                        const uint64_t bdesc = make_desc_sw128(smem_base + xe_off + (uint32_t)kb * DEC_XE_KB_BYTES);
+                        if (el) {
+                            const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
+                            const uint64_t bdesc = make_desc_sw128(smem_base + xe_off + (uint32_t)kb * DEC_XE_KB_BYTES);
 #pragma unroll
-                        for (int kk = 0; kk < KB / 16; ++kk)
-                            umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)((kb | kk) != 0));
-                        umma_commit(empty_bar(stage));
+                            for (int kk = 0; kk < KB / 16; ++kk)
+                                umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)((kb | kk) != 0));
+                            umma_commit(empty_bar(stage));
+                        }
+                        __syncwarp();
                         if (++stage == NS) { stage = 0; phase ^= 1u; }
                     }
-                    umma_commit(a1full(b));
-                    if (g.last(ax)) umma_commit(xempty);            // Xe may be restaged once these MMAs retire
+                    if (el) {
+                        umma_commit(a1full(b));
+                        if (g.last(ax)) umma_commit(xempty);        // Xe may be restaged once these MMAs retire
+                    }
+                    __syncwarp();
                     g.next(ax);
                 }
                 if (i >= 1) {                                       // ---- D(i-1): Y[db] += Wd(e, cb, db) . Hs[b]^T
@@ -350,16 +440,22 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     for (int db = 0; db < D.nDB; ++db) {
                         mbar_wait(full_bar(stage), phase, a.state);
                         tc_fence_after();
-                        const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
-                        const uint32_t d_tmem = tmem_base + 2u * DEC_N + (uint32_t)db * DEC_N;
+                        if (el) {
+                            const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
+                            const uint32_t d_tmem = tmem_base + 2u * DEC_N + (uint32_t)db * DEC_N;
 #pragma unroll
-                        for (int kk = 0; kk < KB / 16; ++kk)
-                            umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)(!first || kk != 0));
-                        umma_commit(empty_bar(stage));
+                            for (int kk = 0; kk < KB / 16; ++kk)
+                                umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)(!first || kk != 0));
+                            umma_commit(empty_bar(stage));
+                        }
+                        __syncwarp();
                         if (++stage == NS) { stage = 0; phase ^= 1u; }
                     }
-                    umma_commit(hempty(b));
-                    if (d.last(ax)) umma_commit(yfull);
+                    if (el) {
+                        umma_commit(hempty(b));
+                        if (d.last(ax)) umma_commit(yfull);
+                    }
+                    __syncwarp();
                     d.next(ax);
                 }
             }
@@ -471,15 +567,20 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     __threadfence();                                               // this thread's reductions are performed
     tc_fence_before();
     __syncthreads();
+    DEC_TR(2);
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, 512);
     }
     if (tid == 0) {
+        DEC_TR(5);
         grid_arrive(a.state, 1, G);
+        DEC_TR(6);
         grid_wait(a.state, 1, ax->gen0[1]);
+        DEC_TR(7);
     }
     __syncthreads();
+    DEC_TR(3);
     {
         const size_t n4 = (size_t)a.T * D.d / 4;
         const float4* src = (const float4*)a.yacc;
@@ -493,6 +594,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             dst[i] = o;
         }
     }
+    DEC_TR(4);
 }
 
 // ---------------------------------------------------------------------------------------------- host side
@@ -523,3 +625,7 @@ cudaError_t launch_decode(const Dims& D, const uint8_t* packed, const int* r_tab
 }
 
 }  // namespace fxm
+
+#ifdef FXM_TRACE
+extern "C" int fxm_dtrace_read(void* dst) { return (int)cudaMemcpyFromSymbol(dst, fxm::g_dtrace, sizeof(fxm::g_dtrace)); }
+#endif

@@ -65,9 +65,11 @@ __host__ __device__ inline size_t dn_bytes(const Dims& D) { return (size_t)D.E *
 struct DevState {           // lives at the tail of the packed blob (zeroed by pack)
     uint32_t flags;         // bit0: expert id out of range; bit1: pipeline wait timed out
     uint32_t ticket;        // route: blocks that have published their histogram (reset by the last one)
-    uint32_t bar_count[2];  // decode kernel: arrivals at grid barrier 0 / 1 (reset by the last arriver)
+    uint32_t bar_count[2];  // decode kernel: top-level arrivals at grid barrier 0 / 1 (reset by the last arriver)
+    uint32_t bar_sub[2][8]; // decode kernel: first-level arrivals, CTA b uses counter b % 8 (reset by their last arrivers)
+    uint32_t pad0[12];      // -> 128 bytes: the polled words below live in their own line
     uint32_t bar_gen[2];    // decode kernel: generation of grid barrier 0 / 1 (sense reversal; never reset)
-    uint32_t pad[58];
+    uint32_t pad1[30];
 };
 
 // ------------------------------------------------------------------------------------------------

@@ -120,7 +120,7 @@ def workspace_bytes_host(E: int, d: int, I: int, T_max: int, k: int) -> int:
 N_KERNELS = 7
 KERNEL_NAMES = ("route_plan", "scatter", "gather", "gemm1_swiglu", "gemm2", "combine", "decode_fused")
 DECODE_DEFAULT_MAX_ASSIGNMENTS = 768
-DECODE_DEFAULT_PREFETCH = 8
+DECODE_DEFAULT_PREFETCH = 0
 
 
 def ratio_to_width(I: int, num: int, den: int) -> int:
