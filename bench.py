@@ -207,9 +207,8 @@ def run_ours(args):
 
     sampler = ClockSampler(local)
     sampler.start()
-    # ---- timed region 1: K steps, inputs resident in HBM, per-kernel events recorded inside it
+    # ---- timed region 1: EXACTLY K steps, inputs resident in HBM, nothing but the calls between the two events
     barrier()
-    L.profile_begin(args.steps)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     w0 = time.perf_counter()
     e0.record(stream)
@@ -219,6 +218,13 @@ def run_ours(args):
     barrier()
     w1 = time.perf_counter()
     ms_total = e0.elapsed_time(e1)
+    # ---- the same K steps again with a CUDA event before every kernel (fxm_profile_begin/end): per-kernel device
+    #      times for the roofline of the dominant kernel.  The events cost ~2-3 us each, which is why this pass is not
+    #      the headline number.
+    L.profile_begin(args.steps)
+    for i in range(args.steps):
+        L.moe_ffn(*dev[i % NB], out=y)
+    barrier()
     kern_ms, n_prof = L.profile_end()
 
     # ---- timed region 2: end to end through fxm_moe_ffn_host (pinned host buffers, H2D + D2H inside)
@@ -381,7 +387,6 @@ def _time_calls(torch, L, dev, y, iters, warm, flush_buf):
     for i in range(warm):
         L.moe_ffn(*dev[i % len(dev)], out=y)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
-    L.profile_begin(iters)
     for i in range(iters):
         if flush_buf is not None:
             flush_buf.add_(1)
@@ -389,8 +394,14 @@ def _time_calls(torch, L, dev, y, iters, warm, flush_buf):
         L.moe_ffn(*dev[i % len(dev)], out=y)
         ev[i][1].record(st)
     torch.cuda.synchronize()
-    kern, n = L.profile_end()
     ms = np.array([a.elapsed_time(b) for a, b in ev])
+    # per-kernel times in a second pass: the per-kernel events cost 2-3 us each and must not sit inside `ms`
+    npk = min(iters, 20)
+    L.profile_begin(npk)
+    for i in range(npk):
+        L.moe_ffn(*dev[i % len(dev)], out=y)
+    torch.cuda.synchronize()
+    kern, n = L.profile_end()
     return ms, {kname: v / n for kname, v in kern.items()}
 
 
