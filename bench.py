@@ -29,6 +29,10 @@ import numpy as np
 
 METRIC = "routed_expert_ffn_tokens_per_s"
 UNIT = "tokens/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+# captures (profiles/r01b_README.md); keyed by (config, T, width, kernel).  --traffic overrides.
+NCU_TRAFFIC = {("C2", 4096, "704", "gemm1_swiglu"): 437.1e6, ("C2", 4096, "704", "gemm2"): 239.8e6,
+               ("C4", 64, "1280", "decode_fused"): 1776.6e6}
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 
 
@@ -151,6 +155,23 @@ def make_table(gen, sh, spec, rng):
     raise SystemExit(f"unknown table spec {spec!r}")
 
 
+def rank_seed0(rank: int) -> int:
+    """First batch seed of a rank: ranks are replicas of the layer that see disjoint seeded token batches."""
+    return 1000 * rank
+
+
+def aggregate(ms_list, T, steps, world, dist=None, device="cpu"):
+    """Whole-job numbers from per-rank device times: every timed region takes the MAX over ranks (all_reduce MAX
+    when `dist` is an initialised torch.distributed module), tokens are summed over ranks (weak scaling: T per rank).
+    Returns (list of max times in ms, total tokens)."""
+    if dist is not None and world > 1:
+        import torch
+        t = torch.tensor(list(ms_list), dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_list = [float(v) for v in t]
+    return list(ms_list), world * T * steps
+
+
 def host_batches(gen, cfg, T, n, seed0):
     """n seeded batches (x, ids, w) of a named config; batch i uses seed seed0+i."""
     out = []
@@ -182,7 +203,7 @@ def run_ours(args):
     peaks = load_peaks()
     NB = args.batches
     lay = gen.layer_for(cfg, 0)                      # same weights on every rank (replicas)
-    hb = host_batches(gen, cfg, T, NB, 1000 * rank)  # each rank its own tokens
+    hb = host_batches(gen, cfg, T, NB, rank_seed0(rank))  # each rank its own tokens
     r = make_table(gen, sh, args.r, hb[0][1])
     L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate), fx.bf16_from_bits(lay.W_up), fx.bf16_from_bits(lay.W_down),
                       lay.channel_rank)
@@ -245,12 +266,7 @@ def run_ours(args):
     sampler.stop()
     clocks = sampler.summary([(w0, w1), (w2, w3)])
 
-    if world > 1:
-        t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_e2e = float(t[0]), float(t[1])
-
-    tokens = world * T * args.steps
+    (ms_total, ms_e2e), tokens = aggregate([ms_total, ms_e2e], T, args.steps, world, dist if world > 1 else None, "cuda")
     value = tokens / (ms_total * 1e-3)
     e2e_value = tokens / (ms_e2e * 1e-3)
     wm = [work_model(b.topk_ids, r, sh.d, T, sh.k) for b, _ in hb]
@@ -269,7 +285,9 @@ def run_ours(args):
     else:
         achieved, peak, unit = kbytes / dur / 1e9, peaks["hbm_gbs"], "GB/s"
     roofline = {"bound": bound, "achieved": round(achieved, 2), "peak": peak, "unit": unit,
-                "frac": round(achieved / peak, 4), "traffic": args.traffic, "kernel": dom,
+                "frac": round(achieved / peak, 4),
+                "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC.get((cfg, T, str(args.r), dom)),
+                "kernel": dom,
                 "kernel_ms": round(per_launch_ms[dom], 5), "peak_source": peaks["source"] + ", burst figure",
                 "frac_of_sustained": round(achieved / peaks["bf16_tflops_sustained"], 4) if bound == "tensor" else None,
                 "algorithmic": {"flops": kflops, "bytes": kbytes}}
