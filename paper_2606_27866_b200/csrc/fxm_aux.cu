@@ -123,6 +123,8 @@ __global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __res
     __shared__ int s_p[MAX_K];
     __shared__ float s_w[MAX_K];
     const int t = blockIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
     if (threadIdx.x < k) {
         s_p[threadIdx.x] = prow[(size_t)t * k + threadIdx.x];
         s_w[threadIdx.x] = topk_w[(size_t)t * k + threadIdx.x];
@@ -164,8 +166,7 @@ __global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __res
 cudaError_t launch_combine(const Dims& D, int T, int k, const float* topk_w, const Workspace& ws, __nv_bfloat16* y,
                            cudaStream_t st) {
     if (T == 0) return cudaSuccess;
-    k_combine<<<T, 128, 0, st>>>(D, k, ws.prow, topk_w, ws.O, ws.P, (uint4*)y);
-    return cudaGetLastError();
+    return launch_pdl(k_combine, dim3(T), dim3(128), 0, st, D, k, (const int*)ws.prow, topk_w, (const uint8_t*)ws.O, ws.P, (uint4*)y);
 }
 
 // --------------------------------------------------------------------------------------------- read_h

@@ -154,6 +154,32 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
 }
 
 // ------------------------------------------------------------------------------------------------
+// Programmatic dependent launch: the kernels of one fxm_moe_ffn are launched with the programmatic-stream-serialization
+// attribute, call pdl_launch_dependents() first thing (the next kernel may be scheduled onto free SMs and run its
+// prologue) and pdl_wait() before their first access to global memory that an earlier kernel of the stream may still
+// be writing or reading (it returns once the preceding kernel has completed and flushed).  Every kernel of the chain
+// waits, so completion is transitive.  This hides the launch latency and the prologue of each of the six kernels.
+// ------------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+#endif
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Launchers (each enqueues on `st` and returns cudaGetLastError()).
 // ------------------------------------------------------------------------------------------------
 cudaError_t launch_pack(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,

@@ -236,12 +236,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
 
     const int warp = shfl0(threadIdx.x >> 5), lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
+    pdl_launch_dependents();
     const Dims& D = a.D;
-
-    // ring geometry of this call: a stage holds one 16 KB weight tile and this CTA's half of the widest token tile
-    const int max_n = a.sched->max_n;
-    const uint32_t stage_bytes = WT_BYTES + (((uint32_t)max_n * (ROW_BYTES / 2) + 1023u) & ~1023u);
-    const int NS = min(PAIR_MAX_STAGES, (int)(PAIR_RING_BYTES / stage_bytes));
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < PAIR_MAX_STAGES; ++s) {
@@ -257,6 +253,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
     cluster_sync_all();                                       // barriers of both CTAs are initialised before any remote use
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot;
+    pdl_wait();                                               // everything above overlapped the previous kernel's tail
+
+    // ring geometry of this call: a stage holds one 16 KB weight tile and this CTA's half of the widest token tile
+    const int max_n = a.sched->max_n;
+    const uint32_t stage_bytes = WT_BYTES + (((uint32_t)max_n * (ROW_BYTES / 2) + 1023u) & ~1023u);
+    const int NS = min(PAIR_MAX_STAGES, (int)(PAIR_RING_BYTES / stage_bytes));
+
 
     const int W = MODE == 1 ? a.sched->W1 : a.sched->W2;
     const int wi0 = (int)cluster_id_x(), wstep = (int)cluster_count_x();
@@ -499,8 +502,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
 // ---------------------------------------------------------------------------------------------- launchers
 template <int MODE>
 static cudaError_t launch_pair_t(const PairArgs& a, int num_sms, cudaStream_t st) {
-    k_gemm_pair<MODE><<<num_sms / 2 * 2, PAIR_THREADS, PAIR_SMEM, st>>>(a);   // cluster dims are compiled in
-    return cudaGetLastError();
+    return launch_pdl(k_gemm_pair<MODE>, dim3(num_sms / 2 * 2), dim3(PAIR_THREADS), PAIR_SMEM, st, a);   // cluster dims are compiled in
 }
 
 cudaError_t init_pair_kernels() {

@@ -60,8 +60,10 @@ k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* _
     __shared__ int s_ntt, s_last;
     const int E = D.E;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    pdl_launch_dependents();
     for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
     __syncthreads();
+    pdl_wait();                                                  // the previous call's kernels may still read the workspace
     const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
     const int sub = chunk / RT_WARPS;
     const int wlo = min(hi, lo + w * sub), whi = min(hi, wlo + sub);
@@ -210,8 +212,10 @@ k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __re
     __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, then per-warp running base
     const int E = D.E;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    pdl_launch_dependents();
     for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
     __syncthreads();
+    pdl_wait();
     const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
     const int sub = chunk / RT_WARPS;
     const int wlo = min(hi, lo + w * sub), whi = min(hi, wlo + sub);
@@ -263,6 +267,8 @@ k_gather(Dims D, const uint4* __restrict__ x, int k, const int* __restrict__ row
          uint8_t* __restrict__ Xs, int P) {
     const int lane = threadIdx.x & 31;
     const int gw = blockIdx.x * 8 + (threadIdx.x >> 5), nw = gridDim.x * 8;
+    pdl_launch_dependents();
+    pdl_wait();
     const int P_used = sched->P_used;
     const int chunks_per_row = D.d >> 3;
     for (int p = gw; p < P_used; p += nw) {
@@ -273,16 +279,14 @@ k_gather(Dims D, const uint4* __restrict__ x, int k, const int* __restrict__ row
 
 cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int grp,
                               int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st) {
-    k_route_plan<<<ws.RB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, r_table, tile_n, grp, counts, offsets, ws.bhist,
-                                               ws.poff, ws.tt, ws.items1, ws.sched, state);
-    return cudaGetLastError();
+    return launch_pdl(k_route_plan, dim3(ws.RB), dim3(RT_THREADS), 0, st, D, ids, T * k, ws.chunk, r_table, tile_n, grp, counts,
+                      offsets, ws.bhist, ws.poff, ws.tt, ws.items1, ws.sched, state);
 }
 
 cudaError_t launch_scatter(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
                            const int* offsets, int* perm, int* inv_perm, const Workspace& ws, cudaStream_t st) {
-    k_scatter<<<ws.RB, RT_THREADS, 0, st>>>(D, ids, T * k, ws.chunk, r_table, counts, offsets, ws.poff, ws.bhist, perm,
-                                            inv_perm, ws.row_flat, ws.prow);
-    return cudaGetLastError();
+    return launch_pdl(k_scatter, dim3(ws.RB), dim3(RT_THREADS), 0, st, D, ids, T * k, ws.chunk, r_table, counts, offsets,
+                      (const int*)ws.poff, (const int*)ws.bhist, perm, inv_perm, ws.row_flat, ws.prow);
 }
 
 cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st) {
@@ -290,8 +294,8 @@ cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, c
     long long blocks = (rows + 7) / 8;
     if (blocks > 148 * 8) blocks = 148 * 8;
     if (blocks < 1) blocks = 1;
-    k_gather<<<(int)blocks, 256, 0, st>>>(D, (const uint4*)x, k, ws.row_flat, ws.sched, ws.Xs, ws.P);
-    return cudaGetLastError();
+    return launch_pdl(k_gather, dim3((unsigned)blocks), dim3(256), 0, st, D, (const uint4*)x, k, (const int*)ws.row_flat,
+                      (const Sched*)ws.sched, ws.Xs, ws.P);
 }
 
 }  // namespace fxm
