@@ -56,6 +56,7 @@ typedef enum {
 #define FXM_IMPL_TCGEN05 0
 #define FXM_IMPL_SIMT_DEBUG 1
 #define FXM_IMPL_TCGEN05_1CTA 2
+#define FXM_IMPL_TCGEN05_XS 3 /* the CTA-pair kernels fed by the separate gather kernel (A/B measurement of the fused gather) */
 
 /* ---- sizes first: the caller owns all device memory -------------------------------------------------- */
 
@@ -107,7 +108,7 @@ int32_t fxm_ratio_to_width(int I, int num, int den);
  * topk_w   : device fp32 [T][k], applied as given (the router is external and frozen)
  * y        : device bf16 [T][d], OVERWRITTEN (Y <- 0 then accumulate); routed experts only.
  * workspace: device, >= fxm_workspace_bytes(E,d,I,T,k), 1024-byte aligned; contents are scratch.
- * Launches: route plan, scatter, gather, grouped GEMM-1(+SwiGLU), grouped GEMM-2, combine (scale + sum) -- or, for
+ * Launches: route plan, scatter, grouped GEMM-1(+X[pi] gather, +SwiGLU), grouped GEMM-2, combine (scale + sum) -- or, for
  * decode-sized calls (fxm_set_decode), ONE fused launch that streams the retained weights once.  Grid sizes
  * do not depend on the budget or on the routing (persistent kernels read the device-side schedule), so a
  * call is CUDA-graph capturable.  T == 0 is a no-op. */
@@ -161,7 +162,8 @@ fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles)
 /* Synchronises `stream`, then returns the sticky device flag word (bit0: expert id out of range,
  * bit1: a pipeline wait timed out -- a bug) in *flags and clears it. */
 fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream);
-/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode) or 6 (bench.py's gpu_launches). */
+/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode), 5 (product path: plan, scatter, GEMM-1 with
+ * the gather fused, GEMM-2, combine) or 6 (debug paths with the separate gather kernel); bench.py's gpu_launches. */
 int fxm_launches_per_ffn(const fxm_layer* L);
 
 const char* fxm_status_string(fxm_status s);

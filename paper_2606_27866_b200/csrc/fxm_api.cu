@@ -22,6 +22,9 @@ struct fxm_layer {
     int dec_max_A;           // the fused decode kernel takes calls with T*k <= dec_max_A (0 = never)
     int dec_pf;              // its L2 prefetch distance in 16 KB tiles
     int last_launches;       // kernels enqueued by the last fxm_moe_ffn
+    alignas(64) unsigned char x_map[128];   // CUtensorMap over the x of the last pair-path call (gather4 source)
+    const void* x_map_ptr;   // the x it was encoded for
+    int x_map_T;
     std::vector<int> host_tables;   // mirror of the resident tables (validation / introspection only)
     std::vector<cudaEvent_t> prof_events;   // fxm_profile_begin: (FXM_N_KERNELS + 1) events per recorded call
     int prof_capacity;       // calls that can still be recorded
@@ -48,13 +51,14 @@ static size_t state_offset(const Dims& D) { return tables_offset(D) + sizeof(int
 static size_t rank_offset(const Dims& D) { return align_up(state_offset(D) + sizeof(DevState), 1024); }
 static size_t packed_total(const Dims& D) { return align_up(rank_offset(D) + sizeof(int) * (size_t)D.E * D.I, 1024); }
 
+static bool is_pair(const fxm_layer* L) { return L->impl == FXM_IMPL_TCGEN05 || L->impl == FXM_IMPL_TCGEN05_XS; }
 static int choose_tile_n(const fxm_layer* L, int T, int k) {
-    if (L->impl == FXM_IMPL_TCGEN05) return PAIR_TILE_N;         // CTA-pair kernels: one or two 256-token sub-tiles
+    if (is_pair(L)) return PAIR_TILE_N;         // CTA-pair kernels: one or two 256-token sub-tiles
     if (L->tile_n_override == 128 || L->tile_n_override == 256) return L->tile_n_override;
     // mean rows per expert > 192: 256-token tiles halve the weight re-reads; below that 128 wastes less
     return ((long long)T * k > 192LL * L->D.E) ? 256 : 128;
 }
-static int plan_grp(const fxm_layer* L) { return L->impl == FXM_IMPL_TCGEN05 ? 2 : 1; }
+static int plan_grp(const fxm_layer* L) { return is_pair(L) ? 2 : 1; }
 // a6: decode-sized calls (a handful of tokens per expert) go to the single-launch weight-streaming kernel
 static bool use_decode(const fxm_layer* L, int T, int k) {
     const long long A = (long long)T * k;
@@ -153,6 +157,7 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
     L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
     L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
     L->prof_capacity = 0; L->prof_calls = 0;
+    L->x_map_ptr = nullptr; L->x_map_T = -1;
     L->dec_max_A = FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS; L->dec_pf = FXM_DECODE_DEFAULT_PREFETCH; L->last_launches = 0;
     *out = L;
     return FXM_OK;
@@ -210,7 +215,7 @@ fxm_status fxm_select_budget(fxm_layer* L, int b) {
 }
 
 fxm_status fxm_set_impl(fxm_layer* L, int impl) {
-    if (!L || (impl != FXM_IMPL_TCGEN05 && impl != FXM_IMPL_SIMT_DEBUG && impl != FXM_IMPL_TCGEN05_1CTA)) return FXM_EINVAL;
+    if (!L || impl < FXM_IMPL_TCGEN05 || impl > FXM_IMPL_TCGEN05_XS) return FXM_EINVAL;
     L->impl = impl;
     return FXM_OK;
 }
@@ -322,12 +327,20 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
     FXM_MARK(1)
     if (launch_scatter(D, topk_ids, T, k, table, ws.counts, ws.offsets, ws.perm, ws.inv_perm, ws, st) != cudaSuccess)
         return FXM_ECUDA;
-    // gather of the x rows into sorted swizzled panels
+    // X[pi] (Alg. 2 l.7): the product path gathers the token rows inside GEMM-1 (TMA gather4 straight from x); the
+    // other paths copy them into sorted swizzled panels first
     FXM_MARK(2)
-    if (launch_gather(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
+    const bool fused_gather = L->impl == FXM_IMPL_TCGEN05;
+    if (fused_gather) {
+        if (L->x_map_ptr != x || L->x_map_T != T) {
+            if (encode_x_map(x, T, D.d, L->x_map) != cudaSuccess) return FXM_ECUDA;
+            L->x_map_ptr = x; L->x_map_T = T;
+        }
+    } else if (launch_gather(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
     FXM_MARK(3)
-    if (L->impl == FXM_IMPL_TCGEN05) {
-        if (launch_gemm1_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
+    if (is_pair(L)) {
+        if (launch_gemm1_pair(D, L->packed, table, ws, L->state, L->num_sms, fused_gather ? L->x_map : nullptr, st) != cudaSuccess)
+            return FXM_ECUDA;
         FXM_MARK(4)
         if (launch_gemm2_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
     } else if (L->impl == FXM_IMPL_TCGEN05_1CTA) {
@@ -344,7 +357,7 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
     FXM_MARK(6)
     FXM_MARK(7)
 #undef FXM_MARK
-    L->last_launches = 6;
+    L->last_launches = fused_gather ? 5 : 6;
     return FXM_OK;
 }
 

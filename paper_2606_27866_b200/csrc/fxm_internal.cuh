@@ -94,6 +94,7 @@ struct Workspace {
     int* inv_perm;          // [A]
     int* row_flat;          // [P]  flat assignment index f = t*k+j of each padded row, -1 for padding
     int* prow;              // [A]  padded row of each flat assignment; -1 = dropped or expert of width 0
+    int* row_tok;           // [P]  token index t = f / k of each padded row (0 for padding rows): the gather4 row coordinates
     int* bhist;             // [RB][E] per-route-block expert histogram, then exclusive base over blocks
     int4* tt;               // [NT] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}
     int4* items1;           // [NT*nCB] GEMM-1 work items {expert, first padded row, valid rows, channel block}
@@ -138,6 +139,7 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.inv_perm = (int*)(b + take(sizeof(int) * (A + 1)));
     w.row_flat = (int*)(b + take(sizeof(int) * (size_t)P));
     w.prow = (int*)(b + take(sizeof(int) * (A + 1)));
+    w.row_tok = (int*)(b + take(sizeof(int) * (size_t)P));
     w.bhist = (int*)(b + take(sizeof(int) * (size_t)RB * D.E));
     w.tt = (int4*)(b + take(sizeof(int4) * (size_t)NT));
     w.items1 = (int4*)(b + take(sizeof(int4) * (size_t)NT * D.nCB));
@@ -217,8 +219,12 @@ cudaError_t init_sm100_kernels();   // cudaFuncSetAttribute for the dynamic shar
 
 // CTA-pair path (cta_group::2, token tiles up to 512 rows); the schedule must have been planned with grp = 2
 constexpr int PAIR_TILE_N = 512;
+// x_map: a CUtensorMap (128 bytes, passed by value to the kernel) over x [T][d] bf16 with box {64, 1} and 128-byte
+// swizzle: GEMM-1 gathers its token rows straight from x with TMA gather4 (no Xs copy).  nullptr = read the Xs panels.
 cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
-                              DevState* state, int num_sms, cudaStream_t st);
+                              DevState* state, int num_sms, const void* x_map, cudaStream_t st);
+// encodes the tensor map above through the driver entry point cuTensorMapEncodeTiled (no libcuda link dependency)
+cudaError_t encode_x_map(const void* x, int T, int d, void* map_out /* 128 bytes, 64-byte aligned */);
 cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
                               DevState* state, int num_sms, cudaStream_t st);
 cudaError_t init_pair_kernels();

@@ -29,18 +29,28 @@
 //   * an L2 prefetch cursor runs ahead of the weight loads so the ring refills at L2 latency.
 //
 // Warp roles (640 threads per CTA): warp 0 = producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA),
-// warps 4-19 = epilogue (each CTA drains its own TMEM lanes; four warps per lane quadrant).
+// GEMM-1 only: warps 2-7 = gather warps (token rows straight from x by TMA gather4, no Xs copy), then 16 epilogue warps
+// (each CTA drains its own TMEM lanes; four warps per lane quadrant).
 #include "fxm_ptx.cuh"
+
+#include <cuda.h>          // CUtensorMap and the cuTensorMapEncodeTiled prototype (resolved at run time, no libcuda link)
 
 namespace fxm {
 
 constexpr int PAIR_NSUB = 256;                  // most tokens per sub-tile (UMMA N max)
 constexpr int PAIR_EPI_WARPS = 16;              // epilogue warps: 4 per TMEM lane quadrant (the SwiGLU epilogue is issue-bound)
-constexpr int PAIR_THREADS = 128 + 32 * PAIR_EPI_WARPS;
+constexpr int PAIR_GW = 6;                      // gather warps of GEMM-1 (TMA gather4 issue costs ~60 cycles per 4 rows and warp)
+// warps: 0 producer, 1 MMA / relay, [GEMM-1: 2..7 gather], then the epilogue warps (first one a multiple of 4)
+template <int MODE> struct PairCfg {
+    static constexpr int EPI0 = MODE == 1 ? 8 : 4;
+    static constexpr int THREADS = 32 * (EPI0 + PAIR_EPI_WARPS);
+};
 constexpr int PAIR_MAX_STAGES = 8;
 constexpr int PAIR_STAGING = 2 * 16384;         // two 16 KB epilogue staging buffers
 constexpr int PAIR_SMEM = 232448;               // 227 KB: everything a CTA can have
-constexpr int PAIR_RING_BYTES = PAIR_SMEM - 1024 /*alignment slack*/ - PAIR_STAGING - 1024 /*barriers*/;
+constexpr int PAIR_AUX = 2048;                  // barriers (264 B) and, at +512, the gather warps' token indices
+constexpr int PAIR_RING_BYTES = PAIR_SMEM - 1024 /*alignment slack*/ - PAIR_STAGING - PAIR_AUX;   // 4 x 48 KB
+constexpr int PAIR_GMAX = (PAIR_NSUB / 4 + PAIR_GW - 1) / PAIR_GW;     // most 4-row groups one gather warp issues per k-block
 constexpr int PAIR_TQ = 8;                      // TMEM sub-tile barrier ring
 #ifndef FXM_PAIR_PF
 #define FXM_PAIR_PF 0
@@ -53,7 +63,8 @@ struct PairArgs {
     const int* r_table;
     const int4* items;         // GEMM-1: pair items {e, row0, valid rows, cbp}; GEMM-2: token tiles {e, row0, valid rows, .}
     const Sched* sched;
-    const uint8_t* Bsrc;       // Xs (GEMM-1) or H (GEMM-2) panels
+    const uint8_t* Bsrc;       // Xs (GEMM-1 fed by the gather kernel) or H (GEMM-2) panels
+    const int* tok;            // GEMM-1 with the gather fused: token index of every padded row (nullptr: read Xs)
     uint8_t* H;                // GEMM-1 output panels
     uint8_t* O;                // GEMM-2 output panels [nDB][P][256 B]
     DevState* state;
@@ -124,6 +135,15 @@ __device__ __forceinline__ void umma2_commit_mc(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
                  ::"r"(bar), "h"(mask)
                  : "memory");
+}
+// TMA gather4: four rows (row coordinates r0..r3) x 64 bf16 columns starting at `col` of the 2-D tensor behind `map`
+// land as four consecutive 128-byte rows at `dst`, 128-byte swizzled by shared-memory address -- the K-major SW128
+// operand layout tcgen05.mma reads.  512 bytes complete on `bar`.
+__device__ __forceinline__ void tma_gather4(uint32_t dst, const void* map, int col, int4 r, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cta.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];"
+        ::"r"(dst), "l"(map), "r"(col), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w), "r"(bar)
+        : "memory");
 }
 __device__ __forceinline__ uint32_t make_idesc2(uint32_t n) {     // M = 256 (pair), N = n
     return (1u << 4) | (1u << 7) | (1u << 10) | ((n >> 3) << 17) | ((256u >> 4) << 24);
@@ -221,7 +241,9 @@ struct TmemRing {
 
 // ------------------------------------------------------------------------------------------------ kernel
 template <int MODE>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_gemm_pair(const PairArgs a) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PairCfg<MODE>::THREADS, 1)
+k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
+    constexpr int EPI0 = PairCfg<MODE>::EPI0;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
@@ -233,6 +255,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
     auto tfull_bar = [&](uint32_t q) { return bar_base + 8u * (2 * PAIR_MAX_STAGES + (q % PAIR_TQ)); };
     auto tempty_bar = [&](uint32_t q) { return bar_base + 8u * (2 * PAIR_MAX_STAGES + PAIR_TQ + (q % PAIR_TQ)); };
     volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + PAIR_RING_BYTES + PAIR_STAGING + 8 * (2 * PAIR_MAX_STAGES + 2 * PAIR_TQ));
+    int4* gidx = (int4*)(smem_gen + PAIR_RING_BYTES + PAIR_STAGING + 512);        // [PAIR_GW][PAIR_GMAX] token indices
 
     const int warp = shfl0(threadIdx.x >> 5), lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
@@ -261,6 +284,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
     const int NS = min(PAIR_MAX_STAGES, (int)(PAIR_RING_BYTES / stage_bytes));
 
 
+    const bool gather = MODE == 1 && a.tok != nullptr;        // GEMM-1 token rows come straight from x via TMA gather4
     const int W = MODE == 1 ? a.sched->W1 : a.sched->W2;
     const int wi0 = (int)cluster_id_x(), wstep = (int)cluster_count_x();
     const uint8_t* dn = a.packed + gu_bytes(D);
@@ -313,13 +337,48 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
                     const uint32_t sb = smem_base + s * stage_bytes;
                     mbar_expect_tx(full_bar(s), tx);
                     bulk_g2s(sb, asrc + kb * astride, WT_BYTES, full_bar(s));
-                    bulk_g2s(sb + WT_BYTES, b0 + kb * bstride, h0 * ROW_BYTES, full_bar(s));
-                    if (h1) bulk_g2s(sb + WT_BYTES + h0 * ROW_BYTES, b1 + kb * bstride, h1 * ROW_BYTES, full_bar(s));
+                    if (!gather) {                                     // else: the gather warps bring the same bytes
+                        bulk_g2s(sb + WT_BYTES, b0 + kb * bstride, h0 * ROW_BYTES, full_bar(s));
+                        if (h1) bulk_g2s(sb + WT_BYTES + h0 * ROW_BYTES, b1 + kb * bstride, h1 * ROW_BYTES, full_bar(s));
+                    }
                 }
                 pf_step();
                 if (++s == NS) { s = 0; ph ^= 1u; }
             }
             if (rank == 0 && leader_lane) FXM_TR(MODE, tj, 6, tw);
+        }
+    } else if (MODE == 1 && gather && warp >= 2 && warp < 2 + PAIR_GW) {
+        // ===================================================== gather warps (both CTAs; GEMM-1 with the gather fused)
+        // X[pi] (Alg. 2 l.7) without a copy of x in global memory: this CTA's half of the token rows of a
+        // k-block comes straight from x, four rows per TMA gather4 (group g = rows 4g..4g+3 of the half, sub-tile 0
+        // first).  Warp gw issues groups gw, gw + PAIR_GW, ...; their token indices sit in this warp's slice of gidx.
+        const int gw = warp - 2;
+        const bool leader_lane = elect_one();
+        int4* myidx = gidx + gw * PAIR_GMAX;
+        int s = 0;
+        uint32_t ph = 0;
+        for (int wi = wi0; wi < W; wi += wstep) {
+            const PairItem it = pair_item<MODE>(a, wi, rank);
+            const int h0 = it.n0 >> 1, h1 = it.n1 >> 1;
+            const int ng0 = h0 >> 2, ng = (h0 + h1) >> 2;
+            const int cnt = ng > gw ? (ng - gw + PAIR_GW - 1) / PAIR_GW : 0;
+            __syncwarp();                                             // the previous item's gather4s have read their indices
+            if (lane < cnt) {
+                const int g = gw + PAIR_GW * lane;
+                const int p = g < ng0 ? it.row0 + (int)rank * h0 + 4 * g : it.row0 + it.n0 + (int)rank * h1 + 4 * (g - ng0);
+                myidx[lane] = __ldg((const int4*)(a.tok + p));
+            }
+            __syncwarp();
+            for (int kb = 0; kb < it.nk; ++kb) {
+                mbar_wait(empty_bar(s), ph ^ 1u, a.state);
+                if (leader_lane) {
+                    const uint32_t dst = smem_base + s * stage_bytes + WT_BYTES + (uint32_t)gw * (4u * ROW_BYTES);
+                    for (int j = 0; j < cnt; ++j)
+                        tma_gather4(dst + (uint32_t)j * (PAIR_GW * 4u * ROW_BYTES), &xmap, kb * KB, myidx[j], full_bar(s));
+                }
+                __syncwarp();
+                if (++s == NS) { s = 0; ph ^= 1u; }
+            }
         }
     } else if (warp == 1 && rank != 0) {
         // ===================================================== relay (peer CTA): "my half of this k-block has landed"
@@ -385,7 +444,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
             }
             __syncwarp();
         }
-    } else if (warp >= 4) {
+    } else if (warp >= EPI0) {
         // ===================================================== epilogue warps 4..19 (both CTAs, own TMEM lanes)
         // A sub-tile is drained in CHUNKS of CH token columns: TMEM -> registers -> (SwiGLU | round) -> a 16 KB staging
         // buffer in the FINAL global layout -> one bulk store per chunk.  Two staging buffers alternate.
@@ -393,8 +452,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
         constexpr int ROWB = MODE == 1 ? ROW_BYTES : 2 * WT_ROWS;   // bytes per token row of this CTA's output
         const int q = warp & 3;                                // TMEM lane quadrant this warp may read
         constexpr int NWQ = PAIR_EPI_WARPS / 4;                // warps per lane quadrant
-        const int wq = (warp - 4) >> 2;                        // which share of a chunk's 16-column groups
-        const int et = threadIdx.x - 128;
+        const int wq = (warp - EPI0) >> 2;                        // which share of a chunk's 16-column groups
+        const int et = threadIdx.x - 32 * EPI0;
         TmemRing ring;
         ring.init();
         uint32_t nchunk = 0;
@@ -501,8 +560,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PAIR_THREADS, 1) k_g
 
 // ---------------------------------------------------------------------------------------------- launchers
 template <int MODE>
-static cudaError_t launch_pair_t(const PairArgs& a, int num_sms, cudaStream_t st) {
-    return launch_pdl(k_gemm_pair<MODE>, dim3(num_sms / 2 * 2), dim3(PAIR_THREADS), PAIR_SMEM, st, a);   // cluster dims are compiled in
+static cudaError_t launch_pair_t(const PairArgs& a, const CUtensorMap& xmap, int num_sms, cudaStream_t st) {
+    return launch_pdl(k_gemm_pair<MODE>, dim3(num_sms / 2 * 2), dim3(PairCfg<MODE>::THREADS), PAIR_SMEM, st, a, xmap);
+}
+
+// x [T][d] bf16 as a 2-D tensor {d, T} with box {64 columns, 1 row} and 128-byte swizzle: the shape tile::gather4 wants
+cudaError_t encode_x_map(const void* x, int T, int d, void* map_out) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres);
+        if (e != cudaSuccess) return e;
+        if (qres != cudaDriverEntryPointSuccess || !p) return cudaErrorNotSupported;
+        fn = (EncodeFn)p;
+    }
+    const cuuint64_t gdim[2] = {(cuuint64_t)d, (cuuint64_t)T};
+    const cuuint64_t gstride[1] = {(cuuint64_t)d * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)KB, 1};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = fn((CUtensorMap*)map_out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(x), gdim, gstride, box,
+                          estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
 cudaError_t init_pair_kernels() {
@@ -512,11 +595,14 @@ cudaError_t init_pair_kernels() {
 }
 
 cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
-                              DevState* state, int num_sms, cudaStream_t st) {
+                              DevState* state, int num_sms, const void* x_map, cudaStream_t st) {
     PairArgs a{};
     a.D = D; a.packed = packed; a.r_table = r_table; a.items = ws.items1; a.sched = ws.sched; a.Bsrc = ws.Xs;
     a.H = ws.H; a.state = state; a.P = ws.P;
-    return launch_pair_t<1>(a, num_sms, st);
+    a.tok = x_map ? ws.row_tok : nullptr;
+    CUtensorMap m{};
+    if (x_map) m = *(const CUtensorMap*)x_map;
+    return launch_pair_t<1>(a, m, num_sms, st);
 }
 
 cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
@@ -524,7 +610,7 @@ cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r
     PairArgs a{};
     a.D = D; a.packed = packed; a.r_table = r_table; a.items = ws.tt; a.sched = ws.sched; a.Bsrc = ws.H;
     a.O = ws.O; a.state = state; a.P = ws.P;
-    return launch_pair_t<2>(a, num_sms, st);
+    return launch_pair_t<2>(a, CUtensorMap{}, num_sms, st);
 }
 
 }  // namespace fxm

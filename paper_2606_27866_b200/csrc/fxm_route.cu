@@ -208,7 +208,7 @@ __global__ void __launch_bounds__(RT_THREADS)
 k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table,
           const int* __restrict__ counts, const int* __restrict__ offsets, const int* __restrict__ poff,
           const int* __restrict__ bbase, int* __restrict__ perm, int* __restrict__ inv_perm,
-          int* __restrict__ row_flat, int* __restrict__ prow) {
+          int* __restrict__ row_flat, int* __restrict__ prow, int* __restrict__ row_tok, int k) {
     __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, then per-warp running base
     const int E = D.E;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
@@ -245,6 +245,7 @@ k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __re
             perm[pos] = f;
             inv_perm[f] = pos;
             row_flat[pr] = f;
+            row_tok[pr] = f / k;
             prow[f] = (!r_table || r_table[id] > 0) ? pr : -1;   // width-0 experts get no tiles: nothing to read back
         } else if (f < whi) {
             inv_perm[f] = -1;                                // dropped (precondition violation, flagged by the plan kernel)
@@ -257,7 +258,7 @@ k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __re
 
     // ---- padding rows of the expert segments carry no assignment
     for (int e = blockIdx.x * RT_THREADS + tid; e < E; e += gridDim.x * RT_THREADS)
-        for (int p = poff[e] + counts[e]; p < poff[e + 1]; ++p) row_flat[p] = -1;
+        for (int p = poff[e] + counts[e]; p < poff[e + 1]; ++p) { row_flat[p] = -1; row_tok[p] = 0; }
 }
 
 // Alg. 2 l.7, X[pi]: one warp per padded row p copies x[token(p)] into the swizzled panels; padding
@@ -286,7 +287,7 @@ cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const
 cudaError_t launch_scatter(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
                            const int* offsets, int* perm, int* inv_perm, const Workspace& ws, cudaStream_t st) {
     return launch_pdl(k_scatter, dim3(ws.RB), dim3(RT_THREADS), 0, st, D, ids, T * k, ws.chunk, r_table, counts, offsets,
-                      (const int*)ws.poff, (const int*)ws.bhist, perm, inv_perm, ws.row_flat, ws.prow);
+                      (const int*)ws.poff, (const int*)ws.bhist, perm, inv_perm, ws.row_flat, ws.prow, ws.row_tok, k);
 }
 
 cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st) {

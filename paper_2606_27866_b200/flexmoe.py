@@ -19,6 +19,7 @@ _HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_CSRC, "fxm_pt
 IMPL_TCGEN05 = 0
 IMPL_SIMT_DEBUG = 1
 IMPL_TCGEN05_1CTA = 2
+IMPL_TCGEN05_XS = 3
 MAX_BUDGETS = 15
 
 _STATUS = ["FXM_OK", "FXM_EINVAL", "FXM_ESHAPE", "FXM_EPERM", "FXM_EBUDGET", "FXM_ENOTNESTED",
