@@ -5,8 +5,8 @@
     python bench.py --impl reference [--steps K] [--warmup W]        the CPU oracle, timed on the host cores
     python bench.py --sweep [--sweep-configs C2,C3,C4,C5]            every config x T x budget -> gpurun_out/sweep.json
 
-A "step" is one fxm_moe_ffn call (route -> gather -> grouped GEMM-1+SwiGLU -> grouped GEMM-2+combine ->
-finalize) over one batch of synthetic tokens.  Default workload = BASELINE.json
+A "step" is one fxm_moe_ffn call (route plan -> scatter -> grouped GEMM-1 with the token gather and SwiGLU fused ->
+grouped GEMM-2 -> combine) over one batch of synthetic tokens.  Default workload = BASELINE.json
 configs[1]: the Qwen1.5-MoE-A2.7B-shaped layer (d=2048, E=60, top-4, I=1408), T=4096, uniform r_e=704 (50 %
 pruned).  N>1 = independent replicas of the layer, tokens sharded across ranks (weak scaling, no data-path
 collective).  Prints ONE JSON line on rank 0.
@@ -30,8 +30,8 @@ import numpy as np
 METRIC = "routed_expert_ffn_tokens_per_s"
 UNIT = "tokens/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# captures (profiles/r01b_README.md); keyed by (config, T, width, kernel).  --traffic overrides.
-NCU_TRAFFIC = {("C2", 4096, "704", "gemm1_swiglu"): 437.1e6, ("C2", 4096, "704", "gemm2"): 239.8e6,
+# captures (profiles/r01c_README.md, r01b_README.md); keyed by (config, T, width, kernel).  --traffic overrides.
+NCU_TRAFFIC = {("C2", 4096, "704", "gemm1_swiglu"): 405.8e6, ("C2", 4096, "704", "gemm2"): 239.8e6,
                ("C4", 64, "1280", "decode_fused"): 1776.6e6}
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 
@@ -60,8 +60,8 @@ def work_model(ids: np.ndarray, r: np.ndarray, d: int, T: int, k: int):
     return {
         "S": S, "R_act": R_act,
         "flops": 6.0 * d * S, "bytes": 6.0 * d * R_act + 4.0 * T * d + 8.0 * A,
-        "gemm1_flops": 4.0 * d * S, "gemm1_bytes": 4.0 * d * R_act + 2.0 * A * d + 2.0 * S,
-        "gemm2_flops": 2.0 * d * S, "gemm2_bytes": 2.0 * d * R_act + 2.0 * S + 4.0 * T * d,
+        "gemm1_flops": 4.0 * d * S, "gemm1_bytes": 4.0 * d * R_act + 2.0 * T * d + 2.0 * S,   # W_gate/up once, x once, H once
+        "gemm2_flops": 2.0 * d * S, "gemm2_bytes": 2.0 * d * R_act + 2.0 * S + 2.0 * A * d,   # W_down once, H once, O once
     }
 
 
