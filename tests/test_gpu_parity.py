@@ -164,6 +164,43 @@ def test_pair_subtile_boundaries(T):
         gu.check_close(gu.run_ffn(L, b, r, decode=False), gu.oracle_ffn(lay, b, r), f"T={T} r={r.tolist()}")
 
 
+def _random_cases():
+    rng = np.random.default_rng(2024)
+    cases = [(64, 1, 1, 16, 1), (64, 1, 1, 16, 40), (128, 256, 16, 32, 33), (64, 2, 2, 1040, 17), (3584, 3, 2, 64, 70)]
+    for _ in range(10):
+        d = int(rng.integers(1, 9)) * 64
+        E = int(rng.integers(1, 24))
+        k = int(rng.integers(1, min(E, 6) + 1))
+        I = int(rng.integers(1, 21)) * 16
+        T = int(rng.choice([1, 2, 7, 31, 64, 129, 300, 700]))
+        cases.append((d, E, k, I, T))
+    return cases
+
+
+@pytest.mark.parametrize("d,E,k,I,T", _random_cases())
+def test_random_small_shapes_product_path_and_decode(d, E, k, I, T):
+    """Seeded sweep over small (d, E, k, I, T) including the extremes of the supported set (d = 64, E = 1 and 256,
+    k = 1 and 16, I = 16, ragged I, d = 3584): random widths in [0, I] (any multiple of 1), skewed routing; the
+    product path and, where T*k <= 1024, the fused decode kernel, every element against the oracle."""
+    import gpu_util as gu
+    sh, lay, rng = _small_layer(1000 + d + E + T, d, E, k, I, w_std=0.08)
+    lg = gen.make_logits(T, E, rng, 1.0, 1.5)
+    ids, w = gen.route(lg, k)
+    b = gen.Batch(gen.make_x(T, d, rng), ids, w)
+    L = gu.pack_layer(lay)
+    r = rng.integers(0, I + 1, size=E).astype(np.int32)
+    r[int(rng.integers(E))] = I
+    ref = gu.oracle_ffn(lay, b, r)
+    if np.abs(ref).max() == 0:
+        r[:] = I
+        ref = gu.oracle_ffn(lay, b, r)
+    gu.check_close(gu.run_ffn(L, b, r, decode=False), ref, f"general d={d} E={E} k={k} I={I} T={T} r={r.tolist()[:8]}")
+    if T * k <= 1024 and d <= 3840:
+        y = gu.run_ffn(L, b, r, decode=True)
+        assert L.launches_per_ffn() == 1
+        gu.check_close(y, ref, f"decode d={d} E={E} k={k} I={I} T={T}")
+
+
 # ------------------------------------------------------------------------------------- fused decode kernel (a6)
 @pytest.mark.parametrize("T,k,E,bias", [(1, 1, 4, 0.0), (3, 2, 5, 0.0), (40, 4, 6, 2.0), (200, 2, 6, 2.5), (64, 16, 16, 0.0),
                                         (128, 8, 256, 1.0), (1024, 1, 7, 1.0)])
@@ -280,6 +317,40 @@ def test_budget_switch_select_and_nested_check():
     assert torch.equal(before[:nw], L.packed[:nw]), "a budget switch must not touch the weights"
     with pytest.raises(fx.FxmError):
         L.select_budget(3)
+
+
+@pytest.mark.parametrize("decode", [False, True])
+def test_cuda_graph_capture_and_replay(decode):
+    """include/flexmoe.h: grid sizes do not depend on the routing or the budget, nothing synchronises -> a call is
+    CUDA-graph capturable.  Capture one fxm_moe_ffn, then replay it on NEW token data and a NEW budget table written
+    into the same buffers (the graph holds no routing- or budget-dependent launch shape)."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    tabs = np.array([[512] * 8, [256, 128, 192, 64, 512, 64, 128, 0]], np.int32)
+    L = gu.pack_layer(lay)
+    L.set_decode(1024 if decode else 0)
+    L.set_budget(tabs[0])
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    y = torch.empty((b.x.shape[0], sh.d), dtype=torch.bfloat16, device="cuda")
+    L.moe_ffn(x, ids, w, out=y)                               # warm-up outside the capture (workspace allocation)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            L.moe_ffn(x, ids, w, out=y)
+    g.replay()
+    torch.cuda.synchronize()
+    gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), gu.oracle_ffn(lay, b, tabs[0]), "replay 1")
+    b2 = gen.make_batch(sh, b.x.shape[0], np.random.default_rng(77))
+    x.copy_(gu.to_dev(b2.x)); ids.copy_(torch.from_numpy(b2.topk_ids).cuda()); w.copy_(torch.from_numpy(b2.topk_w).cuda())
+    L.set_budget(tabs[1])                                     # same device table slot, new widths
+    g.replay()
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
+    gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), gu.oracle_ffn(lay, b2, tabs[1]), "replay 2")
 
 
 def test_errors_and_state():
