@@ -1,7 +1,7 @@
 // fxm_pair.cu -- steps a4/a5 as CTA-PAIR kernels (tcgen05.mma.cta_group::2): two SMs of one TPC share a tile.
 //
 //   a4  GEMM-1 + SwiGLU (Eq. 4; Alg. 2 l.12-16), swap-AB:
-//         D[256 packed weight rows, N tokens] = Wgu[256, d] . Xs[N, d]^T,   UMMA M = 256 over the pair:
+//         D[256 packed weight rows, N tokens] = Wgu[256, d] . X[pi][N, d]^T,   UMMA M = 256 over the pair:
 //         CTA r of the pair owns channel block cb = 2*cbp + r (64 gate + 64 up rows, lanes 0..127 of ITS TMEM).
 //         Epilogue: h = silu(g) * u (gate lane l, up lane l+16: one shuffle), channels >= r_e forced to 0 (the
 //         paper's pad-zero rule), one rounding to bf16 -> the swizzled H panel.
@@ -26,11 +26,13 @@
 //     as soon as the columns they need are drained (tiles of <= 256 tokens are fully double-buffered);
 //   * the epilogue stages its output in shared memory in the final layout and writes it with bulk stores (the H / O
 //     panels make a CTA's output of a sub-tile one contiguous range);
-//   * an L2 prefetch cursor runs ahead of the weight loads so the ring refills at L2 latency.
+//   * GEMM-1 takes its token rows straight from x (X[pi], Alg. 2 l.7): TMA tile::gather4 through a tensor map over
+//     x [T][d], four rows per instruction, landing in the swizzled K-major operand layout -- no gathered copy of x;
+//   * an optional L2 prefetch cursor over the weight tiles exists (FXM_PAIR_PF) but is off: every distance > 0 was slower.
 //
-// Warp roles (640 threads per CTA): warp 0 = producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA),
-// GEMM-1 only: warps 2-7 = gather warps (token rows straight from x by TMA gather4, no Xs copy), then 16 epilogue warps
-// (each CTA drains its own TMEM lanes; four warps per lane quadrant).
+// Warp roles: warp 0 = weight producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA), GEMM-1 only: warps 2-7 =
+// gather warps (a gather4 costs one warp ~60 cycles of issue, six of them keep up with the MMAs), then 16 epilogue
+// warps (each CTA drains its own TMEM lanes; four warps per lane quadrant).  768 threads (GEMM-1) / 640 (GEMM-2).
 #include "fxm_ptx.cuh"
 
 #include <cuda.h>          // CUtensorMap and the cuTensorMapEncodeTiled prototype (resolved at run time, no libcuda link)
