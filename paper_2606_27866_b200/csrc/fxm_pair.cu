@@ -41,10 +41,13 @@ namespace fxm {
 
 constexpr int PAIR_NSUB = 256;                  // most tokens per sub-tile (UMMA N max)
 constexpr int PAIR_EPI_WARPS = 16;              // epilogue warps: 4 per TMEM lane quadrant (the SwiGLU epilogue is issue-bound)
-constexpr int PAIR_GW = 6;                      // gather warps of GEMM-1 (TMA gather4 issue costs ~60 cycles per 4 rows and warp)
+#ifndef FXM_PAIR_GW
+#define FXM_PAIR_GW 6
+#endif
+constexpr int PAIR_GW = FXM_PAIR_GW;                      // gather warps of GEMM-1 (TMA gather4 issue costs ~60 cycles per 4 rows and warp)
 // warps: 0 producer, 1 MMA / relay, [GEMM-1: 2..7 gather], then the epilogue warps (first one a multiple of 4)
 template <int MODE> struct PairCfg {
-    static constexpr int EPI0 = MODE == 1 ? 8 : 4;
+    static constexpr int EPI0 = MODE == 1 ? (2 + PAIR_GW + 3) / 4 * 4 : 4;
     static constexpr int THREADS = 32 * (EPI0 + PAIR_EPI_WARPS);
 };
 constexpr int PAIR_MAX_STAGES = 8;
