@@ -153,7 +153,7 @@ fxm_status fxm_set_impl(fxm_layer* L, int impl);          /* FXM_IMPL_* ; defaul
 /* Token-tile width of the grouped GEMMs: 128, 256, or 0 = choose from T*k/E (default).  Tuning knob only. */
 fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
 /* Step a6: calls with T*k <= max_assignments (<= 1024; 0 = never) run as ONE launch of the fused
- * weight-streaming decode kernel instead of the six launches above; prefetch_tiles = how many 16 KB weight tiles
+ * weight-streaming decode kernel instead of the five launches above; prefetch_tiles = how many 16 KB weight tiles
  * its L2 prefetch cursor runs ahead of the shared-memory ring (0..256).  Tuning knob only: results agree within
  * the stated tolerance either way.  Needs d <= 3840, else the general path is used regardless. */
 #define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 768
