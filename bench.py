@@ -309,7 +309,8 @@ def run_ours(args):
                    "parallelism": f"replicas x{world}, tokens sharded, no data-path collective"},
         "e2e": {"value": round(e2e_value, 1), "unit": UNIT,
                 "h2d_bytes_per_step": int(T * sh.d * 2 + 2 * T * sh.k * 4), "d2h_bytes_per_step": int(T * sh.d * 2),
-                "ms_per_step": round(ms_e2e / args.steps, 5), "api": "fxm_moe_ffn_host (pinned host buffers)"},
+                "ms_per_step": round(ms_e2e / args.steps, 5), "api": "fxm_moe_ffn_host (pinned host buffers; every step copies its x, ids, w in and its y out; the input copy of "
+                       "step i+1 runs on the library's side stream while step i computes)"},
         "gpu_launches": int(L.launches_per_ffn() * args.steps),
         "clocks": clocks, "roofline": roofline, "roofline_step": roofline_step,
     }

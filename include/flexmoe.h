@@ -115,11 +115,14 @@ int32_t fxm_ratio_to_width(int I, int num, int den);
 fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
                        void* y, void* workspace, size_t workspace_bytes, void* stream);
 
-/* Same forward with HOST buffers (pinned memory recommended so the copies are asynchronous): enqueues on
- * `stream` the host->device copies of x [T][d] bf16, topk_ids [T][k] int32 and topk_w [T][k] fp32 into a
- * staging area at the tail of `workspace`, the five kernels of fxm_moe_ffn, and the device->host copy of
- * y [T][d] bf16.  workspace >= fxm_workspace_bytes_host(E,d,I,T,k).  Does not synchronise: y_host is valid
- * once `stream` has passed this call.  This is the end-to-end entry point bench.py times as `e2e`. */
+/* Same forward with HOST buffers (pinned memory recommended so the copies are asynchronous).  The inputs x [T][d] bf16,
+ * topk_ids [T][k] int32 and topk_w [T][k] fp32 are copied on a library-owned side stream into one of two staging
+ * sets at the tail of `workspace`, so the host->device copy of call i+1 overlaps the kernels and the device->host
+ * copy of call i; `stream` waits for the inputs, runs the kernels of fxm_moe_ffn and copies y [T][d] bf16 back.
+ * Contract: the three input buffers must hold their data when the call is made (they are read from call time on, not
+ * in `stream` order) and stay unmodified until `stream` has passed this call; y_host is valid once `stream` has passed
+ * this call.  Does not synchronise.  workspace >= fxm_workspace_bytes_host(E,d,I,T,k).  On a capturing stream the
+ * copies are enqueued in-stream instead.  This is the end-to-end entry point bench.py times as `e2e`. */
 fxm_status fxm_workspace_bytes_host(int E, int d, int I, int T_max, int k, size_t* bytes);
 fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
                             int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream);

@@ -26,14 +26,21 @@ struct fxm_layer {
     const void* x_map_ptr;   // the x it was encoded for
     int x_map_T;
     std::vector<int> host_tables;   // mirror of the resident tables (validation / introspection only)
+    // fxm_moe_ffn_host: inputs travel on a side stream into one of two staging sets so that the host->device copy of
+    // call i+1 overlaps the kernels and the device->host copy of call i
+    cudaStream_t h2d_stream;
+    cudaEvent_t ev_in[2];    // inputs of set b have landed (recorded on h2d_stream)
+    cudaEvent_t ev_done[2];  // the kernels that read set b have finished (recorded on the caller's stream)
+    unsigned host_calls;
     std::vector<cudaEvent_t> prof_events;   // fxm_profile_begin: (FXM_N_KERNELS + 1) events per recorded call
     int prof_capacity;       // calls that can still be recorded
     int prof_calls;          // calls recorded so far
 };
 
 static size_t host_stage_bytes(const Dims& D, int T, int k) {
-    // device staging of the host-buffer entry point: x, y (bf16 [T][d]), ids (int32 [T][k]), w (fp32 [T][k])
-    return 2 * align_up((size_t)T * D.d * 2, 1024) + 2 * align_up((size_t)T * k * 4, 1024);
+    // device staging of the host-buffer entry point: two input sets {x bf16 [T][d], ids int32 [T][k], w fp32 [T][k]}
+    // and one y bf16 [T][d]
+    return 3 * align_up((size_t)T * D.d * 2, 1024) + 4 * align_up((size_t)T * k * 4, 1024);
 }
 
 static bool make_dims(int E, int d, int I, Dims* D) {
@@ -158,6 +165,8 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
     L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
     L->prof_capacity = 0; L->prof_calls = 0;
     L->x_map_ptr = nullptr; L->x_map_T = -1;
+    L->h2d_stream = nullptr; L->host_calls = 0;
+    for (int b = 0; b < 2; ++b) { L->ev_in[b] = nullptr; L->ev_done[b] = nullptr; }
     L->dec_max_A = FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS; L->dec_pf = FXM_DECODE_DEFAULT_PREFETCH; L->last_launches = 0;
     *out = L;
     return FXM_OK;
@@ -166,6 +175,11 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
 void fxm_destroy(fxm_layer* L) {
     if (!L) return;
     for (cudaEvent_t ev : L->prof_events) cudaEventDestroy(ev);
+    for (int b = 0; b < 2; ++b) {
+        if (L->ev_in[b]) cudaEventDestroy(L->ev_in[b]);
+        if (L->ev_done[b]) cudaEventDestroy(L->ev_done[b]);
+    }
+    if (L->h2d_stream) cudaStreamDestroy(L->h2d_stream);
     delete L;
 }
 
@@ -372,16 +386,41 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
     if (L->current < 0) return FXM_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t xb = (size_t)T * L->D.d * 2, ab = (size_t)T * k * 4;
+    const size_t xs = align_up(xb, 1024), as = align_up(ab, 1024);
     uint8_t* p = (uint8_t*)workspace + inner;
-    uint8_t* xd = p;  p += align_up(xb, 1024);
-    uint8_t* yd = p;  p += align_up(xb, 1024);
-    uint8_t* idd = p; p += align_up(ab, 1024);
-    uint8_t* wd = p;
-    if (cudaMemcpyAsync(xd, x_host, xb, cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
-    if (cudaMemcpyAsync(idd, topk_ids_host, ab, cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
-    if (cudaMemcpyAsync(wd, topk_w_host, ab, cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
+    uint8_t* yd = p;
+    p += xs;
+    // a capturing stream cannot wait on events recorded outside the capture: copy in-stream then (no overlap)
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) return FXM_ECUDA;
+    const bool side = cap == cudaStreamCaptureStatusNone;
+    if (side && !L->h2d_stream) {
+        if (cudaStreamCreateWithFlags(&L->h2d_stream, cudaStreamNonBlocking) != cudaSuccess) return FXM_ECUDA;
+        for (int b = 0; b < 2; ++b)
+            if (cudaEventCreateWithFlags(&L->ev_in[b], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&L->ev_done[b], cudaEventDisableTiming) != cudaSuccess)
+                return FXM_ECUDA;
+    }
+    const unsigned set = side ? (L->host_calls & 1u) : 0u;
+    uint8_t* xd = p + set * (xs + 2 * as);
+    uint8_t* idd = xd + xs;
+    uint8_t* wd = idd + as;
+    cudaStream_t cs = side ? L->h2d_stream : st;
+    // the staging set is free once the kernels of the call before last (same set) have read it
+    if (side && L->host_calls >= 2 && cudaStreamWaitEvent(cs, L->ev_done[set], 0) != cudaSuccess) return FXM_ECUDA;
+    if (cudaMemcpyAsync(xd, x_host, xb, cudaMemcpyHostToDevice, cs) != cudaSuccess) return FXM_ECUDA;
+    if (cudaMemcpyAsync(idd, topk_ids_host, ab, cudaMemcpyHostToDevice, cs) != cudaSuccess) return FXM_ECUDA;
+    if (cudaMemcpyAsync(wd, topk_w_host, ab, cudaMemcpyHostToDevice, cs) != cudaSuccess) return FXM_ECUDA;
+    if (side) {
+        if (cudaEventRecord(L->ev_in[set], cs) != cudaSuccess) return FXM_ECUDA;
+        if (cudaStreamWaitEvent(st, L->ev_in[set], 0) != cudaSuccess) return FXM_ECUDA;
+    }
     fxm_status s = fxm_moe_ffn(L, xd, (const int32_t*)idd, (const float*)wd, T, k, yd, workspace, inner, stream);
     if (s != FXM_OK) return s;
+    if (side) {
+        if (cudaEventRecord(L->ev_done[set], st) != cudaSuccess) return FXM_ECUDA;
+        ++L->host_calls;
+    }
     if (cudaMemcpyAsync(y_host, yd, xb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return FXM_ECUDA;
     return FXM_OK;
 }

@@ -353,6 +353,32 @@ def test_cuda_graph_capture_and_replay(decode):
     gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), gu.oracle_ffn(lay, b2, tabs[1]), "replay 2")
 
 
+def test_host_buffer_entry_point_pipelined_calls():
+    """fxm_moe_ffn_host: six back-to-back calls with different pinned inputs and no host synchronisation in between
+    (the input copy of call i+1 runs on the library's side stream while call i computes; the two staging sets
+    alternate), decode-sized and general path; every output against the oracle."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b0, rng = _c1()
+    r = gen.table_c1(sh, rng)
+    L = gu.pack_layer(lay)
+    L.set_budget(r)
+    for max_a in (1024, 0):
+        L.set_decode(max_a)
+        batches = [gen.make_batch(sh, 64, np.random.default_rng(300 + i)) for i in range(6)]
+        hx = [(fx.bf16_from_bits(b.x, "cpu").pin_memory(), torch.from_numpy(b.topk_ids).pin_memory(),
+               torch.from_numpy(b.topk_w).pin_memory()) for b in batches]
+        hy = [torch.empty((64, sh.d), dtype=torch.bfloat16).pin_memory() for _ in batches]
+        for i in range(6):
+            L.moe_ffn_host(*hx[i], hy[i])
+        torch.cuda.synchronize()
+        assert L.device_flags() == 0
+        for i, b in enumerate(batches):
+            y = gen.bf16_bits_to_f32(hy[i].view(torch.int16).numpy().view(np.uint16)).astype(np.float64)
+            gu.check_close(y, gu.oracle_ffn(lay, b, r), f"host call {i} decode_max={max_a}")
+
+
 def test_errors_and_state():
     import torch
     import gpu_util as gu
