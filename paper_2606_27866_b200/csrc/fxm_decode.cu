@@ -365,6 +365,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         // 978 at 64), so the default distance is 0.
         if (n_items > 0) {
             const bool el = dec_elect_one();
+            const uint64_t pol_stream = l2_policy_evict_first();   // every weight byte is read exactly once
             PartStream ld, pf;
             ld.init(ax, a);
             pf.init(ax, a);
@@ -387,7 +388,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
                     if (el) {
                         mbar_expect_tx(full_bar(stage), WT_BYTES);
-                        bulk_g2s(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage));
+                        bulk_g2s_hint(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage), pol_stream);
                     }
                     if (++stage == NS) { stage = 0; phase ^= 1u; }
                 }

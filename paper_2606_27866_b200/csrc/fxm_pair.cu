@@ -302,6 +302,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
     if (warp == 0) {
         // ===================================================== producer (both CTAs): weight tile + token half per k-block
         const bool leader_lane = elect_one();
+        const uint64_t pol_stream = l2_policy_evict_first();     // weight tiles: read once
         int s = 0;
         uint32_t ph = 0;
         const size_t bstride = (size_t)a.P * ROW_BYTES;
@@ -341,7 +342,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                 if (leader_lane) {
                     const uint32_t sb = smem_base + s * stage_bytes;
                     mbar_expect_tx(full_bar(s), tx);
-                    bulk_g2s(sb, asrc + kb * astride, WT_BYTES, full_bar(s));
+                    bulk_g2s_hint(sb, asrc + kb * astride, WT_BYTES, full_bar(s), pol_stream);
                     if (!gather) {                                     // else: the gather warps bring the same bytes
                         bulk_g2s(sb + WT_BYTES, b0 + kb * bstride, h0 * ROW_BYTES, full_bar(s));
                         if (h1) bulk_g2s(sb + WT_BYTES + h0 * ROW_BYTES, b1 + kb * bstride, h1 * ROW_BYTES, full_bar(s));
@@ -459,6 +460,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         constexpr int NWQ = PAIR_EPI_WARPS / 4;                // warps per lane quadrant
         const int wq = (warp - EPI0) >> 2;                        // which share of a chunk's 16-column groups
         const int et = threadIdx.x - 32 * EPI0;
+        const uint64_t pol_keep = l2_policy_evict_last();         // H / O panels: read back by the next kernel
         TmemRing ring;
         ring.init();
         uint32_t nchunk = 0;
@@ -540,7 +542,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                         if (it.valid) {
                             uint8_t* gdst = MODE == 1 ? a.H + ((size_t)it.blk * a.P + rowS + ch0) * ROW_BYTES
                                                       : a.O + ((size_t)it.blk * a.P + rowS + ch0) * ROWB;
-                            bulk_s2g(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROWB);
+                            bulk_s2g_hint(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROWB, pol_keep);
                             bulk_commit();
                         }
                         if (last) {                                // all epilogue warps have drained this sub-tile's columns
