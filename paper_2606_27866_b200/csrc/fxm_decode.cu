@@ -365,7 +365,11 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         // 978 at 64), so the default distance is 0.
         if (n_items > 0) {
             const bool el = dec_elect_one();
-            const uint64_t pol_stream = l2_policy_evict_first();   // every weight byte is read exactly once
+            // every weight byte is read exactly once: evict_first keeps the stream from displacing anything -- measured
+            // -7 % at C4 T=1 and -10 % at C2 T=16, but +3.5 % when the call streams multi-GB at full HBM rate (C4 T=32/64 at
+            // 0 %), so the hint is used below ~1.2 GB per call
+            const uint64_t pol_stream = l2_policy_evict_first();
+            const bool hint = (size_t)W * (size_t)(D.nKB1 + D.nDB) * WT_BYTES < ((size_t)1200 << 20);
             PartStream ld, pf;
             ld.init(ax, a);
             pf.init(ax, a);
@@ -388,7 +392,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
                     if (el) {
                         mbar_expect_tx(full_bar(stage), WT_BYTES);
-                        bulk_g2s_hint(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage), pol_stream);
+                        if (hint) bulk_g2s_hint(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage), pol_stream);
+                        else bulk_g2s(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage));
                     }
                     if (++stage == NS) { stage = 0; phase ^= 1u; }
                 }
