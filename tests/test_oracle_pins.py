@@ -342,3 +342,178 @@ def test_r_zero_expert_contributes_nothing():
     r = np.zeros(sh.E, np.int32)
     y = oracle.moe_ffn(b.x, Gt, Ut, Dt, r, b.topk_ids, b.topk_w)
     assert (y == 0).all()
+
+
+# ------------------------------------------------------------------ P11: saliency (Eq. 2)
+def _sal_inputs(seed=0, B=3, E=3, I=20, d=12):
+    rng = np.random.default_rng(seed)
+    mk = lambda *sh: gen.f32_to_bf16_bits(rng.standard_normal(sh).astype(np.float32) * 0.5)
+    return (mk(E, I, d), mk(E, I, d), mk(E, d, I)), (mk(B, E, I, d), mk(B, E, I, d), mk(B, E, d, I))
+
+
+def test_P11_saliency_constant_gradient_closed_form():
+    """g = c everywhere  =>  s_j = c^2 * sum_{theta in Theta_j} theta^2: row norms of gate/up plus the COLUMN norm of
+    down (Theta_j = row j of W_gate, row j of W_up, column j of W_down), via numpy's own sum of squares."""
+    (Wg, Wu, Wd), (Gg, Gu, Gd) = _sal_inputs(1)
+    c = 0.75
+    cb = gen.f32_to_bf16_bits(np.full(1, c, np.float32))[0]
+    s = oracle.saliency(Wg, Wu, Wd, np.full_like(Gg, cb), np.full_like(Gu, cb), np.full_like(Gd, cb))
+    expect = c * c * ((f64(Wg) ** 2).sum(2) + (f64(Wu) ** 2).sum(2) + (f64(Wd) ** 2).sum(1))
+    assert np.allclose(s, expect, rtol=1e-12, atol=0)
+    # a transposed down operand (row instead of column) would give sum over axis 2 of Wd: must differ
+    wrong = c * c * ((f64(Wg) ** 2).sum(2) + (f64(Wu) ** 2).sum(2))
+    assert not np.allclose(s[:, :Wd.shape[1]], wrong[:, :Wd.shape[1]], rtol=1e-3)
+
+
+def test_P11_saliency_invariants():
+    """a^2 scaling in g, equivariance under a consistent channel permutation, additivity over the three matrices, the
+    mean over batches (duplicating the ranking set changes nothing), non-negativity."""
+    (Wg, Wu, Wd), (Gg, Gu, Gd) = _sal_inputs(2)
+    s = oracle.saliency(Wg, Wu, Wd, Gg, Gu, Gd)
+    assert (s >= 0).all() and s.shape == (3, 20)
+    two = lambda g: gen.f32_to_bf16_bits(gen.bf16_bits_to_f32(g) * np.float32(2.0))      # exact in bf16
+    assert np.allclose(oracle.saliency(Wg, Wu, Wd, two(Gg), two(Gu), two(Gd)), 4.0 * s, rtol=1e-12)
+    zero = lambda g: np.zeros_like(g)
+    parts = (oracle.saliency(Wg, Wu, Wd, Gg, zero(Gu), zero(Gd)) + oracle.saliency(Wg, Wu, Wd, zero(Gg), Gu, zero(Gd)) +
+             oracle.saliency(Wg, Wu, Wd, zero(Gg), zero(Gu), Gd))
+    assert np.allclose(parts, s, rtol=1e-12)
+    dup = lambda g: np.concatenate([g, g])
+    assert np.allclose(oracle.saliency(Wg, Wu, Wd, dup(Gg), dup(Gu), dup(Gd)), s, rtol=1e-12)
+    rng = np.random.default_rng(5)
+    pi = rng.permutation(20)
+    sp = oracle.saliency(Wg[:, pi], Wu[:, pi], Wd[:, :, pi], Gg[:, :, pi], Gu[:, :, pi], Gd[:, :, :, pi])
+    assert np.allclose(sp, s[:, pi], rtol=1e-12)
+    # only batch 0 differs from the mean over batches: B matters as a divisor
+    s0 = oracle.saliency(Wg, Wu, Wd, Gg[:1], Gu[:1], Gd[:1])
+    assert not np.allclose(s0, s, rtol=1e-3)
+
+
+def test_P11_saliency_brute_force_tiny():
+    """pure-python triple loop over (batch, parameter) on a tiny case, grouping parameters by channel through an
+    explicit membership list Theta_j built from index tuples."""
+    (Wg, Wu, Wd), (Gg, Gu, Gd) = _sal_inputs(3, B=2, E=2, I=4, d=3)
+    s = oracle.saliency(Wg, Wu, Wd, Gg, Gu, Gd)
+    W = {"g": f64(Wg), "u": f64(Wu), "d": f64(Wd)}
+    G = {"g": f64(Gg), "u": f64(Gu), "d": f64(Gd)}
+    for e in range(2):
+        for j in range(4):
+            theta = [("g", (e, j, i)) for i in range(3)] + [("u", (e, j, i)) for i in range(3)] + [("d", (e, i, j)) for i in range(3)]
+            tot = 0.0
+            for b in range(2):
+                sb = 0.0
+                for m, idx in theta:
+                    sb += (W[m][idx] * G[m][(b,) + idx]) ** 2
+                tot += sb
+            assert abs(s[e, j] - tot / 2) <= 1e-12 * max(1.0, tot)
+
+
+# ------------------------------------------------------------------ P12: rank (Eq. 3's pi, PAPER.md:82; reading R4)
+def test_P12_rank_vs_numpy_stable_argsort_and_ties():
+    rng = np.random.default_rng(0)
+    s = rng.random((5, 257))
+    s[1, 10:20] = s[1, 3]                     # a run of exact ties
+    s[2, :] = 1.0                             # all equal -> identity
+    s[3, ::2] = 0.0
+    got = oracle.rank(s)
+    for e in range(5):
+        assert np.array_equal(got[e], np.argsort(-s[e], kind="stable"))
+        assert sorted(got[e].tolist()) == list(range(257))
+        assert (np.diff(s[e][got[e]]) <= 0).all()
+    assert np.array_equal(got[2], np.arange(257))
+
+
+def test_P12_rank_recovers_a_planted_importance_order_through_saliency_and_pack():
+    """Plant the importance: channel c of expert e gets weight scale proportional to a planted score, gradients all
+    one -> Eq. 2 orders the channels by the planted score -> rank returns the planted order, and packing with it puts the
+    channels in that order (reading R3: rank[p] = ORIGINAL index of the p-th most important channel)."""
+    rng = np.random.default_rng(7)
+    E, I, d = 2, 16, 8
+    order = np.stack([rng.permutation(I) for _ in range(E)])           # order[e][p] = channel with the p-th largest score
+    scale = np.empty((E, I), np.float32)
+    for e in range(E):
+        scale[e, order[e]] = 2.0 ** (-np.arange(I) / 2.0).astype(np.float32)
+    one = np.ones((E, I, d), np.float32)
+    Wg = gen.f32_to_bf16_bits(one * scale[:, :, None])
+    Wu = gen.f32_to_bf16_bits(one * scale[:, :, None])
+    Wd = gen.f32_to_bf16_bits(np.ones((E, d, I), np.float32) * scale[:, None, :])
+    ones = lambda sh: gen.f32_to_bf16_bits(np.ones(sh, np.float32))
+    s = oracle.saliency(Wg, Wu, Wd, ones((1, E, I, d)), ones((1, E, I, d)), ones((1, E, d, I)))
+    rk = oracle.rank(s)
+    assert np.array_equal(rk, order)
+    Gt, _, Dt = oracle.pack(Wg, Wu, Wd, rk)
+    assert (np.diff(f64(Gt)[:, :, 0], axis=1) < 0).all() and (np.diff(f64(Dt)[:, 0, :], axis=1) < 0).all()
+
+
+# ------------------------------------------------------------------ P13: router front end (reading R10)
+def test_P13_router_topk_vs_generator_and_torch():
+    """The generator plays the same router with the OTHER formulation (softmax over all E, top-k, renormalise);
+    torch.topk / torch.softmax are a third.  ids equal (generic logits), weights within fp32 rounding."""
+    rng = np.random.default_rng(0)
+    lg = gen.make_logits(300, 24, rng)
+    ids, w = oracle.router_topk(lg, 5)
+    gi, gw = gen.route(lg, 5)
+    assert np.array_equal(ids, gi) and np.allclose(w, gw, rtol=0, atol=3e-7)
+    tv, ti = torch.topk(torch.from_numpy(lg).double(), 5, dim=1)
+    assert np.array_equal(ids, ti.numpy().astype(np.int32))
+    assert np.allclose(w, torch.softmax(tv, dim=1).numpy(), atol=1e-7)
+    assert np.allclose(w.sum(1), 1.0, atol=1e-6) and (np.diff(w, axis=1) <= 0).all()
+
+
+def test_P13_router_closed_forms():
+    ids, w = oracle.router_topk(np.zeros((3, 8), np.float32), 3)               # all ties: lowest ids, equal weights
+    assert (ids == np.array([0, 1, 2])).all() and np.allclose(w, 1 / 3, atol=1e-7)
+    lg = np.array([[0.0, np.log(3.0), -50.0, np.log(3.0)]], np.float32)
+    ids, w = oracle.router_topk(lg, 3)
+    assert ids.tolist() == [[1, 3, 0]] and np.allclose(w, [[3 / 7, 3 / 7, 1 / 7]], atol=1e-7)
+    rng = np.random.default_rng(1)
+    lg = rng.standard_normal((50, 12)).astype(np.float32)
+    i1, w1 = oracle.router_topk(lg, 4)
+    i2, w2 = oracle.router_topk(lg + np.float32(8.0), 4)                       # shift invariance (8.0 keeps fp32 sums exact enough)
+    assert np.array_equal(i1, i2) and np.allclose(w1, w2, atol=2e-6)
+    iE, wE = oracle.router_topk(lg, 12)                                          # k = E: plain softmax, sorted
+    sm = torch.softmax(torch.from_numpy(lg).double(), 1).numpy()
+    assert np.allclose(np.take_along_axis(sm, iE.astype(np.int64), 1), wE, atol=1e-7)
+
+
+# ------------------------------------------------------------------ P14: actions (Eq. 6-7, 10-11)
+def test_P14_noise_free_argmax_reproduces_the_printed_mask():
+    """Eq. 11: hardened action = argmax_k p_k.  Build logits whose argmax is the printed action of every
+    cell of Fig. 6; with zero noise the sampled ratios must be the printed ones and Eq. 12 gives the
+    printed budget 0.4031."""
+    mask = _fig6() / 100.0                     # the golden file holds percent
+    assert mask.shape == (32, 8)
+    ratios = np.array([0.1, 0.4, 0.7, 1.0])
+    num, den = np.array([1, 4, 7, 10], np.int32), 10
+    act_true = np.array([[int(np.argmin(np.abs(ratios - v))) for v in row] for row in mask])
+    rng = np.random.default_rng(0)
+    alpha = rng.standard_normal((256, 4)).astype(np.float32)
+    alpha[np.arange(256), act_true.ravel()] += 10.0
+    action, width = oracle.sample_actions(alpha, np.zeros_like(alpha), num, den, 14336)
+    assert np.array_equal(action, act_true.ravel())
+    assert width.tolist().count(1434) == 92 and width.tolist().count(14336) == 117      # ceil(0.1 * 14336) = 1434
+    assert abs(oracle.budget_rho(width, 14336) - 0.40311) < 1e-4
+
+
+def test_P14_gumbel_argmax_properties_and_cost_closed_forms():
+    rng = np.random.default_rng(3)
+    E, K = 40, 4
+    alpha = rng.standard_normal((E, K)).astype(np.float32)
+    g = -np.log(-np.log(rng.random((E, K)))).astype(np.float32)
+    num, den = np.array([1, 4, 7, 10], np.int32), 10
+    a1, w1 = oracle.sample_actions(alpha, g, num, den, 2560)
+    # Eq. 6 with any temperature: argmax of softmax((alpha+g)/tau) == argmax of alpha+g (fp32 sum)
+    for tau in (0.1, 1.0, 5.0):
+        z = torch.softmax(torch.from_numpy((alpha + g).astype(np.float64)) / tau, 1).numpy()
+        assert np.array_equal(a1, z.argmax(1))
+    assert np.array_equal(w1, np.array([256, 1024, 1792, 2560])[a1])
+    # Eq. 10: uniform p (alpha = 0) -> C = mean(r) regardless of the load; one-hot p -> C = sum_e q_e r_{k(e)}
+    counts = rng.integers(0, 100, E).astype(np.int32)
+    assert abs(oracle.action_cost(np.zeros((E, K), np.float32), num, den, counts) - 0.55) < 1e-12
+    hot = np.full((E, K), -1e4, np.float32)
+    hot[np.arange(E), a1] = 0.0
+    q = counts / counts.sum()
+    assert abs(oracle.action_cost(hot, num, den, counts) - float((q * (num[a1] / den)).sum())) < 1e-12
+    # initialisation at the thickest action (PAPER.md:127): cost = 1
+    thick = np.full((E, K), -1e4, np.float32)
+    thick[:, K - 1] = 0.0
+    assert abs(oracle.action_cost(thick, num, den, counts) - 1.0) < 1e-12
