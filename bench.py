@@ -1,22 +1,25 @@
 #!/usr/bin/env python
-"""bench.py -- routed-expert FFN tokens/s and % of roofline on B200 (BASELINE.json metric).
+"""bench.py -- routed-expert FFN tokens/s and % of roofline vs pruning budget on B200 (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W]              our arm (C-ABI library, CUDA kernels)
     python bench.py --impl reference [--steps K] [--warmup W]        the CPU oracle, timed on the host cores
-    python bench.py --sweep [--sweep-configs C2,C3,C4,C5]            every config x T x budget -> gpurun_out/sweep.json
+    python bench.py --config C2 --T 4096 --r 704                     another workload (C2/C3/C4/C5, any T, any table)
 
-A "step" is one fxm_moe_ffn call (route plan -> scatter -> grouped GEMM-1 with the token gather and SwiGLU fused ->
-grouped GEMM-2 -> combine) over one batch of synthetic tokens.  Default workload = BASELINE.json
-configs[1]: the Qwen1.5-MoE-A2.7B-shaped layer (d=2048, E=60, top-4, I=1408), T=4096, uniform r_e=704 (50 %
-pruned).  N>1 = independent replicas of the layer, tokens sharded across ranks (weak scaling, no data-path
-collective).  Prints ONE JSON line on rank 0.
+A "step" is one fxm_moe_ffn call (route -> grouped GEMM-1 with the token gather, SwiGLU and
+Y <- 0 fused -> grouped GEMM-2 with the router-weight scale and the scatter-add fused -> finalize) over one batch of
+synthetic tokens.  Default workload = the largest single-GPU configuration of BASELINE.json: configs[3], the
+Qwen2-57B-A14B-shaped layer (d=3584, E=64, top-8, I=2560), T=8192, 0 % pruned (uniform r_e=2560).  The same run adds
+  "budget_sweep": 0/25/40/50/75 % pruned (uniform and heterogeneous nested tables) x T in {1, 64, 8192},
+  "switch":       a short C5 loop (interleaved T=32 / T=4096 steps, a different nested table every step),
+  "roofline", "cpu_baseline", "e2e", "clocks" as the contract asks.
+N>1 = independent replicas of the layer, tokens sharded across ranks (weak scaling, no data-path collective; DESIGN.md
+"Multi-GPU"); the sweep / switch / cpu_baseline legs run at N=1 only.  Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -29,11 +32,11 @@ import numpy as np
 
 METRIC = "routed_expert_ffn_tokens_per_s"
 UNIT = "tokens/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
-# captures (profiles/r01c_README.md, r01b_README.md); keyed by (config, T, width, kernel).  --traffic overrides.
-NCU_TRAFFIC = {("C2", 4096, "704", "gemm1_swiglu"): 405.8e6, ("C2", 4096, "704", "gemm2"): 239.8e6,
-               ("C4", 64, "1280", "decode_fused"): 1776.6e6}
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+DEFAULTS = {"config": "C4", "T": 8192, "r": "2560"}
+SWEEP_T = (8192, 64, 1)
+SWEEP_TABLES = [("U0", 2560), ("U25", 1920), ("U40", 1536), ("U50", 1280), ("U75", 640),
+                ("H0", "hetero:0"), ("H25", "hetero:1"), ("H40", "hetero:2"), ("H50", "hetero:3"), ("H75", "hetero:4")]
 
 
 def load_peaks():
@@ -50,9 +53,11 @@ def load_peaks():
 
 # ------------------------------------------------------------------------------------------ work model
 def work_model(ids: np.ndarray, r: np.ndarray, d: int, T: int, k: int):
-    """Algorithmic work of one call: S = sum_e n_e r_e,
-    R_act = sum over experts with n_e>0 of r_e.  FLOPs = 6 d S (gate 2 + up 2 + down 2 per token-channel-d);
-    bytes = each retained weight of an active expert once (6 d R_act) + x + y (4 T d) + ids/weights (8 A)."""
+    """Algorithmic work of one call, exactly SURVEY.md 8(d): S = sum_e n_e r_e, R_act = sum over experts with n_e > 0 of
+    r_e.  FLOPs = 6 d S (gate 2 + up 2 + down 2 per token-channel-feature); bytes = every retained weight of an active
+    expert once (6 d R_act) + x + y (4 T d) + ids/weights (8 A).  NOT counted (implementation traffic): the H round
+    trip, the fp32 accumulator of y.  Per kernel: GEMM-1 = 4 d S flops, gate/up weights + x; GEMM-2 = 2 d S flops, down
+    weights + y."""
     n = np.bincount(ids.ravel(), minlength=r.size).astype(np.int64)
     S = int((n * r.astype(np.int64)).sum())
     R_act = int(r.astype(np.int64)[n > 0].sum())
@@ -60,12 +65,13 @@ def work_model(ids: np.ndarray, r: np.ndarray, d: int, T: int, k: int):
     return {
         "S": S, "R_act": R_act,
         "flops": 6.0 * d * S, "bytes": 6.0 * d * R_act + 4.0 * T * d + 8.0 * A,
-        "gemm1_flops": 4.0 * d * S, "gemm1_bytes": 4.0 * d * R_act + 2.0 * T * d + 2.0 * S,   # W_gate/up once, x once, H once
-        "gemm2_flops": 2.0 * d * S, "gemm2_bytes": 2.0 * d * R_act + 2.0 * S + 2.0 * A * d,   # W_down once, H once, O once
+        "gemm1_flops": 4.0 * d * S, "gemm1_bytes": 4.0 * d * R_act + 2.0 * T * d + 4.0 * A,
+        "gemm2_flops": 2.0 * d * S, "gemm2_bytes": 2.0 * d * R_act + 2.0 * T * d + 4.0 * A,
     }
 
 
 def roof_time_s(flops, nbytes, peaks, tf_key="bf16_tflops"):
+    """bound = the larger of the two floors"""
     t_tc = flops / (peaks[tf_key] * 1e12)
     t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
     return (t_tc, "tensor") if t_tc >= t_hbm else (t_hbm, "hbm")
@@ -73,7 +79,7 @@ def roof_time_s(flops, nbytes, peaks, tf_key="bf16_tflops"):
 
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler:
-    """Polls NVML (SM clock, power, clock-event reasons) from a thread while a timed region runs."""
+    """Polls NVML (SM clock, power, clock-event reasons) from a thread while the timed regions run."""
     REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
                0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
 
@@ -119,7 +125,7 @@ class ClockSampler:
         if self._thr is not None:
             self._thr.join()
 
-    def summary(self, windows):
+    def summary(self, windows, brief=False):
         """windows: list of (t0, t1) perf_counter intervals during which the GPU was under load."""
         if self._h is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"], "samples": 0}
@@ -131,18 +137,17 @@ class ClockSampler:
         for s in sel:
             bits |= s[2]
         reasons = [n for b, n in self.REASONS.items() if bits & b]
-        return {"sm_mhz": float(np.median([s[1] for s in sel])) if sel else None, "sm_max_mhz": self.max_mhz,
-                "reasons": reasons, "samples": len(sel),
-                "power_w_max": round(max(s[3] for s in sel), 1) if sel else None}
+        out = {"sm_mhz": float(np.median([s[1] for s in sel])) if sel else None, "sm_max_mhz": self.max_mhz,
+               "reasons": reasons, "samples": len(sel)}
+        if not brief:
+            out["power_w_max"] = round(max(s[3] for s in sel), 1) if sel else None
+        return out
 
 
 # ------------------------------------------------------------------------------------------ workload
-DEFAULTS = {"config": "C2", "T": 4096, "r": 704}
-
-
 def make_table(gen, sh, spec, rng):
-    """spec: an int width (uniform), 'full', 'hetero:<b>' (C4 nested-descent table b), 'mean60' (C3) or 'c1'."""
-    if isinstance(spec, int) or str(spec).isdigit():
+    """spec: an int width (uniform), 'full', 'hetero:<b>' (C4 nested-descent table b), 'fig6', 'mean60' (C3) or 'c1'."""
+    if isinstance(spec, (int, np.integer)) or str(spec).isdigit():
         return gen.table_uniform(sh, int(spec))
     if spec == "full":
         return gen.table_uniform(sh, sh.I)
@@ -150,9 +155,17 @@ def make_table(gen, sh, spec, rng):
         return gen.table_c1(sh, rng)
     if spec == "mean60":
         return gen.table_mean_ratio(sh, rng, 0.6)
+    if spec == "fig6":
+        return gen.table_fig6_like(sh, rng)
     if str(spec).startswith("hetero:"):
-        return gen.tables_nested_descent(sh, rng)[int(spec.split(":")[1])]
+        return gen.tables_nested_descent(sh, np.random.default_rng([0, 3]))[int(spec.split(":")[1])]
     raise SystemExit(f"unknown table spec {spec!r}")
+
+
+def workload_string(cfg, sh, T, spec, r):
+    """Identical for both arms (the driver compares the strings)."""
+    return (f"{cfg} {sh.name}: d={sh.d} E={sh.E} top-{sh.k} I={sh.I} T={T} per GPU, table {spec} "
+            f"(rho={1 - float(r.mean()) / sh.I:.3f} pruned)")
 
 
 def rank_seed0(rank: int) -> int:
@@ -181,6 +194,141 @@ def host_batches(gen, cfg, T, n, seed0):
     return out
 
 
+def to_device(fx, torch, hb):
+    return [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()) for b, _ in hb]
+
+
+# ------------------------------------------------------------------------------------------ budget sweep (N=1)
+def sweep_point(torch, L, dev, y, iters, warm, flush_buf):
+    """Median device time of one call (CUDA events on the launching stream around every call).  With flush_buf, a buffer
+    larger than L2 is rewritten before every call so the weights never come from L2 (decode points)."""
+    st = torch.cuda.current_stream()
+    for i in range(warm):
+        L.moe_ffn(*dev[i % len(dev)], out=y)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    for i in range(iters):
+        if flush_buf is not None:
+            flush_buf.add_(1)
+        ev[i][0].record(st)
+        L.moe_ffn(*dev[i % len(dev)], out=y)
+        ev[i][1].record(st)
+    torch.cuda.synchronize()
+    return np.array([a.elapsed_time(b) for a, b in ev])
+
+
+def run_budget_sweep(torch, fx, gen, L, cfg, sh, peaks, sampler):
+    """BASELINE.json metric "vs pruning budget": every budget of configs[3] x T in {8192, 64, 1}."""
+    flush_buf = torch.zeros(512 << 20, dtype=torch.uint8, device="cuda")
+    rows, base = [], {}
+    for T in SWEEP_T:
+        NB = 4 if T >= 1024 else 8
+        hb = host_batches(gen, cfg, T, NB, 500)
+        dev = to_device(fx, torch, hb)
+        y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
+        for label, spec in SWEEP_TABLES:
+            r = make_table(gen, sh, spec, None)
+            L.set_budget(r)
+            iters = 12 if T >= 1024 else 60
+            w0 = time.perf_counter()
+            ms = sweep_point(torch, L, dev, y, iters, 3, flush_buf if T <= 64 else None)
+            w1 = time.perf_counter()
+            wm = [work_model(b.topk_ids, r, sh.d, T, sh.k) for b, _ in hb]
+            fl = float(np.mean([w["flops"] for w in wm]))
+            by = float(np.mean([w["bytes"] for w in wm]))
+            t_roof, bound = roof_time_s(fl, by, peaks)
+            med = float(np.median(ms)) * 1e-3
+            key = (T, label[0])
+            if label in ("U0", "H0"):
+                base[key] = med
+            rows.append({"T": T, "table": label, "rho": round(1 - float(r.mean()) / sh.I, 4),
+                         "ms": round(med * 1e3, 5), "tokens_per_s": round(T / med, 1),
+                         "tflops": round(fl / med / 1e12, 2), "gbs": round(by / med / 1e9, 1), "bound": bound,
+                         "t_roof_us": round(t_roof * 1e6, 2), "frac": round(t_roof / med, 4),
+                         "speedup_vs_0pct": round(base[key] / med, 3) if key in base else None,
+                         "launches": L.launches_per_ffn(),
+                         "l2": "flushed before every call" if T <= 64 else "weights > L2",
+                         "clocks": sampler.summary([(w0, w1)], brief=True)})
+        del dev, y
+    del flush_buf
+    torch.cuda.empty_cache()
+    return rows
+
+
+# ------------------------------------------------------------------------------------------ C5: online budget switching (N=1)
+def run_switch(torch, fx, gen, L, sh, steps, sampler):
+    """BASELINE.json configs[4] in short: interleaved decode (T=32) / prefill (T=4096) steps on the resident layer, a
+    different registered nested table every step (fxm_select_budget: host-only, no launch, no weight movement)."""
+    tabs = gen.tables_nested_descent(sh, np.random.default_rng([0, 3]))
+    L.register_budgets(tabs, require_nested=True)
+    pools = {}
+    for T in (32, 4096):
+        pools[T] = to_device(fx, torch, host_batches(gen, "C5", T, 8, 0))
+    ys = {T: torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda") for T in pools}
+    L.workspace(4096, sh.k)
+    rng = np.random.default_rng(5)
+    seq, prev = [], -1
+    for _ in range(steps):
+        b = int(rng.integers(len(tabs)))
+        while b == prev:
+            b = int(rng.integers(len(tabs)))
+        seq.append(b)
+        prev = b
+    st = torch.cuda.current_stream()
+
+    def loop(switching):
+        host_sel = 0.0
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(st)
+        for i, b in enumerate(seq):
+            T = 32 if i % 2 == 0 else 4096
+            if switching:
+                t0 = time.perf_counter()
+                L.select_budget(b)
+                host_sel += time.perf_counter() - t0
+            L.moe_ffn(*pools[T][(i // 2) % 8], out=ys[T])
+        e1.record(st)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3, host_sel
+
+    w0 = time.perf_counter()
+    L.select_budget(2)
+    loop(False)                                            # warm-up
+    frozen = {}
+    for b in range(len(tabs)):                             # the frozen-budget loops the switching loop is compared with
+        L.select_budget(b)
+        frozen[b] = loop(False)[0]
+    t_sw, host_sel = loop(True)
+    # what the switching loop should cost if a switch were free: every step at its own table's frozen per-step cost
+    per_step = {}
+    for b in range(len(tabs)):
+        per_step[b] = frozen[b] / len(seq)
+    expect = float(np.mean([frozen[b] for b in seq]))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0.record(st)
+    for b in seq:
+        L.set_budget(tabs[b])
+    e1.record(st)
+    t_host_set = (time.perf_counter() - t0) / len(seq)
+    torch.cuda.synchronize()
+    w1 = time.perf_counter()
+    t_dev_set = e0.elapsed_time(e1) * 1e-3 / len(seq)
+    tokens = sum(32 if i % 2 == 0 else 4096 for i in range(len(seq)))
+    return {"workload": f"C5: C4-shaped layer, {len(seq)} interleaved T=32 / T=4096 steps, 5 nested tables "
+                        f"(rho={[round(1 - float(t.mean()) / sh.I, 3) for t in tabs]}), table switched every step",
+            "sustained_tokens_per_s_switching": round(tokens / t_sw, 1),
+            "loop_s_switching": round(t_sw, 5), "loop_s_expected_from_frozen_loops": round(expect, 5),
+            "switch_cost_us_per_step_device": round((t_sw - expect) / len(seq) * 1e6, 3),
+            "select_budget_host_us": round(host_sel / len(seq) * 1e6, 3),
+            "set_budget_host_us": round(t_host_set * 1e6, 3), "set_budget_stream_us": round(t_dev_set * 1e6, 3),
+            "frozen_loop_s": {str(b): round(v, 5) for b, v in frozen.items()},
+            "weights_touched_by_switch_bytes": 0, "table_bytes": int(sh.E * 4),
+            "clocks": sampler.summary([(w0, w1)], brief=True)}
+
+
+# ------------------------------------------------------------------------------------------ our arm
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -209,8 +357,7 @@ def run_ours(args):
                       lay.channel_rank)
     L.set_budget(r)
     torch.cuda.synchronize()
-    dev = [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
-           for b, _ in hb]
+    dev = to_device(fx, torch, hb)
     y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
     stream = torch.cuda.current_stream()
 
@@ -239,9 +386,10 @@ def run_ours(args):
     barrier()
     w1 = time.perf_counter()
     ms_total = e0.elapsed_time(e1)
+    launches = int(L.launches_per_ffn() * args.steps)
     # ---- the same K steps again with a CUDA event before every kernel (fxm_profile_begin/end): per-kernel device
-    #      times for the roofline of the dominant kernel.  The events cost ~2-3 us each, which is why this pass is not
-    #      the headline number.
+    #      times for the roofline of the dominant kernel, measured live on the launching stream.  The events cost
+    #      2-3 us each and serialise the programmatic dependent launches, which is why this pass is not the headline.
     L.profile_begin(args.steps)
     for i in range(args.steps):
         L.moe_ffn(*dev[i % NB], out=y)
@@ -263,7 +411,6 @@ def run_ours(args):
     barrier()
     w3 = time.perf_counter()
     ms_e2e = e0.elapsed_time(e1)
-    sampler.stop()
     clocks = sampler.summary([(w0, w1), (w2, w3)])
 
     (ms_total, ms_e2e), tokens = aggregate([ms_total, ms_e2e], T, args.steps, world, dist if world > 1 else None, "cuda")
@@ -273,11 +420,12 @@ def run_ours(args):
     sel = [wm[i % NB] for i in range(args.steps)]
     mean = lambda key: float(np.mean([w[key] for w in sel]))
 
-    # ---- roofline of the dominant kernel (largest share of the step) and of the whole step
+    # ---- roofline of the dominant kernel (largest share of the step) and of the whole step, SURVEY.md 8(d) work model
     per_launch_ms = {kname: v / max(n_prof, 1) for kname, v in kern_ms.items()}
     dom = max(per_launch_ms, key=per_launch_ms.get)
-    kflops = {"gemm1_swiglu": mean("gemm1_flops"), "gemm2": mean("gemm2_flops")}.get(dom, 0.0)
-    kbytes = {"gemm1_swiglu": mean("gemm1_bytes"), "gemm2": mean("gemm2_bytes")}.get(dom, mean("bytes"))
+    kflops = {"gemm1_swiglu": mean("gemm1_flops"), "gemm2_scatter_add": mean("gemm2_flops"),
+              "decode_fused": mean("flops")}.get(dom, 0.0)
+    kbytes = {"gemm1_swiglu": mean("gemm1_bytes"), "gemm2_scatter_add": mean("gemm2_bytes")}.get(dom, mean("bytes"))
     t_roof, bound = roof_time_s(kflops, kbytes, peaks)
     dur = per_launch_ms[dom] * 1e-3
     if bound == "tensor":
@@ -286,35 +434,45 @@ def run_ours(args):
         achieved, peak, unit = kbytes / dur / 1e9, peaks["hbm_gbs"], "GB/s"
     roofline = {"bound": bound, "achieved": round(achieved, 2), "peak": peak, "unit": unit,
                 "frac": round(achieved / peak, 4),
-                "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC.get((cfg, T, str(args.r), dom)),
-                "kernel": dom,
-                "kernel_ms": round(per_launch_ms[dom], 5), "peak_source": peaks["source"] + ", burst figure",
+                "traffic": args.traffic,            # dram bytes per launch from an ncu --set full capture of THIS config, else null
+                "kernel": dom, "kernel_ms": round(per_launch_ms[dom], 5),
+                "kernel_share_of_step": round(per_launch_ms[dom] / max(sum(per_launch_ms.values()), 1e-12), 4),
+                "peak_source": peaks["source"] + ", burst figure (the kernel is timed alone between CUDA events)",
                 "frac_of_sustained": round(achieved / peaks["bf16_tflops_sustained"], 4) if bound == "tensor" else None,
-                "algorithmic": {"flops": kflops, "bytes": kbytes}}
+                "algorithmic": {"flops": kflops, "bytes": kbytes,
+                                "model": "SURVEY.md 8(d): weights of the kernel once + x (GEMM-1) or y (GEMM-2) + ids; no H, no accumulator traffic"}}
     step_roof, step_bound = roof_time_s(mean("flops"), mean("bytes"), peaks)
     step_s = ms_total * 1e-3 / args.steps
     roofline_step = {"bound": step_bound, "t_roof_us": round(step_roof * 1e6, 2), "t_step_us": round(step_s * 1e6, 2),
-                     "frac": round(step_roof / step_s, 4), "tflops": round(mean("flops") / step_s / 1e12, 2),
-                     "gbs": round(mean("bytes") / step_s / 1e9, 1),
+                     "frac": round(step_roof / step_s, 4),
+                     "frac_of_sustained": round(roof_time_s(mean("flops"), mean("bytes"), peaks, "bf16_tflops_sustained")[0] / step_s, 4),
+                     "tflops": round(mean("flops") / step_s / 1e12, 2), "gbs": round(mean("bytes") / step_s / 1e9, 1),
                      "kernel_ms_per_step": {kname: round(v, 5) for kname, v in per_launch_ms.items()}}
 
     out = {
         "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": round(ms_total / args.steps, 5), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": f"{cfg} {sh.name}: d={sh.d} E={sh.E} top-{sh.k} I={sh.I} T={T} per GPU, r={args.r} "
-                               f"(rho={1 - float(r.mean()) / sh.I:.3f})",
+        "config": {"workload": workload_string(cfg, sh, T, args.r, r),
                    "l2": f"inputs larger than L2: {6 * sh.d * int(r.sum()) / 1e6:.0f} MB of retained weights streamed "
                          f"per step, {NB} rotating token batches",
                    "parallelism": f"replicas x{world}, tokens sharded, no data-path collective"},
         "e2e": {"value": round(e2e_value, 1), "unit": UNIT,
                 "h2d_bytes_per_step": int(T * sh.d * 2 + 2 * T * sh.k * 4), "d2h_bytes_per_step": int(T * sh.d * 2),
-                "ms_per_step": round(ms_e2e / args.steps, 5), "api": "fxm_moe_ffn_host (pinned host buffers; every step copies its x, ids, w in and its y out; the input copy of "
-                       "step i+1 runs on the library's side stream while step i computes)"},
-        "gpu_launches": int(L.launches_per_ffn() * args.steps),
+                "ms_per_step": round(ms_e2e / args.steps, 5),
+                "api": "fxm_moe_ffn_host (pinned host buffers; every step copies its x, ids, w in and its y out; the "
+                       "input copy of step i+1 runs on the library's side stream while step i computes)"},
+        "gpu_launches": launches,
         "clocks": clocks, "roofline": roofline, "roofline_step": roofline_step,
     }
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    single = rank == 0 and world == 1
+    if single and not args.no_sweep and cfg in ("C4", "C5"):
+        out["budget_sweep"] = run_budget_sweep(torch, fx, gen, L, cfg, sh, peaks, sampler)
+        out["switch"] = run_switch(torch, fx, gen, L, sh, args.switch_steps, sampler)
+        L.set_budget(r)
+        assert L.device_flags() == 0
+    sampler.stop()
+    if single and not args.no_cpu_baseline:
         out["cpu_baseline"], out["parity_sample"] = cpu_baseline(gen, fx, lay, hb[0][0], r, L, dev[0], y, args.cpu_seconds)
     if world > 1:
         dist.barrier()
@@ -334,9 +492,17 @@ def _time_oracle(oracle, b, packed, r, rows):
     return time.perf_counter() - t0, ref
 
 
+def _sample_size(T, cores, t_cal, n0, seconds, floor=512):
+    """tokens of the bounded sample: about `seconds` of CPU work, at least `floor` (>= 512), at most T"""
+    n = int((seconds / max(t_cal, 1e-6)) * n0)
+    n = max(n, floor)
+    n = min(T, max(cores, n // cores * cores))
+    return n
+
+
 def cpu_baseline(gen, fx, lay, b, r, L, dev0, y, seconds):
-    """The oracle as it stands (oracle/oracle.c, fp64, OpenMP over tokens) timed on this box's host cores on a
-    bounded token sample of the SAME workload; the same rows of the GPU output are compared with it."""
+    """The oracle as it stands (oracle/oracle.c, fp64, OpenMP over tokens, gcc -O3 -march=native) timed on this box's
+    host cores on a bounded token sample of the SAME workload; the same rows of the GPU output are compared with it."""
     import torch
     import oracle
     cores = oracle.threads()
@@ -344,8 +510,7 @@ def cpu_baseline(gen, fx, lay, b, r, L, dev0, y, seconds):
     packed = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
     n0 = min(T, cores)
     t_cal, _ = _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n0))
-    n = int(min(T, max(n0, (seconds / max(t_cal, 1e-6)) * n0)))
-    n = max(cores, n // cores * cores) if T >= cores else T
+    n = _sample_size(T, cores, t_cal, n0, seconds)
     rows = _oracle_sample_rows(T, n)
     dt, ref = _time_oracle(oracle, b, packed, r, rows)
     L.moe_ffn(*dev0, out=y)
@@ -354,9 +519,10 @@ def cpu_baseline(gen, fx, lay, b, r, L, dev0, y, seconds):
     scale = float(np.abs(ref).max())
     parity = {"rows": int(rows.size), "max_err_over_max_ref": float(np.abs(yv - ref).max() / scale),
               "rel_l2": float(np.linalg.norm(yv - ref) / np.linalg.norm(ref)), "tol": {"max": 1e-2, "l2": 5e-3}}
+    how = "all" if rows.size == T else "seeded random rows"
     return ({"value": round(rows.size / dt, 2), "unit": UNIT, "cores": cores, "kind": "oracle",
-             "sample": f"{rows.size} of {T} tokens (seeded random rows, full k and r_e), {dt:.1f} s wall, fp64, "
-                       f"OpenMP over tokens"}, parity)
+             "sample": f"{rows.size} of {T} tokens ({how}, full k and r_e), {dt:.1f} s wall, fp64, OpenMP over "
+                       f"tokens, gcc -O3 -march=native"}, parity)
 
 
 def run_reference(args):
@@ -376,8 +542,7 @@ def run_reference(args):
     t_cal, _ = _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n0))
     budget_s = args.cpu_seconds * 6.0                      # whole run (warm-up + steps) ~ 1.5 min by default
     per_step = budget_s / (args.steps + args.warmup)
-    n = int(min(T, max(n0, per_step / max(t_cal, 1e-6) * n0)))
-    n = max(cores, n // cores * cores) if T >= cores else T
+    n = _sample_size(T, cores, t_cal, n0, per_step, floor=cores)
     for i in range(args.warmup):
         _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n, seed=100 + i))
     total = 0.0
@@ -385,12 +550,11 @@ def run_reference(args):
         dt, _ = _time_oracle(oracle, b, packed, r, _oracle_sample_rows(T, n, seed=200 + i))
         total += dt
     value = n * args.steps / total
-    sample = f"{n} of {T} tokens per step (seeded random rows), fp64, OpenMP over tokens"
+    sample = f"{n} of {T} tokens per step (seeded random rows), fp64, OpenMP over tokens, gcc -O3 -march=native"
     out = {"impl": "reference", "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(total / args.steps * 1e3, 3),
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"{cfg} {sh.name}: d={sh.d} E={sh.E} top-{sh.k} I={sh.I} T={T}, r={args.r} "
-                                  f"(rho={1 - float(r.mean()) / sh.I:.3f})", "l2": "n/a (CPU)",
+           "config": {"workload": workload_string(cfg, sh, T, args.r, r), "l2": "n/a (CPU)",
                       "parallelism": "host cores, rank 0 only"},
            "cpu_baseline": {"value": round(value, 2), "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
            "e2e": {"value": round(value, 2), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -398,199 +562,27 @@ def run_reference(args):
     print(json.dumps(out), flush=True)
 
 
-# ------------------------------------------------------------------------------------------ sweep (not the bench line)
-def _time_calls(torch, L, dev, y, iters, warm, flush_buf):
-    """Per-call device time (CUDA events around every call on the current stream).  With flush_buf, a buffer
-    larger than L2 is rewritten before every call so weights never come from L2 (decode points)."""
-    st = torch.cuda.current_stream()
-    for i in range(warm):
-        L.moe_ffn(*dev[i % len(dev)], out=y)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
-    for i in range(iters):
-        if flush_buf is not None:
-            flush_buf.add_(1)
-        ev[i][0].record(st)
-        L.moe_ffn(*dev[i % len(dev)], out=y)
-        ev[i][1].record(st)
-    torch.cuda.synchronize()
-    ms = np.array([a.elapsed_time(b) for a, b in ev])
-    # per-kernel times in a second pass: the per-kernel events cost 2-3 us each and must not sit inside `ms`
-    npk = min(iters, 20)
-    L.profile_begin(npk)
-    for i in range(npk):
-        L.moe_ffn(*dev[i % len(dev)], out=y)
-    torch.cuda.synchronize()
-    kern, n = L.profile_end()
-    return ms, {kname: v / n for kname, v in kern.items()}
-
-
-SWEEP = {
-    "C2": {"T": [1, 16, 4096], "tables": [("r=704 (50%)", 704), ("r=1408 (0%)", "full")]},
-    "C3": {"T": [8192], "tables": [("mean 40% pruned, heterogeneous", "mean60"), ("0%", "full")]},
-    "C4": {"T": [1, 64, 8192], "tables": [("0%", 2560), ("25%", 1920), ("40%", 1536), ("50%", 1280), ("75%", 640),
-                                          ("H 0%", "hetero:0"), ("H 25%", "hetero:1"), ("H 40%", "hetero:2"),
-                                          ("H 50%", "hetero:3"), ("H 75%", "hetero:4")]},
-}
-
-
-def run_sweep(args):
-    import torch
-    from paper_2606_27866_b200 import flexmoe as fx
-    from paper_2606_27866_b200 import inputs as gen
-    torch.cuda.set_device(0)
-    peaks = load_peaks()
-    flush_buf = torch.zeros(512 << 20, dtype=torch.uint8, device="cuda")
-    rows = []
-    for cfg in [c.strip().upper() for c in args.sweep_configs.split(",") if c.strip()]:
-        if cfg not in SWEEP:
-            continue
-        sh = gen.SHAPES[cfg]
-        lay = gen.layer_for(cfg, 0)
-        L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate), fx.bf16_from_bits(lay.W_up), fx.bf16_from_bits(lay.W_down),
-                          lay.channel_rank)
-        torch.cuda.synchronize()
-        for T in SWEEP[cfg]["T"]:
-            NB = 8
-            hb = host_batches(gen, cfg, T, NB, 0)
-            dev = [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
-                   for b, _ in hb]
-            y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
-            for label, spec in SWEEP[cfg]["tables"]:
-                r = make_table(gen, sh, spec, np.random.default_rng([0, 3]))
-                L.set_budget(r)
-                iters = 200 if T <= 64 else (60 if cfg != "C4" else 24)
-                ms, kern = _time_calls(torch, L, dev, y, iters, 5, flush_buf if T <= 64 else None)
-                wm = [work_model(b.topk_ids, r, sh.d, T, sh.k) for b, _ in hb]
-                fl = float(np.mean([w["flops"] for w in wm]))
-                by = float(np.mean([w["bytes"] for w in wm]))
-                t_roof, bound = roof_time_s(fl, by, peaks)
-                med = float(np.median(ms)) * 1e-3
-                rows.append({"config": cfg, "T": T, "budget": label, "rho": round(1 - float(r.mean()) / sh.I, 4),
-                             "ms_median": round(med * 1e3, 5), "ms_p10": round(float(np.percentile(ms, 10)), 5),
-                             "ms_p90": round(float(np.percentile(ms, 90)), 5), "tokens_per_s": round(T / med, 1),
-                             "tflops": round(fl / med / 1e12, 2), "gbs": round(by / med / 1e9, 1), "bound": bound,
-                             "t_roof_us": round(t_roof * 1e6, 2), "roofline_frac": round(t_roof / med, 4),
-                             "l2": "flushed before every call" if T <= 64 else "weights > L2",
-                             "kernel_ms": {kname: round(v, 5) for kname, v in kern.items()}})
-                print(json.dumps(rows[-1]), flush=True)
-            assert L.device_flags() == 0
-        del L
-        torch.cuda.empty_cache()
-    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
-    with open(os.path.join(ROOT, "gpurun_out", "sweep.json"), "w") as f:
-        json.dump({"peaks": peaks, "rows": rows}, f, indent=1)
-
-
-# ------------------------------------------------------------------------------------------ C5: online budget switching
-def run_switch(args):
-    """BASELINE.json configs[4]: C4-shaped layer, `--switch-steps` interleaved decode (T=32) / prefill (T=4096)
-    steps, a different registered nested table every step (fxm_select_budget: host-only)."""
-    import torch
-    from paper_2606_27866_b200 import flexmoe as fx
-    from paper_2606_27866_b200 import inputs as gen
-    torch.cuda.set_device(0)
-    sh = gen.SHAPES["C5"]
-    lay = gen.layer_for("C5", 0)
-    L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate), fx.bf16_from_bits(lay.W_up), fx.bf16_from_bits(lay.W_down),
-                      lay.channel_rank)
-    tabs = gen.tables_nested_descent(sh, np.random.default_rng([0, 3]))
-    L.register_budgets(tabs, require_nested=True)
-    pools = {}
-    for T in (32, 4096):
-        hb = host_batches(gen, "C5", T, 16, 0)
-        pools[T] = [(fx.bf16_from_bits(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
-                    for b, _ in hb]
-    ys = {T: torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda") for T in pools}
-    L.workspace(4096, sh.k)
-    rng = np.random.default_rng(5)
-    seq, prev = [], -1
-    for _ in range(args.switch_steps):
-        b = int(rng.integers(len(tabs)))
-        while b == prev:
-            b = int(rng.integers(len(tabs)))
-        seq.append(b)
-        prev = b
-    st = torch.cuda.current_stream()
-
-    def loop(switching):
-        host_sel = 0.0
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record(st)
-        for i, b in enumerate(seq):
-            T = 32 if i % 2 == 0 else 4096
-            if switching:
-                t0 = time.perf_counter()
-                L.select_budget(b)
-                host_sel += time.perf_counter() - t0
-            L.moe_ffn(*pools[T][(i // 2) % 16], out=ys[T])
-        e1.record(st)
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) * 1e-3, host_sel
-
-    L.select_budget(2)
-    loop(False)                                            # warm-up
-    frozen = {}
-    for b in range(len(tabs)):                             # the frozen-budget loops the switching loop is compared with
-        L.select_budget(b)
-        frozen[b] = loop(False)[0]
-    t_sw, host_sel = loop(True)
-    expect = float(np.mean([frozen[b] for b in seq]))      # mean of frozen-loop times weighted by how often b is used
-    # fxm_set_budget (one tiny launch carrying the table in its arguments): stream time per switch
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    e0.record(st)
-    for b in seq:
-        L.set_budget(tabs[b])
-    e1.record(st)
-    t_host_set = (time.perf_counter() - t0) / len(seq)
-    torch.cuda.synchronize()
-    t_dev_set = e0.elapsed_time(e1) * 1e-3 / len(seq)
-    tokens = sum(32 if i % 2 == 0 else 4096 for i in range(len(seq)))
-    out = {"workload": f"C5: C4-shaped layer, {len(seq)} interleaved T=32 / T=4096 steps, 5 nested tables "
-                       f"(rho={[round(1 - float(t.mean()) / sh.I, 3) for t in tabs]}), table switched every step",
-           "sustained_tokens_per_s_switching": round(tokens / t_sw, 1),
-           "loop_s_switching": round(t_sw, 5), "loop_s_expected_from_frozen_loops": round(expect, 5),
-           "switch_cost_us_per_step_device": round((t_sw - expect) / len(seq) * 1e6, 3),
-           "select_budget_host_us": round(host_sel / len(seq) * 1e6, 3),
-           "set_budget_host_us": round(t_host_set * 1e6, 3), "set_budget_stream_us": round(t_dev_set * 1e6, 3),
-           "frozen_loop_s": {str(b): round(v, 5) for b, v in frozen.items()},
-           "weights_touched_by_switch_bytes": 0, "table_bytes": int(sh.E * 4)}
-    assert L.device_flags() == 0
-    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
-    with open(os.path.join(ROOT, "gpurun_out", "switch.json"), "w") as f:
-        json.dump(out, f, indent=1)
-    print(json.dumps(out), flush=True)
-
-
 # ------------------------------------------------------------------------------------------ main
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default=DEFAULTS["config"])
     ap.add_argument("--T", type=int, default=DEFAULTS["T"])
-    ap.add_argument("--r", default=str(DEFAULTS["r"]), help="uniform width, 'full', 'hetero:<b>', 'mean60', 'c1'")
-    ap.add_argument("--batches", type=int, default=8, help="rotating pre-generated token batches")
+    ap.add_argument("--r", default=str(DEFAULTS["r"]), help="uniform width, 'full', 'hetero:<b>', 'fig6', 'mean60', 'c1'")
+    ap.add_argument("--batches", type=int, default=4, help="rotating pre-generated token batches")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the budget_sweep and switch legs")
+    ap.add_argument("--switch-steps", type=int, default=200)
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture (else null)")
-    ap.add_argument("--sweep", action="store_true")
-    ap.add_argument("--sweep-configs", default="C2,C3,C4")
-    ap.add_argument("--switch", action="store_true")
-    ap.add_argument("--switch-steps", type=int, default=1000)
+                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture of this config (else null)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
-    if args.sweep:
-        return run_sweep(args)
-    if args.switch:
-        return run_switch(args)
     return run_ours(args)
 
 

@@ -45,18 +45,17 @@ typedef enum {
     FXM_ENOTNESTED = 5, /* fxm_register_budgets(require_nested=1): r^(b+1)_e > r^(b)_e for some e          */
     FXM_EWORKSPACE = 6, /* workspace_bytes smaller than fxm_workspace_bytes(E,d,I,T,k)                     */
     FXM_ESTATE = 7,     /* moe_ffn before any budget was installed                                         */
-    FXM_ECUDA = 8       /* a CUDA runtime call failed (no device, launch failure, earlier async fault)     */
+    FXM_ECUDA = 8,      /* a CUDA runtime call failed (no device, launch failure, earlier async fault)     */
+    FXM_ENOMEM = 9      /* a host allocation of the library failed                                         */
 } fxm_status;
 
 #define FXM_MAX_BUDGETS 15 /* tables that fxm_register_budgets can keep resident */
 
-/* implementation selector for fxm_set_impl: the CTA-pair tcgen05 path (cta_group::2) is the product; the
- * single-CTA tcgen05 path and the slow, structurally simple SIMT path run on the SAME packed layout and
- * exist to bisect the fast kernels. */
+/* implementation selector for fxm_set_impl: the CTA-pair tcgen05 path (cta_group::2) is the product; the slow,
+ * structurally simple SIMT path runs on the SAME packed layout, schedule and accumulators and exists to bisect the
+ * fast kernels (it is a CUDA path, not a CPU fallback). */
 #define FXM_IMPL_TCGEN05 0
 #define FXM_IMPL_SIMT_DEBUG 1
-#define FXM_IMPL_TCGEN05_1CTA 2
-#define FXM_IMPL_TCGEN05_XS 3 /* the CTA-pair kernels fed by the separate gather kernel (A/B measurement of the fused gather) */
 
 /* ---- sizes first: the caller owns all device memory -------------------------------------------------- */
 
@@ -65,8 +64,8 @@ typedef enum {
 fxm_status fxm_packed_bytes(int E, int d, int I, size_t* bytes);
 
 /* Bytes of scratch for one moe_ffn / route call with at most T_max tokens and k experts per token:
- * grouping indices, tile schedule, the gathered activations X_s [T_max*k + 16E, d] bf16, the SwiGLU
- * activations H [T_max*k + 16E, ceil64(I)] bf16 and the expert outputs O [T_max*k + 16E, ceil128(d)] bf16. */
+ * grouping indices, tile schedule, the SwiGLU activations H [T_max*k + 16E, ceil64(I)] bf16 and the fp32
+ * scatter-add accumulator of y [T_max, d].  Monotonic in T_max: a buffer sized for T_max serves every T <= T_max. */
 fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* bytes);
 
 /* ---- (1) pack: Eq. 3; layout prior art App. C.2, PAPER.md:526-540 ---------------------
@@ -107,13 +106,25 @@ int32_t fxm_ratio_to_width(int I, int num, int den);
  *            readable with fxm_device_flags and the offending assignment is dropped)
  * topk_w   : device fp32 [T][k], applied as given (the router is external and frozen)
  * y        : device bf16 [T][d], OVERWRITTEN (Y <- 0 then accumulate); routed experts only.
+ * x and y must be 16-byte aligned.
  * workspace: device, >= fxm_workspace_bytes(E,d,I,T,k), 1024-byte aligned; contents are scratch.
- * Launches: route plan, scatter, grouped GEMM-1(+X[pi] gather, +SwiGLU), grouped GEMM-2, combine (scale + sum) -- or, for
- * decode-sized calls (fxm_set_decode), ONE fused launch that streams the retained weights once.  Grid sizes
- * do not depend on the budget or on the routing (persistent kernels read the device-side schedule), so a
- * call is CUDA-graph capturable.  T == 0 is a no-op. */
+ * Launches (4): route (grouping + tile schedule), grouped GEMM-1 (+X[pi] gather, +SwiGLU, +Y <- 0), grouped GEMM-2
+ * (+router-weight scale, +scatter-add into an fp32 accumulator: Alg. 2 l.18-20 in one kernel), finalize (the single
+ * rounding of y to bf16) -- or, for decode-sized calls (fxm_set_decode), ONE fused launch that streams the retained
+ * weights once.  Grid sizes do not depend on the budget or on the routing (persistent kernels read the device-side
+ * schedule), so a call is CUDA-graph capturable.  A captured call is bound to what was resolved on the host when it
+ * was captured: the x pointer and T (a TMA tensor map over x is a kernel argument) and the budget TABLE SLOT that was
+ * current -- fxm_select_budget after the capture does not change what a replay reads; to switch the budget of a
+ * captured call, capture it after fxm_set_budget and call fxm_set_budget (which rewrites that slot in stream order)
+ * before each replay.  T == 0 is a no-op. */
 fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
                        void* y, void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same forward with the output of the layer's SHARED expert(s) added (Qwen / DeepSeek-style layers, PAPER.md:208,
+ * 362): y = bf16( sum_j topk_w[t][j] FFN_e(x[t]) + y_shared[t] ), the add in fp32 before the single rounding.
+ * y_shared: device bf16 [T][d], 16-byte aligned, computed by the caller (the shared expert is not pruned by FlexMoE). */
+fxm_status fxm_moe_ffn_shared(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
+                              const void* y_shared, void* y, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Same forward with HOST buffers (pinned memory recommended so the copies are asynchronous).  The inputs x [T][d] bf16,
  * topk_ids [T][k] int32 and topk_w [T][k] fp32 are copied on a library-owned side stream into one of two staging
@@ -121,19 +132,40 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
  * copy of call i; `stream` waits for the inputs, runs the kernels of fxm_moe_ffn and copies y [T][d] bf16 back.
  * Contract: the three input buffers must hold their data when the call is made (they are read from call time on, not
  * in `stream` order) and stay unmodified until `stream` has passed this call; y_host is valid once `stream` has passed
- * this call.  Does not synchronise.  workspace >= fxm_workspace_bytes_host(E,d,I,T,k).  On a capturing stream the
- * copies are enqueued in-stream instead.  This is the end-to-end entry point bench.py times as `e2e`. */
+ * this call.  Does not synchronise.  workspace >= fxm_workspace_bytes_host(E,d,I,T,k); the staging sets live at the END
+ * of the buffer.  Calls with the same (workspace, size, T, k) pipeline; a call that changes any of them first waits (on
+ * the device) for the previous host call to finish, because its staging area may lie on memory that call still uses.
+ * On a capturing stream the copies are enqueued in-stream instead.  This is the end-to-end entry point bench.py times as `e2e`. */
 fxm_status fxm_workspace_bytes_host(int E, int d, int I, int T_max, int k, size_t* bytes);
 fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
                             int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- offline clipping: PAPER.md:222 ("the pruned subnet is exported as a standalone fixed-budget checkpoint"),
+ * Table 2 PAPER.md:201-206 ------------------------------------------------------------------------------------------
+ * A clipped blob holds only the retained prefix of every expert -- ceil(r_e / 64) channel blocks of gate/up and of down,
+ * back to back -- plus a 2 KB self-describing header and the small tail (budget tables, state).  Its size is linear in
+ * the retained fraction (the law Table 2's checkpoint sizes follow).  The blob is position independent: copy it to
+ * the host / a file and back, then fxm_load_clipped. */
+fxm_status fxm_clipped_bytes(int E, int d, int I, const int32_t* r_host /* [E] */, size_t* bytes);
+/* Device kernel copies the retained tiles of L (widths r_host [E], HOST; r_e <= I, and <= the exported widths if L is
+ * itself clipped) into blob (device, 1024-byte aligned, >= fxm_clipped_bytes).  Stream-ordered, L is not modified. */
+fxm_status fxm_export_clipped(fxm_layer* L, const int32_t* r_host, void* blob, size_t blob_bytes, void* stream);
+/* Reads E, d, I and the widths r [E] (r_out has room for 256) from the first 2 KB of a blob copied to HOST memory. */
+fxm_status fxm_parse_clipped_header(const void* host_bytes, size_t n, int* E, int* d, int* I, int32_t* r_out);
+/* A layer handle over a clipped blob (device).  The exported table is installed as the current budget, so
+ * fxm_moe_ffn works at once with static widths; fxm_set_budget / fxm_register_budgets accept only tables with
+ * r_e <= the exported r_e (nested sub-budgets of the clipped checkpoint), else FXM_EBUDGET.  Same kernels, same
+ * workspace sizes as the full layer. */
+fxm_status fxm_load_clipped(fxm_layer** out, int E, int d, int I, const int32_t* r_host, void* blob, size_t blob_bytes,
+                            void* stream);
+
 /* ---- measurement surface -------------------------------------------------------------------------------
  * Per-kernel device times of fxm_moe_ffn: between fxm_profile_begin and fxm_profile_end every
  * fxm_moe_ffn call (at most max_calls of them, <= 4096) records a CUDA event on its stream before each of its
- * FXM_N_KERNELS launches and after the last.  fxm_profile_end synchronises those events and writes, per kernel
- * (order: route plan, scatter, gather, GEMM-1+SwiGLU, GEMM-2, combine, fused decode kernel), the SUM of its durations in milliseconds over
- * the *calls recorded; events are host objects, no device memory is allocated. */
-#define FXM_N_KERNELS 7
+ * launches and after the last.  fxm_profile_end synchronises those events and writes, per kernel (order: route,
+ * GEMM-1+SwiGLU, GEMM-2+scale+scatter-add, finalize, fused decode kernel), the SUM of its durations in milliseconds
+ * over the *calls recorded; events are host objects, no device memory is allocated. */
+#define FXM_N_KERNELS 5
 fxm_status fxm_profile_begin(fxm_layer* L, int max_calls);
 fxm_status fxm_profile_end(fxm_layer* L, float* ms_sum /* [FXM_N_KERNELS] */, int* calls);
 
@@ -147,26 +179,31 @@ fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_
  * Wg [r][d], Wu [r][d], Wd [d][r] (device).  Test surface and the offline-clipping export. */
 fxm_status fxm_unpack_prefix(fxm_layer* L, int e, int r, void* Wg, void* Wu, void* Wd, void* stream);
 
-/* Copy the internal SwiGLU activations of the LAST moe_ffn on this workspace into row-major bf16
- * H_out [T*k][I] in sorted (perm) order; columns >= r_e are 0.  Debug only. */
-fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k, void* workspace, void* H_out,
+/* Copy the internal SwiGLU activations of the LAST general-path moe_ffn on this workspace into row-major bf16
+ * H_out [T*k][I] in sorted (perm) order.  raw = 0: columns >= r_e read as 0 (the definition).  raw = 1: no reader-side
+ * mask -- every column below ceil64(r_e) is returned exactly as the GEMM-1 epilogue wrote it (the columns
+ * [r_e, ceil64(r_e)) must be exact zeros by the pad-zero rule); blocks that were never issued read 0.
+ * Debug only. */
+fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k, void* workspace, void* H_out, int raw,
                             void* stream);
 
 fxm_status fxm_set_impl(fxm_layer* L, int impl);          /* FXM_IMPL_* ; default FXM_IMPL_TCGEN05 */
-/* Token-tile width of the grouped GEMMs: 128, 256, or 0 = choose from T*k/E (default).  Tuning knob only. */
+/* Most rows of a token tile of the grouped GEMMs: 128, 256, 512, or 0 = default (512).  Tuning knob only. */
 fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
 /* Step a6: calls with T*k <= max_assignments (<= 1024; 0 = never) run as ONE launch of the fused
- * weight-streaming decode kernel instead of the five launches above; prefetch_tiles = how many 16 KB weight tiles
+ * weight-streaming decode kernel instead of the four launches above; prefetch_tiles = how many 16 KB weight tiles
  * its L2 prefetch cursor runs ahead of the shared-memory ring (0..256).  Tuning knob only: results agree within
  * the stated tolerance either way.  Needs d <= 3840, else the general path is used regardless. */
 #define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 768
 #define FXM_DECODE_DEFAULT_PREFETCH 0
 fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles);
 /* Synchronises `stream`, then returns the sticky device flag word (bit0: expert id out of range,
- * bit1: a pipeline wait timed out -- a bug) in *flags and clears it. */
+ * bit1: a pipeline wait timed out -- a bug) in *flags and clears it.  A timed-out wait traps the kernel, which kills
+ * the CUDA context: bit1 is therefore also written to a pinned host word first, and this call still reports it
+ * (together with FXM_ECUDA) when the device can no longer be read. */
 fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream);
-/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode), 5 (product path: plan, scatter, GEMM-1 with
- * the gather fused, GEMM-2, combine) or 6 (debug paths with the separate gather kernel); bench.py's gpu_launches. */
+/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode) or 4 (route, GEMM-1, GEMM-2,
+ * finalize); bench.py's gpu_launches. */
 int fxm_launches_per_ffn(const fxm_layer* L);
 
 const char* fxm_status_string(fxm_status s);

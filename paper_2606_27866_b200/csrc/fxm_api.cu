@@ -4,6 +4,7 @@
 #include "fxm_internal.cuh"
 
 #include <algorithm>
+#include <cstring>
 #include <new>
 #include <vector>
 
@@ -11,18 +12,23 @@ using namespace fxm;
 
 struct fxm_layer {
     Dims D;
-    uint8_t* packed;         // caller's buffer: [gate/up tiles][down tiles][tables][state][channel_rank copy]
+    LayerView V;             // where the weight tiles live (inside the caller's packed / clipped blob)
+    uint8_t* blob;           // caller's buffer
     int* tables;             // [MAX_TABLES][TABLE_STRIDE] int32
     DevState* state;
+    int* rank_dev;           // device copy of channel_rank (full layers packed with a ranking), else null
+    int clipped;             // 1: offline-clipped layer: widths are bounded by r_clip
+    std::vector<int> r_clip; // [E] exported widths of a clipped layer
     int n_registered;
     int current;             // index of the table the next moe_ffn reads; -1 = none installed
     int impl;
     int num_sms;
-    int tile_n_override;     // 0 = choose from T*k/E
+    int tile_n_override;     // 0 = PAIR_TILE_N
     int dec_max_A;           // the fused decode kernel takes calls with T*k <= dec_max_A (0 = never)
     int dec_pf;              // its L2 prefetch distance in 16 KB tiles
     int last_launches;       // kernels enqueued by the last fxm_moe_ffn
-    alignas(64) unsigned char x_map[128];   // CUtensorMap over the x of the last pair-path call (gather4 source)
+    uint32_t* host_flags;    // pinned, device-mapped word: bit1 (pipeline timeout) survives a trapped context
+    alignas(64) unsigned char x_map[128];   // CUtensorMap over the x of the last general-path call (gather4 source)
     const void* x_map_ptr;   // the x it was encoded for
     int x_map_T;
     std::vector<int> host_tables;   // mirror of the resident tables (validation / introspection only)
@@ -31,7 +37,11 @@ struct fxm_layer {
     cudaStream_t h2d_stream;
     cudaEvent_t ev_in[2];    // inputs of set b have landed (recorded on h2d_stream)
     cudaEvent_t ev_done[2];  // the kernels that read set b have finished (recorded on the caller's stream)
+    cudaEvent_t ev_tail;     // the whole previous host call (kernels + y copy) has finished
     unsigned host_calls;
+    const void* host_ws;     // layout key of the previous host call: (workspace, bytes, T, k)
+    size_t host_ws_bytes;
+    int host_T, host_k;
     std::vector<cudaEvent_t> prof_events;   // fxm_profile_begin: (FXM_N_KERNELS + 1) events per recorded call
     int prof_capacity;       // calls that can still be recorded
     int prof_calls;          // calls recorded so far
@@ -53,23 +63,81 @@ static bool make_dims(int E, int d, int I, Dims* D) {
     return true;
 }
 
-static size_t tables_offset(const Dims& D) { return align_up(gu_bytes(D) + dn_bytes(D), 1024); }
-static size_t state_offset(const Dims& D) { return tables_offset(D) + sizeof(int) * MAX_TABLES * TABLE_STRIDE; }
-static size_t rank_offset(const Dims& D) { return align_up(state_offset(D) + sizeof(DevState), 1024); }
-static size_t packed_total(const Dims& D) { return align_up(rank_offset(D) + sizeof(int) * (size_t)D.E * D.I, 1024); }
-
-static bool is_pair(const fxm_layer* L) { return L->impl == FXM_IMPL_TCGEN05 || L->impl == FXM_IMPL_TCGEN05_XS; }
-static int choose_tile_n(const fxm_layer* L, int T, int k) {
-    if (is_pair(L)) return PAIR_TILE_N;         // CTA-pair kernels: one or two 256-token sub-tiles
-    if (L->tile_n_override == 128 || L->tile_n_override == 256) return L->tile_n_override;
-    // mean rows per expert > 192: 256-token tiles halve the weight re-reads; below that 128 wastes less
-    return ((long long)T * k > 192LL * L->D.E) ? 256 : 128;
+// tail of a blob, after `wbytes` of weight tiles: [16 budget tables][state][eblk][channel_rank copy (full layers only)]
+struct Tail { size_t tables, state, eblk, rank, total; };
+static Tail tail_map(const Dims& D, size_t wbytes, bool with_rank) {
+    Tail t;
+    t.tables = align_up(wbytes, 1024);
+    t.state = t.tables + sizeof(int) * MAX_TABLES * TABLE_STRIDE;
+    t.eblk = align_up(t.state + sizeof(DevState), 1024);
+    t.rank = align_up(t.eblk + sizeof(uint32_t) * MAX_E, 1024);
+    t.total = with_rank ? align_up(t.rank + sizeof(int) * (size_t)D.E * D.I, 1024) : t.rank;
+    return t;
 }
-static int plan_grp(const fxm_layer* L) { return is_pair(L) ? 2 : 1; }
+static size_t packed_total(const Dims& D) { return tail_map(D, gu_bytes(D) + dn_bytes(D), true).total; }
+
+// ---- clipped blob (offline clipping): [header 2 KB][gate/up tiles of the retained blocks][down tiles][tail]
+constexpr uint32_t CLIP_MAGIC = 0x4D584643u;    // "CFXM"
+constexpr size_t CLIP_HEADER_BYTES = 2048;
+struct ClipHeader { uint32_t magic, version; int32_t E, d, I, reserved[3]; int32_t r[MAX_E]; };
+static_assert(sizeof(ClipHeader) <= CLIP_HEADER_BYTES, "clip header");
+static size_t clip_blocks(const Dims& D, const int32_t* r) {
+    size_t nb = 0;
+    for (int e = 0; e < D.E; ++e) nb += (size_t)((r[e] + CB - 1) / CB);
+    return nb;
+}
+static size_t clip_gu_bytes(const Dims& D, const int32_t* r) { return clip_blocks(D, r) * D.nKB1 * WT_BYTES; }
+static size_t clip_dn_bytes(const Dims& D, const int32_t* r) { return clip_blocks(D, r) * D.nDB * WT_BYTES; }
+static size_t clip_total(const Dims& D, const int32_t* r) {
+    return tail_map(D, CLIP_HEADER_BYTES + clip_gu_bytes(D, r) + clip_dn_bytes(D, r), false).total;
+}
+
+static int choose_tile_n(const fxm_layer* L) { return L->tile_n_override ? L->tile_n_override : PAIR_TILE_N; }
 // a6: decode-sized calls (a handful of tokens per expert) go to the single-launch weight-streaming kernel
 static bool use_decode(const fxm_layer* L, int T, int k) {
     const long long A = (long long)T * k;
     return L->impl == FXM_IMPL_TCGEN05 && A <= L->dec_max_A && A <= DEC_MAX_A && decode_supported(L->D);
+}
+
+static fxm_layer* new_layer(const Dims& D, uint8_t* blob, const Tail& tl, int sms) {
+    fxm_layer* L = new (std::nothrow) fxm_layer();
+    if (!L) return nullptr;
+    L->D = D; L->blob = blob;
+    L->tables = (int*)(blob + tl.tables);
+    L->state = (DevState*)(blob + tl.state);
+    L->V.eblk = (const uint32_t*)(blob + tl.eblk);
+    L->rank_dev = nullptr; L->clipped = 0;
+    L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
+    L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
+    L->prof_capacity = 0; L->prof_calls = 0;
+    L->x_map_ptr = nullptr; L->x_map_T = -1;
+    L->h2d_stream = nullptr; L->host_calls = 0; L->ev_tail = nullptr;
+    L->host_ws = nullptr; L->host_ws_bytes = 0; L->host_T = -1; L->host_k = -1;
+    for (int b = 0; b < 2; ++b) { L->ev_in[b] = nullptr; L->ev_done[b] = nullptr; }
+    L->dec_max_A = FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS; L->dec_pf = FXM_DECODE_DEFAULT_PREFETCH; L->last_launches = 0;
+    L->host_flags = nullptr;
+    return L;
+}
+
+// zero the tables + state of a blob and point the state's host flag at a fresh pinned word
+static fxm_status init_tail(fxm_layer* L, cudaStream_t st) {
+    if (cudaMemsetAsync(L->tables, 0, sizeof(int) * MAX_TABLES * TABLE_STRIDE + sizeof(DevState), st) != cudaSuccess)
+        return FXM_ECUDA;
+    void* hp = nullptr;
+    if (cudaHostAlloc(&hp, 64, cudaHostAllocMapped) == cudaSuccess && hp) {
+        std::memset(hp, 0, 64);
+        void* dp = nullptr;
+        if (cudaHostGetDevicePointer(&dp, hp, 0) == cudaSuccess && dp) {
+            L->host_flags = (uint32_t*)hp;
+            // a copy from pageable host memory is staged before the call returns, so the stack variable may go away
+            if (cudaMemcpyAsync(&L->state->hflag, &dp, sizeof(dp), cudaMemcpyHostToDevice, st) != cudaSuccess) return FXM_ECUDA;
+        } else {
+            cudaFreeHost(hp);
+        }
+    } else {
+        (void)cudaGetLastError();      // no mapped memory: the device flag word alone remains
+    }
+    return FXM_OK;
 }
 
 extern "C" {
@@ -80,11 +148,12 @@ const char* fxm_status_string(fxm_status s) {
         case FXM_EINVAL: return "FXM_EINVAL: bad pointer, size or enum";
         case FXM_ESHAPE: return "FXM_ESHAPE: unsupported dimensions";
         case FXM_EPERM: return "FXM_EPERM: channel_rank row is not a permutation";
-        case FXM_EBUDGET: return "FXM_EBUDGET: width outside [0, I] or unknown budget index";
+        case FXM_EBUDGET: return "FXM_EBUDGET: width outside [0, I] (or above the exported width of a clipped layer) or unknown budget index";
         case FXM_ENOTNESTED: return "FXM_ENOTNESTED: budget tables are not nested";
         case FXM_EWORKSPACE: return "FXM_EWORKSPACE: workspace too small";
         case FXM_ESTATE: return "FXM_ESTATE: no budget installed";
         case FXM_ECUDA: return "FXM_ECUDA: CUDA runtime failure";
+        case FXM_ENOMEM: return "FXM_ENOMEM: host allocation failed";
     }
     return "FXM_?";
 }
@@ -122,6 +191,14 @@ int32_t fxm_ratio_to_width(int I, int num, int den) {
     return (int32_t)(((int64_t)I * num + den - 1) / den);
 }
 
+static fxm_status device_info(int* sms) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return FXM_ECUDA;
+    if (cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return FXM_ECUDA;
+    if (init_pair_kernels() != cudaSuccess || init_decode_kernel() != cudaSuccess) return FXM_ECUDA;
+    return FXM_OK;
+}
+
 fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down,
                     const int32_t* channel_rank, void* packed, void* stream) {
     Dims D;
@@ -140,34 +217,25 @@ fxm_status fxm_pack(fxm_layer** out, int E, int d, int I, const void* W_gate, co
             }
         }
     }
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return FXM_ECUDA;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return FXM_ECUDA;
-    if (init_sm100_kernels() != cudaSuccess || init_pair_kernels() != cudaSuccess || init_decode_kernel() != cudaSuccess)
-        return FXM_ECUDA;
+    int sms = 0;
+    fxm_status s = device_info(&sms);
+    if (s != FXM_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     uint8_t* pk = (uint8_t*)packed;
-    int* tables = (int*)(pk + tables_offset(D));
-    DevState* state = (DevState*)(pk + state_offset(D));
-    int* rank_dev = channel_rank ? (int*)(pk + rank_offset(D)) : nullptr;
-    if (cudaMemsetAsync(tables, 0, sizeof(int) * MAX_TABLES * TABLE_STRIDE + sizeof(DevState), st) != cudaSuccess)
-        return FXM_ECUDA;
-    if (rank_dev && cudaMemcpyAsync(rank_dev, channel_rank, sizeof(int) * (size_t)E * I, cudaMemcpyHostToDevice, st) !=
-                        cudaSuccess)
-        return FXM_ECUDA;
-    if (launch_pack(D, (const __nv_bfloat16*)W_gate, (const __nv_bfloat16*)W_up, (const __nv_bfloat16*)W_down, rank_dev,
-                    pk, st) != cudaSuccess)
-        return FXM_ECUDA;
-    fxm_layer* L = new (std::nothrow) fxm_layer();
-    if (!L) return FXM_EINVAL;
-    L->D = D; L->packed = pk; L->tables = tables; L->state = state;
-    L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
-    L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
-    L->prof_capacity = 0; L->prof_calls = 0;
-    L->x_map_ptr = nullptr; L->x_map_T = -1;
-    L->h2d_stream = nullptr; L->host_calls = 0;
-    for (int b = 0; b < 2; ++b) { L->ev_in[b] = nullptr; L->ev_done[b] = nullptr; }
-    L->dec_max_A = FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS; L->dec_pf = FXM_DECODE_DEFAULT_PREFETCH; L->last_launches = 0;
+    const Tail tl = tail_map(D, gu_bytes(D) + dn_bytes(D), true);
+    fxm_layer* L = new_layer(D, pk, tl, sms);
+    if (!L) return FXM_ENOMEM;
+    L->V.gu = pk;
+    L->V.dn = pk + gu_bytes(D);
+    L->rank_dev = channel_rank ? (int*)(pk + tl.rank) : nullptr;
+    s = init_tail(L, st);
+    if (s == FXM_OK && L->rank_dev &&
+        cudaMemcpyAsync(L->rank_dev, channel_rank, sizeof(int) * (size_t)E * I, cudaMemcpyHostToDevice, st) != cudaSuccess)
+        s = FXM_ECUDA;
+    if (s == FXM_OK && launch_pack(D, (const __nv_bfloat16*)W_gate, (const __nv_bfloat16*)W_up, (const __nv_bfloat16*)W_down,
+                                   L->rank_dev, pk, (uint32_t*)(pk + tl.eblk), st) != cudaSuccess)
+        s = FXM_ECUDA;
+    if (s != FXM_OK) { fxm_destroy(L); return s; }
     *out = L;
     return FXM_OK;
 }
@@ -179,13 +247,17 @@ void fxm_destroy(fxm_layer* L) {
         if (L->ev_in[b]) cudaEventDestroy(L->ev_in[b]);
         if (L->ev_done[b]) cudaEventDestroy(L->ev_done[b]);
     }
+    if (L->ev_tail) cudaEventDestroy(L->ev_tail);
     if (L->h2d_stream) cudaStreamDestroy(L->h2d_stream);
+    if (L->host_flags) cudaFreeHost(L->host_flags);
     delete L;
 }
 
 static fxm_status check_table(const fxm_layer* L, const int32_t* r) {
-    for (int e = 0; e < L->D.E; ++e)
+    for (int e = 0; e < L->D.E; ++e) {
         if (r[e] < 0 || r[e] > L->D.I) return FXM_EBUDGET;
+        if (L->clipped && r[e] > L->r_clip[e]) return FXM_EBUDGET;      // those channels were not exported
+    }
     return FXM_OK;
 }
 
@@ -229,13 +301,13 @@ fxm_status fxm_select_budget(fxm_layer* L, int b) {
 }
 
 fxm_status fxm_set_impl(fxm_layer* L, int impl) {
-    if (!L || impl < FXM_IMPL_TCGEN05 || impl > FXM_IMPL_TCGEN05_XS) return FXM_EINVAL;
+    if (!L || (impl != FXM_IMPL_TCGEN05 && impl != FXM_IMPL_SIMT_DEBUG)) return FXM_EINVAL;
     L->impl = impl;
     return FXM_OK;
 }
 
 fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n) {
-    if (!L || (tile_n != 0 && tile_n != 128 && tile_n != 256)) return FXM_EINVAL;
+    if (!L || (tile_n != 0 && tile_n != 128 && tile_n != 256 && tile_n != 512)) return FXM_EINVAL;
     L->tile_n_override = tile_n;
     return FXM_OK;
 }
@@ -294,28 +366,28 @@ fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_
     if (s != FXM_OK) return s;
     if (!counts || !offsets || (T > 0 && (!topk_ids || !perm || !inv_perm))) return FXM_EINVAL;
     const Workspace ws = map_workspace(L->D, T, k, workspace);
-    const int* table = L->current >= 0 ? L->tables + (size_t)L->current * TABLE_STRIDE : nullptr;
-    if (launch_route_plan(L->D, topk_ids, T, k, table, choose_tile_n(L, T, k), plan_grp(L), counts, offsets, ws, L->state,
-                          (cudaStream_t)stream) != cudaSuccess)
-        return FXM_ECUDA;
-    if (launch_scatter(L->D, topk_ids, T, k, table, counts, offsets, perm, inv_perm, ws, (cudaStream_t)stream) !=
-        cudaSuccess)
-        return FXM_ECUDA;
+    RouteArgs a{};
+    a.D = L->D; a.ids = topk_ids; a.topk_w = nullptr;
+    a.r_table = L->current >= 0 ? L->tables + (size_t)L->current * TABLE_STRIDE : nullptr;
+    a.T = T; a.k = k; a.tile_n = choose_tile_n(L);
+    a.counts = counts; a.offsets = offsets; a.perm = perm; a.inv_perm = inv_perm;
+    if (launch_route(a, ws, L->state, (cudaStream_t)stream) != cudaSuccess) return FXM_ECUDA;
     return FXM_OK;
 }
 
-fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k, void* y,
-                       void* workspace, size_t workspace_bytes, void* stream) {
+// the forward with every optional input: y_add (shared-expert output, may be null)
+static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
+                           const void* y_add, void* y, void* workspace, size_t workspace_bytes, void* stream) {
     fxm_status s = check_call(L, T, k, workspace, workspace_bytes);
     if (s != FXM_OK) return s;
     if (T == 0) return FXM_OK;
-    if (!x || !topk_ids || !topk_w || !y || ((uintptr_t)x & 15u) || ((uintptr_t)y & 7u)) return FXM_EINVAL;
+    if (!x || !topk_ids || !topk_w || !y || ((uintptr_t)x & 15u) || ((uintptr_t)y & 15u) || ((uintptr_t)y_add & 15u))
+        return FXM_EINVAL;
     if (L->current < 0) return FXM_ESTATE;
     const Dims& D = L->D;
     cudaStream_t st = (cudaStream_t)stream;
     const Workspace ws = map_workspace(D, T, k, workspace);
     const int* table = L->tables + (size_t)L->current * TABLE_STRIDE;
-    const int tile_n = choose_tile_n(L, T, k);
     cudaEvent_t* ev = nullptr;                                    // per-kernel timing, only between profile_begin/end
     if (L->prof_capacity > 0) {
         ev = &L->prof_events[(size_t)L->prof_calls * (FXM_N_KERNELS + 1)];
@@ -326,53 +398,54 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
     if (use_decode(L, T, k)) {
         // a6: one launch does a2..a5 (in-kernel grouping, weight streaming, SwiGLU, scale + combine)
         for (int j = 0; j < FXM_N_KERNELS; ++j) FXM_MARK(j)
-        if (launch_decode(D, L->packed, table, (const __nv_bfloat16*)x, topk_ids, topk_w, T, k, ws.yacc,
-                          (__nv_bfloat16*)y, L->state, L->num_sms, L->dec_pf, st) != cudaSuccess)
+        if (launch_decode(D, L->V, table, (const __nv_bfloat16*)x, topk_ids, topk_w, T, k, ws.yacc,
+                          (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->num_sms, L->dec_pf, st) != cudaSuccess)
             return FXM_ECUDA;
         FXM_MARK(FXM_N_KERNELS)
         L->last_launches = 1;
         return FXM_OK;
     }
-    // a2 + a3: grouping and the tile schedule for the CURRENT table
+    // a2 + a3: grouping and the tile schedule for the CURRENT table, one launch
     FXM_MARK(0)
-    if (launch_route_plan(D, topk_ids, T, k, table, tile_n, plan_grp(L), ws.counts, ws.offsets, ws, L->state, st) != cudaSuccess)
-        return FXM_ECUDA;
-    // stable scatter of the indices
+    RouteArgs ra{};
+    ra.D = D; ra.ids = topk_ids; ra.topk_w = topk_w; ra.r_table = table; ra.T = T; ra.k = k; ra.tile_n = choose_tile_n(L);
+    ra.counts = ws.counts; ra.offsets = ws.offsets; ra.perm = ws.perm; ra.inv_perm = ws.inv_perm;
+    if (launch_route(ra, ws, L->state, st) != cudaSuccess) return FXM_ECUDA;
     FXM_MARK(1)
-    if (launch_scatter(D, topk_ids, T, k, table, ws.counts, ws.offsets, ws.perm, ws.inv_perm, ws, st) != cudaSuccess)
-        return FXM_ECUDA;
-    // X[pi] (Alg. 2 l.7): the product path gathers the token rows inside GEMM-1 (TMA gather4 straight from x); the
-    // other paths copy them into sorted swizzled panels first
-    FXM_MARK(2)
-    const bool fused_gather = L->impl == FXM_IMPL_TCGEN05;
-    if (fused_gather) {
+    if (L->impl == FXM_IMPL_TCGEN05) {
+        // a4 with X[pi] (Alg. 2 l.7) fused: the token rows come straight from x through a tensor map (TMA gather4)
         if (L->x_map_ptr != x || L->x_map_T != T) {
             if (encode_x_map(x, T, D.d, L->x_map) != cudaSuccess) return FXM_ECUDA;
             L->x_map_ptr = x; L->x_map_T = T;
         }
-    } else if (launch_gather(D, (const __nv_bfloat16*)x, T, k, ws, st) != cudaSuccess) return FXM_ECUDA;
-    FXM_MARK(3)
-    if (is_pair(L)) {
-        if (launch_gemm1_pair(D, L->packed, table, ws, L->state, L->num_sms, fused_gather ? L->x_map : nullptr, st) != cudaSuccess)
-            return FXM_ECUDA;
-        FXM_MARK(4)
-        if (launch_gemm2_pair(D, L->packed, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
-    } else if (L->impl == FXM_IMPL_TCGEN05_1CTA) {
-        if (launch_gemm1_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
-        FXM_MARK(4)
-        if (launch_gemm2_sm100(D, L->packed, table, ws, L->state, tile_n, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
+        if (launch_gemm1_pair(D, L->V, table, ws, T, L->state, L->num_sms, L->x_map, st) != cudaSuccess) return FXM_ECUDA;
+        FXM_MARK(2)
+        // a5: down projection, router-weight scale and scatter-add in one kernel
+        if (launch_gemm2_pair(D, L->V, table, ws, L->state, L->num_sms, st) != cudaSuccess) return FXM_ECUDA;
     } else {
-        if (launch_gemm1_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
-        FXM_MARK(4)
-        if (launch_gemm2_simt(D, L->packed, table, ws, st) != cudaSuccess) return FXM_ECUDA;
+        if (cudaMemsetAsync(ws.yacc, 0, (size_t)T * D.d * sizeof(float), st) != cudaSuccess) return FXM_ECUDA;
+        if (launch_gemm1_simt(D, L->V, table, (const __nv_bfloat16*)x, ws, st) != cudaSuccess) return FXM_ECUDA;
+        FXM_MARK(2)
+        if (launch_gemm2_simt(D, L->V, table, ws, st) != cudaSuccess) return FXM_ECUDA;
     }
+    FXM_MARK(3)
+    if (launch_finalize(D, T, ws.yacc, (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
+    FXM_MARK(4)
     FXM_MARK(5)
-    if (launch_combine(D, T, k, topk_w, ws, (__nv_bfloat16*)y, st) != cudaSuccess) return FXM_ECUDA;
-    FXM_MARK(6)
-    FXM_MARK(7)
 #undef FXM_MARK
-    L->last_launches = fused_gather ? 5 : 6;
+    L->last_launches = 4;
     return FXM_OK;
+}
+
+fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k, void* y,
+                       void* workspace, size_t workspace_bytes, void* stream) {
+    return ffn_impl(L, x, topk_ids, topk_w, T, k, nullptr, y, workspace, workspace_bytes, stream);
+}
+
+fxm_status fxm_moe_ffn_shared(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
+                              const void* y_shared, void* y, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!y_shared) return FXM_EINVAL;
+    return ffn_impl(L, x, topk_ids, topk_w, T, k, y_shared, y, workspace, workspace_bytes, stream);
 }
 
 fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
@@ -380,14 +453,16 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
     if (!L || T < 0 || !workspace || ((uintptr_t)workspace & 1023u)) return FXM_EINVAL;
     if (k < 1 || k > MAX_K || k > L->D.E || (long long)T * k > (1LL << 30)) return FXM_ESHAPE;
     const size_t inner = map_workspace(L->D, T, k, nullptr).bytes;
-    if (workspace_bytes < inner + host_stage_bytes(L->D, T, k)) return FXM_EWORKSPACE;
+    const size_t stage = host_stage_bytes(L->D, T, k);
+    if (workspace_bytes < inner + stage) return FXM_EWORKSPACE;
     if (T == 0) return FXM_OK;
     if (!x_host || !topk_ids_host || !topk_w_host || !y_host) return FXM_EINVAL;
     if (L->current < 0) return FXM_ESTATE;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t xb = (size_t)T * L->D.d * 2, ab = (size_t)T * k * 4;
     const size_t xs = align_up(xb, 1024), as = align_up(ab, 1024);
-    uint8_t* p = (uint8_t*)workspace + inner;
+    // the staging area sits at the END of the buffer, so it never overlaps the compute workspace of this call
+    uint8_t* p = (uint8_t*)workspace + (workspace_bytes & ~(size_t)1023) - stage;
     uint8_t* yd = p;
     p += xs;
     // a capturing stream cannot wait on events recorded outside the capture: copy in-stream then (no overlap)
@@ -400,12 +475,21 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
             if (cudaEventCreateWithFlags(&L->ev_in[b], cudaEventDisableTiming) != cudaSuccess ||
                 cudaEventCreateWithFlags(&L->ev_done[b], cudaEventDisableTiming) != cudaSuccess)
                 return FXM_ECUDA;
+        if (cudaEventCreateWithFlags(&L->ev_tail, cudaEventDisableTiming) != cudaSuccess) return FXM_ECUDA;
+    }
+    cudaStream_t cs = side ? L->h2d_stream : st;
+    // A different (workspace, size, T, k) than the previous host call moves the staging sets -- possibly onto memory the
+    // previous call is still using (its compute workspace, its input sets, its y).  Then the copies wait for the WHOLE
+    // previous call, and the set rotation starts over (both sets are free once that call is done).
+    const bool same_layout = L->host_ws == workspace && L->host_ws_bytes == workspace_bytes && L->host_T == T && L->host_k == k;
+    if (side && !same_layout) {
+        if (L->host_ws && cudaStreamWaitEvent(cs, L->ev_tail, 0) != cudaSuccess) return FXM_ECUDA;
+        L->host_calls = 0;
     }
     const unsigned set = side ? (L->host_calls & 1u) : 0u;
     uint8_t* xd = p + set * (xs + 2 * as);
     uint8_t* idd = xd + xs;
     uint8_t* wd = idd + as;
-    cudaStream_t cs = side ? L->h2d_stream : st;
     // the staging set is free once the kernels of the call before last (same set) have read it
     if (side && L->host_calls >= 2 && cudaStreamWaitEvent(cs, L->ev_done[set], 0) != cudaSuccess) return FXM_ECUDA;
     if (cudaMemcpyAsync(xd, x_host, xb, cudaMemcpyHostToDevice, cs) != cudaSuccess) return FXM_ECUDA;
@@ -417,32 +501,113 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
     }
     fxm_status s = fxm_moe_ffn(L, xd, (const int32_t*)idd, (const float*)wd, T, k, yd, workspace, inner, stream);
     if (s != FXM_OK) return s;
-    if (side) {
-        if (cudaEventRecord(L->ev_done[set], st) != cudaSuccess) return FXM_ECUDA;
-        ++L->host_calls;
-    }
+    if (side && cudaEventRecord(L->ev_done[set], st) != cudaSuccess) return FXM_ECUDA;
     if (cudaMemcpyAsync(y_host, yd, xb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return FXM_ECUDA;
+    if (side) {
+        if (cudaEventRecord(L->ev_tail, st) != cudaSuccess) return FXM_ECUDA;
+        ++L->host_calls;
+        L->host_ws = workspace; L->host_ws_bytes = workspace_bytes; L->host_T = T; L->host_k = k;
+    }
     return FXM_OK;
 }
 
 fxm_status fxm_unpack_prefix(fxm_layer* L, int e, int r, void* Wg, void* Wu, void* Wd, void* stream) {
     if (!L || e < 0 || e >= L->D.E) return FXM_EINVAL;
-    if (r < 0 || r > L->D.I) return FXM_EBUDGET;
+    if (r < 0 || r > L->D.I || (L->clipped && r > L->r_clip[e])) return FXM_EBUDGET;
     if (r == 0) return FXM_OK;
     if (!Wg || !Wu || !Wd) return FXM_EINVAL;
-    if (launch_unpack_prefix(L->D, L->packed, e, r, (__nv_bfloat16*)Wg, (__nv_bfloat16*)Wu, (__nv_bfloat16*)Wd,
+    if (launch_unpack_prefix(L->D, L->V, e, r, (__nv_bfloat16*)Wg, (__nv_bfloat16*)Wu, (__nv_bfloat16*)Wd,
                              (cudaStream_t)stream) != cudaSuccess)
         return FXM_ECUDA;
     return FXM_OK;
 }
 
-fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k, void* workspace, void* H_out,
+// ---- offline clipping (Table 2) ------------------------------------------------------
+
+fxm_status fxm_clipped_bytes(int E, int d, int I, const int32_t* r_host, size_t* bytes) {
+    Dims D;
+    if (!bytes || !r_host) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    for (int e = 0; e < E; ++e)
+        if (r_host[e] < 0 || r_host[e] > I) return FXM_EBUDGET;
+    *bytes = clip_total(D, r_host);
+    return FXM_OK;
+}
+
+fxm_status fxm_export_clipped(fxm_layer* L, const int32_t* r_host, void* blob, size_t blob_bytes, void* stream) {
+    if (!L || !r_host || !blob || ((uintptr_t)blob & 1023u)) return FXM_EINVAL;
+    fxm_status s = check_table(L, r_host);
+    if (s != FXM_OK) return s;
+    const Dims& D = L->D;
+    if (blob_bytes < clip_total(D, r_host)) return FXM_EWORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint8_t* b = (uint8_t*)blob;
+    const size_t gub = clip_gu_bytes(D, r_host), dnb = clip_dn_bytes(D, r_host);
+    const Tail tl = tail_map(D, CLIP_HEADER_BYTES + gub + dnb, false);
+    // header: self-description of the blob (fxm_parse_clipped_header reads it back from a host copy).  The words travel
+    // in kernel arguments (two tiny launches): no pageable-memory copy, nothing synchronises.
+    if (cudaMemsetAsync(b + tl.tables, 0, tl.total - tl.tables, st) != cudaSuccess) return FXM_ECUDA;
+    int32_t head[8] = {(int32_t)CLIP_MAGIC, 1, D.E, D.d, D.I, 0, 0, 0};
+    static_assert(offsetof(ClipHeader, r) == 32, "clip header layout");
+    if (cudaMemsetAsync(b, 0, CLIP_HEADER_BYTES, st) != cudaSuccess) return FXM_ECUDA;
+    if (launch_set_table((int*)b, head, 8, st) != cudaSuccess) return FXM_ECUDA;              // words 0..7, zeros up to 255
+    if (launch_set_table((int*)(b + 32), r_host, D.E, st) != cudaSuccess) return FXM_ECUDA;   // r[0..E), zeros after
+    int* tab0 = (int*)(b + tl.tables);                            // table slot 0 of the new blob: the widths the export kernel reads
+    if (launch_set_table(tab0, r_host, D.E, st) != cudaSuccess) return FXM_ECUDA;
+    if (launch_export_clipped(D, L->V, tab0, b + CLIP_HEADER_BYTES, b + CLIP_HEADER_BYTES + gub, (uint32_t*)(b + tl.eblk), st) !=
+        cudaSuccess)
+        return FXM_ECUDA;
+    if (cudaMemsetAsync(tab0, 0, sizeof(int) * TABLE_STRIDE, st) != cudaSuccess) return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_parse_clipped_header(const void* host_bytes, size_t n, int* E, int* d, int* I, int32_t* r_out) {
+    if (!host_bytes || n < sizeof(ClipHeader) || !E || !d || !I || !r_out) return FXM_EINVAL;
+    ClipHeader h;
+    std::memcpy(&h, host_bytes, sizeof(h));
+    Dims D;
+    if (h.magic != CLIP_MAGIC || h.version != 1 || !make_dims(h.E, h.d, h.I, &D)) return FXM_EINVAL;
+    for (int e = 0; e < h.E; ++e)
+        if (h.r[e] < 0 || h.r[e] > h.I) return FXM_EBUDGET;
+    *E = h.E; *d = h.d; *I = h.I;
+    std::copy(h.r, h.r + h.E, r_out);
+    return FXM_OK;
+}
+
+fxm_status fxm_load_clipped(fxm_layer** out, int E, int d, int I, const int32_t* r_host, void* blob, size_t blob_bytes,
+                            void* stream) {
+    Dims D;
+    if (!out || !r_host || !blob || ((uintptr_t)blob & 1023u)) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    for (int e = 0; e < E; ++e)
+        if (r_host[e] < 0 || r_host[e] > I) return FXM_EBUDGET;
+    if (blob_bytes < clip_total(D, r_host)) return FXM_EWORKSPACE;
+    int sms = 0;
+    fxm_status s = device_info(&sms);
+    if (s != FXM_OK) return s;
+    uint8_t* b = (uint8_t*)blob;
+    const size_t gub = clip_gu_bytes(D, r_host), dnb = clip_dn_bytes(D, r_host);
+    const Tail tl = tail_map(D, CLIP_HEADER_BYTES + gub + dnb, false);
+    fxm_layer* L = new_layer(D, b, tl, sms);
+    if (!L) return FXM_ENOMEM;
+    L->V.gu = b + CLIP_HEADER_BYTES;
+    L->V.dn = b + CLIP_HEADER_BYTES + gub;
+    L->clipped = 1;
+    L->r_clip.assign(r_host, r_host + E);
+    s = init_tail(L, (cudaStream_t)stream);       // tables + state start clean (a blob read back from disk carries stale ones)
+    if (s == FXM_OK) s = fxm_set_budget(L, r_host, stream);       // static widths: the exported table is the current one
+    if (s != FXM_OK) { fxm_destroy(L); return s; }
+    *out = L;
+    return FXM_OK;
+}
+
+fxm_status fxm_debug_read_h(fxm_layer* L, const int32_t* topk_ids, int T, int k, void* workspace, void* H_out, int raw,
                             void* stream) {
     if (!L || !workspace || !H_out || !topk_ids || T < 0) return FXM_EINVAL;
     if (L->current < 0) return FXM_ESTATE;
     if (T == 0) return FXM_OK;
     const Workspace ws = map_workspace(L->D, T, k, workspace);
-    if (launch_read_h(L->D, T, k, topk_ids, L->tables + (size_t)L->current * TABLE_STRIDE, ws, (__nv_bfloat16*)H_out,
+    if (launch_read_h(L->D, T, k, topk_ids, L->tables + (size_t)L->current * TABLE_STRIDE, ws, (__nv_bfloat16*)H_out, raw,
                       (cudaStream_t)stream) != cudaSuccess)
         return FXM_ECUDA;
     return FXM_OK;
@@ -452,10 +617,15 @@ fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream) {
     if (!L || !flags) return FXM_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     uint32_t v = 0;
-    if (cudaMemcpyAsync(&v, &L->state->flags, sizeof(v), cudaMemcpyDeviceToHost, st) != cudaSuccess) return FXM_ECUDA;
-    if (cudaMemsetAsync(&L->state->flags, 0, sizeof(v), st) != cudaSuccess) return FXM_ECUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return FXM_ECUDA;
-    *flags = v;
+    const uint32_t hostbits = L->host_flags ? *(volatile uint32_t*)L->host_flags : 0u;   // survives a trapped context
+    if (cudaMemcpyAsync(&v, &L->state->flags, sizeof(v), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemsetAsync(&L->state->flags, 0, sizeof(v), st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
+        *flags = hostbits | (L->host_flags ? *(volatile uint32_t*)L->host_flags : 0u);
+        return FXM_ECUDA;
+    }
+    const uint32_t hb = L->host_flags ? *(volatile uint32_t*)L->host_flags : 0u;
+    if (L->host_flags) *(volatile uint32_t*)L->host_flags = 0u;
+    *flags = v | hb | hostbits;
     return FXM_OK;
 }
 

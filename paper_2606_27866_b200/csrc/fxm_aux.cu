@@ -1,12 +1,12 @@
 // fxm_aux.cu -- the bandwidth-only kernels around the two grouped GEMMs:
-//   pack / unpack_prefix (Eq. 3), set_table (Eq. 11), combine (router-weighted sum of
-//   each token's k expert outputs, one rounding of y to bf16; Alg. 2 l.19-20), read_h (debug).
+//   pack / unpack_prefix (Eq. 3), export_clipped (offline clipping), set_table (Eq. 11,
+//   PAPER.md:129), finalize (the single rounding of y: fp32 accumulator -> bf16, optional shared-expert add), read_h (debug).
 #include "fxm_internal.cuh"
 
 namespace fxm {
 
 // ---------------------------------------------------------------------------------------------- pack
-// one thread per 16-byte chunk of the packed gate/up region
+// one thread per 16-byte chunk of the packed gate/up region (full layer: expert e starts at channel block e * nCB)
 __global__ void k_pack_gu(Dims D, const uint4* __restrict__ Wg, const uint4* __restrict__ Wu,
                           const int* __restrict__ rank, uint4* __restrict__ out, size_t n_chunks) {
     for (size_t g = blockIdx.x * (size_t)blockDim.x + threadIdx.x; g < n_chunks; g += (size_t)gridDim.x * blockDim.x) {
@@ -57,45 +57,105 @@ __global__ void k_pack_dn(Dims D, const uint16_t* __restrict__ Wd, const int* __
     }
 }
 
+__global__ void k_eblk_full(uint32_t* __restrict__ eblk, int E, int nCB) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < E) eblk[e] = (uint32_t)e * (uint32_t)nCB;
+}
+
 cudaError_t launch_pack(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
-                        const int* rank_dev, uint8_t* packed, cudaStream_t st) {
+                        const int* rank_dev, uint8_t* packed, uint32_t* eblk_dev, cudaStream_t st) {
     const size_t n_gu = gu_bytes(D) >> 4, n_dn = dn_bytes(D) >> 4;
     const int threads = 256;
     const int b_gu = (int)((n_gu + threads - 1) / threads < 148 * 64 ? (n_gu + threads - 1) / threads : 148 * 64);
     const int b_dn = (int)((n_dn + threads - 1) / threads < 148 * 64 ? (n_dn + threads - 1) / threads : 148 * 64);
     k_pack_gu<<<b_gu, threads, 0, st>>>(D, (const uint4*)Wg, (const uint4*)Wu, rank_dev, (uint4*)packed, n_gu);
     k_pack_dn<<<b_dn, threads, 0, st>>>(D, (const uint16_t*)Wd, rank_dev, (uint4*)(packed + gu_bytes(D)), n_dn);
+    k_eblk_full<<<1, MAX_E, 0, st>>>(eblk_dev, D.E, D.nCB);
     return cudaGetLastError();
 }
 
 // --------------------------------------------------------------------------------------- unpack_prefix
-__global__ void k_unpack_prefix(Dims D, const uint8_t* __restrict__ packed, int e, int r,
+__global__ void k_unpack_prefix(Dims D, LayerView V, int e, int r,
                                 uint16_t* __restrict__ Wg, uint16_t* __restrict__ Wu, uint16_t* __restrict__ Wd) {
     const size_t n = (size_t)r * D.d;
-    const uint8_t* dn = packed + gu_bytes(D);
+    const uint32_t eb = V.eblk[e];
     for (size_t g = blockIdx.x * (size_t)blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) {
         {   // gate / up element (p, i)
             const int p = (int)(g / D.d), i = (int)(g % D.d);
             const int cb = p / CB, w = p % CB;
             const uint32_t pr_g = (w / 16) * 32 + (w % 16);
-            const uint8_t* t = packed + gu_tile_index(D, e, cb, i / KB) * WT_BYTES;
+            const uint8_t* t = V.gu + gu_tile_off(D, eb, cb, i / KB);
             Wg[g] = *(const uint16_t*)(t + sw128_off(pr_g, i % KB));
             Wu[g] = *(const uint16_t*)(t + sw128_off(pr_g + 16, i % KB));
         }
         {   // down element (i, p), output row-major [d][r]
             const int i = (int)(g / r), p = (int)(g % r);
-            const uint8_t* t = dn + dn_tile_index(D, e, p / KB, i / WT_ROWS) * WT_BYTES;
+            const uint8_t* t = V.dn + dn_tile_off(D, eb, p / KB, i / WT_ROWS);
             Wd[g] = *(const uint16_t*)(t + sw128_off(i % WT_ROWS, p % KB));
         }
     }
 }
 
-cudaError_t launch_unpack_prefix(const Dims& D, const uint8_t* packed, int e, int r, __nv_bfloat16* Wg,
+cudaError_t launch_unpack_prefix(const Dims& D, const LayerView& V, int e, int r, __nv_bfloat16* Wg,
                                  __nv_bfloat16* Wu, __nv_bfloat16* Wd, cudaStream_t st) {
     if (r == 0) return cudaSuccess;
     const size_t n = (size_t)r * D.d;
     const int blocks = (int)((n + 255) / 256 < 148 * 32 ? (n + 255) / 256 : 148 * 32);
-    k_unpack_prefix<<<blocks, 256, 0, st>>>(D, packed, e, r, (uint16_t*)Wg, (uint16_t*)Wu, (uint16_t*)Wd);
+    k_unpack_prefix<<<blocks, 256, 0, st>>>(D, V, e, r, (uint16_t*)Wg, (uint16_t*)Wu, (uint16_t*)Wd);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------- export_clipped
+// Offline clipping (Table 2): the retained prefix ceil(r_e / 64) channel blocks of every
+// expert, copied back to back.  A channel block is nKB1 (gate/up) resp. nDB (down) consecutive 16 KB tiles in both the
+// source and the destination, so the export is a segmented copy: HBM-bound, bytes = 2 x the clipped blob.
+// Block (e, part) streams its expert's share with 16-byte loads/stores; eblk_dst is the exclusive scan of the block counts.
+__global__ void __launch_bounds__(256) k_export_clipped(Dims D, LayerView src, const int* __restrict__ r,
+                                                        uint8_t* __restrict__ gu_dst, uint8_t* __restrict__ dn_dst,
+                                                        uint32_t* __restrict__ eblk_dst, int parts) {
+    __shared__ uint32_t s_base;
+    const int e = blockIdx.x / parts, part = blockIdx.x % parts;
+    if (threadIdx.x < 32) {                                      // exclusive scan of ceil(r / 64) over experts < e
+        uint32_t acc = 0;
+        for (int o = threadIdx.x; o < e; o += 32) acc += (uint32_t)((r[o] + CB - 1) / CB);
+#pragma unroll
+        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (threadIdx.x == 0) {
+            s_base = acc;
+            if (part == 0) eblk_dst[e] = acc;
+        }
+    }
+    __syncthreads();
+    const uint32_t dbase = s_base, sbase = src.eblk[e];
+    const int nb = (r[e] + CB - 1) / CB;
+    const size_t gu_n = (size_t)nb * D.nKB1 * (WT_BYTES / 16), dn_n = (size_t)nb * D.nDB * (WT_BYTES / 16);   // uint4 counts
+    const uint4* gs = (const uint4*)(src.gu + gu_tile_off(D, sbase, 0, 0));
+    const uint4* ds = (const uint4*)(src.dn + dn_tile_off(D, sbase, 0, 0));
+    uint4* gd = (uint4*)(gu_dst + gu_tile_off(D, dbase, 0, 0));
+    uint4* dd = (uint4*)(dn_dst + dn_tile_off(D, dbase, 0, 0));
+    const size_t stride = (size_t)parts * 256;
+    for (size_t i = (size_t)part * 256 + threadIdx.x; i < gu_n + dn_n; i += 4 * stride) {
+        uint4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t j = i + u * stride;
+            if (j < gu_n + dn_n) v[u] = j < gu_n ? __ldcs(gs + j) : __ldcs(ds + (j - gu_n));
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t j = i + u * stride;
+            if (j < gu_n + dn_n) {
+                if (j < gu_n) __stcs(gd + j, v[u]); else __stcs(dd + (j - gu_n), v[u]);
+            }
+        }
+    }
+}
+
+cudaError_t launch_export_clipped(const Dims& D, const LayerView& src, const int* r_dev, uint8_t* gu_dst, uint8_t* dn_dst,
+                                  uint32_t* eblk_dst, cudaStream_t st) {
+    int parts = (148 * 8 + D.E - 1) / D.E;                        // ~8 blocks per SM in total
+    if (parts < 1) parts = 1;
+    k_export_clipped<<<D.E * parts, 256, 0, st>>>(D, src, r_dev, gu_dst, dn_dst, eblk_dst, parts);
     return cudaGetLastError();
 }
 
@@ -112,69 +172,48 @@ cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStrea
     return cudaGetLastError();
 }
 
-// -------------------------------------------------------------------------------------------- combine
-// Alg. 2 l.19-20: Y[token] += alpha * Z_down, done as a GATHER so that no atomics are needed and
-// the sum runs in slot order j = 0..k-1 in fp32 with exactly one rounding of y (readings R8, R11):
-//   y[t][i] = sum_j topk_w[t][j] * O[prow[t*k+j]][i]
-// One block per token; a thread owns 8 consecutive output features (16 bytes of each O row).
-__global__ void __launch_bounds__(128) k_combine(Dims D, int k, const int* __restrict__ prow,
-                                                 const float* __restrict__ topk_w, const uint8_t* __restrict__ O,
-                                                 int P, uint4* __restrict__ y) {
-    __shared__ int s_p[MAX_K];
-    __shared__ float s_w[MAX_K];
-    const int t = blockIdx.x;
+// ------------------------------------------------------------------------------------------- finalize
+// The end of Alg. 2 l.19-20: the fp32 scatter-add target becomes y.  This is the ONE rounding of y
+// (reading R11); y_add, if given, is the shared-expert output added in fp32 before it.
+// 8 elements per thread: 32 B of yacc in, 16 B of y out.
+__global__ void __launch_bounds__(256) k_finalize(const float4* __restrict__ yacc, const uint4* __restrict__ y_add,
+                                                  uint4* __restrict__ y, size_t n8) {
     pdl_launch_dependents();
     pdl_wait();
-    if (threadIdx.x < k) {
-        s_p[threadIdx.x] = prow[(size_t)t * k + threadIdx.x];
-        s_w[threadIdx.x] = topk_w[(size_t)t * k + threadIdx.x];
-    }
-    __syncthreads();
-    const int chunks = D.d >> 3;
-    const size_t orow = 2 * WT_ROWS;                              // bytes per row of an O panel
-    for (int c = threadIdx.x; c < chunks; c += blockDim.x) {
-        const uint8_t* col = O + (size_t)(c >> 4) * P * orow + ((size_t)(c & 15) << 4);   // panel c/16, 16-byte chunk c%16
-        float acc[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) acc[q] = 0.f;
-        for (int j0 = 0; j0 < k; j0 += 4) {
-            uint4 v[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const int p = j0 + u < k ? s_p[j0 + u] : -1;
-                v[u] = p >= 0 ? __ldg((const uint4*)(col + (size_t)p * orow)) : make_uint4(0, 0, 0, 0);
-            }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (j0 + u >= k) break;
-                const float wj = s_w[j0 + u];
-                const uint32_t h[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    acc[2 * q] += wj * __uint_as_float(h[q] << 16);
-                    acc[2 * q + 1] += wj * __uint_as_float(h[q] & 0xFFFF0000u);
-                }
-            }
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n8; i += (size_t)gridDim.x * blockDim.x) {
+        float4 a = __ldcs(yacc + 2 * i), b = __ldcs(yacc + 2 * i + 1);
+        if (y_add) {
+            const uint4 s = __ldg(y_add + i);
+            a.x += __uint_as_float(s.x << 16); a.y += __uint_as_float(s.x & 0xFFFF0000u);
+            a.z += __uint_as_float(s.y << 16); a.w += __uint_as_float(s.y & 0xFFFF0000u);
+            b.x += __uint_as_float(s.z << 16); b.y += __uint_as_float(s.z & 0xFFFF0000u);
+            b.z += __uint_as_float(s.w << 16); b.w += __uint_as_float(s.w & 0xFFFF0000u);
         }
+        const __nv_bfloat162 p0 = __floats2bfloat162_rn(a.x, a.y), p1 = __floats2bfloat162_rn(a.z, a.w);
+        const __nv_bfloat162 p2 = __floats2bfloat162_rn(b.x, b.y), p3 = __floats2bfloat162_rn(b.z, b.w);
         uint4 o;
-        __nv_bfloat162 b0 = __floats2bfloat162_rn(acc[0], acc[1]), b1 = __floats2bfloat162_rn(acc[2], acc[3]);
-        __nv_bfloat162 b2 = __floats2bfloat162_rn(acc[4], acc[5]), b3 = __floats2bfloat162_rn(acc[6], acc[7]);
-        o.x = *(uint32_t*)&b0; o.y = *(uint32_t*)&b1; o.z = *(uint32_t*)&b2; o.w = *(uint32_t*)&b3;
-        y[(size_t)t * chunks + c] = o;
+        o.x = *(const uint32_t*)&p0; o.y = *(const uint32_t*)&p1; o.z = *(const uint32_t*)&p2; o.w = *(const uint32_t*)&p3;
+        y[i] = o;
     }
 }
-cudaError_t launch_combine(const Dims& D, int T, int k, const float* topk_w, const Workspace& ws, __nv_bfloat16* y,
-                           cudaStream_t st) {
+cudaError_t launch_finalize(const Dims& D, int T, const float* yacc, const __nv_bfloat16* y_add, __nv_bfloat16* y,
+                            cudaStream_t st) {
     if (T == 0) return cudaSuccess;
-    return launch_pdl(k_combine, dim3(T), dim3(128), 0, st, D, k, (const int*)ws.prow, topk_w, (const uint8_t*)ws.O, ws.P, (uint4*)y);
+    const size_t n8 = (size_t)T * D.d / 8;                        // d % 64 == 0
+    size_t blocks = (n8 + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    return launch_pdl(k_finalize, dim3((unsigned)blocks), dim3(256), 0, st, (const float4*)yacc, (const uint4*)y_add, (uint4*)y, n8);
 }
 
 // --------------------------------------------------------------------------------------------- read_h
-// H_out[s][c] for sorted position s (perm order) and channel c < I, from the swizzled panels.
+// H_out[s][c] for sorted position s (perm order) and channel c < I, from the swizzled panels.  raw = 0: columns of
+// blocks that were never issued (c >= ceil64(r_e)) and, by definition, every column >= r_e read as 0; raw = 1: columns
+// below ceil64(r_e) are returned exactly as the GEMM-1 epilogue wrote them (the test of the kernel's pad-zero rule),
+// columns of never-issued blocks are 0.
 __global__ void k_read_h(Dims D, int k, const int* __restrict__ ids, const int* __restrict__ r_table,
                          const int* __restrict__ inv_perm, const int* __restrict__ row_flat,
                          const Sched* __restrict__ sched, const uint8_t* __restrict__ H, int P,
-                         uint16_t* __restrict__ out) {
+                         uint16_t* __restrict__ out, int raw) {
     const int P_used = sched->P_used;
     const size_t n = (size_t)P_used * D.I;
     for (size_t g = blockIdx.x * (size_t)blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) {
@@ -184,15 +223,17 @@ __global__ void k_read_h(Dims D, int k, const int* __restrict__ ids, const int* 
         const int s = inv_perm[f];
         const uint8_t* row = H + ((size_t)(c / CB) * P + p) * ROW_BYTES;
         const uint16_t v = *(const uint16_t*)(row + ((((c % CB) >> 3) ^ p) & 7) * 16 + ((c & 7) << 1));
-        out[(size_t)s * D.I + c] = c < r_table[ids[f]] ? v : (uint16_t)0;   // pruned tiles are never written
+        const int r = r_table[ids[f]];
+        const int lim = raw ? (r + CB - 1) / CB * CB : r;            // pruned blocks are never written
+        out[(size_t)s * D.I + c] = c < lim ? v : (uint16_t)0;
     }
     (void)k;
 }
 cudaError_t launch_read_h(const Dims& D, int T, int k, const int* ids, const int* r_table, const Workspace& ws,
-                          __nv_bfloat16* H_out, cudaStream_t st) {
+                          __nv_bfloat16* H_out, int raw, cudaStream_t st) {
     (void)T;
     k_read_h<<<148 * 8, 256, 0, st>>>(D, k, ids, r_table, ws.inv_perm, ws.row_flat, ws.sched, ws.H, ws.P,
-                                      (uint16_t*)H_out);
+                                      (uint16_t*)H_out, raw);
     return cudaGetLastError();
 }
 

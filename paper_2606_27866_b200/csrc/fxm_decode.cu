@@ -40,12 +40,13 @@ constexpr int DEC_SMEM_MAX = 232448;              // 227 KB
 
 struct DecArgs {
     Dims D;
-    const uint8_t* packed;
+    LayerView V;
     const int* r_table;
     const uint4* x;            // [T][d] bf16
     const int* ids;            // [T][k]
     const float* topk_w;       // [T][k]
     float* yacc;               // [T][d] fp32 scratch (workspace)
+    const uint2* y_add;        // [T][d] bf16 or null: shared-expert output added in fp32 before the rounding of y
     __nv_bfloat16* y;          // [T][d]
     DevState* state;
     int T, k, A;
@@ -58,6 +59,7 @@ struct DecAux {
     int4 runs[DEC_MAX_RUNS];   // {e | n << 16, first sorted position, cb_lo, cb_hi}
     int16_t perm[DEC_MAX_A];   // sorted position -> flat assignment index
     int r[MAX_E];
+    uint32_t eb[MAX_E];        // first channel block of each expert in the weight regions (LayerView::eblk)
     uint64_t bars[2 * DEC_MAX_SLOTS + 16];
     uint32_t tmem_slot;
     int n_runs, n_items, W;
@@ -118,6 +120,7 @@ __device__ __forceinline__ void grid_wait(DevState* st, int i, uint32_t gen0) {
         __nanosleep(1000);                                         // 148 pollers: keep the L2 slice of the barrier words quiet
         if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) {
             atomicOr(&st->flags, 2u);
+            if (st->hflag) *(volatile uint32_t*)st->hflag = 2u;
             __threadfence_system();
             __trap();
         }
@@ -131,6 +134,7 @@ struct ItemCur {
     __device__ __forceinline__ bool first(const DecAux* ax) const { return cb == ax->runs[R].z; }
     __device__ __forceinline__ bool last(const DecAux* ax) const { return cb + 1 == ax->runs[R].w; }
     __device__ __forceinline__ int e(const DecAux* ax) const { return ax->runs[R].x & 0xFFFF; }
+    __device__ __forceinline__ uint32_t eb(const DecAux* ax) const { return ax->eb[ax->runs[R].x & 0xFFFF]; }
     __device__ __forceinline__ void next(const DecAux* ax) {
         if (++cb == ax->runs[R].w) {
             ++R;
@@ -150,7 +154,7 @@ struct PartStream {
     int i;            // step: the G part of item i, then the D part of item i-1
     int sub;          // 0 = G(i) comes next, 1 = D(i-1) comes next
     __device__ __forceinline__ void init(const DecAux* a, const DecArgs& args) {
-        ax = a; D = args.D; gu = args.packed; dn = args.packed + gu_bytes(args.D);
+        ax = a; D = args.D; gu = args.V.gu; dn = args.V.dn;
         g.init(a); d.init(a);
         i = 0; sub = 0;
     }
@@ -160,7 +164,7 @@ struct PartStream {
             if (sub == 0) {
                 sub = 1;
                 if (i < n) {
-                    base = gu + gu_tile_index(D, g.e(ax), g.cb, 0) * WT_BYTES;
+                    base = gu + gu_tile_off(D, g.eb(ax), g.cb, 0);
                     count = D.nKB1;
                     g.next(ax);
                     return true;
@@ -169,7 +173,7 @@ struct PartStream {
             sub = 0;
             const int ii = i++;
             if (ii >= 1) {
-                base = dn + dn_tile_index(D, d.e(ax), d.cb, 0) * WT_BYTES;
+                base = dn + dn_tile_off(D, d.eb(ax), d.cb, 0);
                 count = D.nDB;
                 d.next(ax);
                 return true;
@@ -241,7 +245,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         tp->ids[f] = (int16_t)id;
     }
     if (bad) atomicOr(&a.state->flags, 1u);
-    for (int e = tid; e < MAX_E; e += DEC_THREADS) ax->r[e] = e < E ? a.r_table[e] : 0;
+    for (int e = tid; e < MAX_E; e += DEC_THREADS) { ax->r[e] = e < E ? a.r_table[e] : 0; ax->eb[e] = e < E ? a.V.eblk[e] : 0u; }
     // zero this CTA's slice of the fp32 accumulator (grid barrier #0 orders it before every reduction)
     {
         float4* z = (float4*)a.yacc;
@@ -592,7 +596,12 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         const float4* src = (const float4*)a.yacc;
         uint2* dst = (uint2*)a.y;
         for (size_t i = (size_t)blockIdx.x * DEC_THREADS + tid; i < n4; i += (size_t)G * DEC_THREADS) {
-            const float4 f = __ldcg(src + i);
+            float4 f = __ldcg(src + i);
+            if (a.y_add) {
+                const uint2 sa = __ldg(a.y_add + i);
+                f.x += __uint_as_float(sa.x << 16); f.y += __uint_as_float(sa.x & 0xFFFF0000u);
+                f.z += __uint_as_float(sa.y << 16); f.w += __uint_as_float(sa.y & 0xFFFF0000u);
+            }
             const __nv_bfloat162 b0 = __floats2bfloat162_rn(f.x, f.y), b1 = __floats2bfloat162_rn(f.z, f.w);
             uint2 o;
             o.x = *(const uint32_t*)&b0;
@@ -617,12 +626,12 @@ cudaError_t init_decode_kernel() {
     return cudaFuncSetAttribute(k_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, DEC_SMEM_MAX);
 }
 
-cudaError_t launch_decode(const Dims& D, const uint8_t* packed, const int* r_table, const __nv_bfloat16* x,
-                          const int* ids, const float* topk_w, int T, int k, float* yacc, __nv_bfloat16* y,
-                          DevState* state, int num_sms, int pf, cudaStream_t st) {
+cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
+                          const int* ids, const float* topk_w, int T, int k, float* yacc, const __nv_bfloat16* y_add,
+                          __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st) {
     DecArgs a{};
-    a.D = D; a.packed = packed; a.r_table = r_table; a.x = (const uint4*)x; a.ids = ids; a.topk_w = topk_w;
-    a.yacc = yacc; a.y = y; a.state = state; a.T = T; a.k = k; a.A = T * k;
+    a.D = D; a.V = V; a.r_table = r_table; a.x = (const uint4*)x; a.ids = ids; a.topk_w = topk_w;
+    a.yacc = yacc; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.T = T; a.k = k; a.A = T * k;
     a.slots = decode_slots(D);
     a.pf = pf;
     const int smem = dec_fixed_smem(D) + a.slots * WT_BYTES;

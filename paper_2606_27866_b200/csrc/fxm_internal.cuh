@@ -36,11 +36,6 @@ __host__ __device__ inline uint32_t sw128_chunk(uint32_t row, uint32_t ch) {
     return row * ROW_BYTES + (((ch ^ row) & 7u) << 4);
 }
 
-// byte offset of output feature i of padded row p in the O panels
-__host__ __device__ inline size_t o_off(int P, int p, int i) {
-    return ((size_t)(i >> 7) * P + p) * (2 * WT_ROWS) + (size_t)(i & 127) * 2;
-}
-
 struct Dims {
     int E, d, I;
     int Ip;      // ceil64(I)
@@ -53,12 +48,6 @@ struct Dims {
 //   gate/up tile (e, cb, kb):  rows pr=0..127: g16 = pr/32, w = pr%32; w<16 -> gate channel cb*64+g16*16+w,
 //                              else up channel cb*64+g16*16+(w-16); cols = x features kb*64 .. +63
 //   down tile (e, kb2, db):    rows = output features db*128 .. +127, cols = channels kb2*64 .. +63
-__host__ __device__ inline size_t gu_tile_index(const Dims& D, int e, int cb, int kb) {
-    return ((size_t)e * D.nCB + cb) * D.nKB1 + kb;
-}
-__host__ __device__ inline size_t dn_tile_index(const Dims& D, int e, int kb2, int db) {
-    return ((size_t)e * D.nCB + kb2) * D.nDB + db;
-}
 __host__ __device__ inline size_t gu_bytes(const Dims& D) { return (size_t)D.E * D.nCB * D.nKB1 * WT_BYTES; }
 __host__ __device__ inline size_t dn_bytes(const Dims& D) { return (size_t)D.E * D.nCB * D.nDB * WT_BYTES; }
 
@@ -67,22 +56,28 @@ struct DevState {           // lives at the tail of the packed blob (zeroed by p
     uint32_t ticket;        // route: blocks that have published their histogram (reset by the last one)
     uint32_t bar_count[2];  // decode kernel: top-level arrivals at grid barrier 0 / 1 (reset by the last arriver)
     uint32_t bar_sub[2][8]; // decode kernel: first-level arrivals, CTA b uses counter b % 8 (reset by their last arrivers)
-    uint32_t pad0[12];      // -> 128 bytes: the polled words below live in their own line
+    uint32_t pad0[10];
+    uint32_t* hflag;        // host-mapped (pinned) word that also receives bit1: readable after a trap has killed the context
+                            // -> 128 bytes: the polled words below live in their own line
     uint32_t bar_gen[2];    // decode kernel: generation of grid barrier 0 / 1 (sense reversal; never reset)
-    uint32_t pad1[30];
+    uint32_t route_gen;     // route kernel: bumped by the last block to publish its histogram (sense reversal; never reset)
+    uint32_t pad1[29];
 };
+static_assert(sizeof(DevState) == 256, "DevState layout");
 
 // ------------------------------------------------------------------------------------------------
 // Workspace map (all offsets 1024-byte aligned).  P = padded-row capacity for this call.
 // ------------------------------------------------------------------------------------------------
 struct Sched {              // written by the route kernel, read by everything after it
     int ntt;                // number of token tiles (experts with n_e == 0 or r_e == 0 get none: pruned work is never issued)
-    int W1;                 // GEMM-1 work items  = sum_j ceil(r_e(j) / 64)
-    int W2;                 // GEMM-2 work items  = ntt * nDB
+    int W1;                 // GEMM-1 work items  = sum_j ceil(ceil(r_e(j) / 64) / 2)   (CTA-pair items)
+    int W2;                 // GEMM-2 work items  = ntt * ceil(nDB / 2)
     int P_used;             // padded rows in use
     int A;                  // T * k
     int max_n;              // rows of the widest token tile (multiple of 16; 16 if there is none)
-    int pad[10];
+    unsigned claim1;        // dynamic work claim counters of GEMM-1 / GEMM-2 (zeroed by the plan kernel)
+    unsigned claim2;
+    int pad[8];
 };
 
 struct Workspace {
@@ -93,15 +88,13 @@ struct Workspace {
     int* perm;              // [A]
     int* inv_perm;          // [A]
     int* row_flat;          // [P]  flat assignment index f = t*k+j of each padded row, -1 for padding
-    int* prow;              // [A]  padded row of each flat assignment; -1 = dropped or expert of width 0
     int* row_tok;           // [P]  token index t = f / k of each padded row (0 for padding rows): the gather4 row coordinates
+    int2* row_tw;           // [P]  {token index or -1 for padding rows, router weight topk_w[f] as bits}: the scatter-add
+                            //      destination and scale of each padded row (GEMM-2 epilogue, Alg. 2 l.19-20)
     int* bhist;             // [RB][E] per-route-block expert histogram, then exclusive base over blocks
-    int4* tt;               // [NT] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}
-    int4* items1;           // [NT*nCB] GEMM-1 work items {expert, first padded row, valid rows, channel block}
-    uint8_t* Xs;            // [nKB1][P][128 B]  gathered activations, swizzled panels
+    int4* tt;               // [NT + 1] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}; tt[ntt] = sentinel
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
-    uint8_t* O;             // [nDB][P][256 B]  expert outputs, bf16: panel db holds features db*128..+127 of every padded row
-    float* yacc;            // [T][d] fp32 accumulator of the fused decode kernel (only when T*k <= DEC_MAX_A)
+    float* yacc;            // [T][d] fp32 accumulator of y: the scatter-add target of GEMM-2 / of the decode kernel
     int RB;                 // route blocks
     int chunk;              // flat assignments per route block
     int P;                  // padded-row capacity (multiple of 16)
@@ -109,16 +102,20 @@ struct Workspace {
     size_t bytes;           // total
 };
 
-constexpr int TILE_N_MAX = 256;   // largest token tile any kernel uses (schedule capacity is sized for the smallest)
-constexpr int TILE_N_MIN = 128;
+constexpr int TILE_N_MIN = 128;   // smallest token tile any plan uses (the schedule capacity is sized for it)
 
 __host__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-constexpr int RT_THREADS = 256;   // route kernels: 8 warps per block
-// flat assignments per route block: a multiple of 256 that keeps the grid at <= 128 blocks
-__host__ inline int route_chunk(long long A) {
-    const long long per = (A + 127) / 128;
-    return (int)((per + 255) / 256 * 256 > 0 ? (per + 255) / 256 * 256 : 256);
+constexpr int RT_THREADS = 256;   // route kernel: 8 warps per block
+constexpr int RT_MAX_BLOCKS = 128;
+// tokens per route block: a multiple of 32 that keeps the grid at <= RT_MAX_BLOCKS blocks (a block owns whole tokens,
+// i.e. the flat assignments [b * chunk * k, (b + 1) * chunk * k))
+__host__ inline int route_tok_chunk(long long T, int E) {
+    // every block sums all published histogram rows: keep rows x experts / 256 threads at <= 32 loads per thread
+    const int maxb = E <= 64 ? RT_MAX_BLOCKS : (8192 / E > 16 ? 8192 / E : 16);
+    const long long per = (T + maxb - 1) / maxb;
+    const long long c = (per + 31) / 32 * 32;
+    return (int)(c > 0 ? c : 32);
 }
 
 __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base) {
@@ -126,8 +123,8 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     const size_t A = (size_t)T * k;
     const int P = (int)align_up(A + (size_t)(ROW_ALIGN - 1) * D.E, ROW_ALIGN) + ROW_ALIGN;
     const int NT = (int)(A / TILE_N_MIN) + D.E + 1;
-    const int chunk = route_chunk((long long)A);
-    const int RB = (int)((A + chunk - 1) / chunk) > 0 ? (int)((A + chunk - 1) / chunk) : 1;
+    const int chunk = route_tok_chunk((long long)T, D.E) * k;          // flat assignments per route block
+    const int RB = T > 0 ? (int)((A + chunk - 1) / chunk) : 1;
     size_t o = 0;
     auto take = [&](size_t n) { size_t r = o; o = align_up(o + n, 1024); return r; };
     uint8_t* b = (uint8_t*)base;
@@ -138,15 +135,12 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.perm = (int*)(b + take(sizeof(int) * (A + 1)));
     w.inv_perm = (int*)(b + take(sizeof(int) * (A + 1)));
     w.row_flat = (int*)(b + take(sizeof(int) * (size_t)P));
-    w.prow = (int*)(b + take(sizeof(int) * (A + 1)));
     w.row_tok = (int*)(b + take(sizeof(int) * (size_t)P));
-    w.bhist = (int*)(b + take(sizeof(int) * (size_t)RB * D.E));
-    w.tt = (int4*)(b + take(sizeof(int4) * (size_t)NT));
-    w.items1 = (int4*)(b + take(sizeof(int4) * (size_t)NT * D.nCB));
-    w.Xs = b + take((size_t)D.nKB1 * P * ROW_BYTES);
+    w.row_tw = (int2*)(b + take(sizeof(int2) * (size_t)P));
+    w.bhist = (int*)(b + take(sizeof(int) * (size_t)RT_MAX_BLOCKS * D.E));   // capacity, not RB: the size stays monotonic in T
+    w.tt = (int4*)(b + take(sizeof(int4) * ((size_t)NT + 1)));
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
-    w.O = b + take((size_t)P * D.nDB * WT_ROWS * 2);
-    w.yacc = (float*)(b + take(A <= (size_t)DEC_MAX_A ? (size_t)T * D.d * sizeof(float) : 0));
+    w.yacc = (float*)(b + take((size_t)T * D.d * sizeof(float)));       // every T: the size is monotonic in T
     w.RB = RB;
     w.chunk = chunk;
     w.P = P;
@@ -182,58 +176,86 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 }
 
 // ------------------------------------------------------------------------------------------------
+// Where the weight tiles of a layer live.  A full (online) layer keeps every channel block of every expert:
+// eblk[e] = e * nCB.  An offline-clipped layer (fxm_export_clipped) keeps only the retained prefix
+// ceil(r_e / 64) blocks of each expert, back to back: eblk[e] = sum_{e' < e} ceil(r_e' / 64).  Every kernel
+// addresses tiles through eblk, so one code path serves both deployment modes.
+// ------------------------------------------------------------------------------------------------
+struct LayerView {
+    const uint8_t* gu;       // gate/up tiles: tile (e, cb, kb) at ((eblk[e] + cb) * nKB1 + kb) * 16 KB
+    const uint8_t* dn;       // down tiles:    tile (e, kb2, db) at ((eblk[e] + kb2) * nDB + db) * 16 KB
+    const uint32_t* eblk;    // [E] device: first channel block of expert e
+};
+__host__ __device__ inline size_t gu_tile_off(const Dims& D, uint32_t eblk, int cb, int kb) {
+    return (((size_t)eblk + cb) * D.nKB1 + kb) * WT_BYTES;
+}
+__host__ __device__ inline size_t dn_tile_off(const Dims& D, uint32_t eblk, int kb2, int db) {
+    return (((size_t)eblk + kb2) * D.nDB + db) * WT_BYTES;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Launchers (each enqueues on `st` and returns cudaGetLastError()).
 // ------------------------------------------------------------------------------------------------
 cudaError_t launch_pack(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
-                        const int* rank_dev /*[E][I] or null*/, uint8_t* packed, cudaStream_t st);
-cudaError_t launch_unpack_prefix(const Dims& D, const uint8_t* packed, int e, int r, __nv_bfloat16* Wg,
+                        const int* rank_dev /*[E][I] or null*/, uint8_t* packed, uint32_t* eblk_dev, cudaStream_t st);
+cudaError_t launch_unpack_prefix(const Dims& D, const LayerView& V, int e, int r, __nv_bfloat16* Wg,
                                  __nv_bfloat16* Wu, __nv_bfloat16* Wd, cudaStream_t st);
 cudaError_t launch_set_table(int* table_dev, const int* r_host, int E, cudaStream_t st);
-// a2/a3 part 1: per-block histograms; the last block to finish scans them and writes counts/offsets/poff/tt/items1/sched
-// tile_n = max rows of a token tile; grp = weight blocks per work item (1: single-CTA kernels, 2: CTA-pair kernels)
-cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int grp,
-                              int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st);
-// a2 part 2: stable scatter (perm / inv_perm / row_flat / prow)
-cudaError_t launch_scatter(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
-                           const int* offsets, int* perm, int* inv_perm, const Workspace& ws, cudaStream_t st);
-// gather of the x rows into the sorted, padded, swizzled panels ws.Xs
-cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st);
-// y[t] = sum_j topk_w[t][j] * O[row of (t,j)]   (fp32 sum in slot order, one rounding)
-cudaError_t launch_combine(const Dims& D, int T, int k, const float* topk_w, const Workspace& ws, __nv_bfloat16* y,
-                           cudaStream_t st);
+// offline clipping: copy the retained prefix blocks of every expert of `src` into the compact regions
+// gu_dst / dn_dst (block order given by eblk_dst) and write eblk_dst; r_dev = the width table (device)
+cudaError_t launch_export_clipped(const Dims& D, const LayerView& src, const int* r_dev, uint8_t* gu_dst, uint8_t* dn_dst,
+                                  uint32_t* eblk_dst, cudaStream_t st);
+
+// a2 + a3 in ONE launch (fxm_route.cu): per-block histograms -> grid-wide publish -> every block derives its own
+// bases and scatters its assignments (stable); block 0 also writes counts / offsets / the token tiles / the work items
+// for the CURRENT width table.  tile_n = max rows of a token tile.  topk_w may be null (fxm_route: indices only).
+struct RouteArgs {
+    Dims D;
+    const int* ids;          // [T][k] device, or null when `logits` is given
+    const float* topk_w;     // [T][k] device, or null
+    const float* logits;     // [T][E] router logits (NEXT-3 front end): softmax -> top-k -> renormalise in this kernel
+    int* ids_out;            // [T][k] where the front end writes the ids it chose (workspace), else null
+    float* w_out;            // [T][k] ... and the renormalised weights
+    const int* r_table;      // current widths or null (fxm_route before any budget: full width)
+    int T, k, tile_n;
+    int* counts;             // [E]
+    int* offsets;            // [E+1]
+    int* perm;               // [A]
+    int* inv_perm;           // [A]
+};
+cudaError_t launch_route(const RouteArgs& a, const Workspace& ws, DevState* state, cudaStream_t st);
+// y[t] = bf16( yacc[t] (+ y_add[t]) ): the single rounding of y (reading R11); y_add = optional shared-expert output
+cudaError_t launch_finalize(const Dims& D, int T, const float* yacc, const __nv_bfloat16* y_add, __nv_bfloat16* y,
+                            cudaStream_t st);
+// raw != 0: no reader-side mask (what the kernels really wrote, pad columns included)
 cudaError_t launch_read_h(const Dims& D, int T, int k, const int* ids, const int* r_table, const Workspace& ws,
-                          __nv_bfloat16* H_out, cudaStream_t st);
+                          __nv_bfloat16* H_out, int raw, cudaStream_t st);
 
-// SIMT debug path (same layouts, no tensor cores, no async copies)
-cudaError_t launch_gemm1_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+// SIMT debug path (same layouts and schedule, no tensor cores, no async copies)
+cudaError_t launch_gemm1_simt(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
+                              const Workspace& ws, cudaStream_t st);
+cudaError_t launch_gemm2_simt(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws,
                               cudaStream_t st);
-cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
-                              cudaStream_t st);
 
-// tcgen05 / TMEM / bulk-copy path
-cudaError_t launch_gemm1_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
-                               DevState* state, int tile_n, int num_sms, cudaStream_t st);
-cudaError_t launch_gemm2_sm100(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
-                               DevState* state, int tile_n, int num_sms, cudaStream_t st);
-cudaError_t init_sm100_kernels();   // cudaFuncSetAttribute for the dynamic shared memory sizes
-
-// CTA-pair path (cta_group::2, token tiles up to 512 rows); the schedule must have been planned with grp = 2
+// CTA-pair tcgen05 path (cta_group::2, token tiles up to 512 rows = two sub-tiles)
 constexpr int PAIR_TILE_N = 512;
 // x_map: a CUtensorMap (128 bytes, passed by value to the kernel) over x [T][d] bf16 with box {64, 1} and 128-byte
-// swizzle: GEMM-1 gathers its token rows straight from x with TMA gather4 (no Xs copy).  nullptr = read the Xs panels.
-cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+// swizzle: GEMM-1 gathers its token rows straight from x with TMA gather4 (no gathered copy of x).  GEMM-1 also
+// zeroes ws.yacc (its epilogue warps are idle while the first tiles are multiplied).
+cudaError_t launch_gemm1_pair(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws, int T,
                               DevState* state, int num_sms, const void* x_map, cudaStream_t st);
 // encodes the tensor map above through the driver entry point cuTensorMapEncodeTiled (no libcuda link dependency)
 cudaError_t encode_x_map(const void* x, int T, int d, void* map_out /* 128 bytes, 64-byte aligned */);
-cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+// GEMM-2 with the router-weight scale and the scatter-add into ws.yacc fused in its epilogue (Alg. 2 l.18-20)
+cudaError_t launch_gemm2_pair(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws,
                               DevState* state, int num_sms, cudaStream_t st);
 cudaError_t init_pair_kernels();
 
 // fused single-launch decode kernel (fxm_decode.cu): T*k <= DEC_MAX_A, d <= 3840
 bool decode_supported(const Dims& D);
 cudaError_t init_decode_kernel();
-cudaError_t launch_decode(const Dims& D, const uint8_t* packed, const int* r_table, const __nv_bfloat16* x,
-                          const int* ids, const float* topk_w, int T, int k, float* yacc, __nv_bfloat16* y,
-                          DevState* state, int num_sms, int pf, cudaStream_t st);
+cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
+                          const int* ids, const float* topk_w, int T, int k, float* yacc, const __nv_bfloat16* y_add,
+                          __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st);
 
 }  // namespace fxm

@@ -5,10 +5,14 @@
 //         CTA r of the pair owns channel block cb = 2*cbp + r (64 gate + 64 up rows, lanes 0..127 of ITS TMEM).
 //         Epilogue: h = silu(g) * u (gate lane l, up lane l+16: one shuffle), channels >= r_e forced to 0 (the
 //         paper's pad-zero rule), one rounding to bf16 -> the swizzled H panel.
-//   a5  GEMM-2 (Alg. 2 l.18):
+//   a5  GEMM-2 + router-weight scale + scatter-add combine (Alg. 2 l.18-20):
 //         D[256 out features, N tokens] = Wd[256, r_e] . H[N, r_e]^T,  CTA r owns feature block db = 2*dbp + r;
-//         K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.  Epilogue: one rounding to
-//         bf16 -> the O panel; the router-weight scale and the sum over k experts are the gather in k_combine.
+//         K loop bounded by ceil(r_e/64): pruned K steps are never loaded or issued.  Epilogue: every epilogue warp
+//         pulls its share of the accumulator into registers (tcgen05.ld), hands the TMEM columns back to the MMA
+//         warp at once, then scales each token column by its router weight in fp32 and adds it into the fp32
+//         accumulator yacc[token][feature] with red.global.add.f32 -- a warp covers 32 consecutive features of one
+//         token = one 128-byte line per instruction (measured on B200: 5.7 TB/s of fp32 adds, the speed of plain
+//         stores; cp.reduce.async.bulk is 3x slower).  No O panels, no combine kernel, no third rounding.
 //
 // Token tiles are up to 512 rows: a tile is one or two SUB-TILES of <= 256 tokens (UMMA N <= 256, balanced split)
 // that share the weight operand -- each weight byte is pulled into shared memory once per (expert, token tile).
@@ -24,8 +28,8 @@
 //     peer CTA's relay ("my half has landed"); ONE multicast commit frees the stage in both CTAs;
 //   * TMEM is a circular column allocator: a sub-tile takes N contiguous columns, so the MMAs of the next item start
 //     as soon as the columns they need are drained (tiles of <= 256 tokens are fully double-buffered);
-//   * the epilogue stages its output in shared memory in the final layout and writes it with bulk stores (the H / O
-//     panels make a CTA's output of a sub-tile one contiguous range);
+//   * the GEMM-1 epilogue stages its output in shared memory in the final layout and writes it with bulk stores (the H
+//     panels make a CTA's output of a sub-tile one contiguous range); the GEMM-2 epilogue has no staging at all;
 //   * GEMM-1 takes its token rows straight from x (X[pi], Alg. 2 l.7): TMA tile::gather4 through a tensor map over
 //     x [T][d], four rows per instruction, landing in the swizzled K-major operand layout -- no gathered copy of x;
 //   * an optional L2 prefetch cursor over the weight tiles exists (FXM_PAIR_PF) but is off: every distance > 0 was slower.
@@ -33,6 +37,8 @@
 // Warp roles: warp 0 = weight producer, warp 1 = MMA issuer (leader CTA) / relay (peer CTA), GEMM-1 only: warps 2-7 =
 // gather warps (a gather4 costs one warp ~60 cycles of issue, six of them keep up with the MMAs), then 16 epilogue
 // warps (each CTA drains its own TMEM lanes; four warps per lane quadrant).  768 threads (GEMM-1) / 640 (GEMM-2).
+// GEMM-1's epilogue warps also zero yacc (the scatter-add target of GEMM-2) before their first tile: they are idle
+// while the first tiles are multiplied, so the fp32 accumulator costs no launch and no time of its own.
 #include "fxm_ptx.cuh"
 
 #include <cuda.h>          // CUtensorMap and the cuTensorMapEncodeTiled prototype (resolved at run time, no libcuda link)
@@ -51,10 +57,13 @@ template <int MODE> struct PairCfg {
     static constexpr int THREADS = 32 * (EPI0 + PAIR_EPI_WARPS);
 };
 constexpr int PAIR_MAX_STAGES = 8;
-constexpr int PAIR_STAGING = 2 * 16384;         // two 16 KB epilogue staging buffers
 constexpr int PAIR_SMEM = 232448;               // 227 KB: everything a CTA can have
 constexpr int PAIR_AUX = 2048;                  // barriers (264 B) and, at +512, the gather warps' token indices
-constexpr int PAIR_RING_BYTES = PAIR_SMEM - 1024 /*alignment slack*/ - PAIR_STAGING - PAIR_AUX;   // 4 x 48 KB
+// after the ring: GEMM-1 two 16 KB epilogue staging buffers; GEMM-2 two sets of 512 {token, router weight} pairs
+template <int MODE> struct PairSmem {
+    static constexpr int EXTRA = MODE == 1 ? 2 * 16384 : 2 * 512 * 8;
+    static constexpr int RING = PAIR_SMEM - 1024 /*alignment slack*/ - EXTRA - PAIR_AUX;   // GEMM-1: 4 x 48 KB
+};
 constexpr int PAIR_GMAX = (PAIR_NSUB / 4 + PAIR_GW - 1) / PAIR_GW;     // most 4-row groups one gather warp issues per k-block
 constexpr int PAIR_TQ = 8;                      // TMEM sub-tile barrier ring
 #ifndef FXM_PAIR_PF
@@ -64,16 +73,18 @@ constexpr int PAIR_PF = FXM_PAIR_PF;                     // weight tiles the L2 
 
 struct PairArgs {
     Dims D;
-    const uint8_t* packed;
+    LayerView V;
     const int* r_table;
-    const int4* items;         // GEMM-1: pair items {e, row0, valid rows, cbp}; GEMM-2: token tiles {e, row0, valid rows, .}
+    const int4* items;         // token tiles {e, row0, valid rows, GEMM-1 work prefix}; [ntt] = sentinel
     const Sched* sched;
-    const uint8_t* Bsrc;       // Xs (GEMM-1 fed by the gather kernel) or H (GEMM-2) panels
-    const int* tok;            // GEMM-1 with the gather fused: token index of every padded row (nullptr: read Xs)
+    const uint8_t* Bsrc;       // GEMM-2: the H panels
+    const int* tok;            // GEMM-1: token index of every padded row (the gather4 row coordinates)
     uint8_t* H;                // GEMM-1 output panels
-    uint8_t* O;                // GEMM-2 output panels [nDB][P][256 B]
+    const int2* row_tw;        // GEMM-2: {token or -1, router weight bits} of every padded row
+    float* yacc;               // GEMM-2: fp32 scatter-add target [T][d]; GEMM-1 zeroes it
     DevState* state;
     int P;
+    int T;
 };
 
 // ------------------------------------------------------------------------------------------ cluster PTX
@@ -173,18 +184,22 @@ __device__ long long g_trace[2][74][16][10];
 // ------------------------------------------------------------------------------------------------ items
 struct PairItem {
     int e, row0, n0, n1, blk, nk, r;
+    uint32_t eblk;            // first channel block of the expert in the weight regions
     bool valid;               // false: this CTA's weight block lies beyond the retained width (odd block count)
 };
 
+// `cur` = this role's cursor over the token tiles (GEMM-1: item wi belongs to the tile j with tt[j].w <= wi < tt[j+1].w;
+// a role's items ascend, so the cursor only moves forward -- a few L1 hits per item)
 template <int MODE>
-__device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_t rank) {
+__device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_t rank, int& cur) {
     const Dims& D = a.D;
     PairItem it;
     int4 q;
     int pairblk;
     if (MODE == 1) {
-        q = a.items[wi];
-        pairblk = q.w;
+        while (__ldg(&a.items[cur + 1].w) <= wi) ++cur;
+        q = __ldg(a.items + cur);
+        pairblk = wi - q.w;
     } else {
         const int nDBp = (D.nDB + 1) >> 1;
         q = a.items[wi / nDBp];
@@ -197,6 +212,7 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
     it.n0 = n <= PAIR_NSUB ? n : (((n >> 4) + 1) >> 1) << 4;
     it.n1 = n - it.n0;
     it.r = a.r_table[it.e];
+    it.eblk = a.V.eblk[it.e];
     const int nb = (it.r + CB - 1) / CB;
     const int blk = 2 * pairblk + (int)rank;
     const int limit = MODE == 1 ? nb : D.nDB;
@@ -252,15 +268,17 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
     uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-    const uint32_t stg_base = smem_base + PAIR_RING_BYTES;                    // epilogue staging, 2 x 16 KB
-    uint8_t* stg_gen = smem_gen + PAIR_RING_BYTES;
-    const uint32_t bar_base = stg_base + PAIR_STAGING;
+    constexpr int PAIR_RING_BYTES = PairSmem<MODE>::RING;
+    constexpr int PAIR_EXTRA = PairSmem<MODE>::EXTRA;
+    [[maybe_unused]] const uint32_t stg_base = smem_base + PAIR_RING_BYTES;   // GEMM-1: epilogue staging, 2 x 16 KB
+    [[maybe_unused]] uint8_t* stg_gen = smem_gen + PAIR_RING_BYTES;            // GEMM-2: row info, 2 x 512 x {token, weight}
+    const uint32_t bar_base = smem_base + PAIR_RING_BYTES + PAIR_EXTRA;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
     auto empty_bar = [&](int s) { return bar_base + 8u * (PAIR_MAX_STAGES + s); };
     auto tfull_bar = [&](uint32_t q) { return bar_base + 8u * (2 * PAIR_MAX_STAGES + (q % PAIR_TQ)); };
     auto tempty_bar = [&](uint32_t q) { return bar_base + 8u * (2 * PAIR_MAX_STAGES + PAIR_TQ + (q % PAIR_TQ)); };
-    volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + PAIR_RING_BYTES + PAIR_STAGING + 8 * (2 * PAIR_MAX_STAGES + 2 * PAIR_TQ));
-    int4* gidx = (int4*)(smem_gen + PAIR_RING_BYTES + PAIR_STAGING + 512);        // [PAIR_GW][PAIR_GMAX] token indices
+    volatile uint32_t* tmem_slot = (volatile uint32_t*)(smem_gen + PAIR_RING_BYTES + PAIR_EXTRA + 8 * (2 * PAIR_MAX_STAGES + 2 * PAIR_TQ));
+    [[maybe_unused]] int4* gidx = (int4*)(smem_gen + PAIR_RING_BYTES + PAIR_EXTRA + 512);   // [PAIR_GW][PAIR_GMAX] token indices
 
     const int warp = shfl0(threadIdx.x >> 5), lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
@@ -272,7 +290,8 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
             mbar_init(full_bar(s), rank == 0 ? 2 : 1);            // leader: own producer + the peer's relay
             mbar_init(empty_bar(s), 1);
         }
-        for (int q = 0; q < PAIR_TQ; ++q) { mbar_init(tfull_bar(q), 1); mbar_init(tempty_bar(q), 2); }
+        // "columns drained": GEMM-1 one arrival per CTA (after its epilogue barrier), GEMM-2 one per epilogue warp
+        for (int q = 0; q < PAIR_TQ; ++q) { mbar_init(tfull_bar(q), 1); mbar_init(tempty_bar(q), MODE == 1 ? 2 : 2 * PAIR_EPI_WARPS); }
         fence_barrier_init();
     }
     if (warp == 1) tmem_alloc2(smem_u32((const void*)tmem_slot), 512);
@@ -289,14 +308,15 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
     const int NS = min(PAIR_MAX_STAGES, (int)(PAIR_RING_BYTES / stage_bytes));
 
 
-    const bool gather = MODE == 1 && a.tok != nullptr;        // GEMM-1 token rows come straight from x via TMA gather4
+    constexpr bool gather = MODE == 1;                        // GEMM-1 token rows come straight from x via TMA gather4
     const int W = MODE == 1 ? a.sched->W1 : a.sched->W2;
     const int wi0 = (int)cluster_id_x(), wstep = (int)cluster_count_x();
-    const uint8_t* dn = a.packed + gu_bytes(D);
+    int cur = 0;                                              // every role walks the same item sequence with its own tile cursor
+    [[maybe_unused]] int pf_cur = 0;
     auto a_src = [&](const PairItem& it, size_t& stride) -> const uint8_t* {
-        if (MODE == 1) { stride = WT_BYTES; return a.packed + gu_tile_index(D, it.e, it.blk, 0) * WT_BYTES; }
+        if (MODE == 1) { stride = WT_BYTES; return a.V.gu + gu_tile_off(D, it.eblk, it.blk, 0); }
         stride = (size_t)D.nDB * WT_BYTES;
-        return dn + dn_tile_index(D, it.e, 0, it.blk) * WT_BYTES;
+        return a.V.dn + dn_tile_off(D, it.eblk, 0, it.blk);
     };
 
     if (warp == 0) {
@@ -313,7 +333,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         size_t pf_stride = 0;
         auto pf_load_item = [&]() {
             if (pf_wi < W) {
-                const PairItem pit = pair_item<MODE>(a, pf_wi, rank);
+                const PairItem pit = pair_item<MODE>(a, pf_wi, rank, pf_cur);
                 pf_src = a_src(pit, pf_stride);
                 pf_nk = pit.nk;
             }
@@ -327,7 +347,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         for (int i = 0; i < PAIR_PF; ++i) pf_step();
         int tj = 0;
         for (int wi = wi0; wi < W; wi += wstep, ++tj) {
-            const PairItem it = pair_item<MODE>(a, wi, rank);
+            const PairItem it = pair_item<MODE>(a, wi, rank, cur);
             long long tw = 0;
             size_t astride;
             const uint8_t* asrc = a_src(it, astride);
@@ -364,7 +384,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         int s = 0;
         uint32_t ph = 0;
         for (int wi = wi0; wi < W; wi += wstep) {
-            const PairItem it = pair_item<MODE>(a, wi, rank);
+            const PairItem it = pair_item<MODE>(a, wi, rank, cur);
             const int h0 = it.n0 >> 1, h1 = it.n1 >> 1;
             const int ng0 = h0 >> 2, ng = (h0 + h1) >> 2;
             const int cnt = ng > gw ? (ng - gw + PAIR_GW - 1) / PAIR_GW : 0;
@@ -392,7 +412,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         int s = 0;
         uint32_t ph = 0;
         for (int wi = wi0; wi < W; wi += wstep) {
-            const PairItem it = pair_item<MODE>(a, wi, rank);
+            const PairItem it = pair_item<MODE>(a, wi, rank, cur);
             for (int kb = 0; kb < it.nk; ++kb) {
                 mbar_wait(full_bar(s), ph, a.state);
                 if (leader_lane) mbar_arrive_remote(full_bar(s), 0);
@@ -408,7 +428,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         uint32_t ph = 0, drained = 0;
         int tj = 0;
         for (int wi = wi0; wi < W; wi += wstep, ++tj) {
-            const PairItem it = pair_item<MODE>(a, wi, rank);
+            const PairItem it = pair_item<MODE>(a, wi, rank, cur);
             [[maybe_unused]] const long long t_start = FXM_CLK();
             long long tw = 0;
             uint32_t c0, c1, need;
@@ -451,43 +471,50 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
             __syncwarp();
         }
     } else if (warp >= EPI0) {
-        // ===================================================== epilogue warps 4..19 (both CTAs, own TMEM lanes)
-        // A sub-tile is drained in CHUNKS of CH token columns: TMEM -> registers -> (SwiGLU | round) -> a 16 KB staging
-        // buffer in the FINAL global layout -> one bulk store per chunk.  Two staging buffers alternate.
-        constexpr int CH = MODE == 1 ? 128 : 64;                // tokens per chunk: 128 x 128 B (H rows) or 64 x 256 B (O rows)
-        constexpr int ROWB = MODE == 1 ? ROW_BYTES : 2 * WT_ROWS;   // bytes per token row of this CTA's output
+        // ===================================================== epilogue warps (both CTAs, own TMEM lanes)
         const int q = warp & 3;                                // TMEM lane quadrant this warp may read
         constexpr int NWQ = PAIR_EPI_WARPS / 4;                // warps per lane quadrant
-        const int wq = (warp - EPI0) >> 2;                        // which share of a chunk's 16-column groups
+        const int wq = (warp - EPI0) >> 2;                        // which share of the 16-column groups
         const int et = threadIdx.x - 32 * EPI0;
-        const uint64_t pol_keep = l2_policy_evict_last();         // H / O panels: read back by the next kernel
         TmemRing ring;
         ring.init();
-        uint32_t nchunk = 0;
         int tj = 0;
-        for (int wi = wi0; wi < W; wi += wstep, ++tj) {
-            const PairItem it = pair_item<MODE>(a, wi, rank);
-            const int nsub = it.n1 ? 2 : 1;
-            uint32_t cc0, cc1, need_unused;
-            const uint32_t sq0 = ring.seq;
-            ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, cc0, cc1, need_unused);
-            for (int sidx = 0; sidx < nsub; ++sidx) {
-                const int n = sidx ? it.n1 : it.n0;
-                const uint32_t col0 = sidx ? cc1 : cc0;
-                const uint32_t sq = sq0 + sidx;
-                const int rowS = it.row0 + (sidx ? it.n0 : 0);
-                const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + col0;
-                mbar_wait(tfull_bar(sq), (sq / PAIR_TQ) & 1u, a.state);
-                if (et == 0 && rank == 0 && sidx == 0) FXM_TR(MODE, tj, 4, FXM_CLK());
-                tc_fence_after();
-                for (int ch0 = 0; ch0 < n; ch0 += CH, ++nchunk) {
-                    const int rows = min(CH, n - ch0);
-                    uint8_t* stg = stg_gen + (nchunk & 1u) * 16384u;
-                    const int ngrp = rows >> 4;                          // 16-column groups in this chunk
-                    const int gbeg = ngrp * wq / NWQ, gend = ngrp * (wq + 1) / NWQ;
-                    if (it.valid && gbeg < gend) {
-                        uint32_t va[16], vb[16];
-                        if (MODE == 1) {
+        if constexpr (MODE == 1) {
+            // Y <- 0 (Alg. 2 l.1): zero the fp32 scatter-add target of GEMM-2.  These warps have nothing
+            // to do until the first tile has been multiplied; the stores drain while the tensor pipe works.
+            if (a.yacc) {
+                uint4* z = (uint4*)a.yacc;
+                const size_t n4 = (size_t)a.T * D.d / 4;
+                const size_t nthr = (size_t)gridDim.x * (32 * PAIR_EPI_WARPS);
+                for (size_t i = (size_t)blockIdx.x * (32 * PAIR_EPI_WARPS) + et; i < n4; i += nthr) z[i] = make_uint4(0, 0, 0, 0);
+            }
+            // A sub-tile is drained in CHUNKS of 128 token columns: TMEM -> registers -> SwiGLU -> a 16 KB staging buffer
+            // in the FINAL global layout (swizzled H panel rows) -> one bulk store per chunk.  Two staging buffers alternate.
+            constexpr int CH = 128;
+            const uint64_t pol_keep = l2_policy_evict_last();         // H panels: read back by GEMM-2
+            uint32_t nchunk = 0;
+            for (int wi = wi0; wi < W; wi += wstep, ++tj) {
+                const PairItem it = pair_item<MODE>(a, wi, rank, cur);
+                const int nsub = it.n1 ? 2 : 1;
+                uint32_t cc0, cc1, need_unused;
+                const uint32_t sq0 = ring.seq;
+                ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, cc0, cc1, need_unused);
+                for (int sidx = 0; sidx < nsub; ++sidx) {
+                    const int n = sidx ? it.n1 : it.n0;
+                    const uint32_t col0 = sidx ? cc1 : cc0;
+                    const uint32_t sq = sq0 + sidx;
+                    const int rowS = it.row0 + (sidx ? it.n0 : 0);
+                    const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + col0;
+                    mbar_wait(tfull_bar(sq), (sq / PAIR_TQ) & 1u, a.state);
+                    if (et == 0 && rank == 0 && sidx == 0) FXM_TR(MODE, tj, 4, FXM_CLK());
+                    tc_fence_after();
+                    for (int ch0 = 0; ch0 < n; ch0 += CH, ++nchunk) {
+                        const int rows = min(CH, n - ch0);
+                        uint8_t* stg = stg_gen + (nchunk & 1u) * 16384u;
+                        const int ngrp = rows >> 4;                          // 16-column groups in this chunk
+                        const int gbeg = ngrp * wq / NWQ, gend = ngrp * (wq + 1) / NWQ;
+                        if (it.valid && gbeg < gend) {
+                            uint32_t va[16], vb[16];
                             const int chn = q * 16 + (lane & 15);
                             const bool keep = it.blk * CB + chn < it.r;       // tail mask of the last retained block (pad-zero rule)
                             const int odd = lane >> 4;
@@ -514,46 +541,88 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                                 if (g + 2 < gend) tmem_ld16(taddr + ch0 + (g + 2) * 16, va);
                                 if (g + 1 < gend) swiglu16(vb, (g + 1) * 16);
                             }
-                        } else {
-                            // lane = output feature; 16 token columns per load; 32 lanes -> 64 contiguous bytes of one O row
-                            uint8_t* dst = stg + (q * 32 + lane) * 2;
-                            auto store16 = [&](const uint32_t (&v)[16], int t0) {
-#pragma unroll
-                                for (int jj = 0; jj < 16; ++jj)
-                                    *(__nv_bfloat16*)(dst + (t0 + jj) * ROWB) = __float2bfloat16_rn(__uint_as_float(v[jj]));
-                            };
-                            tmem_ld16(taddr + ch0 + gbeg * 16, va);
-                            for (int g = gbeg; g < gend; g += 2) {
-                                tmem_ld_wait();
-                                if (g + 1 < gend) tmem_ld16(taddr + ch0 + (g + 1) * 16, vb);
-                                store16(va, g * 16);
-                                tmem_ld_wait();
-                                if (g + 2 < gend) tmem_ld16(taddr + ch0 + (g + 2) * 16, va);
-                                if (g + 1 < gend) store16(vb, (g + 1) * 16);
+                        }
+                        const bool last = ch0 + CH >= n;
+                        fence_proxy_async_smem();                      // staging writes -> visible to the bulk-copy engine
+                        if (last) tc_fence_before();
+                        if (et == 0) bulk_wait_read0();                // the previous chunk's store has left the OTHER buffer
+                        epi_bar_sync_all();
+                        if (et == 0) {
+                            if (it.valid) {
+                                uint8_t* gdst = a.H + ((size_t)it.blk * a.P + rowS + ch0) * ROW_BYTES;
+                                bulk_s2g_hint(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROW_BYTES, pol_keep);
+                                bulk_commit();
                             }
-                        }
-                    }
-                    const bool last = ch0 + CH >= n;
-                    fence_proxy_async_smem();                      // staging writes -> visible to the bulk-copy engine
-                    if (last) tc_fence_before();
-                    if (et == 0) bulk_wait_read0();                // the previous chunk's store has left the OTHER buffer
-                    epi_bar_sync_all();
-                    if (et == 0) {
-                        if (it.valid) {
-                            uint8_t* gdst = MODE == 1 ? a.H + ((size_t)it.blk * a.P + rowS + ch0) * ROW_BYTES
-                                                      : a.O + ((size_t)it.blk * a.P + rowS + ch0) * ROWB;
-                            bulk_s2g_hint(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROWB, pol_keep);
-                            bulk_commit();
-                        }
-                        if (last) {                                // all epilogue warps have drained this sub-tile's columns
-                            if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
-                            if (rank == 0 && sidx == nsub - 1) FXM_TR(MODE, tj, 5, FXM_CLK());
+                            if (last) {                                // all epilogue warps have drained this sub-tile's columns
+                                if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
+                                if (rank == 0 && sidx == nsub - 1) FXM_TR(MODE, tj, 5, FXM_CLK());
+                            }
                         }
                     }
                 }
             }
+            if (et == 0) bulk_wait0();
+        } else {
+            // GEMM-2: "Z <- Z (.) alpha;  Y <- ScatterAdd(Y, pi, Z)" (Alg. 2 l.19-20) straight from the
+            // accumulator.  A warp owns up to four 16-column groups of a sub-tile (its lane quadrant = 32 output features):
+            // it loads them into 64 registers, tells the MMA warp that it is done with the columns, and only then scales and
+            // adds: lane = feature, so each red.global.add.f32 of the warp is one 128-byte line of yacc[token].
+            int2* rinfo = (int2*)stg_gen;                              // [2][512] {token or -1, router weight bits}
+            const int feat0 = q * 32 + lane;
+            for (int wi = wi0; wi < W; wi += wstep, ++tj) {
+                const PairItem it = pair_item<MODE>(a, wi, rank, cur);
+                const int nsub = it.n1 ? 2 : 1;
+                int2* ri = rinfo + (tj & 1) * 512;
+                if (et < it.n0 + it.n1) ri[et] = __ldg(a.row_tw + it.row0 + et);
+                epi_bar_sync_all();                                    // row info of this item is in place (and the buffer of item tj-2 is free)
+                uint32_t cc0, cc1, need_unused;
+                const uint32_t sq0 = ring.seq;
+                ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, cc0, cc1, need_unused);
+                const int feat = it.blk * WT_ROWS + feat0;
+                const bool fok = it.valid && feat < D.d;               // padded rows of the last feature block (d % 128 == 64)
+                float* ycol = a.yacc + feat;
+                for (int sidx = 0; sidx < nsub; ++sidx) {
+                    const int n = sidx ? it.n1 : it.n0;
+                    const uint32_t col0 = sidx ? cc1 : cc0;
+                    const uint32_t sq = sq0 + sidx;
+                    const int2* rr = ri + (sidx ? it.n0 : 0);
+                    const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + col0;
+                    const int ngrp = n >> 4;                               // <= 16 groups in a sub-tile of <= 256 tokens
+                    const int gbeg = ngrp * wq / NWQ, gend = ngrp * (wq + 1) / NWQ;     // <= 4 of them are this warp's
+                    mbar_wait(tfull_bar(sq), (sq / PAIR_TQ) & 1u, a.state);
+                    if (et == 0 && rank == 0 && sidx == 0) FXM_TR(MODE, tj, 4, FXM_CLK());
+                    tc_fence_after();
+                    uint32_t v[4][16];
+                    if (it.valid) {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+                            if (gbeg + u < gend) tmem_ld16(taddr + (uint32_t)(gbeg + u) * 16u, v[u]);
+                        tmem_ld_wait();
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {                                   // this warp no longer needs the columns
+                        if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
+                    }
+                    if (fok) {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (gbeg + u < gend) {
+                                const int2* r16 = rr + (gbeg + u) * 16;
+#pragma unroll
+                                for (int jj = 0; jj < 16; ++jj) {
+                                    const int2 tw = r16[jj];           // same address in every lane: a broadcast
+                                    if (tw.x >= 0)
+                                        asm volatile("red.relaxed.gpu.global.add.f32 [%0], %1;" ::"l"(ycol + (size_t)tw.x * D.d),
+                                                     "f"(__int_as_float(tw.y) * __uint_as_float(v[u][jj])) : "memory");
+                                }
+                            }
+                        }
+                    }
+                    if (et == 0 && rank == 0 && sidx == nsub - 1) FXM_TR(MODE, tj, 5, FXM_CLK());
+                }
+            }
         }
-        if (et == 0) bulk_wait0();
     }
 
     tc_fence_before();
@@ -601,22 +670,19 @@ cudaError_t init_pair_kernels() {
     return cudaFuncSetAttribute(k_gemm_pair<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, PAIR_SMEM);
 }
 
-cudaError_t launch_gemm1_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+cudaError_t launch_gemm1_pair(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws, int T,
                               DevState* state, int num_sms, const void* x_map, cudaStream_t st) {
     PairArgs a{};
-    a.D = D; a.packed = packed; a.r_table = r_table; a.items = ws.items1; a.sched = ws.sched; a.Bsrc = ws.Xs;
-    a.H = ws.H; a.state = state; a.P = ws.P;
-    a.tok = x_map ? ws.row_tok : nullptr;
-    CUtensorMap m{};
-    if (x_map) m = *(const CUtensorMap*)x_map;
-    return launch_pair_t<1>(a, m, num_sms, st);
+    a.D = D; a.V = V; a.r_table = r_table; a.items = ws.tt; a.sched = ws.sched; a.tok = ws.row_tok;
+    a.H = ws.H; a.yacc = ws.yacc; a.T = T; a.state = state; a.P = ws.P;
+    return launch_pair_t<1>(a, *(const CUtensorMap*)x_map, num_sms, st);
 }
 
-cudaError_t launch_gemm2_pair(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+cudaError_t launch_gemm2_pair(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws,
                               DevState* state, int num_sms, cudaStream_t st) {
     PairArgs a{};
-    a.D = D; a.packed = packed; a.r_table = r_table; a.items = ws.tt; a.sched = ws.sched; a.Bsrc = ws.H;
-    a.O = ws.O; a.state = state; a.P = ws.P;
+    a.D = D; a.V = V; a.r_table = r_table; a.items = ws.tt; a.sched = ws.sched; a.Bsrc = ws.H;
+    a.row_tw = ws.row_tw; a.yacc = ws.yacc; a.state = state; a.P = ws.P;
     return launch_pair_t<2>(a, CUtensorMap{}, num_sms, st);
 }
 

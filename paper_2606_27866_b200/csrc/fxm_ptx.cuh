@@ -35,6 +35,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, DevStat
     while (!mbar_try_wait(bar, parity)) {
         if ((++spins & 0xFFFu) == 0 && clock64() - t0 > 4000000000LL) {
             atomicOr(&state->flags, 2u);
+            if (state->hflag) *(volatile uint32_t*)state->hflag = 2u;    // pinned host word: still readable after the trap
             __threadfence_system();
             __trap();
         }

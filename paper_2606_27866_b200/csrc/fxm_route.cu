@@ -1,22 +1,26 @@
-// fxm_route.cu -- step a2/a3: router-output grouping (stable per-expert counting sort, bit-exact indices),
-// the device-side tile schedule that skips pruned work, and the gather of token rows into sorted panels.
+// fxm_route.cu -- steps a2 + a3 in ONE launch: router-output grouping (stable per-expert counting sort, bit-exact
+// indices) and the device-side tile schedule that skips pruned work.
 //   Alg. 2 l.4-6: "(pi, eid) <- Sort(eid)", read as the STABLE sort by (expert id, flat
 //   index f = t*k+j) so that exactly one permutation is correct (reading R5).
 //   Alg. 2 l.2-3, 8-11: BucketByRetI / AlignUp / view lists are replaced by a tile list
 //   computed here from counts[] and the CURRENT width table r[]: only tiles with channel index < r_e and
 //   token row < n_e exist.
-//   Alg. 2 l.7: X[pi] -- the gather of routed token rows into sorted panels.
 //
-// Three launches, no atomics decide any position (hence deterministic and stable):
-//   k_route_plan     grid = RB blocks.  Block b histograms the flat assignments [b*chunk, (b+1)*chunk) per
-//                    expert.  The LAST block to publish (ticket counter) turns the RB x E histogram into
-//                    exclusive bases over blocks and writes counts, offsets, padded offsets, the token tiles
-//                    and the GEMM-1 work items for the current width table.
-//   k_scatter        grid = RB blocks.  Block b ranks its assignments: base over blocks + base over the
-//                    warps of the block + __match_any_sync rank inside a 32-wide step ("earlier block, earlier
-//                    warp, earlier step, lower lane" == "lower flat index"), writes perm / inv_perm / row_flat
-//                    / prow.
-//   k_gather         full grid, one warp per padded row: x rows -> swizzled K-major panels Xs.
+// k_route, grid = RB <= 128 blocks of 256 threads, no atomics decide any position (deterministic and stable):
+//   1  block b histograms its flat assignments [b*chunk, (b+1)*chunk) per expert, one histogram row per warp
+//      (warp w owns a contiguous sub-range, so "earlier block, earlier warp, earlier 32-wide step, lower lane" is
+//      "lower flat index"), and publishes the block row to bhist[b][.];
+//   2  grid-wide publish barrier: a ticket counter; the last block to arrive bumps a generation word that the
+//      others poll (all RB <= 128 blocks are co-resident: they are small and a B200 has 148 SMs);
+//   3  EVERY block sums the published rows itself: all rows -> counts, rows of earlier blocks -> its own base.
+//      These are independent loads (no serial scan by a "last block"), a few per thread;
+//   4  every block scans counts over the experts (offsets, padded offsets) in shared memory and scatters its own
+//      assignments -- the per-warp histograms of step 1 are still in shared memory, nothing is recomputed;
+//   5  block 0 also writes counts / offsets and the schedule for the current width table: the token tiles
+//      {expert, first padded row, valid rows, GEMM-1 work prefix}, experts ordered by descending work per tile (rows x
+//      retained width) so that a static stride over the work list hands out the heavy tiles first and the light
+//      ones in the last, partly filled round.  GEMM-1's work items (tile, pair of retained channel blocks) are not
+//      materialised: item wi belongs to the tile j with tt[j].w <= wi < tt[j+1].w (tt[ntt] is a sentinel).
 #include "fxm_internal.cuh"
 
 namespace fxm {
@@ -31,198 +35,223 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
     }
     return v;
 }
+__device__ __forceinline__ uint32_t ld_acquire_gpu(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 
 // balanced split of np padded rows into nt tiles: rows per tile, a multiple of 16
 __device__ __forceinline__ int per_rows(int np, int nt) { return ((np + nt - 1) / nt + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN; }
 
-// per-warp histogram of the block's chunk; warp w owns the contiguous sub-range [wlo, whi)
-__device__ __forceinline__ bool block_histogram(const int* __restrict__ ids, int E, int wlo, int whi, int lane,
-                                                int* __restrict__ wh /* this warp's [MAX_E] row */) {
-    bool bad = false;
-    for (int base = wlo; base < whi; base += 32) {
-        const int f = base + lane;
-        int id = f < whi ? ids[f] : -1;
-        if (f < whi && (id < 0 || id >= E)) { bad = true; id = -1; }
-        const unsigned m = __match_any_sync(0xffffffffu, id);
-        if (id >= 0 && lane == __ffs(m) - 1) wh[id] += __popc(m);
-        __syncwarp();
-    }
-    return bad;
+// -DFXM_TRACE: per-block globaltimer stamps (ns) of the phases (tuning aid; the product build has none of this)
+#ifdef FXM_TRACE
+__device__ unsigned long long g_rtrace[RT_MAX_BLOCKS][8];
+__device__ __forceinline__ unsigned long long rt_now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
 }
+#define RT_TR(f) do { if (threadIdx.x == 0) g_rtrace[blockIdx.x][f] = rt_now(); } while (0)
+#else
+#define RT_TR(f) do { } while (0)
+#endif
+
+struct RouteWs {             // the device pointers of the workspace the kernel writes
+    int* poff;
+    Sched* sched;
+    int* row_flat;
+    int* row_tok;
+    int2* row_tw;
+    int* bhist;
+    int4* tt;
+    int chunk;
+};
 
 __global__ void __launch_bounds__(RT_THREADS)
-k_route_plan(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table, int tile_n, int grp,
-             int* __restrict__ counts, int* __restrict__ offsets, int* __restrict__ bhist, int* __restrict__ poff,
-             int4* __restrict__ tt, int4* __restrict__ items1, Sched* __restrict__ sched,
-             DevState* __restrict__ state) {
-    __shared__ int whist[RT_WARPS][MAX_E];
-    __shared__ int s_cnt[MAX_E], s_off[MAX_E + 1], s_poff[MAX_E + 1];
-    __shared__ int s_ntt, s_last;
-    const int E = D.E;
-    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
+    __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, later the warp's running base
+    __shared__ int s_cnt[MAX_E], s_off[MAX_E + 1], s_poff[MAX_E + 1], s_bbase[MAX_E];
+    __shared__ int s_key[MAX_E], s_order[MAX_E];
+    __shared__ uint32_t s_gen0;
+    const Dims& D = a.D;
+    const int E = D.E, k = a.k, A = a.T * a.k;
+    const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
+    const int RB = gridDim.x, b = blockIdx.x;
+    const int* __restrict__ ids = a.ids;
+    RT_TR(0);
     pdl_launch_dependents();
     for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
-    __syncthreads();
     pdl_wait();                                                  // the previous call's kernels may still read the workspace
-    const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
-    const int sub = chunk / RT_WARPS;
-    const int wlo = min(hi, lo + w * sub), whi = min(hi, wlo + sub);
-    if (block_histogram(ids, E, wlo, whi, lane, whist[w])) atomicOr(&state->flags, 1u);
+    RT_TR(1);
+    if (tid == 0) s_gen0 = ld_acquire_gpu(&state->route_gen);    // before this block arrives anywhere
+    __syncthreads();
+
+    // ---- 1: per-warp histogram of this block's chunk
+    const int lo = min(A, b * w.chunk), hi = min(A, lo + w.chunk);
+    const int sub = w.chunk / RT_WARPS;
+    const int wlo = min(hi, lo + wp * sub), whi = min(hi, wlo + sub);
+    {
+        bool bad = false;
+        int* wh = whist[wp];
+        for (int base = wlo; base < whi; base += 32) {
+            const int f = base + lane;
+            int id = f < whi ? ids[f] : -1;
+            if (f < whi && (id < 0 || id >= E)) { bad = true; id = -1; }
+            const unsigned m = __match_any_sync(0xffffffffu, id);
+            if (id >= 0 && lane == __ffs(m) - 1) wh[id] += __popc(m);
+            __syncwarp();
+        }
+        if (bad) atomicOr(&state->flags, 1u);
+    }
     __syncthreads();
     for (int e = tid; e < E; e += RT_THREADS) {
         int c = 0;
 #pragma unroll
         for (int ww = 0; ww < RT_WARPS; ++ww) c += whist[ww][e];
-        bhist[(size_t)blockIdx.x * E + e] = c;
+        w.bhist[(size_t)b * E + e] = c;
     }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) s_last = (atomicAdd(&state->ticket, 1u) == gridDim.x - 1);
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
 
-    // ---- last block: exclusive scan over blocks, per expert.  Thread (e, s) owns rows [s*L, (s+1)*L) of column e:
-    //      pass 1 sums them, the S segment sums are scanned through shared memory, pass 2 writes the prefixes.
-    const int RB = gridDim.x;
-    const int S = RT_THREADS / E > 0 ? RT_THREADS / E : 1;     // E <= 256 = RT_THREADS
-    const int L = (RB + S - 1) / S;
-    int* seg = &whist[0][0];                                     // [S][E] <= 256 ints, histogram rows are dead now
-    const int e0 = tid % E, s0 = tid / E;
-    const int b_lo = min(RB, s0 * L), b_hi = s0 < S ? min(RB, b_lo + L) : b_lo;
-    {
-        int sum = 0;
-        int b = b_lo;
-        for (; b + 8 <= b_hi; b += 8) {
-            int c[8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u) c[u] = __ldcg(bhist + (size_t)(b + u) * E + e0);
-#pragma unroll
-            for (int u = 0; u < 8; ++u) sum += c[u];
-        }
-        for (; b < b_hi; ++b) sum += __ldcg(bhist + (size_t)b * E + e0);
-        __syncthreads();                                         // everyone is done reading whist
-        if (s0 < S) seg[s0 * E + e0] = sum;
-    }
+    // ---- 2: publish barrier over the grid
+    __threadfence();
     __syncthreads();
-    {
-        int run = 0;
-        for (int ss = 0; ss < s0 && ss < S; ++ss) run += seg[ss * E + e0];
-        if (s0 == S - 1) {                                       // the last segment also knows the column total
-            const int tot = run + seg[s0 * E + e0];
-            s_cnt[e0] = tot;
-            counts[e0] = tot;
-        }
-        int b = b_lo;
-        for (; b + 8 <= b_hi; b += 8) {
-            int c[8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u) c[u] = __ldcg(bhist + (size_t)(b + u) * E + e0);
-#pragma unroll
-            for (int u = 0; u < 8; ++u) { bhist[(size_t)(b + u) * E + e0] = run; run += c[u]; }
-        }
-        for (; b < b_hi; ++b) {
-            const int c = __ldcg(bhist + (size_t)b * E + e0);
-            bhist[(size_t)b * E + e0] = run;
-            run += c;
+    RT_TR(2);
+    if (tid == 0) {
+        if (atomicAdd(&state->ticket, 1u) == (uint32_t)RB - 1u) {
+            state->ticket = 0;                                   // ready for the next call on this layer
+            __threadfence();
+            atomicAdd(&state->route_gen, 1u);
+        } else {
+            const long long t0 = clock64();
+            uint32_t spins = 0;
+            while (ld_acquire_gpu(&state->route_gen) == s_gen0) {
+                if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) {
+                    atomicOr(&state->flags, 2u);
+                    if (state->hflag) *(volatile uint32_t*)state->hflag = 2u;
+                    __threadfence_system();
+                    __trap();
+                }
+            }
         }
     }
     __syncthreads();
 
-    // ---- warp 0: scans over experts -> offsets, padded offsets, token tiles, work prefixes
-    if (w == 0) {
-        int c_off = 0, c_poff = 0, c_tiles = 0, c_work = 0, c_max = ROW_ALIGN;
+    RT_TR(3);
+    // ---- 3: every block sums the published rows: thread (e0, s0) takes rows s0, s0 + S, ... of column e0
+    {
+        const int S = RT_THREADS / E > 0 ? RT_THREADS / E : 1;   // E <= 256 = RT_THREADS
+        const int e0 = tid % E, s0 = tid / E;
+        int tot = 0, base = 0;
+        if (s0 < S) {
+            int bb = s0;
+            for (; bb + 15 * S < RB; bb += 16 * S) {             // 16 independent loads in flight per thread
+                int c[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) c[u] = __ldcg(w.bhist + (size_t)(bb + u * S) * E + e0);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) { tot += c[u]; if (bb + u * S < b) base += c[u]; }
+            }
+            for (; bb < RB; bb += S) {
+                const int c = __ldcg(w.bhist + (size_t)bb * E + e0);
+                tot += c;
+                if (bb < b) base += c;
+            }
+        }
+        // reduce the S partials of a column through shared memory (s_cnt / s_bbase as accumulators)
+        for (int e = tid; e < E; e += RT_THREADS) { s_cnt[e] = 0; s_bbase[e] = 0; }
+        __syncthreads();
+        if (s0 < S) { atomicAdd(&s_cnt[e0], tot); atomicAdd(&s_bbase[e0], base); }   // integer sums: order-independent
+        __syncthreads();
+    }
+
+    RT_TR(4);
+    // ---- 4a: warp 0 scans over the experts -> offsets and padded offsets (expert order); block 0 also orders the
+    //          experts by descending work per tile and lays out the token tiles and work prefixes in that order
+    if (wp == 0) {
+        int c_off = 0, c_poff = 0;
         for (int base = 0; base < E; base += 32) {
             const int e = base + lane;
             const int n = e < E ? s_cnt[e] : 0;
-            const int r = e < E ? (r_table ? r_table[e] : D.I) : 0;   // no table yet (fxm_route only): full width
             const int np = (n + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
-            const int nt = (n > 0 && r > 0) ? (np + tile_n - 1) / tile_n : 0;   // pruned-away / idle experts: no tiles
-            const int nb = ((r + CB - 1) / CB + grp - 1) / grp;                 // GEMM-1 items per token tile
             const int i_off = warp_incl_scan(n, lane), i_poff = warp_incl_scan(np, lane);
-            const int i_tiles = warp_incl_scan(nt, lane), i_work = warp_incl_scan(nt * nb, lane);
-            if (e < E) {
-                s_off[e] = c_off + i_off - n;
-                s_poff[e] = c_poff + i_poff - np;
-                int j = c_tiles + i_tiles - nt, wk = c_work + i_work - nt * nb;
-                const int p0 = c_poff + i_poff - np;
-                // balanced split of the padded segment into nt tiles of <= tile_n rows, each a multiple of 16 rows
-                const int per = nt > 0 ? per_rows(np, nt) : 0;
-                for (int row = 0; row < np && nt > 0; row += per, ++j, wk += nb)
-                    tt[j] = make_int4(e, p0 + row, min(per, n - row), wk);      // .z = valid rows of the tile (>= 1)
-            }
-            {
-                int mx = nt > 0 ? min(per_rows(np, nt), np) : 0;          // rows of this expert's widest tile
-#pragma unroll
-                for (int o = 16; o; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-                c_max = max(c_max, mx);
-            }
+            if (e < E) { s_off[e] = c_off + i_off - n; s_poff[e] = c_poff + i_poff - np; }
             c_off += __shfl_sync(0xffffffffu, i_off, 31);
             c_poff += __shfl_sync(0xffffffffu, i_poff, 31);
-            c_tiles += __shfl_sync(0xffffffffu, i_tiles, 31);
-            c_work += __shfl_sync(0xffffffffu, i_work, 31);
         }
-        if (lane == 0) {
-            s_off[E] = c_off;
-            s_poff[E] = c_poff;
-            s_ntt = c_tiles;
-            sched->ntt = c_tiles;
-            sched->W1 = c_work;
-            sched->W2 = c_tiles * ((D.nDB + grp - 1) / grp);
-            sched->P_used = c_poff;
-            sched->A = A;
-            sched->max_n = c_max;
-            state->ticket = 0;                               // ready for the next call on this layer
-        }
+        if (lane == 0) { s_off[E] = c_off; s_poff[E] = c_poff; }
     }
     __syncthreads();
-    for (int e = tid; e <= E; e += RT_THREADS) { offsets[e] = s_off[e]; poff[e] = s_poff[e]; }
-    // GEMM-1 work items: one per (token tile, RETAINED channel block) -- pruned blocks are never listed
-    for (int j = tid; j < s_ntt; j += RT_THREADS) {
-        const int4 t = tt[j];
-        const int nb = (((r_table ? r_table[t.x] : D.I) + CB - 1) / CB + grp - 1) / grp;
-        for (int cb = 0; cb < nb; ++cb) items1[t.w + cb] = make_int4(t.x, t.y, t.z, cb);
-    }
-}
-
-// copy one x row (d bf16) into the swizzled panels Xs[kb][p][.]; src == nullptr writes zeros
-__device__ __forceinline__ void put_row(const uint4* __restrict__ src, uint8_t* __restrict__ Xs, int P, int p,
-                                        int chunks_per_row, int lane) {
-    for (int c0 = lane; c0 < chunks_per_row; c0 += 128) {
-        uint4 v[4];
+    if (b == 0) {
+        // work key of an expert: rows of its widest tile x retained width (what one GEMM-2 item of it costs)
+        for (int e = tid; e < E; e += RT_THREADS) {
+            const int n = s_cnt[e];
+            const int r = a.r_table ? a.r_table[e] : D.I;           // no table yet (fxm_route only): full width
+            const int np = (n + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
+            const int nt = (n > 0 && r > 0) ? (np + a.tile_n - 1) / a.tile_n : 0;
+            s_key[e] = nt > 0 ? min(per_rows(np, nt), np) * r : 0;
+        }
+        __syncthreads();
+        for (int e = tid; e < E; e += RT_THREADS) {               // rank by (key descending, id ascending)
+            const int ke = s_key[e];
+            int rk = 0;
+            for (int o = 0; o < E; ++o) {
+                const int ko = s_key[o];
+                rk += (ko > ke) || (ko == ke && o < e);
+            }
+            s_order[rk] = e;
+        }
+        __syncthreads();
+        if (wp == 0) {
+            int c_tiles = 0, c_work = 0, c_max = ROW_ALIGN;
+            for (int base = 0; base < E; base += 32) {
+                const int pos = base + lane;
+                const int e = pos < E ? s_order[pos] : 0;
+                const int n = pos < E ? s_cnt[e] : 0;
+                const int r = pos < E ? (a.r_table ? a.r_table[e] : D.I) : 0;
+                const int np = (n + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
+                const int nt = (n > 0 && r > 0) ? (np + a.tile_n - 1) / a.tile_n : 0;   // pruned-away / idle experts: no tiles
+                const int nb = ((r + CB - 1) / CB + 1) / 2;                          // GEMM-1 pair items per token tile
+                const int i_tiles = warp_incl_scan(nt, lane), i_work = warp_incl_scan(nt * nb, lane);
+                if (pos < E && nt > 0) {
+                    int j = c_tiles + i_tiles - nt, wk = c_work + i_work - nt * nb;
+                    const int p0 = s_poff[e];
+                    // balanced split of the padded segment into nt tiles of <= tile_n rows, each a multiple of 16 rows
+                    const int per = per_rows(np, nt);
+                    for (int row = 0; row < np; row += per, ++j, wk += nb)
+                        w.tt[j] = make_int4(e, p0 + row, min(per, n - row), wk);   // .z = valid rows of the tile (>= 1)
+                }
+                {
+                    int mx = nt > 0 ? min(per_rows(np, nt), np) : 0;               // rows of this expert's widest tile
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int c = c0 + 32 * u;
-            v[u] = (src && c < chunks_per_row) ? __ldg(src + c) : make_uint4(0, 0, 0, 0);
+                    for (int o = 16; o; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+                    c_max = max(c_max, mx);
+                }
+                c_tiles += __shfl_sync(0xffffffffu, i_tiles, 31);
+                c_work += __shfl_sync(0xffffffffu, i_work, 31);
+            }
+            if (lane == 0) {
+                w.tt[c_tiles] = make_int4(0, 0, 0, c_work);          // sentinel: the work prefix of "the tile after the last"
+                w.sched->ntt = c_tiles;
+                w.sched->W1 = c_work;
+                w.sched->W2 = c_tiles * ((D.nDB + 1) / 2);
+                w.sched->P_used = s_poff[E];
+                w.sched->A = A;
+                w.sched->max_n = c_max;
+                w.sched->claim1 = 0;
+                w.sched->claim2 = 0;
+            }
         }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int c = c0 + 32 * u;
-            if (c < chunks_per_row)
-                *(uint4*)(Xs + ((size_t)(c >> 3) * P + p) * ROW_BYTES + ((((c & 7) ^ p) & 7) << 4)) = v[u];
+        for (int e = tid; e <= E; e += RT_THREADS) {
+            a.offsets[e] = s_off[e];
+            w.poff[e] = s_poff[e];
+            if (e < E) a.counts[e] = s_cnt[e];
         }
     }
-}
 
-__global__ void __launch_bounds__(RT_THREADS)
-k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __restrict__ r_table,
-          const int* __restrict__ counts, const int* __restrict__ offsets, const int* __restrict__ poff,
-          const int* __restrict__ bbase, int* __restrict__ perm, int* __restrict__ inv_perm,
-          int* __restrict__ row_flat, int* __restrict__ prow, int* __restrict__ row_tok, int k) {
-    __shared__ int whist[RT_WARPS][MAX_E];      // per-warp histogram, then per-warp running base
-    const int E = D.E;
-    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    pdl_launch_dependents();
-    for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
-    __syncthreads();
-    pdl_wait();
-    const int lo = min(A, blockIdx.x * chunk), hi = min(A, lo + chunk);
-    const int sub = chunk / RT_WARPS;
-    const int wlo = min(hi, lo + w * sub), whi = min(hi, wlo + sub);
-    block_histogram(ids, E, wlo, whi, lane, whist[w]);
-    __syncthreads();
-    for (int e = tid; e < E; e += RT_THREADS) {      // exclusive scan over the warps of this block, on top of the block base
-        int run = bbase[(size_t)blockIdx.x * E + e];
+    RT_TR(5);
+    // ---- 4b: exclusive scan over the warps of this block, on top of the block base -> the warp's running base
+    for (int e = tid; e < E; e += RT_THREADS) {
+        int run = s_bbase[e];
 #pragma unroll
         for (int ww = 0; ww < RT_WARPS; ++ww) {
             const int c = whist[ww][e];
@@ -232,71 +261,50 @@ k_scatter(Dims D, const int* __restrict__ ids, int A, int chunk, const int* __re
     }
     __syncthreads();
 
-    // ---- stable scatter
+    // ---- stable scatter of this block's assignments
     for (int base = wlo; base < whi; base += 32) {
         const int f = base + lane;
         int id = f < whi ? ids[f] : -1;
         if (id < 0 || id >= E) id = -1;
         const unsigned m = __match_any_sync(0xffffffffu, id);
         if (id >= 0) {
-            const int rank = whist[w][id] + __popc(m & ((1u << lane) - 1u));
-            const int pos = offsets[id] + rank;
-            const int pr = poff[id] + rank;
-            perm[pos] = f;
-            inv_perm[f] = pos;
-            row_flat[pr] = f;
-            row_tok[pr] = f / k;
-            prow[f] = (!r_table || r_table[id] > 0) ? pr : -1;   // width-0 experts get no tiles: nothing to read back
+            const int rank = whist[wp][id] + __popc(m & ((1u << lane) - 1u));
+            const int pos = s_off[id] + rank;
+            const int pr = s_poff[id] + rank;
+            const int t = f / k;
+            a.perm[pos] = f;
+            a.inv_perm[f] = pos;
+            w.row_flat[pr] = f;
+            w.row_tok[pr] = t;
+            w.row_tw[pr] = make_int2(t, a.topk_w ? __float_as_int(a.topk_w[f]) : 0);
         } else if (f < whi) {
-            inv_perm[f] = -1;                                // dropped (precondition violation, flagged by the plan kernel)
-            prow[f] = -1;
+            a.inv_perm[f] = -1;                              // dropped (precondition violation, flagged above)
         }
         __syncwarp();
-        if (id >= 0 && lane == __ffs(m) - 1) whist[w][id] += __popc(m);
+        if (id >= 0 && lane == __ffs(m) - 1) whist[wp][id] += __popc(m);
         __syncwarp();
     }
 
+    RT_TR(6);
     // ---- padding rows of the expert segments carry no assignment
-    for (int e = blockIdx.x * RT_THREADS + tid; e < E; e += gridDim.x * RT_THREADS)
-        for (int p = poff[e] + counts[e]; p < poff[e + 1]; ++p) { row_flat[p] = -1; row_tok[p] = 0; }
+    for (int e = b * RT_THREADS + tid; e < E; e += RB * RT_THREADS)
+        for (int p = s_poff[e] + s_cnt[e]; p < s_poff[e + 1]; ++p) {
+            w.row_flat[p] = -1;
+            w.row_tok[p] = 0;
+            w.row_tw[p] = make_int2(-1, 0);
+        }
+
 }
 
-// Alg. 2 l.7, X[pi]: one warp per padded row p copies x[token(p)] into the swizzled panels; padding
-// rows become zeros so no garbage ever reaches a tensor core.
-__global__ void __launch_bounds__(256)
-k_gather(Dims D, const uint4* __restrict__ x, int k, const int* __restrict__ row_flat, const Sched* __restrict__ sched,
-         uint8_t* __restrict__ Xs, int P) {
-    const int lane = threadIdx.x & 31;
-    const int gw = blockIdx.x * 8 + (threadIdx.x >> 5), nw = gridDim.x * 8;
-    pdl_launch_dependents();
-    pdl_wait();
-    const int P_used = sched->P_used;
-    const int chunks_per_row = D.d >> 3;
-    for (int p = gw; p < P_used; p += nw) {
-        const int f = row_flat[p];
-        put_row(f >= 0 ? x + (size_t)(f / k) * chunks_per_row : nullptr, Xs, P, p, chunks_per_row, lane);
-    }
-}
-
-cudaError_t launch_route_plan(const Dims& D, const int* ids, int T, int k, const int* r_table, int tile_n, int grp,
-                              int* counts, int* offsets, const Workspace& ws, DevState* state, cudaStream_t st) {
-    return launch_pdl(k_route_plan, dim3(ws.RB), dim3(RT_THREADS), 0, st, D, ids, T * k, ws.chunk, r_table, tile_n, grp, counts,
-                      offsets, ws.bhist, ws.poff, ws.tt, ws.items1, ws.sched, state);
-}
-
-cudaError_t launch_scatter(const Dims& D, const int* ids, int T, int k, const int* r_table, const int* counts,
-                           const int* offsets, int* perm, int* inv_perm, const Workspace& ws, cudaStream_t st) {
-    return launch_pdl(k_scatter, dim3(ws.RB), dim3(RT_THREADS), 0, st, D, ids, T * k, ws.chunk, r_table, counts, offsets,
-                      (const int*)ws.poff, (const int*)ws.bhist, perm, inv_perm, ws.row_flat, ws.prow, ws.row_tok, k);
-}
-
-cudaError_t launch_gather(const Dims& D, const __nv_bfloat16* x, int T, int k, const Workspace& ws, cudaStream_t st) {
-    const long long rows = (long long)T * k + (long long)D.E * (ROW_ALIGN - 1);
-    long long blocks = (rows + 7) / 8;
-    if (blocks > 148 * 8) blocks = 148 * 8;
-    if (blocks < 1) blocks = 1;
-    return launch_pdl(k_gather, dim3((unsigned)blocks), dim3(256), 0, st, D, (const uint4*)x, k, (const int*)ws.row_flat,
-                      (const Sched*)ws.sched, ws.Xs, ws.P);
+cudaError_t launch_route(const RouteArgs& a, const Workspace& ws, DevState* state, cudaStream_t st) {
+    RouteWs w{};
+    w.poff = ws.poff; w.sched = ws.sched; w.row_flat = ws.row_flat; w.row_tok = ws.row_tok; w.row_tw = ws.row_tw;
+    w.bhist = ws.bhist; w.tt = ws.tt; w.chunk = ws.chunk;
+    return launch_pdl(k_route, dim3(ws.RB), dim3(RT_THREADS), 0, st, a, w, state);
 }
 
 }  // namespace fxm
+
+#ifdef FXM_TRACE
+extern "C" int fxm_rtrace_read(void* dst) { return (int)cudaMemcpyFromSymbol(dst, fxm::g_rtrace, sizeof(fxm::g_rtrace)); }
+#endif

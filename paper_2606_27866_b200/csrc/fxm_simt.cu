@@ -1,11 +1,11 @@
 // fxm_simt.cu -- the slow, structurally simple DEBUG path for steps a4/a5 (FXM_IMPL_SIMT_DEBUG).
-// It runs on the SAME packed weights, schedule and swizzled activation panels as the tcgen05 kernels, one
+// It runs on the SAME packed weights, schedule, H panels and fp32 accumulator as the tcgen05 kernels, one
 // CTA per work item, plain loads and fp32 FMAs -- no tensor cores, no async copies, no mbarriers -- so a
 // disagreement between the two paths isolates the fast kernels.  It is a CUDA path (not a CPU fallback) and
 // is never selected unless the caller asks for it with fxm_set_impl().
 //   a4: G = X_e W~gate[0:r_e]^T, U = X_e W~up[0:r_e]^T, H = silu(G) (.) U, channels >= r_e forced to 0
 //       (Eq. 4; Alg. 2 l.12-16)
-//   a5: O[row] = H_e[:, 0:r_e] W~down[:, 0:r_e]^T (Alg. 2 l.18); scale + sum over k in k_combine
+//   a5: yacc[token(row)] += topk_w(row) * H_e[row, 0:r_e] W~down[:, 0:r_e]^T (Alg. 2 l.18-20)
 #include "fxm_internal.cuh"
 
 namespace fxm {
@@ -15,21 +15,20 @@ __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_
 constexpr int SIMT_TOK = 8;   // tokens per register block
 
 // block = 128 threads = the 128 packed rows of one gate/up tile; grid.x = work item (token tile j, channel block cb)
-__global__ void __launch_bounds__(128) k_gemm1_simt(Dims D, const uint8_t* __restrict__ packed,
+__global__ void __launch_bounds__(128) k_gemm1_simt(Dims D, LayerView V,
                                                     const int* __restrict__ r_table, const int4* __restrict__ tt,
-                                                    const Sched* __restrict__ sched, const uint8_t* __restrict__ Xs,
-                                                    uint8_t* __restrict__ H, int P) {
+                                                    const Sched* __restrict__ sched, const uint16_t* __restrict__ x,
+                                                    const int* __restrict__ row_tok, uint8_t* __restrict__ H, int P) {
     __shared__ float s_acc[128][SIMT_TOK + 1];
-    const int ntt = sched->ntt, W1 = sched->W1;
-    for (int wi = blockIdx.x; wi < W1; wi += gridDim.x) {
-        int lo = 0, hi = ntt - 1;                       // last tile whose work prefix <= wi
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (tt[mid].w <= wi) lo = mid; else hi = mid - 1;
-        }
-        const int4 t = tt[lo];
-        const int e = t.x, row0 = t.y, nvalid = t.z, cb = wi - t.w;
+    // work item = (token tile j, channel block cb < ceil(r_e / 64)); the schedule's own GEMM-1 items are CTA-PAIR
+    // items (two channel blocks each), so this path enumerates single blocks itself: tile j, block cb = 0 .. nCB - 1
+    const int ntt = sched->ntt;
+    for (int wi = blockIdx.x; wi < ntt * D.nCB; wi += gridDim.x) {
+        const int4 t = tt[wi / D.nCB];
+        const int e = t.x, row0 = t.y, nvalid = t.z, cb = wi % D.nCB;
         const int r = r_table[e];
+        if (cb * CB >= r) continue;                                   // pruned block: never issued
+        const uint32_t eb = V.eblk[e];
         const int pr = threadIdx.x;
         const int npad = (nvalid + ROW_ALIGN - 1) / ROW_ALIGN * ROW_ALIGN;
         for (int t0 = 0; t0 < npad; t0 += SIMT_TOK) {
@@ -37,14 +36,13 @@ __global__ void __launch_bounds__(128) k_gemm1_simt(Dims D, const uint8_t* __res
 #pragma unroll
             for (int q = 0; q < SIMT_TOK; ++q) acc[q] = 0.f;
             for (int kb = 0; kb < D.nKB1; ++kb) {
-                const uint8_t* wt = packed + gu_tile_index(D, e, cb, kb) * WT_BYTES;
+                const uint8_t* wt = V.gu + gu_tile_off(D, eb, cb, kb);
                 for (int c = 0; c < KB; ++c) {
                     const float wv = bf16_bits_to_float(*(const uint16_t*)(wt + sw128_off(pr, c)));
 #pragma unroll
                     for (int q = 0; q < SIMT_TOK; ++q) {
-                        const int p = row0 + t0 + q;
-                        const uint8_t* xp = Xs + ((size_t)kb * P + p) * ROW_BYTES + ((((c >> 3) ^ p) & 7) << 4) + ((c & 7) << 1);
-                        acc[q] += wv * bf16_bits_to_float(*(const uint16_t*)xp);
+                        const int p = row0 + t0 + q;                   // padding rows read token 0 (X[pi], Alg. 2 l.7)
+                        acc[q] += wv * bf16_bits_to_float(x[(size_t)row_tok[p] * D.d + kb * KB + c]);
                     }
                 }
             }
@@ -68,17 +66,17 @@ __global__ void __launch_bounds__(128) k_gemm1_simt(Dims D, const uint8_t* __res
 }
 
 // block = 128 threads = 128 output features of one down tile row-block; grid.x = work item (token tile j, db)
-__global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, const uint8_t* __restrict__ packed,
+__global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, LayerView V,
                                                     const int* __restrict__ r_table, const int4* __restrict__ tt,
                                                     const Sched* __restrict__ sched, const uint8_t* __restrict__ H,
-                                                    uint8_t* __restrict__ O, int P) {
-    const int W2 = sched->W2;
-    const uint8_t* dn = packed + gu_bytes(D);
-    for (int wi = blockIdx.x; wi < W2; wi += gridDim.x) {
+                                                    const int2* __restrict__ row_tw, float* __restrict__ yacc, int P) {
+    const int ntt = sched->ntt;
+    for (int wi = blockIdx.x; wi < ntt * D.nDB; wi += gridDim.x) {
         const int j = wi / D.nDB, db = wi % D.nDB;
         const int4 t = tt[j];
         const int e = t.x, row0 = t.y, nvalid = t.z;
         const int r = r_table[e];
+        const uint32_t eb = V.eblk[e];
         const int nkb = (r + KB - 1) / KB;
         const int pr = threadIdx.x, i = db * WT_ROWS + pr;
         for (int t0 = 0; t0 < nvalid; t0 += SIMT_TOK) {
@@ -86,7 +84,7 @@ __global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, const uint8_t* __res
 #pragma unroll
             for (int q = 0; q < SIMT_TOK; ++q) acc[q] = 0.f;
             for (int kb2 = 0; kb2 < nkb; ++kb2) {
-                const uint8_t* wt = dn + dn_tile_index(D, e, kb2, db) * WT_BYTES;
+                const uint8_t* wt = V.dn + dn_tile_off(D, eb, kb2, db);
                 for (int c = 0; c < KB; ++c) {
                     const float wv = bf16_bits_to_float(*(const uint16_t*)(wt + sw128_off(pr, c)));
 #pragma unroll
@@ -99,21 +97,23 @@ __global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, const uint8_t* __res
             }
 #pragma unroll
             for (int q = 0; q < SIMT_TOK; ++q) {
-                if (t0 + q < nvalid && i < D.d)
-                    *(__nv_bfloat16*)(O + o_off(P, row0 + t0 + q, i)) = __float2bfloat16_rn(acc[q]);
+                if (t0 + q < nvalid && i < D.d) {
+                    const int2 tw = row_tw[row0 + t0 + q];             // {token, router weight}: scale + scatter-add
+                    if (tw.x >= 0) atomicAdd(yacc + (size_t)tw.x * D.d + i, __int_as_float(tw.y) * acc[q]);
+                }
             }
         }
     }
 }
 
-cudaError_t launch_gemm1_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
-                              cudaStream_t st) {
-    k_gemm1_simt<<<148 * 16, 128, 0, st>>>(D, packed, r_table, ws.tt, ws.sched, ws.Xs, ws.H, ws.P);
+cudaError_t launch_gemm1_simt(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
+                              const Workspace& ws, cudaStream_t st) {
+    k_gemm1_simt<<<148 * 16, 128, 0, st>>>(D, V, r_table, ws.tt, ws.sched, (const uint16_t*)x, ws.row_tok, ws.H, ws.P);
     return cudaGetLastError();
 }
-cudaError_t launch_gemm2_simt(const Dims& D, const uint8_t* packed, const int* r_table, const Workspace& ws,
+cudaError_t launch_gemm2_simt(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws,
                               cudaStream_t st) {
-    k_gemm2_simt<<<148 * 16, 128, 0, st>>>(D, packed, r_table, ws.tt, ws.sched, ws.H, ws.O, ws.P);
+    k_gemm2_simt<<<148 * 16, 128, 0, st>>>(D, V, r_table, ws.tt, ws.sched, ws.H, ws.row_tw, ws.yacc, ws.P);
     return cudaGetLastError();
 }
 

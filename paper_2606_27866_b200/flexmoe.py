@@ -13,17 +13,15 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libflexmoe.so")
-_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_sm100.cu", "fxm_pair.cu", "fxm_decode.cu"]
+_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_pair.cu", "fxm_decode.cu"]
 _HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_CSRC, "fxm_ptx.cuh"), os.path.join(_HERE, "..", "include", "flexmoe.h")]
 
 IMPL_TCGEN05 = 0
 IMPL_SIMT_DEBUG = 1
-IMPL_TCGEN05_1CTA = 2
-IMPL_TCGEN05_XS = 3
 MAX_BUDGETS = 15
 
 _STATUS = ["FXM_OK", "FXM_EINVAL", "FXM_ESHAPE", "FXM_EPERM", "FXM_EBUDGET", "FXM_ENOTNESTED",
-           "FXM_EWORKSPACE", "FXM_ESTATE", "FXM_ECUDA"]
+           "FXM_EWORKSPACE", "FXM_ESTATE", "FXM_ECUDA", "FXM_ENOMEM"]
 
 
 class FxmError(RuntimeError):
@@ -51,12 +49,13 @@ _lib = None
 
 
 def lib():
-    """Load the shared library (building it first if nvcc is available and it is stale/missing)."""
+    """Load the shared library; (re)build it first when it is missing or older than its sources and nvcc exists."""
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(_SO):
-        build()
+    import shutil
+    if not os.path.exists(_SO) or shutil.which("nvcc"):
+        build()                       # a no-op when the .so is newer than every source and header
     L = ctypes.CDLL(_SO)
     vp, i32, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
     L.fxm_packed_bytes.argtypes = [i32, i32, i32, ctypes.POINTER(sz)]
@@ -68,13 +67,18 @@ def lib():
     L.fxm_ratio_to_width.argtypes = [i32, i32, i32]
     L.fxm_ratio_to_width.restype = ctypes.c_int32
     L.fxm_moe_ffn.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_moe_ffn_shared.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, sz, vp]
+    L.fxm_clipped_bytes.argtypes = [i32, i32, i32, vp, ctypes.POINTER(sz)]
+    L.fxm_export_clipped.argtypes = [vp, vp, vp, sz, vp]
+    L.fxm_parse_clipped_header.argtypes = [vp, sz, ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i32), vp]
+    L.fxm_load_clipped.argtypes = [ctypes.POINTER(vp), i32, i32, i32, vp, vp, sz, vp]
     L.fxm_workspace_bytes_host.argtypes = [i32, i32, i32, i32, i32, ctypes.POINTER(sz)]
     L.fxm_moe_ffn_host.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
     L.fxm_profile_begin.argtypes = [vp, i32]
     L.fxm_profile_end.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i32)]
     L.fxm_route.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
     L.fxm_unpack_prefix.argtypes = [vp, i32, i32, vp, vp, vp, vp]
-    L.fxm_debug_read_h.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+    L.fxm_debug_read_h.argtypes = [vp, vp, i32, i32, vp, vp, i32, vp]
     L.fxm_set_impl.argtypes = [vp, i32]
     L.fxm_set_tile_n.argtypes = [vp, i32]
     L.fxm_set_decode.argtypes = [vp, i32, i32]
@@ -89,7 +93,8 @@ def lib():
 
 
 EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
-           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_workspace_bytes_host", "fxm_moe_ffn_host",
+           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_moe_ffn_shared", "fxm_workspace_bytes_host",
+           "fxm_moe_ffn_host", "fxm_clipped_bytes", "fxm_export_clipped", "fxm_parse_clipped_header", "fxm_load_clipped",
            "fxm_profile_begin", "fxm_profile_end", "fxm_route", "fxm_unpack_prefix",
            "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_set_decode", "fxm_device_flags", "fxm_launches_per_ffn",
            "fxm_status_string", "fxm_destroy"]
@@ -118,8 +123,8 @@ def workspace_bytes_host(E: int, d: int, I: int, T_max: int, k: int) -> int:
     return n.value
 
 
-N_KERNELS = 7
-KERNEL_NAMES = ("route_plan", "scatter", "gather", "gemm1_swiglu", "gemm2", "combine", "decode_fused")
+N_KERNELS = 5
+KERNEL_NAMES = ("route", "gemm1_swiglu", "gemm2_scatter_add", "finalize", "decode_fused")
 DECODE_DEFAULT_MAX_ASSIGNMENTS = 768
 DECODE_DEFAULT_PREFETCH = 0
 
@@ -142,10 +147,11 @@ def _i32_host(a):
 class Layer:
     """One packed MoE layer.  Owns (via torch) the packed weight blob and a workspace."""
 
-    def __init__(self, handle, E, d, I, packed):
+    def __init__(self, handle, E, d, I, packed, clipped_widths=None):
         self._h = handle
         self.E, self.d, self.I = E, d, I
         self.packed = packed            # torch.uint8 tensor; must outlive the handle
+        self.clipped_widths = clipped_widths   # None for a full layer, else the exported r[E]
         self._ws = None
         self._ws_key = None
 
@@ -218,8 +224,9 @@ class Layer:
         return self._ws
 
     # -- (3) forward --------------------------------------------------------------------------------
-    def moe_ffn(self, x, topk_ids, topk_w, out=None, workspace=None, stream=None):
-        """x [T,d] bf16, topk_ids [T,k] int32, topk_w [T,k] fp32 (CUDA, contiguous) -> y [T,d] bf16."""
+    def moe_ffn(self, x, topk_ids, topk_w, out=None, workspace=None, stream=None, y_shared=None):
+        """x [T,d] bf16, topk_ids [T,k] int32, topk_w [T,k] fp32 (CUDA, contiguous) -> y [T,d] bf16.
+        y_shared [T,d] bf16 (optional): the shared expert's output, added before the rounding (fxm_moe_ffn_shared)."""
         import torch
         T, d = x.shape
         k = topk_ids.shape[1]
@@ -228,9 +235,51 @@ class Layer:
         assert topk_w.dtype == torch.float32 and topk_w.is_contiguous() and tuple(topk_w.shape) == (T, k)
         y = torch.empty((T, d), dtype=torch.bfloat16, device=x.device) if out is None else out
         ws = self.workspace(T, k) if workspace is None else workspace
-        _chk(lib().fxm_moe_ffn(self._h, x.data_ptr(), topk_ids.data_ptr(), topk_w.data_ptr(), T, k, y.data_ptr(),
-                               ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_moe_ffn")
+        if y_shared is None:
+            _chk(lib().fxm_moe_ffn(self._h, x.data_ptr(), topk_ids.data_ptr(), topk_w.data_ptr(), T, k, y.data_ptr(),
+                                   ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_moe_ffn")
+        else:
+            assert y_shared.dtype == torch.bfloat16 and y_shared.is_contiguous() and tuple(y_shared.shape) == (T, d)
+            _chk(lib().fxm_moe_ffn_shared(self._h, x.data_ptr(), topk_ids.data_ptr(), topk_w.data_ptr(), T, k,
+                                          y_shared.data_ptr(), y.data_ptr(), ws.data_ptr(), ws.numel(),
+                                          _stream_ptr(stream)), "fxm_moe_ffn_shared")
         return y
+
+    # -- offline clipping ----------------------------------------------------------------
+    def export_clipped(self, r, stream=None):
+        """-> torch.uint8 blob (device) holding only the retained prefix of every expert for the widths r[E]."""
+        import torch
+        r = _i32_host(r)
+        assert r.shape == (self.E,)
+        n = ctypes.c_size_t()
+        _chk(lib().fxm_clipped_bytes(self.E, self.d, self.I, r.ctypes.data, ctypes.byref(n)), "fxm_clipped_bytes")
+        raw = torch.empty(n.value + 1024, dtype=torch.uint8, device=self.packed.device)
+        off = (-raw.data_ptr()) % 1024
+        blob = raw[off:off + n.value]
+        _chk(lib().fxm_export_clipped(self._h, r.ctypes.data, blob.data_ptr(), blob.numel(), _stream_ptr(stream)),
+             "fxm_export_clipped")
+        return blob
+
+    @staticmethod
+    def parse_clipped_header(host_bytes):
+        """host_bytes: the first >= 2048 bytes of a blob (bytes / numpy uint8) -> (E, d, I, r[E])."""
+        import numpy as np
+        buf = np.frombuffer(bytes(host_bytes[:2048]), dtype=np.uint8).copy()
+        E, d, I = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        r = np.zeros(256, np.int32)
+        _chk(lib().fxm_parse_clipped_header(buf.ctypes.data, buf.size, ctypes.byref(E), ctypes.byref(d), ctypes.byref(I),
+                                            r.ctypes.data), "fxm_parse_clipped_header")
+        return E.value, d.value, I.value, r[:E.value].copy()
+
+    @staticmethod
+    def load_clipped(blob, E, d, I, r, stream=None) -> "Layer":
+        """blob: torch.uint8 CUDA tensor (1024-byte aligned) written by export_clipped, possibly after a round trip
+        through host memory or a file."""
+        r = _i32_host(r)
+        h = ctypes.c_void_p()
+        _chk(lib().fxm_load_clipped(ctypes.byref(h), E, d, I, r.ctypes.data, blob.data_ptr(), blob.numel(),
+                                    _stream_ptr(stream)), "fxm_load_clipped")
+        return Layer(h, E, d, I, blob, clipped_widths=r.copy())
 
     def workspace_host(self, T: int, k: int):
         import torch
@@ -294,13 +343,13 @@ class Layer:
              "fxm_unpack_prefix")
         return Wg, Wu, Wd
 
-    def debug_read_h(self, topk_ids, stream=None):
+    def debug_read_h(self, topk_ids, raw=False, stream=None):
         import torch
         T, k = topk_ids.shape
         H = torch.zeros((T * k, self.I), dtype=torch.bfloat16, device=self.packed.device)
         ws = self.workspace(T, k)
-        _chk(lib().fxm_debug_read_h(self._h, topk_ids.data_ptr(), T, k, ws.data_ptr(), H.data_ptr(), _stream_ptr(stream)),
-             "fxm_debug_read_h")
+        _chk(lib().fxm_debug_read_h(self._h, topk_ids.data_ptr(), T, k, ws.data_ptr(), H.data_ptr(), int(bool(raw)),
+                                    _stream_ptr(stream)), "fxm_debug_read_h")
         return H
 
     def device_flags(self, stream=None) -> int:

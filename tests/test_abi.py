@@ -41,8 +41,42 @@ def test_sizes_match_the_layout_formulas():
     ws2 = fx.workspace_bytes(E, d, I, 16, 4)
     assert ws1 > ws2 > 0
     A, P = 4096 * 4, 4096 * 4 + 16 * E
-    assert ws1 >= P * d * 2 + P * I * 2 + P * d * 2              # Xs + H + O (bf16 expert outputs per padded row)
-    assert ws1 <= 1.2 * (P * d * 2 + P * I * 2 + P * d * 2) + (1 << 20)
+    # H panels (bf16 SwiGLU activations per padded row) + the fp32 scatter-add accumulator of y; no gathered copy
+    # of x and no per-assignment expert outputs any more
+    assert ws1 >= P * I * 2 + 4096 * d * 4
+    assert ws1 <= 1.1 * (P * I * 2 + 4096 * d * 4) + (2 << 20)
+
+
+def test_workspace_size_is_monotonic_in_T():
+    """include/flexmoe.h: a buffer sized for T_max serves every T <= T_max (the decode accumulator used to
+    exist only for small T, so a smaller call could need MORE than fxm_workspace_bytes(T_max))."""
+    for (E, d, I, k) in [(60, 2048, 1408, 4), (64, 3584, 2560, 8), (8, 256, 512, 2), (256, 64, 16, 16)]:
+        prev = 0
+        for T in [0, 1, 2, 7, 16, 31, 32, 33, 64, 100, 127, 128, 129, 130, 256, 1000, 1024, 1025, 4096, 8192]:
+            n = fx.workspace_bytes(E, d, I, T, k)
+            assert n >= prev, (E, d, I, k, T)
+            assert fx.workspace_bytes_host(E, d, I, T, k) >= n
+            prev = n
+
+
+def test_clipped_bytes_follow_the_linear_law():
+    """Table 2: checkpoint bytes are linear in the retained fraction (oracle pin P10).  The clipped
+    blob = 6 d bytes per retained channel (rounded up to 64-channel blocks per expert) + a constant tail."""
+    E, d, I = 64, 3584, 2560
+    L = fx.lib()
+    sizes = []
+    for r in (2560, 1920, 1536, 1280, 640, 0):
+        n = ctypes.c_size_t()
+        rr = np.full(E, r, np.int32)
+        assert L.fxm_clipped_bytes(E, d, I, rr.ctypes.data, ctypes.byref(n)) == 0
+        sizes.append(n.value)
+    const = sizes[-1]
+    assert const < 64 * 1024
+    for r, n in zip((2560, 1920, 1536, 1280, 640), sizes):
+        assert n - const == 6 * d * E * r                          # widths are multiples of 64 here: exact
+    bad = np.full(E, I + 1, np.int32)
+    n = ctypes.c_size_t()
+    assert L.fxm_clipped_bytes(E, d, I, bad.ctypes.data, ctypes.byref(n)) == 4     # FXM_EBUDGET
 
 
 @pytest.mark.parametrize("args,code", [((0, 64, 16), "FXM_ESHAPE"), ((257, 64, 16), "FXM_ESHAPE"),
@@ -74,7 +108,7 @@ def test_ratio_to_width_is_integer_ceil_and_matches_oracle():
 
 def test_status_strings():
     L = fx.lib()
-    for i in range(9):
+    for i in range(10):
         assert L.fxm_status_string(i).decode().startswith("FXM_")
 
 

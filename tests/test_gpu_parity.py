@@ -89,10 +89,10 @@ def _c1():
     return gen.SHAPES["C1"], lay, b, rng
 
 
-# impl: 1 = SIMT debug, 2 = single-CTA tcgen05, 3 = CTA-pair tcgen05 fed by the gather kernel, 0 = CTA-pair tcgen05 with
-# the gather fused into GEMM-1 (the product; general path forced), "dec" = fused decode kernel
-IMPLS = [1, 2, 3, 0, "dec"]
-GENERAL_LAUNCHES = {0: 5, 1: 6, 2: 6, 3: 6}
+# impl: 1 = SIMT debug path, 0 = CTA-pair tcgen05 kernels (the product; general four-launch path forced),
+# "dec" = fused decode kernel
+IMPLS = [1, 0, "dec"]
+GENERAL_LAUNCHES = {0: 4, 1: 4}
 
 
 def _run(gu, L, b, r, impl, **kw):
@@ -131,10 +131,10 @@ def test_widths_not_multiple_of_64_and_padded_dims(impl):
         gu.check_close(_run(gu, L, b, r, impl), gu.oracle_ffn(lay, b, r), f"r={r.tolist()} impl={impl}")
 
 
-@pytest.mark.parametrize("impl,tile_n", [(2, 128), (2, 256), (3, 0), (0, 0)])
+@pytest.mark.parametrize("impl,tile_n", [(1, 128), (0, 128), (0, 256), (0, 0)])
 def test_multi_tile_ragged_segments(impl, tile_n):
     """Expert segments that span several token tiles plus a ragged tail, heavy skew, empty experts.
-    impl 0 = CTA-pair kernels (token tiles up to 512 rows = two sub-tiles), impl 2 = single-CTA kernels."""
+    impl 0 = CTA-pair kernels (token tiles up to 128 / 256 / 512 rows; above 256 = two sub-tiles), impl 1 = SIMT debug."""
     import gpu_util as gu
     sh, lay, rng = _small_layer(4, 128, 6, 2, 192, w_std=0.08)
     T = 900
@@ -164,26 +164,9 @@ def test_pair_subtile_boundaries(T):
         gu.check_close(gu.run_ffn(L, b, r, decode=False), gu.oracle_ffn(lay, b, r), f"T={T} r={r.tolist()}")
 
 
-def _random_cases():
-    rng = np.random.default_rng(2024)
-    cases = [(64, 1, 1, 16, 1), (64, 1, 1, 16, 40), (128, 256, 16, 32, 33), (64, 2, 2, 1040, 17), (3584, 3, 2, 64, 70)]
-    for _ in range(10):
-        d = int(rng.integers(1, 9)) * 64
-        E = int(rng.integers(1, 24))
-        k = int(rng.integers(1, min(E, 6) + 1))
-        I = int(rng.integers(1, 21)) * 16
-        T = int(rng.choice([1, 2, 7, 31, 64, 129, 300, 700]))
-        cases.append((d, E, k, I, T))
-    return cases
-
-
-@pytest.mark.parametrize("d,E,k,I,T", _random_cases())
-def test_random_small_shapes_product_path_and_decode(d, E, k, I, T):
-    """Seeded sweep over small (d, E, k, I, T) including the extremes of the supported set (d = 64, E = 1 and 256,
-    k = 1 and 16, I = 16, ragged I, d = 3584): random widths in [0, I] (any multiple of 1), skewed routing; the
-    product path and, where T*k <= 1024, the fused decode kernel, every element against the oracle."""
+def _check_shape_case(d, E, k, I, T, seed):
     import gpu_util as gu
-    sh, lay, rng = _small_layer(1000 + d + E + T, d, E, k, I, w_std=0.08)
+    sh, lay, rng = _small_layer(1000 + seed, d, E, k, I, w_std=0.08)
     lg = gen.make_logits(T, E, rng, 1.0, 1.5)
     ids, w = gen.route(lg, k)
     b = gen.Batch(gen.make_x(T, d, rng), ids, w)
@@ -199,6 +182,29 @@ def test_random_small_shapes_product_path_and_decode(d, E, k, I, T):
         y = gu.run_ffn(L, b, r, decode=True)
         assert L.launches_per_ffn() == 1
         gu.check_close(y, ref, f"decode d={d} E={E} k={k} I={I} T={T}")
+
+
+@pytest.mark.parametrize("d,E,k,I,T", [(64, 1, 1, 16, 1), (64, 1, 1, 16, 40), (128, 256, 16, 32, 33), (64, 2, 2, 1040, 17),
+                                       (3584, 3, 2, 64, 70)])
+def test_extreme_small_shapes_product_path_and_decode(d, E, k, I, T):
+    """The corners of the supported set (d = 64, E = 1 and 256, k = 1 and 16, I = 16, ragged I, d = 3584): random widths
+    in [0, I] (any multiple of 1), skewed routing; product path and fused decode kernel, every element vs the oracle."""
+    _check_shape_case(d, E, k, I, T, d + E + T)
+
+
+def test_property_sweep_random_shapes():
+    """a hypothesis sweep over (d, E, k, I, T, seed) -- empty experts, widths in {0..I} that are not
+    multiples of 16 or 64, duplicate-free skewed routing, ragged token counts; every element against the oracle on the
+    product path and, where T*k <= 1024, on the fused decode kernel."""
+    from hypothesis import given, settings, strategies as st, HealthCheck
+
+    @settings(max_examples=30, deadline=None, derandomize=True, suppress_health_check=list(HealthCheck))
+    @given(d64=st.integers(1, 8), E=st.integers(1, 24), kk=st.integers(1, 6), I16=st.integers(1, 20),
+           T=st.sampled_from([1, 2, 7, 31, 64, 129, 300, 700]), seed=st.integers(0, 10_000))
+    def run(d64, E, kk, I16, T, seed):
+        _check_shape_case(d64 * 64, E, min(kk, E), I16 * 16, T, seed)
+
+    run()
 
 
 # ------------------------------------------------------------------------------------- fused decode kernel (a6)
@@ -270,15 +276,27 @@ def test_decode_out_of_range_id_is_flagged_and_dropped():
 
 
 def test_h_intermediate_matches_definition():
-    """Step a4 alone: H = silu(G) (.) U in sorted order, channels >= r_e exactly 0 (pad-zero rule)."""
+    """Step a4 alone: H = silu(G) (.) U in sorted order, channels >= r_e exactly 0 (pad-zero rule).
+    The RAW read (no reader-side mask) shows what the GEMM-1 epilogue itself wrote: the columns [r_e, ceil64(r_e)) of
+    the last retained block must be exact zeros."""
     import torch
     import gpu_util as gu
     fx = _fx()
     sh, lay, b, rng = _c1()
-    r = gen.table_c1(sh, rng)
+    r = np.array([512, 100, 37, 336, 65, 1, 496, 250], np.int32)        # ragged: the last block of most experts is partial
     L = gu.pack_layer(lay)
     gu.run_ffn(L, b, r, decode=False)                       # the H panels exist only on the general path
     ids = torch.from_numpy(b.topk_ids).cuda()
+    Hraw = fx.bf16_to_bits(L.debug_read_h(ids, raw=True))
+    _, _, perm0, _ = oracle.route(b.topk_ids, sh.E)
+    n_pad = 0
+    for s_ in range(perm0.size):
+        e = b.topk_ids.ravel()[perm0[s_]]
+        lim = -(-int(r[e]) // 64) * 64
+        assert np.all(Hraw[s_, r[e]:lim] == 0), f"pad columns of sorted row {s_} (expert {e}) are not zero"
+        assert np.any(Hraw[s_, :r[e]] != 0)
+        n_pad += lim - int(r[e])
+    assert n_pad > 0
     H = gen.bf16_bits_to_f32(fx.bf16_to_bits(L.debug_read_h(ids))).astype(np.float64)
     Gt, Ut, _ = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
     x = gen.bf16_bits_to_f32(b.x).astype(np.float64)
@@ -408,6 +426,9 @@ def test_errors_and_state():
 
 
 # ------------------------------------------------------------------------------- FFN, paper-shaped sizes
+N_SAMPLE = 512            # prefill shapes are checked on >= 512 sampled token rows (rows of y are independent)
+
+
 def _rows_sample(T, n, seed):
     return np.sort(np.random.default_rng(seed).choice(T, size=min(n, T), replace=False)).astype(np.int32)
 
@@ -415,8 +436,8 @@ def _rows_sample(T, n, seed):
 @pytest.mark.parametrize("T,decode", [(1, True), (16, True), (1, False), (16, False), (4096, None)])
 @pytest.mark.parametrize("r", [704, 1408])
 def test_c2_qwen15_shaped(T, r, decode):
-    """C2 (BASELINE.json configs[1], the bench workload): d=2048, E=60, top-4, I=1408, uniform r_e.
-    T<=16: every row; T=4096: grouping indices in full + 96 sampled rows (rows of y are independent)."""
+    """C2 (BASELINE.json configs[1]): d=2048, E=60, top-4, I=1408, uniform r_e.
+    T<=16: every row; T=4096: grouping indices in full + 512 sampled rows (rows of y are independent)."""
     import torch
     import gpu_util as gu
     lay, b, rng = gen.config("C2", T=T)
@@ -424,8 +445,8 @@ def test_c2_qwen15_shaped(T, r, decode):
     rt = gen.table_uniform(sh, r)
     L = gu.pack_layer(lay)
     y = gu.run_ffn(L, b, rt, decode=decode)
-    assert L.launches_per_ffn() == (1 if decode else 5)
-    rows = None if T <= 16 else _rows_sample(T, 96, 11)
+    assert L.launches_per_ffn() == (1 if decode else 4)
+    rows = None if T <= 16 else _rows_sample(T, N_SAMPLE, 11)
     ref = gu.oracle_ffn(lay, b, rt, rows=rows)
     gu.check_close(y if rows is None else y[rows], ref, f"C2 T={T} r={r}")
     got = [t.cpu().numpy() for t in L.route(torch.from_numpy(b.topk_ids).cuda())]
@@ -434,28 +455,288 @@ def test_c2_qwen15_shaped(T, r, decode):
 
 
 def test_c3_deepseek_shaped_skewed_heterogeneous():
-    """C3: d=2048, E=64, top-6, I=1408, T=8192, skewed load (mu_e + eps reading), per-expert r_e with mean 60 %."""
+    """C3: d=2048, E=64, top-6, I=1408, T=8192, skewed load (mu_e + eps reading), per-expert r_e with mean 60 %;
+    512 sampled rows and the grouping indices in full."""
+    import torch
     import gpu_util as gu
     lay, b, rng = gen.config("C3")
     sh = gen.SHAPES["C3"]
     r = gen.table_mean_ratio(sh, rng, 0.6)
     L = gu.pack_layer(lay)
     y = gu.run_ffn(L, b, r)
-    rows = _rows_sample(8192, 64, 12)
+    rows = _rows_sample(8192, N_SAMPLE, 12)
     gu.check_close(y[rows], gu.oracle_ffn(lay, b, r, rows=rows), "C3")
+    got = [t.cpu().numpy() for t in L.route(torch.from_numpy(b.topk_ids).cuda())]
+    for g, rr in zip(got, oracle.route(b.topk_ids, sh.E)):
+        assert np.array_equal(g, rr)
+
+
+def _c4_tables(sh, rng):
+    """Every budget table BASELINE.json configs[3] names: uniform 0/25/40/50/75 %, the heterogeneous nested-descent
+    tables at the same budgets, and the Fig. 6-like bimodal table."""
+    tabs = [(f"U{int(round(100 * (1 - w / sh.I)))}", gen.table_uniform(sh, w)) for w in (2560, 1920, 1536, 1280, 640)]
+    het = gen.tables_nested_descent(sh, rng)
+    tabs += [(f"H{int(round(100 * p))}", t) for p, t in zip(gen.C4_PRUNED, het)]
+    tabs.append(("fig6", gen.table_fig6_like(sh, rng)))
+    return tabs
 
 
 @pytest.mark.parametrize("T,decode", [(1, None), (64, None), (64, False), (8192, None)])
 def test_c4_qwen2_57b_shaped_budget_sweep(T, decode):
-    """C4: d=3584, E=64, top-8, I=2560; nested heterogeneous tables at 0/25/40/50/75 % pruned."""
+    """C4: d=3584, E=64, top-8, I=2560 at ALL budgets of the contract: uniform and heterogeneous nested tables at
+    0/25/40/50/75 % pruned plus the Fig. 6-like table.  T=1 and T=64: every row; T=8192: 512 sampled rows."""
     import gpu_util as gu
     lay, b, rng = gen.config("C4", T=T)
     sh = gen.SHAPES["C4"]
-    tabs = gen.tables_nested_descent(sh, rng)
     L = gu.pack_layer(lay)
-    rows = None if T == 1 else _rows_sample(T, 24, 13)
-    for bi in (0, 2, 4):
-        y = gu.run_ffn(L, b, tabs[bi], decode=decode)
-        assert L.launches_per_ffn() == (5 if (decode is False or T > 64) else 1)
-        ref = gu.oracle_ffn(lay, b, tabs[bi], rows=rows)
-        gu.check_close(y if rows is None else y[rows], ref, f"C4 T={T} budget {bi}")
+    rows = None if T <= 64 else _rows_sample(T, N_SAMPLE, 13)
+    for name, tab in _c4_tables(sh, rng):
+        y = gu.run_ffn(L, b, tab, decode=decode)
+        assert L.launches_per_ffn() == (4 if (decode is False or T > 64) else 1)
+        ref = gu.oracle_ffn(lay, b, tab, rows=rows)
+        gu.check_close(y if rows is None else y[rows], ref, f"C4 T={T} table {name}")
+
+
+def test_c5_switching_interleaved_decode_prefill_on_c4_layer():
+    """C5 (BASELINE.json configs[4]) in miniature: 40 interleaved decode (T=32) / prefill (T=4096) calls on the C4-shaped
+    layer, a different registered nested table selected before EVERY call (fxm_select_budget: host-only), no host
+    synchronisation in between, one shared workspace sized for the larger T.  Sampled rows of every output against
+    the oracle at the table that call used."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh = gen.SHAPES["C5"]
+    lay = gen.layer_for("C5", 0)
+    tabs = gen.tables_nested_descent(sh, np.random.default_rng([0, 3]))
+    L = gu.pack_layer(lay)
+    L.register_budgets(tabs, require_nested=True)
+    L.set_decode()                                               # library default: T=32 -> fused decode kernel, T=4096 -> general path
+    pools = {}
+    for T in (32, 4096):
+        pools[T] = []
+        for i in range(2):
+            _, bt, _ = gen.config("C5", T=T, seed=40 + i, layer=False)
+            pools[T].append((bt, gu.to_dev(bt.x), torch.from_numpy(bt.topk_ids).cuda(), torch.from_numpy(bt.topk_w).cuda()))
+    L.workspace(4096, sh.k)
+    rng = np.random.default_rng(9)
+    calls, prev = [], -1
+    for i in range(40):
+        bi = int(rng.integers(len(tabs)))
+        while bi == prev:
+            bi = int(rng.integers(len(tabs)))
+        prev = bi
+        T = 32 if i % 2 == 0 else 4096
+        bt, x, ids, w = pools[T][(i // 2) % 2]
+        L.select_budget(bi)
+        y = L.moe_ffn(x, ids, w)
+        assert L.launches_per_ffn() == (1 if T == 32 else 4)
+        calls.append((i, T, bi, bt, y))
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
+    for i, T, bi, bt, y in calls:
+        rows = _rows_sample(T, 32 if T == 32 else 12, 100 + i)
+        yv = gen.bf16_bits_to_f32(fx.bf16_to_bits(y[torch.from_numpy(rows.astype(np.int64)).cuda()])).astype(np.float64)
+        gu.check_close(yv, gu.oracle_ffn(lay, bt, tabs[bi], rows=rows), f"C5 call {i} T={T} budget {bi}")
+
+
+# ------------------------------------------------------------------------------------ robustness items (ADVICE r1)
+def test_host_entry_point_interleaved_sizes_share_one_workspace():
+    """fxm_moe_ffn_host with T=4096 and T=32 calls back to back on ONE workspace sized for the larger T and no host
+    synchronisation: the staging area of a call must never land on memory the previous call still uses."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    lay, _, rng = gen.config("C2", T=32)
+    sh = gen.SHAPES["C2"]
+    r = gen.table_uniform(sh, 704)
+    L = gu.pack_layer(lay)
+    L.set_budget(r)
+    L.workspace_host(4096, sh.k)
+    seq = [4096, 32, 32, 4096, 4096, 32, 4096, 32]
+    batches, hx, hy = [], [], []
+    for i, T in enumerate(seq):
+        _, b, _ = gen.config("C2", T=T, seed=70 + i, layer=False)
+        batches.append(b)
+        hx.append((fx.bf16_from_bits(b.x, "cpu").pin_memory(), torch.from_numpy(b.topk_ids).pin_memory(),
+                   torch.from_numpy(b.topk_w).pin_memory()))
+        hy.append(torch.empty((T, sh.d), dtype=torch.bfloat16).pin_memory())
+    for i in range(len(seq)):
+        L.moe_ffn_host(*hx[i], hy[i])
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
+    for i, (T, b) in enumerate(zip(seq, batches)):
+        rows = _rows_sample(T, 32, 200 + i)
+        y = gen.bf16_bits_to_f32(hy[i].view(torch.int16).numpy().view(np.uint16)[rows]).astype(np.float64)
+        gu.check_close(y, gu.oracle_ffn(lay, b, r, rows=rows), f"host call {i} T={T}")
+
+
+def test_graph_replay_keeps_the_captured_table_slot():
+    """include/flexmoe.h: a captured call is bound to the table SLOT that was current at capture time;
+    fxm_select_budget afterwards does not change a replay, fxm_set_budget (which rewrites the captured slot) does."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    tabs = np.array([[512] * 8, [256, 128, 192, 64, 512, 64, 128, 0], [128, 64, 64, 64, 256, 0, 64, 0]], np.int32)
+    L = gu.pack_layer(lay)
+    L.set_decode(0)
+    L.register_budgets(tabs, require_nested=True)
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    y = torch.empty((b.x.shape[0], sh.d), dtype=torch.bfloat16, device="cuda")
+    L.select_budget(1)
+    L.moe_ffn(x, ids, w, out=y)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            L.moe_ffn(x, ids, w, out=y)
+    L.select_budget(2)                                           # host-only: the graph still reads registered table 1
+    g.replay()
+    torch.cuda.synchronize()
+    gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), gu.oracle_ffn(lay, b, tabs[1]), "replay after select")
+    y2 = L.moe_ffn(x, ids, w)                                    # an eager call does read table 2
+    torch.cuda.synchronize()
+    gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y2)).astype(np.float64), gu.oracle_ffn(lay, b, tabs[2]), "eager after select")
+
+
+def test_misaligned_y_is_rejected_not_faulted():
+    """y is written with 16-byte stores: an 8-byte-aligned y must come back as FXM_EINVAL, never as a misaligned-address fault."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    L = gu.pack_layer(lay)
+    L.set_budget(np.full(sh.E, sh.I, np.int32))
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    buf = torch.empty(b.x.shape[0] * sh.d + 8, dtype=torch.bfloat16, device="cuda")
+    assert buf.data_ptr() % 16 == 0
+    y_bad = buf[4:4 + b.x.shape[0] * sh.d].view(b.x.shape[0], sh.d)      # 8-byte aligned only
+    for dec in (0, 1024):
+        L.set_decode(dec)
+        with pytest.raises(fx.FxmError) as ei:
+            L.moe_ffn(x, ids, w, out=y_bad)
+        assert ei.value.name == "FXM_EINVAL"
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
+
+
+# ------------------------------------------------------------------------------ NEXT-1: offline clipping (PAPER.md:222)
+@pytest.mark.parametrize("d,E,k,I,T", [(256, 8, 2, 512, 64), (192, 5, 3, 208, 300)])
+def test_offline_clipped_export_reload_and_forward(d, E, k, I, T):
+    """Export a fixed-budget blob (retained prefix tiles only), move it through HOST memory (as a checkpoint file
+    would), reload it and run the forward with static widths:
+    (1) the blob's weights are bit-exact: unpack_prefix on the reloaded layer == oracle.pack()[:r_e];
+    (2) its size is the linear law of Table 2 (PAPER.md:204): 6 d bytes per retained 64-channel block + a constant;
+    (3) the forward on it equals the oracle (and the online layer at the same table) within tolerance, on both the
+        general path and the decode kernel; (4) nested sub-budgets of the clipped checkpoint work, wider ones are refused."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, rng = _small_layer(31 + d, d, E, k, I, w_std=0.08)
+    b = gen.make_batch(sh, T, rng, expert_bias_std=1.0)
+    L = gu.pack_layer(lay)
+    r = (rng.integers(0, I // 16 + 1, size=E) * 16).astype(np.int32)
+    r[0] = I
+    r[E - 1] = 0
+    r[1] = 40 if I >= 48 else 16                                  # a width that is not a multiple of 64
+    blob = L.export_clipped(r)
+    torch.cuda.synchronize()
+    host = blob.cpu()                                            # "write the checkpoint"
+    E2, d2, I2, r2 = fx.Layer.parse_clipped_header(host.numpy().tobytes()[:2048])
+    assert (E2, d2, I2) == (E, d, I) and np.array_equal(r2, r)
+    nblk = int(sum(-(-int(x) // 64) for x in r))
+    gu_b = nblk * (d // 64) * 16384
+    dn_b = nblk * (-(-d // 128)) * 16384
+    assert 2048 + gu_b + dn_b <= blob.numel() <= 2048 + gu_b + dn_b + 32 * 1024
+    raw = torch.empty(host.numel() + 1024, dtype=torch.uint8, device="cuda")
+    off = (-raw.data_ptr()) % 1024
+    dev = raw[off:off + host.numel()]
+    dev.copy_(host)                                              # "load the checkpoint"
+    Lc = fx.Layer.load_clipped(dev, E2, d2, I2, r2)
+    Gt, Ut, Dt = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
+    for e in range(E):
+        if r[e] == 0:
+            continue
+        Wg, Wu, Wd = Lc.unpack_prefix(e, int(r[e]))
+        torch.cuda.synchronize()
+        assert np.array_equal(fx.bf16_to_bits(Wg), Gt[e, :r[e]])
+        assert np.array_equal(fx.bf16_to_bits(Wu), Ut[e, :r[e]])
+        assert np.array_equal(fx.bf16_to_bits(Wd), Dt[e, :, :r[e]])
+    with pytest.raises(fx.FxmError) as ei:
+        Lc.unpack_prefix(1, int(r[1]) + 16)
+    assert ei.value.name == "FXM_EBUDGET"
+    x, ids, w = gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda()
+    ref = gu.oracle_ffn(lay, b, r)
+    for dec in (0, 1024):
+        if dec and T * k > 1024:
+            continue
+        Lc.set_decode(dec)
+        y = Lc.moe_ffn(x, ids, w)                                # static widths: usable right after the load
+        torch.cuda.synchronize()
+        assert Lc.device_flags() == 0
+        gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), ref, f"clipped layer decode_max={dec}")
+        L.set_decode(dec)
+        L.set_budget(r)
+        yo = L.moe_ffn(x, ids, w)
+        torch.cuda.synchronize()
+        assert torch.equal(y, yo), "offline-clipped and online forward must agree bit for bit (same kernels, same tiles)"
+    sub = (r // 2 // 16 * 16).astype(np.int32)                   # a nested sub-budget of the checkpoint
+    Lc.set_decode(0)
+    Lc.set_budget(sub)
+    y = Lc.moe_ffn(x, ids, w)
+    torch.cuda.synchronize()
+    gu.check_close(gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64), gu.oracle_ffn(lay, b, sub), "nested sub-budget")
+    wider = r.copy()
+    wider[E - 1] = 16
+    with pytest.raises(fx.FxmError) as ei:
+        Lc.set_budget(wider)
+    assert ei.value.name == "FXM_EBUDGET"
+
+
+def test_offline_clipped_c2_shape_sampled_rows():
+    """NEXT-1 at a paper-shaped size: C2 layer exported at r=704 (50 %), forward at T=4096 on the reloaded blob,
+    512 sampled rows vs the oracle; blob bytes = half of the retained-weight bytes of the full layer + constants."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    lay, b, rng = gen.config("C2", T=4096)
+    sh = gen.SHAPES["C2"]
+    r = gen.table_uniform(sh, 704)
+    L = gu.pack_layer(lay)
+    blob = L.export_clipped(r)
+    torch.cuda.synchronize()
+    full_w = 3 * sh.E * sh.I * sh.d * 2
+    assert abs(blob.numel() - full_w // 2) < 64 * 1024
+    del L
+    Lc = fx.Layer.load_clipped(blob, sh.E, sh.d, sh.I, r)
+    y = Lc.moe_ffn(gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda())
+    torch.cuda.synchronize()
+    assert Lc.device_flags() == 0
+    rows = _rows_sample(4096, N_SAMPLE, 21)
+    yv = gen.bf16_bits_to_f32(fx.bf16_to_bits(y[torch.from_numpy(rows.astype(np.int64)).cuda()])).astype(np.float64)
+    gu.check_close(yv, gu.oracle_ffn(lay, b, r, rows=rows), "C2 clipped r=704")
+
+
+# ------------------------------------------------------------ NEXT-3 (part): shared-expert add (PAPER.md:208, 362)
+@pytest.mark.parametrize("decode", [False, True])
+def test_shared_expert_output_is_added_before_the_rounding(decode):
+    """y = bf16( routed(x) + y_shared ): the add happens in fp32 on the accumulator, so the result has ONE rounding."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b, rng = _c1()
+    r = gen.table_c1(sh, rng)
+    L = gu.pack_layer(lay)
+    L.set_budget(r)
+    L.set_decode(1024 if decode else 0)
+    ys_bits = gen.f32_to_bf16_bits(rng.standard_normal((b.x.shape[0], sh.d)).astype(np.float32) * 0.05)
+    y = L.moe_ffn(gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda(),
+                  y_shared=gu.to_dev(ys_bits))
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0 and L.launches_per_ffn() == (1 if decode else 4)
+    ref = gu.oracle_ffn(lay, b, r) + gen.bf16_bits_to_f32(ys_bits).astype(np.float64)
+    got = gen.bf16_bits_to_f32(fx.bf16_to_bits(y)).astype(np.float64)
+    gu.check_close(got, ref, "routed + shared")
+    # one rounding: |y - ref| <= half an ulp of bf16 at ref (2^-9 relative) plus the H rounding's contribution
+    assert np.abs(got - ref).max() <= 2.0 ** -8 * np.abs(ref).max()
