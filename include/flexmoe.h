@@ -126,6 +126,16 @@ fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, con
 fxm_status fxm_moe_ffn_shared(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
                               const void* y_shared, void* y, void* workspace, size_t workspace_bytes, void* stream);
 
+/* NEXT-3 of SURVEY.md 8(f): the forward fed by the router's LOGITS instead of its top-k output.  The front end --
+ * the k largest logits of each token (fp32 comparison, ties -> lower expert id), weights = softmax over those k logits,
+ * i.e. the full softmax renormalised (reading R10) -- runs INSIDE the route kernel, so the launch count stays
+ * 4; for decode-sized calls it is one small kernel in front of the fused decode kernel (2 launches).
+ * router_logits : device fp32 [T][E].   y_shared : device bf16 [T][d] or NULL.
+ * topk_ids_out / topk_w_out : device [T][k] int32 / fp32 or NULL: where the chosen ids and weights are written. */
+fxm_status fxm_moe_ffn_router(fxm_layer* L, const void* x, const float* router_logits, int T, int k, const void* y_shared,
+                              void* y, int32_t* topk_ids_out, float* topk_w_out, void* workspace, size_t workspace_bytes,
+                              void* stream);
+
 /* Same forward with HOST buffers (pinned memory recommended so the copies are asynchronous).  The inputs x [T][d] bf16,
  * topk_ids [T][k] int32 and topk_w [T][k] fp32 are copied on a library-owned side stream into one of two staging
  * sets at the tail of `workspace`, so the host->device copy of call i+1 overlaps the kernels and the device->host
@@ -158,6 +168,35 @@ fxm_status fxm_parse_clipped_header(const void* host_bytes, size_t n, int* E, in
  * workspace sizes as the full layer. */
 fxm_status fxm_load_clipped(fxm_layer** out, int E, int d, int I, const int32_t* r_host, void* blob, size_t blob_bytes,
                             void* stream);
+
+/* ---- NEXT-2 of SURVEY.md 8(f): channel saliency and ranking, the step in front of pack (Eq. 2-3) ----
+ * s[e][j] = (1/B) sum_b sum_{theta in Theta_j} (theta * g_theta^(b))^2 with Theta_j = row j of W_gate, row j of W_up and
+ * column j of W_down.  All tensors are DEVICE bf16, 16-byte aligned: weights [E][I][d], [E][I][d], [E][d][I]
+ * in ORIGINAL channel order, gradients of the B ranking batches [B][E][I][d], [B][E][I][d], [B][E][d][I].
+ * s_out: device fp32 [E][I].  workspace: device, >= fxm_saliency_workspace_bytes, 16-byte aligned (partial sums).
+ * fp32 accumulation in a fixed order (no floating-point atomics): reproducible.  HBM-bound: (1 + B) 6 E I d bytes. */
+fxm_status fxm_saliency_workspace_bytes(int E, int d, int I, size_t* bytes);
+fxm_status fxm_saliency(int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down, const void* G_gate,
+                        const void* G_up, const void* G_down, int B, float* s_out, void* workspace, size_t workspace_bytes,
+                        void* stream);
+/* channel_rank_out[e][p] (device int32 [E][I]) = ORIGINAL index of the p-th most important channel of expert e: s sorted
+ * in descending order, equal saliencies keep ascending original index (readings R3, R4) -- exactly the
+ * channel_rank fxm_pack takes (copy it to the host first: pack validates it there).  I <= 16384. */
+fxm_status fxm_rank_channels(int E, int I, const float* s, int32_t* channel_rank_out, void* stream);
+
+/* ---- NEXT-4 of SURVEY.md 8(f): training-time action sampling and cost (Eq. 6-7, Eq. 10) --
+ * fxm_sample_budget: for every expert k* = argmax_k (alpha[e][k] + gumbel[e][k]) -- the hard action of Eq. 6 for any
+ * temperature tau > 0 (fp32 sum, ties -> lower k); the straight-through forward value (Eq. 7) is the hard one-hot, so
+ * the width ceil(num[k*] I / den) is written into the layer's current table ON THE DEVICE: the masked
+ * forward of Eq. 4 is then fxm_moe_ffn, no host round trip.  alpha, gumbel: device fp32 [E][K] (gumbel NULL = no
+ * noise: the hardened mask of Eq. 11); the Gumbel noise is an input.  num_host [K], den: the action set as exact
+ * ratios.  action_out: device int32 [E] or NULL.  K <= 16.  Not available on a clipped layer (FXM_ESTATE).
+ * fxm_action_cost: C = sum_e q_e sum_k softmax(alpha_e)_k r_k with q_e = counts[e] / sum counts (counts: device int32
+ * [E], e.g. from fxm_route); cost_out: device fp32 [1]. */
+fxm_status fxm_sample_budget(fxm_layer* L, const float* alpha, const float* gumbel, int K, const int32_t* num_host, int den,
+                             int32_t* action_out, void* stream);
+fxm_status fxm_action_cost(fxm_layer* L, const float* alpha, int K, const int32_t* num_host, int den, const int32_t* counts,
+                           float* cost_out, void* stream);
 
 /* ---- measurement surface -------------------------------------------------------------------------------
  * Per-kernel device times of fxm_moe_ffn: between fxm_profile_begin and fxm_profile_end every
@@ -202,8 +241,8 @@ fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles)
  * the CUDA context: bit1 is therefore also written to a pinned host word first, and this call still reports it
  * (together with FXM_ECUDA) when the device can no longer be read. */
 fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream);
-/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode) or 4 (route, GEMM-1, GEMM-2,
- * finalize); bench.py's gpu_launches. */
+/* Number of kernels the LAST fxm_moe_ffn on this layer enqueued: 1 (fused decode; 2 with the router front end) or 4
+ * (route, GEMM-1, GEMM-2, finalize); bench.py's gpu_launches. */
 int fxm_launches_per_ffn(const fxm_layer* L);
 
 const char* fxm_status_string(fxm_status s);

@@ -375,19 +375,22 @@ fxm_status fxm_route(fxm_layer* L, const int32_t* topk_ids, int T, int k, int32_
     return FXM_OK;
 }
 
-// the forward with every optional input: y_add (shared-expert output, may be null)
-static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
-                           const void* y_add, void* y, void* workspace, size_t workspace_bytes, void* stream) {
+// the forward with every optional input: y_add (shared-expert output, may be null); logits (router front end: then
+// topk_ids / topk_w are OUTPUT buffers, or null to keep the chosen ids / weights in the workspace only)
+static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, const float* logits,
+                           int T, int k, const void* y_add, void* y, void* workspace, size_t workspace_bytes, void* stream) {
     fxm_status s = check_call(L, T, k, workspace, workspace_bytes);
     if (s != FXM_OK) return s;
     if (T == 0) return FXM_OK;
-    if (!x || !topk_ids || !topk_w || !y || ((uintptr_t)x & 15u) || ((uintptr_t)y & 15u) || ((uintptr_t)y_add & 15u))
-        return FXM_EINVAL;
+    if (!x || !y || ((uintptr_t)x & 15u) || ((uintptr_t)y & 15u) || ((uintptr_t)y_add & 15u)) return FXM_EINVAL;
+    if (!logits && (!topk_ids || !topk_w)) return FXM_EINVAL;
     if (L->current < 0) return FXM_ESTATE;
     const Dims& D = L->D;
     cudaStream_t st = (cudaStream_t)stream;
     const Workspace ws = map_workspace(D, T, k, workspace);
     const int* table = L->tables + (size_t)L->current * TABLE_STRIDE;
+    int* fe_ids = logits ? (topk_ids ? const_cast<int32_t*>(topk_ids) : ws.fe_ids) : nullptr;   // where the front end writes
+    float* fe_w = logits ? (topk_w ? const_cast<float*>(topk_w) : ws.fe_w) : nullptr;
     cudaEvent_t* ev = nullptr;                                    // per-kernel timing, only between profile_begin/end
     if (L->prof_capacity > 0) {
         ev = &L->prof_events[(size_t)L->prof_calls * (FXM_N_KERNELS + 1)];
@@ -397,18 +400,21 @@ static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids,
 #define FXM_MARK(j) if (ev && cudaEventRecord(ev[j], st) != cudaSuccess) return FXM_ECUDA;
     if (use_decode(L, T, k)) {
         // a6: one launch does a2..a5 (in-kernel grouping, weight streaming, SwiGLU, scale + combine)
+        if (logits && launch_router_topk(logits, T, D.E, k, fe_ids, fe_w, st) != cudaSuccess) return FXM_ECUDA;
         for (int j = 0; j < FXM_N_KERNELS; ++j) FXM_MARK(j)
-        if (launch_decode(D, L->V, table, (const __nv_bfloat16*)x, topk_ids, topk_w, T, k, ws.yacc,
-                          (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->num_sms, L->dec_pf, st) != cudaSuccess)
+        if (launch_decode(D, L->V, table, (const __nv_bfloat16*)x, logits ? fe_ids : topk_ids, logits ? fe_w : topk_w, T, k,
+                          ws.yacc, (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->num_sms, L->dec_pf, st) !=
+            cudaSuccess)
             return FXM_ECUDA;
         FXM_MARK(FXM_N_KERNELS)
-        L->last_launches = 1;
+        L->last_launches = logits ? 2 : 1;
         return FXM_OK;
     }
     // a2 + a3: grouping and the tile schedule for the CURRENT table, one launch
     FXM_MARK(0)
     RouteArgs ra{};
     ra.D = D; ra.ids = topk_ids; ra.topk_w = topk_w; ra.r_table = table; ra.T = T; ra.k = k; ra.tile_n = choose_tile_n(L);
+    ra.logits = logits; ra.ids_out = fe_ids; ra.w_out = fe_w;      // front end fused into the route kernel (same launch count)
     ra.counts = ws.counts; ra.offsets = ws.offsets; ra.perm = ws.perm; ra.inv_perm = ws.inv_perm;
     if (launch_route(ra, ws, L->state, st) != cudaSuccess) return FXM_ECUDA;
     FXM_MARK(1)
@@ -439,13 +445,20 @@ static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids,
 
 fxm_status fxm_moe_ffn(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k, void* y,
                        void* workspace, size_t workspace_bytes, void* stream) {
-    return ffn_impl(L, x, topk_ids, topk_w, T, k, nullptr, y, workspace, workspace_bytes, stream);
+    return ffn_impl(L, x, topk_ids, topk_w, nullptr, T, k, nullptr, y, workspace, workspace_bytes, stream);
+}
+
+fxm_status fxm_moe_ffn_router(fxm_layer* L, const void* x, const float* router_logits, int T, int k, const void* y_shared,
+                              void* y, int32_t* topk_ids_out, float* topk_w_out, void* workspace, size_t workspace_bytes,
+                              void* stream) {
+    if (!router_logits) return FXM_EINVAL;
+    return ffn_impl(L, x, topk_ids_out, topk_w_out, router_logits, T, k, y_shared, y, workspace, workspace_bytes, stream);
 }
 
 fxm_status fxm_moe_ffn_shared(fxm_layer* L, const void* x, const int32_t* topk_ids, const float* topk_w, int T, int k,
                               const void* y_shared, void* y, void* workspace, size_t workspace_bytes, void* stream) {
     if (!y_shared) return FXM_EINVAL;
-    return ffn_impl(L, x, topk_ids, topk_w, T, k, y_shared, y, workspace, workspace_bytes, stream);
+    return ffn_impl(L, x, topk_ids, topk_w, nullptr, T, k, y_shared, y, workspace, workspace_bytes, stream);
 }
 
 fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
@@ -598,6 +611,71 @@ fxm_status fxm_load_clipped(fxm_layer** out, int E, int d, int I, const int32_t*
     if (s == FXM_OK) s = fxm_set_budget(L, r_host, stream);       // static widths: the exported table is the current one
     if (s != FXM_OK) { fxm_destroy(L); return s; }
     *out = L;
+    return FXM_OK;
+}
+
+// ---- NEXT-2: channel saliency and ranking (Eq. 2-3) ----------------------------------------------------
+
+fxm_status fxm_saliency_workspace_bytes(int E, int d, int I, size_t* bytes) {
+    Dims D;
+    if (!bytes) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    *bytes = saliency_workspace_bytes(D);
+    return FXM_OK;
+}
+
+fxm_status fxm_saliency(int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down, const void* G_gate,
+                        const void* G_up, const void* G_down, int B, float* s_out, void* workspace, size_t workspace_bytes,
+                        void* stream) {
+    Dims D;
+    if (!W_gate || !W_up || !W_down || !G_gate || !G_up || !G_down || !s_out || !workspace || B < 1) return FXM_EINVAL;
+    const uintptr_t al = (uintptr_t)W_gate | (uintptr_t)W_up | (uintptr_t)W_down | (uintptr_t)G_gate | (uintptr_t)G_up |
+                         (uintptr_t)G_down | (uintptr_t)workspace;
+    if (al & 15u) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    if (workspace_bytes < saliency_workspace_bytes(D)) return FXM_EWORKSPACE;
+    if (launch_saliency(D, (const __nv_bfloat16*)W_gate, (const __nv_bfloat16*)W_up, (const __nv_bfloat16*)W_down,
+                        (const __nv_bfloat16*)G_gate, (const __nv_bfloat16*)G_up, (const __nv_bfloat16*)G_down, B, s_out,
+                        (float*)workspace, (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_rank_channels(int E, int I, const float* s, int32_t* channel_rank_out, void* stream) {
+    if (!s || !channel_rank_out) return FXM_EINVAL;
+    if (E < 1 || E > MAX_E || I < 1 || !rank_supported(I)) return FXM_ESHAPE;
+    if (init_rank_kernel() != cudaSuccess) return FXM_ECUDA;
+    if (launch_rank(E, I, s, channel_rank_out, (cudaStream_t)stream) != cudaSuccess) return FXM_ECUDA;
+    return FXM_OK;
+}
+
+// ---- NEXT-4: training-time action sampling and cost (Eq. 6-7, 10) ------------------------------------------------------
+
+static bool check_ratios(int K, const int32_t* num, int den) {
+    if (K < 1 || K > MAX_K || !num || den <= 0) return false;
+    for (int k = 0; k < K; ++k)
+        if (num[k] < 0 || num[k] > den) return false;
+    return true;
+}
+
+fxm_status fxm_sample_budget(fxm_layer* L, const float* alpha, const float* gumbel, int K, const int32_t* num_host, int den,
+                             int32_t* action_out, void* stream) {
+    if (!L || !alpha || !check_ratios(K, num_host, den)) return FXM_EINVAL;
+    if (L->clipped) return FXM_ESTATE;                            // a sampled width may exceed what a clipped blob holds
+    const int slot = MAX_TABLES - 1;
+    if (launch_sample_actions(alpha, gumbel, K, num_host, den, L->D.E, L->D.I, L->tables + (size_t)slot * TABLE_STRIDE,
+                              action_out, (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    std::fill(L->host_tables.begin() + (size_t)slot * TABLE_STRIDE, L->host_tables.begin() + (size_t)(slot + 1) * TABLE_STRIDE, -1);
+    L->current = slot;
+    return FXM_OK;
+}
+
+fxm_status fxm_action_cost(fxm_layer* L, const float* alpha, int K, const int32_t* num_host, int den, const int32_t* counts,
+                           float* cost_out, void* stream) {
+    if (!L || !alpha || !counts || !cost_out || !check_ratios(K, num_host, den)) return FXM_EINVAL;
+    if (launch_action_cost(alpha, K, num_host, den, L->D.E, counts, cost_out, (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
     return FXM_OK;
 }
 

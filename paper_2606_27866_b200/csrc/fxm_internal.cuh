@@ -91,6 +91,8 @@ struct Workspace {
     int* row_tok;           // [P]  token index t = f / k of each padded row (0 for padding rows): the gather4 row coordinates
     int2* row_tw;           // [P]  {token index or -1 for padding rows, router weight topk_w[f] as bits}: the scatter-add
                             //      destination and scale of each padded row (GEMM-2 epilogue, Alg. 2 l.19-20)
+    int* fe_ids;            // [A]  router front end (fxm_moe_ffn_router): the ids it chose ...
+    float* fe_w;            // [A]  ... and the renormalised weights
     int* bhist;             // [RB][E] per-route-block expert histogram, then exclusive base over blocks
     int4* tt;               // [NT + 1] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}; tt[ntt] = sentinel
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
@@ -137,6 +139,8 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.row_flat = (int*)(b + take(sizeof(int) * (size_t)P));
     w.row_tok = (int*)(b + take(sizeof(int) * (size_t)P));
     w.row_tw = (int2*)(b + take(sizeof(int2) * (size_t)P));
+    w.fe_ids = (int*)(b + take(sizeof(int) * (A + 1)));
+    w.fe_w = (float*)(b + take(sizeof(float) * (A + 1)));
     w.bhist = (int*)(b + take(sizeof(int) * (size_t)RT_MAX_BLOCKS * D.E));   // capacity, not RB: the size stays monotonic in T
     w.tt = (int4*)(b + take(sizeof(int4) * ((size_t)NT + 1)));
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
@@ -224,6 +228,8 @@ struct RouteArgs {
     int* inv_perm;           // [A]
 };
 cudaError_t launch_route(const RouteArgs& a, const Workspace& ws, DevState* state, cudaStream_t st);
+// the router front end alone (softmax -> top-k -> renormalise): feeds the fused decode kernel
+cudaError_t launch_router_topk(const float* logits, int T, int E, int k, int* ids_out, float* w_out, cudaStream_t st);
 // y[t] = bf16( yacc[t] (+ y_add[t]) ): the single rounding of y (reading R11); y_add = optional shared-expert output
 cudaError_t launch_finalize(const Dims& D, int T, const float* yacc, const __nv_bfloat16* y_add, __nv_bfloat16* y,
                             cudaStream_t st);
@@ -250,6 +256,19 @@ cudaError_t encode_x_map(const void* x, int T, int d, void* map_out /* 128 bytes
 cudaError_t launch_gemm2_pair(const Dims& D, const LayerView& V, const int* r_table, const Workspace& ws,
                               DevState* state, int num_sms, cudaStream_t st);
 cudaError_t init_pair_kernels();
+
+// NEXT-2 / NEXT-4 (fxm_rank.cu): channel saliency + ranking, action sampling + cost
+size_t saliency_workspace_bytes(const Dims& D);
+cudaError_t launch_saliency(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
+                            const __nv_bfloat16* Gg, const __nv_bfloat16* Gu, const __nv_bfloat16* Gd, int B, float* s,
+                            float* part, cudaStream_t st);
+cudaError_t init_rank_kernel();
+bool rank_supported(int I);
+cudaError_t launch_rank(int E, int I, const float* s, int* rank, cudaStream_t st);
+cudaError_t launch_sample_actions(const float* alpha, const float* gumbel, int K, const int* num_host, int den, int E, int I,
+                                  int* table, int* action, cudaStream_t st);
+cudaError_t launch_action_cost(const float* alpha, int K, const int* num_host, int den, int E, const int* counts, float* cost,
+                               cudaStream_t st);
 
 // fused single-launch decode kernel (fxm_decode.cu): T*k <= DEC_MAX_A, d <= 3840
 bool decode_supported(const Dims& D);

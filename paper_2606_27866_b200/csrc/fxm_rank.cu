@@ -1,0 +1,220 @@
+// fxm_rank.cu -- the steps immediately around the hot path that SURVEY.md 8(f) lists as NEXT-2 and NEXT-4:
+//   NEXT-2  channel saliency (Eq. 2) and the descending ranking that defines P (Eq. 3):
+//             s[e][j] = (1/B) sum_b sum_{theta in Theta_j} (theta * g_theta^(b))^2,
+//             Theta_j = row j of W_gate, row j of W_up, column j of W_down
+//           -> channel_rank[e][p] = ORIGINAL index of the p-th most important channel (readings R3, R4), the input of pack.
+//           A streaming reduction over the weights and B gradient sets: HBM-bound, (1 + B) * 6 E I d bytes, each read once.
+//   NEXT-4  the training-time action sampling that turns logits into a width table on the device (Eq. 6-7, PAPER.md:104-113:
+//           the forward value of the straight-through estimator is the hard one-hot), and the load-sensitive cost of
+//           Eq. 10.  With these the masked forward of Eq. 4 is "sample -> moe_ffn" with no host round trip.
+// All sums are fixed-order (no floating-point atomics): results are reproducible run to run.
+#include "fxm_internal.cuh"
+
+namespace fxm {
+
+__device__ __forceinline__ float bf_lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
+__device__ __forceinline__ float sq8(const uint4& w, const uint4& g) {
+    const float p0 = bf_lo(w.x) * bf_lo(g.x), p1 = bf_hi(w.x) * bf_hi(g.x), p2 = bf_lo(w.y) * bf_lo(g.y), p3 = bf_hi(w.y) * bf_hi(g.y);
+    const float p4 = bf_lo(w.z) * bf_lo(g.z), p5 = bf_hi(w.z) * bf_hi(g.z), p6 = bf_lo(w.w) * bf_lo(g.w), p7 = bf_hi(w.w) * bf_hi(g.w);
+    return ((p0 * p0 + p1 * p1) + (p2 * p2 + p3 * p3)) + ((p4 * p4 + p5 * p5) + (p6 * p6 + p7 * p7));
+}
+
+// gate and up rows: one warp per (e, j); the row of d bf16 is read with 16-byte loads, weights once, gradients B times
+__global__ void __launch_bounds__(256) k_saliency_gu(int d, size_t rows, size_t per, const uint4* __restrict__ Wg,
+                                                     const uint4* __restrict__ Wu, const uint4* __restrict__ Gg,
+                                                     const uint4* __restrict__ Gu, int B, float* __restrict__ part0) {
+    const int lane = threadIdx.x & 31;
+    const int cpr = d >> 3;                                      // 16-byte chunks per row
+    const size_t per4 = per >> 3;                                // chunks per gradient set
+    for (size_t row = blockIdx.x * 8ull + (threadIdx.x >> 5); row < rows; row += (size_t)gridDim.x * 8) {
+        float acc = 0.f;
+        for (int c = lane; c < cpr; c += 32) {
+            const size_t o = row * cpr + c;
+            const uint4 wg = __ldcs(Wg + o), wu = __ldcs(Wu + o);
+            for (int b = 0; b < B; ++b) {
+                const uint4 gg = __ldcs(Gg + b * per4 + o), gu = __ldcs(Gu + b * per4 + o);
+                acc += sq8(wg, gg) + sq8(wu, gu);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) part0[row] = acc;
+    }
+}
+
+// down columns: block (e, r) owns the rows [r0, r1) of W_down[e] [d][I]; a thread owns 8 consecutive columns of a 2048-wide
+// column tile, so a row segment is read as 256 consecutive 16-byte chunks.  Partial column sums go to slot 1 + r.
+__global__ void __launch_bounds__(256) k_saliency_dn(int d, int I, int R, size_t per, const uint4* __restrict__ Wd,
+                                                     const uint4* __restrict__ Gd, int B, float* __restrict__ part) {
+    const int e = blockIdx.x / R, r = blockIdx.x % R;
+    const int E = gridDim.x / R;
+    const int r0 = (int)((long long)d * r / R), r1 = (int)((long long)d * (r + 1) / R);
+    const int cpr = I >> 3;                                      // chunks per row (I % 16 == 0)
+    const size_t per4 = per >> 3;
+    float* out = part + ((size_t)(1 + r) * E + e) * I;
+    for (int c0 = threadIdx.x; c0 < cpr; c0 += 256) {
+        float acc[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = 0.f;
+#pragma unroll 4
+        for (int i = r0; i < r1; ++i) {
+            const size_t o = ((size_t)e * d + i) * cpr + c0;
+            const uint4 w = __ldcs(Wd + o);
+            for (int b = 0; b < B; ++b) {
+                const uint4 g = __ldcs(Gd + b * per4 + o);
+                const float p0 = bf_lo(w.x) * bf_lo(g.x), p1 = bf_hi(w.x) * bf_hi(g.x), p2 = bf_lo(w.y) * bf_lo(g.y), p3 = bf_hi(w.y) * bf_hi(g.y);
+                const float p4 = bf_lo(w.z) * bf_lo(g.z), p5 = bf_hi(w.z) * bf_hi(g.z), p6 = bf_lo(w.w) * bf_lo(g.w), p7 = bf_hi(w.w) * bf_hi(g.w);
+                acc[0] += p0 * p0; acc[1] += p1 * p1; acc[2] += p2 * p2; acc[3] += p3 * p3;
+                acc[4] += p4 * p4; acc[5] += p5 * p5; acc[6] += p6 * p6; acc[7] += p7 * p7;
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) out[(size_t)c0 * 8 + q] = acc[q];
+    }
+}
+
+// s = (slot 0 + slot 1 + ... + slot R) / B, slots summed in index order
+__global__ void k_saliency_sum(const float* __restrict__ part, int slots, size_t n, float inv_b, float* __restrict__ s) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        float acc = 0.f;
+        for (int q = 0; q < slots; ++q) acc += part[(size_t)q * n + i];
+        s[i] = acc * inv_b;
+    }
+}
+
+int saliency_row_chunks(const Dims& D) {
+    int R = (148 * 2 + D.E - 1) / D.E;                           // about two blocks per SM
+    if (R > 16) R = 16;
+    if (R > D.d) R = D.d;
+    return R < 1 ? 1 : R;
+}
+size_t saliency_workspace_bytes(const Dims& D) { return align_up((size_t)(1 + saliency_row_chunks(D)) * D.E * D.I * sizeof(float), 1024); }
+
+cudaError_t launch_saliency(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
+                            const __nv_bfloat16* Gg, const __nv_bfloat16* Gu, const __nv_bfloat16* Gd, int B, float* s,
+                            float* part, cudaStream_t st) {
+    const size_t rows = (size_t)D.E * D.I, per = rows * D.d;
+    const int R = saliency_row_chunks(D);
+    size_t b1 = (rows + 7) / 8;
+    if (b1 > 148 * 16) b1 = 148 * 16;
+    k_saliency_gu<<<(unsigned)b1, 256, 0, st>>>(D.d, rows, per, (const uint4*)Wg, (const uint4*)Wu, (const uint4*)Gg,
+                                                 (const uint4*)Gu, B, part);
+    k_saliency_dn<<<D.E * R, 256, 0, st>>>(D.d, D.I, R, per, (const uint4*)Wd, (const uint4*)Gd, B, part);
+    size_t b3 = (rows + 255) / 256;
+    if (b3 > 148 * 8) b3 = 148 * 8;
+    k_saliency_sum<<<(unsigned)b3, 256, 0, st>>>(part, 1 + R, rows, 1.0f / (float)B, s);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ rank
+// One block per expert: bitonic sort of 64-bit keys (~orderable(s) << 32 | index) in shared memory.  The keys are
+// distinct, so "descending s, ties -> lower original index" (reading R4) is the ascending key order -- one result.
+constexpr int RANK_THREADS = 1024;
+constexpr int RANK_MAX_I = 16384;
+__global__ void __launch_bounds__(RANK_THREADS) k_rank(const float* __restrict__ s, int I, int Np, int* __restrict__ rank) {
+    extern __shared__ unsigned long long keys[];
+    const int e = blockIdx.x;
+    for (int i = threadIdx.x; i < Np; i += RANK_THREADS) {
+        unsigned long long key = ~0ull;                          // padding sorts last
+        if (i < I) {
+            float v = s[(size_t)e * I + i];
+            if (v == 0.f) v = 0.f;                               // -0 and +0 are one value
+            uint32_t u = __float_as_uint(v);
+            u ^= (u >> 31) ? 0xFFFFFFFFu : 0x80000000u;          // ascending-orderable
+            key = ((unsigned long long)(~u) << 32) | (uint32_t)i;
+        }
+        keys[i] = key;
+    }
+    __syncthreads();
+    for (int k = 2; k <= Np; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < (Np >> 1); t += RANK_THREADS) {
+                const int lo = ((t & ~(j - 1)) << 1) | (t & (j - 1));      // index with bit j clear
+                const int hi = lo | j;
+                const bool up = (lo & k) == 0;
+                const unsigned long long a = keys[lo], b = keys[hi];
+                if ((a > b) == up) { keys[lo] = b; keys[hi] = a; }
+            }
+            __syncthreads();
+        }
+    }
+    for (int i = threadIdx.x; i < I; i += RANK_THREADS) rank[(size_t)e * I + i] = (int)(uint32_t)keys[i];
+}
+cudaError_t init_rank_kernel() {
+    return cudaFuncSetAttribute(k_rank, cudaFuncAttributeMaxDynamicSharedMemorySize, RANK_MAX_I * 8);
+}
+bool rank_supported(int I) { return I <= RANK_MAX_I; }
+cudaError_t launch_rank(int E, int I, const float* s, int* rank, cudaStream_t st) {
+    int Np = 2;
+    while (Np < I) Np <<= 1;
+    k_rank<<<E, RANK_THREADS, (size_t)Np * 8, st>>>(s, I, Np, rank);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------- action sampling
+struct RatioArg { int num[MAX_K]; int den; int K; };
+// Eq. 6: k* = argmax_k softmax((alpha + g) / tau) = argmax_k (alpha_k + g_k) for any tau > 0 (fp32 sum,
+// ties -> lower k); Eq. 7: the forward pass uses the hard one-hot, so the sampled width is ceil(r_k* I).
+__global__ void k_sample_actions(const float* __restrict__ alpha, const float* __restrict__ gumbel, RatioArg ra, int E, int I,
+                                 int* __restrict__ table, int* __restrict__ action) {
+    const int e = threadIdx.x;
+    if (e >= MAX_E) return;
+    int width = 0;
+    if (e < E) {
+        int best = 0;
+        float vbest = alpha[(size_t)e * ra.K] + (gumbel ? gumbel[(size_t)e * ra.K] : 0.f);
+        for (int k = 1; k < ra.K; ++k) {
+            const float v = alpha[(size_t)e * ra.K + k] + (gumbel ? gumbel[(size_t)e * ra.K + k] : 0.f);
+            if (v > vbest) { vbest = v; best = k; }
+        }
+        width = (int)(((long long)I * ra.num[best] + ra.den - 1) / ra.den);
+        if (action) action[e] = best;
+    }
+    table[e] = width;
+}
+// Eq. 10 for one layer: C = sum_e q_e sum_k p_ek r_k, p_e = softmax(alpha_e), q_e = n_e / sum n
+__global__ void __launch_bounds__(MAX_E) k_action_cost(const float* __restrict__ alpha, RatioArg ra, int E,
+                                                       const int* __restrict__ counts, float* __restrict__ cost) {
+    __shared__ float s_c[MAX_E], s_n[MAX_E];
+    const int e = threadIdx.x;
+    float er = 0.f, n = 0.f;
+    if (e < E) {
+        float mx = alpha[(size_t)e * ra.K];
+        for (int k = 1; k < ra.K; ++k) mx = fmaxf(mx, alpha[(size_t)e * ra.K + k]);
+        float z = 0.f, acc = 0.f;
+        for (int k = 0; k < ra.K; ++k) {
+            const float p = expf(alpha[(size_t)e * ra.K + k] - mx);
+            z += p;
+            acc += p * ((float)ra.num[k] / (float)ra.den);
+        }
+        er = acc / z;
+        n = (float)counts[e];
+    }
+    s_c[e] = er * n;
+    s_n[e] = n;
+    __syncthreads();
+    for (int o = MAX_E / 2; o > 0; o >>= 1) {                    // fixed-order tree
+        if (e < o) { s_c[e] += s_c[e + o]; s_n[e] += s_n[e + o]; }
+        __syncthreads();
+    }
+    if (e == 0) *cost = s_n[0] > 0.f ? s_c[0] / s_n[0] : 0.f;
+}
+cudaError_t launch_sample_actions(const float* alpha, const float* gumbel, int K, const int* num_host, int den, int E, int I,
+                                  int* table, int* action, cudaStream_t st) {
+    RatioArg ra{};
+    for (int k = 0; k < K; ++k) ra.num[k] = num_host[k];
+    ra.den = den; ra.K = K;
+    k_sample_actions<<<1, MAX_E, 0, st>>>(alpha, gumbel, ra, E, I, table, action);
+    return cudaGetLastError();
+}
+cudaError_t launch_action_cost(const float* alpha, int K, const int* num_host, int den, int E, const int* counts, float* cost,
+                               cudaStream_t st) {
+    RatioArg ra{};
+    for (int k = 0; k < K; ++k) ra.num[k] = num_host[k];
+    ra.den = den; ra.K = K;
+    k_action_cost<<<1, MAX_E, 0, st>>>(alpha, ra, E, counts, cost);
+    return cudaGetLastError();
+}
+
+}  // namespace fxm

@@ -6,7 +6,8 @@
 //   computed here from counts[] and the CURRENT width table r[]: only tiles with channel index < r_e and
 //   token row < n_e exist.
 //
-// k_route, grid = RB <= 128 blocks of 256 threads, no atomics decide any position (deterministic and stable):
+// k_route, grid = RB <= 128 scatter blocks + 1 planner block of 256 threads, no atomics decide any position
+// (deterministic and stable):
 //   1  block b histograms its flat assignments [b*chunk, (b+1)*chunk) per expert, one histogram row per warp
 //      (warp w owns a contiguous sub-range, so "earlier block, earlier warp, earlier 32-wide step, lower lane" is
 //      "lower flat index"), and publishes the block row to bhist[b][.];
@@ -16,12 +17,15 @@
 //      These are independent loads (no serial scan by a "last block"), a few per thread;
 //   4  every block scans counts over the experts (offsets, padded offsets) in shared memory and scatters its own
 //      assignments -- the per-warp histograms of step 1 are still in shared memory, nothing is recomputed;
-//   5  block 0 also writes counts / offsets and the schedule for the current width table: the token tiles
+//   5  the PLANNER block (the extra, last block: it has no assignments of its own, so the schedule is written while the
+//      others scatter) writes counts / offsets and the schedule for the current width table: the token tiles
 //      {expert, first padded row, valid rows, GEMM-1 work prefix}, experts ordered by descending work per tile (rows x
 //      retained width) so that a static stride over the work list hands out the heavy tiles first and the light
 //      ones in the last, partly filled round.  GEMM-1's work items (tile, pair of retained channel blocks) are not
 //      materialised: item wi belongs to the tile j with tt[j].w <= wi < tt[j+1].w (tt[ntt] is a sentinel).
 #include "fxm_internal.cuh"
+
+#include <math_constants.h>
 
 namespace fxm {
 
@@ -57,6 +61,44 @@ __device__ __forceinline__ unsigned long long rt_now() {
 #define RT_TR(f) do { } while (0)
 #endif
 
+// NEXT-3, the router front end (reading R10; the paper takes the router's OUTPUT as given): for one
+// token, the k largest of its E logits in descending order (fp32 comparison, ties -> lower expert id) and the softmax
+// over those k logits (= the softmax over all E renormalised to sum 1).  One warp per token; lane l holds the logits
+// l, l + 32, ...  Each round: every lane offers its best unused logit, a butterfly keeps (larger value, then lower id).
+__device__ __forceinline__ void warp_router_topk(const float* __restrict__ lg, int E, int k, int lane,
+                                                 int* __restrict__ ids_out, float* __restrict__ w_out) {
+    float v[MAX_E / 32];
+#pragma unroll
+    for (int u = 0; u < MAX_E / 32; ++u) v[u] = (lane + 32 * u) < E ? lg[lane + 32 * u] : -CUDART_INF_F;
+    unsigned used = 0;
+    float top = 0.f, mine = 0.f, den = 0.f;
+    int my_id = 0;
+    for (int j = 0; j < k; ++j) {
+        float bv = -CUDART_INF_F;
+        int bi = 0x7fffffff;
+#pragma unroll
+        for (int u = 0; u < MAX_E / 32; ++u) {
+            const int id = lane + 32 * u;
+            if (id < E && !((used >> u) & 1u) && (v[u] > bv || (v[u] == bv && id < bi))) { bv = v[u]; bi = id; }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        if ((bi & 31) == lane && bi < E) used |= 1u << (bi >> 5);
+        if (j == 0) top = bv;
+        const float ex = expf(bv - top);
+        den += ex;
+        if (lane == j) { mine = ex; my_id = bi; }
+    }
+    if (lane < k) {
+        ids_out[lane] = my_id;
+        w_out[lane] = mine / den;
+    }
+}
+
 struct RouteWs {             // the device pointers of the workspace the kernel writes
     int* poff;
     Sched* sched;
@@ -77,14 +119,22 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
     const Dims& D = a.D;
     const int E = D.E, k = a.k, A = a.T * a.k;
     const int tid = threadIdx.x, lane = tid & 31, wp = tid >> 5;
-    const int RB = gridDim.x, b = blockIdx.x;
-    const int* __restrict__ ids = a.ids;
+    const int RB = gridDim.x - 1, b = blockIdx.x;              // block RB is the planner
+    const bool planner = b == RB;
+    const int* ids = a.logits ? a.ids_out : a.ids;
     RT_TR(0);
     pdl_launch_dependents();
     for (int i = tid; i < RT_WARPS * MAX_E; i += RT_THREADS) (&whist[0][0])[i] = 0;
     pdl_wait();                                                  // the previous call's kernels may still read the workspace
     RT_TR(1);
     if (tid == 0) s_gen0 = ld_acquire_gpu(&state->route_gen);    // before this block arrives anywhere
+    if (a.logits && !planner) {
+        // ---- 0: the router front end for this block's own tokens (a block owns whole tokens): ids / weights go to the
+        //         workspace, the grouping below reads them back (same block: visible after the barrier)
+        const int t_lo = min(a.T, b * (w.chunk / k)), t_hi = min(a.T, t_lo + w.chunk / k);
+        for (int t = t_lo + wp; t < t_hi; t += RT_WARPS)
+            warp_router_topk(a.logits + (size_t)t * E, E, k, lane, a.ids_out + (size_t)t * k, a.w_out + (size_t)t * k);
+    }
     __syncthreads();
 
     // ---- 1: per-warp histogram of this block's chunk
@@ -105,19 +155,20 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
         if (bad) atomicOr(&state->flags, 1u);
     }
     __syncthreads();
-    for (int e = tid; e < E; e += RT_THREADS) {
-        int c = 0;
+    if (!planner)
+        for (int e = tid; e < E; e += RT_THREADS) {
+            int c = 0;
 #pragma unroll
-        for (int ww = 0; ww < RT_WARPS; ++ww) c += whist[ww][e];
-        w.bhist[(size_t)b * E + e] = c;
-    }
+            for (int ww = 0; ww < RT_WARPS; ++ww) c += whist[ww][e];
+            w.bhist[(size_t)b * E + e] = c;
+        }
 
     // ---- 2: publish barrier over the grid
     __threadfence();
     __syncthreads();
     RT_TR(2);
     if (tid == 0) {
-        if (atomicAdd(&state->ticket, 1u) == (uint32_t)RB - 1u) {
+        if (atomicAdd(&state->ticket, 1u) == gridDim.x - 1u) {
             state->ticket = 0;                                   // ready for the next call on this layer
             __threadfence();
             atomicAdd(&state->route_gen, 1u);
@@ -181,7 +232,7 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
         if (lane == 0) { s_off[E] = c_off; s_poff[E] = c_poff; }
     }
     __syncthreads();
-    if (b == 0) {
+    if (planner) {
         // work key of an expert: rows of its widest tile x retained width (what one GEMM-2 item of it costs)
         for (int e = tid; e < E; e += RT_THREADS) {
             const int n = s_cnt[e];
@@ -246,6 +297,14 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
             w.poff[e] = s_poff[e];
             if (e < E) a.counts[e] = s_cnt[e];
         }
+        // padding rows of the expert segments carry no assignment
+        for (int e = tid; e < E; e += RT_THREADS)
+            for (int p = s_poff[e] + s_cnt[e]; p < s_poff[e + 1]; ++p) {
+                w.row_flat[p] = -1;
+                w.row_tok[p] = 0;
+                w.row_tw[p] = make_int2(-1, 0);
+            }
+        return;
     }
 
     RT_TR(5);
@@ -276,7 +335,8 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
             a.inv_perm[f] = pos;
             w.row_flat[pr] = f;
             w.row_tok[pr] = t;
-            w.row_tw[pr] = make_int2(t, a.topk_w ? __float_as_int(a.topk_w[f]) : 0);
+            const float* tw = a.logits ? a.w_out : a.topk_w;
+            w.row_tw[pr] = make_int2(t, tw ? __float_as_int(tw[f]) : 0);
         } else if (f < whi) {
             a.inv_perm[f] = -1;                              // dropped (precondition violation, flagged above)
         }
@@ -286,21 +346,30 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
     }
 
     RT_TR(6);
-    // ---- padding rows of the expert segments carry no assignment
-    for (int e = b * RT_THREADS + tid; e < E; e += RB * RT_THREADS)
-        for (int p = s_poff[e] + s_cnt[e]; p < s_poff[e + 1]; ++p) {
-            w.row_flat[p] = -1;
-            w.row_tok[p] = 0;
-            w.row_tw[p] = make_int2(-1, 0);
-        }
+}
 
+// the same front end as a kernel of its own: feeds the fused decode kernel (which re-derives the grouping in every CTA
+// and should not redo the top-k there)
+__global__ void __launch_bounds__(RT_THREADS) k_router_topk(const float* __restrict__ logits, int T, int E, int k,
+                                                            int* __restrict__ ids_out, float* __restrict__ w_out) {
+    pdl_launch_dependents();
+    pdl_wait();
+    const int lane = threadIdx.x & 31;
+    for (int t = blockIdx.x * RT_WARPS + (threadIdx.x >> 5); t < T; t += gridDim.x * RT_WARPS)
+        warp_router_topk(logits + (size_t)t * E, E, k, lane, ids_out + (size_t)t * k, w_out + (size_t)t * k);
+}
+cudaError_t launch_router_topk(const float* logits, int T, int E, int k, int* ids_out, float* w_out, cudaStream_t st) {
+    int blocks = (T + RT_WARPS - 1) / RT_WARPS;
+    if (blocks > 148 * 4) blocks = 148 * 4;
+    if (blocks < 1) blocks = 1;
+    return launch_pdl(k_router_topk, dim3(blocks), dim3(RT_THREADS), 0, st, logits, T, E, k, ids_out, w_out);
 }
 
 cudaError_t launch_route(const RouteArgs& a, const Workspace& ws, DevState* state, cudaStream_t st) {
     RouteWs w{};
     w.poff = ws.poff; w.sched = ws.sched; w.row_flat = ws.row_flat; w.row_tok = ws.row_tok; w.row_tw = ws.row_tw;
     w.bhist = ws.bhist; w.tt = ws.tt; w.chunk = ws.chunk;
-    return launch_pdl(k_route, dim3(ws.RB), dim3(RT_THREADS), 0, st, a, w, state);
+    return launch_pdl(k_route, dim3(ws.RB + 1), dim3(RT_THREADS), 0, st, a, w, state);
 }
 
 }  // namespace fxm

@@ -13,7 +13,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _SO = os.path.join(_HERE, "libflexmoe.so")
-_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_pair.cu", "fxm_decode.cu"]
+_SOURCES = ["fxm_api.cu", "fxm_aux.cu", "fxm_route.cu", "fxm_simt.cu", "fxm_pair.cu", "fxm_decode.cu", "fxm_rank.cu"]
 _HEADERS = [os.path.join(_CSRC, "fxm_internal.cuh"), os.path.join(_CSRC, "fxm_ptx.cuh"), os.path.join(_HERE, "..", "include", "flexmoe.h")]
 
 IMPL_TCGEN05 = 0
@@ -68,12 +68,18 @@ def lib():
     L.fxm_ratio_to_width.restype = ctypes.c_int32
     L.fxm_moe_ffn.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
     L.fxm_moe_ffn_shared.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, sz, vp]
+    L.fxm_moe_ffn_router.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
     L.fxm_clipped_bytes.argtypes = [i32, i32, i32, vp, ctypes.POINTER(sz)]
     L.fxm_export_clipped.argtypes = [vp, vp, vp, sz, vp]
     L.fxm_parse_clipped_header.argtypes = [vp, sz, ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i32), vp]
     L.fxm_load_clipped.argtypes = [ctypes.POINTER(vp), i32, i32, i32, vp, vp, sz, vp]
     L.fxm_workspace_bytes_host.argtypes = [i32, i32, i32, i32, i32, ctypes.POINTER(sz)]
     L.fxm_moe_ffn_host.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_saliency_workspace_bytes.argtypes = [i32, i32, i32, ctypes.POINTER(sz)]
+    L.fxm_saliency.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, i32, vp, vp, sz, vp]
+    L.fxm_rank_channels.argtypes = [i32, i32, vp, vp, vp]
+    L.fxm_sample_budget.argtypes = [vp, vp, vp, i32, vp, i32, vp, vp]
+    L.fxm_action_cost.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp]
     L.fxm_profile_begin.argtypes = [vp, i32]
     L.fxm_profile_end.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i32)]
     L.fxm_route.argtypes = [vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
@@ -93,8 +99,9 @@ def lib():
 
 
 EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
-           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_moe_ffn_shared", "fxm_workspace_bytes_host",
+           "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_moe_ffn_shared", "fxm_moe_ffn_router", "fxm_workspace_bytes_host",
            "fxm_moe_ffn_host", "fxm_clipped_bytes", "fxm_export_clipped", "fxm_parse_clipped_header", "fxm_load_clipped",
+           "fxm_saliency_workspace_bytes", "fxm_saliency", "fxm_rank_channels", "fxm_sample_budget", "fxm_action_cost",
            "fxm_profile_begin", "fxm_profile_end", "fxm_route", "fxm_unpack_prefix",
            "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_set_decode", "fxm_device_flags", "fxm_launches_per_ffn",
            "fxm_status_string", "fxm_destroy"]
@@ -127,6 +134,35 @@ N_KERNELS = 5
 KERNEL_NAMES = ("route", "gemm1_swiglu", "gemm2_scatter_add", "finalize", "decode_fused")
 DECODE_DEFAULT_MAX_ASSIGNMENTS = 768
 DECODE_DEFAULT_PREFETCH = 0
+
+
+def saliency(W_gate, W_up, W_down, G_gate, G_up, G_down, stream=None):
+    """Eq. 2 (fxm_saliency).  CUDA bf16 tensors: weights [E,I,d],[E,I,d],[E,d,I]; gradients [B,E,I,d],[B,E,I,d],[B,E,d,I]
+    -> s [E,I] fp32."""
+    import torch
+    E, I, d = W_gate.shape
+    B = G_gate.shape[0]
+    for t in (W_gate, W_up, W_down, G_gate, G_up, G_down):
+        assert t.is_cuda and t.dtype == torch.bfloat16 and t.is_contiguous()
+    assert tuple(W_down.shape) == (E, d, I) and tuple(G_gate.shape) == (B, E, I, d) and tuple(G_down.shape) == (B, E, d, I)
+    n = ctypes.c_size_t()
+    _chk(lib().fxm_saliency_workspace_bytes(E, d, I, ctypes.byref(n)), "fxm_saliency_workspace_bytes")
+    ws = torch.empty(n.value, dtype=torch.uint8, device=W_gate.device)
+    s = torch.empty((E, I), dtype=torch.float32, device=W_gate.device)
+    _chk(lib().fxm_saliency(E, d, I, W_gate.data_ptr(), W_up.data_ptr(), W_down.data_ptr(), G_gate.data_ptr(),
+                            G_up.data_ptr(), G_down.data_ptr(), B, s.data_ptr(), ws.data_ptr(), ws.numel(),
+                            _stream_ptr(stream)), "fxm_saliency")
+    return s
+
+
+def rank_channels(s, stream=None):
+    """Eq. 3's permutation (fxm_rank_channels): s [E,I] fp32 CUDA -> channel_rank [E,I] int32 CUDA."""
+    import torch
+    E, I = s.shape
+    assert s.is_cuda and s.dtype == torch.float32 and s.is_contiguous()
+    out = torch.empty((E, I), dtype=torch.int32, device=s.device)
+    _chk(lib().fxm_rank_channels(E, I, s.data_ptr(), out.data_ptr(), _stream_ptr(stream)), "fxm_rank_channels")
+    return out
 
 
 def ratio_to_width(I: int, num: int, den: int) -> int:
@@ -200,6 +236,27 @@ class Layer:
         _chk(lib().fxm_register_budgets(self._h, t.shape[0], t.ctypes.data, int(bool(require_nested)),
                                         _stream_ptr(stream)), "fxm_register_budgets")
 
+    def sample_budget(self, alpha, gumbel, num, den, return_actions=False, stream=None):
+        """Eq. 6-7 on the device (fxm_sample_budget): alpha, gumbel [E,K] fp32 CUDA (gumbel may be None)."""
+        import torch
+        num = _i32_host(num)
+        K = num.shape[0]
+        assert alpha.is_cuda and alpha.dtype == torch.float32 and alpha.is_contiguous() and tuple(alpha.shape) == (self.E, K)
+        act = torch.empty(self.E, dtype=torch.int32, device=alpha.device) if return_actions else None
+        _chk(lib().fxm_sample_budget(self._h, alpha.data_ptr(), gumbel.data_ptr() if gumbel is not None else None, K,
+                                     num.ctypes.data, int(den), act.data_ptr() if act is not None else None,
+                                     _stream_ptr(stream)), "fxm_sample_budget")
+        return act
+
+    def action_cost(self, alpha, num, den, counts, stream=None):
+        """Eq. 10 on the device (fxm_action_cost) -> 1-element fp32 CUDA tensor."""
+        import torch
+        num = _i32_host(num)
+        out = torch.empty(1, dtype=torch.float32, device=alpha.device)
+        _chk(lib().fxm_action_cost(self._h, alpha.data_ptr(), num.shape[0], num.ctypes.data, int(den), counts.data_ptr(),
+                                   out.data_ptr(), _stream_ptr(stream)), "fxm_action_cost")
+        return out
+
     def select_budget(self, b: int):
         _chk(lib().fxm_select_budget(self._h, int(b)), "fxm_select_budget")
 
@@ -244,6 +301,23 @@ class Layer:
                                           y_shared.data_ptr(), y.data_ptr(), ws.data_ptr(), ws.numel(),
                                           _stream_ptr(stream)), "fxm_moe_ffn_shared")
         return y
+
+    def moe_ffn_router(self, x, logits, k, y_shared=None, out=None, return_routing=False, workspace=None, stream=None):
+        """Forward from router LOGITS [T,E] fp32 (fxm_moe_ffn_router): softmax -> top-k -> renormalise runs on the device
+        in the route kernel.  -> y, or (y, topk_ids, topk_w) with return_routing."""
+        import torch
+        T, d = x.shape
+        assert d == self.d and x.dtype == torch.bfloat16 and x.is_cuda and x.is_contiguous()
+        assert logits.dtype == torch.float32 and logits.is_contiguous() and tuple(logits.shape) == (T, self.E)
+        y = torch.empty((T, d), dtype=torch.bfloat16, device=x.device) if out is None else out
+        ids = torch.empty((T, k), dtype=torch.int32, device=x.device) if return_routing else None
+        w = torch.empty((T, k), dtype=torch.float32, device=x.device) if return_routing else None
+        ws = self.workspace(T, k) if workspace is None else workspace
+        _chk(lib().fxm_moe_ffn_router(self._h, x.data_ptr(), logits.data_ptr(), T, k,
+                                      y_shared.data_ptr() if y_shared is not None else None, y.data_ptr(),
+                                      ids.data_ptr() if ids is not None else None, w.data_ptr() if w is not None else None,
+                                      ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_moe_ffn_router")
+        return (y, ids, w) if return_routing else y
 
     # -- offline clipping (PAPER.md:222) ----------------------------------------------------------------
     def export_clipped(self, r, stream=None):
