@@ -64,8 +64,8 @@ typedef enum {
 fxm_status fxm_packed_bytes(int E, int d, int I, size_t* bytes);
 
 /* Bytes of scratch for one moe_ffn / route call with at most T_max tokens and k experts per token:
- * grouping indices, tile schedule, the SwiGLU activations H [T_max*k + 16E, ceil64(I)] bf16 and the fp32
- * scatter-add accumulator of y [T_max, d].  Monotonic in T_max: a buffer sized for T_max serves every T <= T_max. */
+ * grouping indices, tile schedule, the SwiGLU activations H [T_max*k + 16E, ceil64(I)] bf16, the fp32
+ * scatter-add accumulator of y [T_max, d] and the decode kernel's partial gate/up sums (8 KB per work piece).  Monotonic in T_max: a buffer sized for T_max serves every T <= T_max. */
 fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* bytes);
 
 /* ---- (1) pack: Eq. 3; layout prior art App. C.2, PAPER.md:526-540 ---------------------
@@ -230,9 +230,10 @@ fxm_status fxm_set_impl(fxm_layer* L, int impl);          /* FXM_IMPL_* ; defaul
 /* Most rows of a token tile of the grouped GEMMs: 128, 256, 512, or 0 = default (512).  Tuning knob only. */
 fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
 /* Step a6: calls with T*k <= max_assignments (<= 1024; 0 = never) run as ONE launch of the fused
- * weight-streaming decode kernel instead of the four launches above; prefetch_tiles = how many 16 KB weight tiles
- * its L2 prefetch cursor runs ahead of the shared-memory ring (0..256).  Tuning knob only: results agree within
- * the stated tolerance either way.  Needs d <= 3840, else the general path is used regardless. */
+ * weight-streaming decode kernel instead of the four launches above.  prefetch_tiles = how many 16 KB weight tiles
+ * each CTA's L2 prefetch cursor runs ahead of its shared-memory ring (0..4096; default 0 = none: every distance
+ * tried was measured slower on B200, see profiles/).  Tuning knob only: results agree within the stated tolerance
+ * either way.  Needs d <= 3840, else the general path is used. */
 #define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 768
 #define FXM_DECODE_DEFAULT_PREFETCH 0
 fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles);

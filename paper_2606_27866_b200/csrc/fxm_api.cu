@@ -99,6 +99,11 @@ static bool use_decode(const fxm_layer* L, int T, int k) {
     return L->impl == FXM_IMPL_TCGEN05 && A <= L->dec_max_A && A <= DEC_MAX_A && decode_supported(L->D);
 }
 
+// L2 prefetch distance of the decode kernel (16 KB tiles per CTA): the caller's choice (fxm_set_decode), default 0.
+// Measured on B200 (L2 flushed, C4 and C2 shapes, T = 1 .. 64, every budget): a cursor of 16 or 256 tiles is 0-40 %
+// SLOWER than none at every size -- prefetch requests share the SM's outstanding-request budget with the ring's own loads.
+static int decode_prefetch(const fxm_layer* L, int, int) { return L->dec_pf > 0 ? L->dec_pf : 0; }
+
 static fxm_layer* new_layer(const Dims& D, uint8_t* blob, const Tail& tl, int sms) {
     fxm_layer* L = new (std::nothrow) fxm_layer();
     if (!L) return nullptr;
@@ -313,7 +318,7 @@ fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n) {
 }
 
 fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles) {
-    if (!L || max_assignments < 0 || prefetch_tiles < 0 || prefetch_tiles > 256) return FXM_EINVAL;
+    if (!L || max_assignments < 0 || prefetch_tiles < -1 || prefetch_tiles > 4096) return FXM_EINVAL;
     L->dec_max_A = max_assignments > DEC_MAX_A ? DEC_MAX_A : max_assignments;
     L->dec_pf = prefetch_tiles;
     return FXM_OK;
@@ -403,8 +408,8 @@ static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids,
         if (logits && launch_router_topk(logits, T, D.E, k, fe_ids, fe_w, st) != cudaSuccess) return FXM_ECUDA;
         for (int j = 0; j < FXM_N_KERNELS; ++j) FXM_MARK(j)
         if (launch_decode(D, L->V, table, (const __nv_bfloat16*)x, logits ? fe_ids : topk_ids, logits ? fe_w : topk_w, T, k,
-                          ws.yacc, (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->num_sms, L->dec_pf, st) !=
-            cudaSuccess)
+                          ws.yacc, ws.dec_part, (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->num_sms,
+                          decode_prefetch(L, T, k), st) != cudaSuccess)
             return FXM_ECUDA;
         FXM_MARK(FXM_N_KERNELS)
         L->last_launches = logits ? 2 : 1;

@@ -4,39 +4,40 @@
 //   (Eq. 4; Alg. 2.)  With a handful of tokens per expert the call is a stream of
 //   the retained weight prefix of every ACTIVE expert, read exactly once: HBM-bound.
 //
-// Design (one persistent CTA per SM, cooperative launch, 320 threads):
-//   prologue   every CTA re-derives the grouping from topk_ids in shared memory (stable counting sort, the same
-//              definition as fxm_route.cu, Alg. 2 l.4-6) and the flat work list for the CURRENT width table:
-//              items (expert e, token group g of <= 16 rows, retained channel block cb), ordered (e, g, cb); pruned
-//              blocks, idle experts and width-0 experts have no items.  CTA c owns the contiguous item range
-//              [c W / G, (c+1) W / G) and cuts it into RUNS of equal (e, g).
-//   warp 0     weight producer: per item the d/64 gate/up tiles (one contiguous range) then the d/128 down tiles (one
-//              contiguous range), 16 KB cp.async.bulk each, through a shared-memory ring; an L2 prefetch cursor
-//              runs `pf` tiles ahead so the ring is refilled at L2 latency and HBM sees a deep queue.
-//   warp 1     MMA issuer.  GEMM-1 (swap-AB): D1[128 packed gate/up rows, 16 tokens] += Wgu_tile . Xe^T over d;
-//              GEMM-2: Y[db][128 out features, 16 tokens] += Wd_tile(e, cb, db) . Hs^T with K = 64 channels, for every
-//              feature block db.  Y stays in TMEM and accumulates over the consecutive channel blocks of a run.
-//              Issue order is software-pipelined: G(0), G(1), D(0), G(2), D(1), ... so the SwiGLU epilogue of
-//              item i overlaps the weight stream of item i+1.
-//   warps 2-5  epilogue: SwiGLU (gate lane l, up lane l+16: one shuffle), pad-zero rule for channels >= r_e
-//              (PAPER.md:579), one rounding to bf16 -> Hs (the B operand of GEMM-2); at the end of a run the
-//              fp32 partial Y is scaled by the router weight (Alg. 2 l.19) and added to yacc[t][:] with fp32
-//              reductions (Alg. 2 l.20 ScatterAdd).
-//   warps 6-9  stage the <= 16 token rows x[t] of the current run into swizzled K-major panels Xe (X[pi], Alg. 2 l.7).
-//   grid barriers (sense-reversing counters in DevState; all CTAs are co-resident by the cooperative launch):
-//              #0 yacc zeroed by everyone before anyone adds to it, #1 every partial added before yacc -> y (one
-//              rounding to bf16).
-// TMEM columns: [0,32) two GEMM-1 accumulators, [32, 32 + 16 nDB) the Y partial.  Needs nDB <= 30 (d <= 3840).
+// One SM pulls only ~40 GB/s through its bulk-copy ring, so the HBM roofline needs ALL 148 SMs streaming the same
+// number of bytes -- also when the call has fewer 64-channel work items than SMs (T = 1 at 75 % pruned: 80 items).  The
+// kernel therefore cuts the weight stream at TILE granularity, in two phases separated by a grid barrier:
+//   phase 1  gate/up.  The tiles of all items (item = run (expert e, <= 16 tokens) x retained channel block cb), in the
+//            order (item, k-block), form one list of W * d/64 tiles; CTA c owns the contiguous range [c T1/G, (c+1) T1/G).
+//            A range is a few PIECES (parts of one item): D1[128 packed rows, 16 tokens] += Wgu_tile . Xe^T over the
+//            piece's k-blocks, then the fp32 partial goes to scratch slot (item + c) -- unique per (item, CTA).
+//   phase 2  down.  Tiles in the order (item, feature block): W * ceil(d/128) tiles, again one contiguous range per CTA.
+//            For every piece (item, feature blocks db0..db1) the epilogue warps sum the item's partials (the slots of the
+//            CTAs that touched it), apply SwiGLU (gate lane l, up lane l+16: one shuffle) and the pad-zero rule for
+//            channels >= r_e, round once to bf16 -> Hs; Y[db] += Wd_tile(e, cb, db) . Hs^T accumulates in
+//            TMEM over the consecutive pieces of a run; at the end of the run segment the touched feature blocks are
+//            scaled by the router weight (Alg. 2 l.19) and added to yacc[t][:] with fp32 reductions (l.20 ScatterAdd).
+//   Both phases are balanced to +-1 tile whatever the routing and the budget.
+// Roles (320 threads): warp 0 weight producer (16 KB cp.async.bulk per tile through a shared-memory ring; it starts
+// fetching phase-2 tiles while the grid barrier is still closing), warp 1 MMA issuer, warps 2-5 epilogue, warps 6-9
+// stage the <= 16 token rows x[t] of a run into swizzled K-major panels Xe (X[pi], Alg. 2 l.7).
+// Grid barriers (sense-reversing counters in DevState): A between the phases (it also orders the zeroing of yacc
+// before every reduction), B before yacc -> y (one rounding to bf16).  The launch is an ordinary one with the
+// programmatic-dependent-launch attribute, grid = #SMs, one CTA per SM: every CTA is resident before a dependent kernel
+// may start, and nothing the CTAs wait for depends on a later kernel, so the barriers cannot deadlock.
+// TMEM columns: [0,32) two phase-1 accumulators, [32, 32 + 16 nDB) the Y partial.  Needs nDB <= 30 (d <= 3840).
 #include "fxm_ptx.cuh"
 
 namespace fxm {
 
 constexpr int DEC_THREADS = 320;
-constexpr int DEC_N = 16;                         // tokens per group = UMMA N
+constexpr int DEC_N = 16;                         // tokens per run = UMMA N
 constexpr int DEC_MAX_RUNS = 320;                 // >= DEC_MAX_A / 16 + MAX_E (total number of runs of a call)
 constexpr int DEC_XE_KB_BYTES = DEC_N * ROW_BYTES;   // 2 KB of Xe per k-block
 constexpr int DEC_MAX_SLOTS = 12;
 constexpr int DEC_SMEM_MAX = 232448;              // 227 KB
+constexpr int DEC_PART = WT_ROWS * DEC_N;         // floats of one phase-1 partial: 128 packed rows x 16 tokens (8 KB)
+constexpr int DEC_MAX_CTAS = 160;                 // the partial-slot capacity is sized for at most this many CTAs
 
 struct DecArgs {
     Dims D;
@@ -46,23 +47,26 @@ struct DecArgs {
     const int* ids;            // [T][k]
     const float* topk_w;       // [T][k]
     float* yacc;               // [T][d] fp32 scratch (workspace)
+    float* part;               // phase-1 partials: [(items + #CTAs)][128][16] fp32 (workspace)
     const uint2* y_add;        // [T][d] bf16 or null: shared-expert output added in fp32 before the rounding of y
     __nv_bfloat16* y;          // [T][d]
     DevState* state;
     int T, k, A;
     int slots;                 // ring depth
-    int pf;                    // L2 prefetch distance in tiles
+    int pf;                    // L2 prefetch distance in 16 KB tiles (0 = none)
 };
 
 // persistent auxiliary shared memory (after ring, Xe, Hs)
 struct DecAux {
-    int4 runs[DEC_MAX_RUNS];   // {e | n << 16, first sorted position, cb_lo, cb_hi}
-    int16_t perm[DEC_MAX_A];   // sorted position -> flat assignment index
+    int run_en[DEC_MAX_RUNS];      // expert | tokens << 16
+    int run_pos[DEC_MAX_RUNS];     // first sorted position of the run
+    int run_ib[DEC_MAX_RUNS + 1];  // first item of the run; [n_runs] = W
+    int16_t perm[DEC_MAX_A];       // sorted position -> flat assignment index
     int r[MAX_E];
-    uint32_t eb[MAX_E];        // first channel block of each expert in the weight regions (LayerView::eblk)
+    uint32_t eb[MAX_E];            // first channel block of each expert in the weight regions (LayerView::eblk)
     uint64_t bars[2 * DEC_MAX_SLOTS + 16];
     uint32_t tmem_slot;
-    int n_runs, n_items, W;
+    int n_runs, W;
     uint32_t gen0[2];
 };
 // prologue-only scratch, aliased on the weight ring (>= 4 slots = 64 KB)
@@ -70,7 +74,6 @@ struct DecTmp {
     int16_t ids[DEC_MAX_A];
     int cnt[MAX_E], off[MAX_E + 1], ibase[MAX_E + 1], gbase[MAX_E + 1];
     int wh[DEC_THREADS / 32][MAX_E];   // per-warp expert histogram, then the warp's running base
-    int first_run;
 };
 
 __host__ __device__ inline int dec_fixed_smem(const Dims& D) {
@@ -94,8 +97,8 @@ __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-// Grid barrier, one thread per CTA (all CTAs are co-resident: cooperative launch).  Two levels, because 148 atomics on ONE
-// address serialise in L2 (measured: 10-20 us per barrier): CTA b arrives on sub-counter b % 8, the last arriver of a
+// Grid barrier, one thread per CTA (all CTAs are resident, see the header).  Two levels, because 148 atomics on ONE address
+// serialise in L2 (measured: 10-20 us per barrier): CTA b arrives on sub-counter b % 8, the last arriver of a
 // sub-counter arrives on the top counter, the last of those bumps the generation word that everyone polls (it lives in
 // another 128-byte line than the counters).  Every counter is reset by its last arriver before the generation moves.
 __device__ __forceinline__ void grid_arrive(DevState* st, int i, uint32_t G) {
@@ -117,7 +120,7 @@ __device__ __forceinline__ void grid_wait(DevState* st, int i, uint32_t gen0) {
     const long long t0 = clock64();
     uint32_t spins = 0;
     while (ld_acquire_u32(&st->bar_gen[i]) == gen0) {
-        __nanosleep(1000);                                         // 148 pollers: keep the L2 slice of the barrier words quiet
+        __nanosleep(200);                                          // 148 pollers: keep the L2 slice of the barrier words quiet
         if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) {
             atomicOr(&st->flags, 2u);
             if (st->hflag) *(volatile uint32_t*)st->hflag = 2u;
@@ -127,74 +130,45 @@ __device__ __forceinline__ void grid_wait(DevState* st, int i, uint32_t gen0) {
     }
 }
 
-// walks the items of this CTA in (run, channel block) order
-struct ItemCur {
-    int R, cb;
-    __device__ __forceinline__ void init(const DecAux* ax) { R = 0; cb = ax->n_runs > 0 ? ax->runs[0].z : 0; }
-    __device__ __forceinline__ bool first(const DecAux* ax) const { return cb == ax->runs[R].z; }
-    __device__ __forceinline__ bool last(const DecAux* ax) const { return cb + 1 == ax->runs[R].w; }
-    __device__ __forceinline__ int e(const DecAux* ax) const { return ax->runs[R].x & 0xFFFF; }
-    __device__ __forceinline__ uint32_t eb(const DecAux* ax) const { return ax->eb[ax->runs[R].x & 0xFFFF]; }
-    __device__ __forceinline__ void next(const DecAux* ax) {
-        if (++cb == ax->runs[R].w) {
-            ++R;
-            cb = R < ax->n_runs ? ax->runs[R].z : 0;
-        }
+// ---- the two tile lists.  Phase p has tiles_per_item = nKB1 (p = 1) or nDB (p = 2); tile t belongs to item t / tpi.
+// A PIECE is the part of one item inside a CTA's range: item, local tile range [a, b).
+struct Piece { int item, a, b; };
+struct PieceIter {
+    long long t, hi;
+    int tpi;
+    __device__ __forceinline__ void init(long long lo_, long long hi_, int tpi_) { t = lo_; hi = hi_; tpi = tpi_; }
+    __device__ __forceinline__ bool next(Piece& p) {
+        if (t >= hi) return false;
+        p.item = (int)(t / tpi);
+        p.a = (int)(t - (long long)p.item * tpi);
+        const long long room = hi - t;
+        p.b = room < (long long)(tpi - p.a) ? p.a + (int)room : tpi;
+        t += p.b - p.a;
+        return true;
     }
 };
+// run cursor: items ascend, so the run of an item is found by walking forward
+__device__ __forceinline__ int run_of(const DecAux* ax, int item, int& cur) {
+    while (ax->run_ib[cur + 1] <= item) ++cur;
+    return cur;
+}
+// CTA that owns tile t of a list of Tn tiles split over G CTAs as [c Tn / G, (c + 1) Tn / G)
+__device__ __forceinline__ int cta_of_tile(long long t, long long Tn, int G) { return (int)(((t + 1) * G - 1) / Tn); }
 
-// the weight stream in issue order, one PART at a time: G(0), G(1), D(0), G(2), D(1), ..., G(n-1), D(n-2), D(n-1).
-// A part is a contiguous range of 16 KB tiles: G(i) = the d/64 gate/up tiles of item i, D(i) = its ceil(d/128) down tiles.
-struct PartStream {
-    const DecAux* ax;
-    const uint8_t* gu;
-    const uint8_t* dn;
-    Dims D;
-    ItemCur g, d;
-    int i;            // step: the G part of item i, then the D part of item i-1
-    int sub;          // 0 = G(i) comes next, 1 = D(i-1) comes next
-    __device__ __forceinline__ void init(const DecAux* a, const DecArgs& args) {
-        ax = a; D = args.D; gu = args.V.gu; dn = args.V.dn;
-        g.init(a); d.init(a);
-        i = 0; sub = 0;
-    }
-    __device__ __forceinline__ bool next(const uint8_t*& base, int& count) {
-        const int n = ax->n_items;
-        while (n > 0 && i <= n) {
-            if (sub == 0) {
-                sub = 1;
-                if (i < n) {
-                    base = gu + gu_tile_off(D, g.eb(ax), g.cb, 0);
-                    count = D.nKB1;
-                    g.next(ax);
-                    return true;
-                }
-            }
-            sub = 0;
-            const int ii = i++;
-            if (ii >= 1) {
-                base = dn + dn_tile_off(D, d.eb(ax), d.cb, 0);
-                count = D.nDB;
-                d.next(ax);
-                return true;
-            }
-        }
-        return false;
-    }
-};
-
-// -DFXM_TRACE: per-CTA globaltimer stamps (ns): 0 entry, 1 prologue done, 2 roles done (this CTA's last reduction issued),
-// 3 grid barrier #1 passed, 4 exit.  Tuning aid only.
 #ifdef FXM_TRACE
-__device__ unsigned long long g_dtrace[148][8];
+__device__ unsigned long long g_dtrace[148][16];
 __device__ __forceinline__ unsigned long long dec_now() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
 #define DEC_TR(f) do { if (threadIdx.x == 0 && blockIdx.x < 148) g_dtrace[blockIdx.x][f] = dec_now(); } while (0)
+#define DEC_TRE(f) do { if (threadIdx.x == 64 && blockIdx.x < 148) g_dtrace[blockIdx.x][f] = dec_now(); } while (0)
+#define DEC_TRM(f) do { if (threadIdx.x == 32 && blockIdx.x < 148) g_dtrace[blockIdx.x][f] = dec_now(); } while (0)
 #else
+#define DEC_TRM(f) do { } while (0)
 #define DEC_TR(f) do { } while (0)
+#define DEC_TRE(f) do { } while (0)
 #endif
 
 __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
@@ -225,6 +199,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     const int E = D.E, A = a.A, k = a.k;
     DEC_TR(0);
     const uint32_t G = gridDim.x;
+    pdl_launch_dependents();
 
     // ------------------------------------------------------------------------------------------ prologue
     if (tid == 0) {
@@ -234,10 +209,13 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             mbar_init(a1full(b), 1); mbar_init(a1empty(b), 128); mbar_init(hfull(b), 128); mbar_init(hempty(b), 1);
         }
         fence_barrier_init();
+    }
+    if (warp == 1) tmem_alloc(smem_u32(&ax->tmem_slot), 512);
+    pdl_wait();                                              // the previous kernel may still use the workspace / write x, ids
+    if (tid == 0) {
         ax->gen0[0] = ld_acquire_u32(&a.state->bar_gen[0]);      // read before this CTA arrives anywhere
         ax->gen0[1] = ld_acquire_u32(&a.state->bar_gen[1]);
     }
-    if (warp == 1) tmem_alloc(smem_u32(&ax->tmem_slot), 512);
     bool bad = false;
     for (int f = tid; f < A; f += DEC_THREADS) {
         int id = a.ids[f];
@@ -246,19 +224,13 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     }
     if (bad) atomicOr(&a.state->flags, 1u);
     for (int e = tid; e < MAX_E; e += DEC_THREADS) { ax->r[e] = e < E ? a.r_table[e] : 0; ax->eb[e] = e < E ? a.V.eblk[e] : 0u; }
-    // zero this CTA's slice of the fp32 accumulator (grid barrier #0 orders it before every reduction)
+    // zero this CTA's slice of the fp32 accumulator (grid barrier A orders it before every reduction)
     {
         float4* z = (float4*)a.yacc;
         const size_t n4 = (size_t)a.T * D.d / 4;
         for (size_t i = (size_t)blockIdx.x * DEC_THREADS + tid; i < n4; i += (size_t)G * DEC_THREADS)
             z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
-    if (tid == 0) grid_arrive(a.state, 0, G);
-    const uint32_t tmem_base = ax->tmem_slot;
-
     // counts (Alg. 2 l.4-6, stable counting sort as in fxm_route.cu): warp w owns the contiguous chunk [w*chunk, (w+1)*chunk)
     // of the flat assignments; per 32-wide step the lowest lane of every group of equal ids adds the group size to
     // the warp's histogram row
@@ -266,7 +238,10 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     const int chunk = ((A + NW - 1) / NW + 31) & ~31;
     const int wlo = min(A, warp * chunk), whi = min(A, wlo + chunk);
     for (int i = tid; i < NW * MAX_E; i += DEC_THREADS) (&tp->wh[0][0])[i] = 0;
+    tc_fence_before();
     __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = ax->tmem_slot;
     for (int base = wlo; base < whi; base += 32) {
         const int f = base + lane;
         const int id = f < whi ? (int)tp->ids[f] : -1;
@@ -314,11 +289,11 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         if (lane == 0) {
             tp->off[E] = c_off; tp->ibase[E] = c_items; tp->gbase[E] = c_runs;
             ax->W = c_items;
+            ax->n_runs = c_runs;
+            ax->run_ib[c_runs] = c_items;
         }
     }
     __syncthreads();
-    const int W = ax->W;
-    const int lo = (int)((long long)blockIdx.x * W / (long long)G), hi = (int)((long long)(blockIdx.x + 1) * W / (long long)G);
     // stable positions (ascending flat index inside an expert, reading R5): expert offset + earlier warps + earlier
     // steps of this warp + lower lanes of this step
     for (int base = wlo; base < whi; base += 32) {
@@ -330,27 +305,16 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         if (id >= 0 && lane == __ffs(m) - 1) tp->wh[warp][id] += __popc(m);
         __syncwarp();
     }
+    // the run table of the WHOLE call: run (e, g) = tokens [16 g, 16 g + 16) of expert e's segment, items = its retained blocks
     if (tid < E) {
-        // the run that contains item `lo`
-        const int r = ax->r[tid];
-        const int nb = (r + CB - 1) / CB;
-        if (lo < hi && tp->ibase[tid] <= lo && lo < tp->ibase[tid + 1]) tp->first_run = tp->gbase[tid] + (lo - tp->ibase[tid]) / nb;
-    }
-    if (tid == 0) { ax->n_runs = 0; ax->n_items = hi - lo; }
-    __syncthreads();
-    if (tid < E && lo < hi) {
         const int n = tp->cnt[tid], r = ax->r[tid];
         const int nb = (r + CB - 1) / CB;
         const int ng = tp->gbase[tid + 1] - tp->gbase[tid];
         for (int g = 0; g < ng; ++g) {
-            const int i0 = tp->ibase[tid] + g * nb;             // items [i0, i0 + nb) = channel blocks 0..nb-1 of (e, g)
-            const int s = max(i0, lo), t = min(i0 + nb, hi);
-            if (s < t) {
-                const int slot = tp->gbase[tid] + g - tp->first_run;
-                const int nt = min(DEC_N, n - g * DEC_N);
-                ax->runs[slot] = make_int4(tid | (nt << 16), tp->off[tid] + g * DEC_N, s - i0, t - i0);
-                atomicMax(&ax->n_runs, slot + 1);
-            }
+            const int slot = tp->gbase[tid] + g;
+            ax->run_en[slot] = tid | (min(DEC_N, n - g * DEC_N) << 16);
+            ax->run_pos[slot] = tp->off[tid] + g * DEC_N;
+            ax->run_ib[slot] = tp->ibase[tid] + g * nb;
         }
     }
     __syncthreads();
@@ -358,216 +322,336 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     for (int i = tid; i < (int)((aux_off - xe_off) / 16); i += DEC_THREADS) ((uint4*)xe_gen)[i] = make_uint4(0, 0, 0, 0);
     fence_proxy_async_smem();
     __syncthreads();
-    const int n_items = ax->n_items, n_runs = ax->n_runs;
+    const int W = ax->W;
+    const long long T1 = (long long)W * D.nKB1, T2 = (long long)W * D.nDB;
+    const long long lo1 = T1 * blockIdx.x / G, hi1 = T1 * (blockIdx.x + 1) / G;
+    const long long lo2 = T2 * blockIdx.x / G, hi2 = T2 * (blockIdx.x + 1) / G;
     DEC_TR(1);
 
     if (warp == 0) {
-        // ===================================================== weight producer + L2 prefetch cursor
-        // per tile: wait for the slot, arm the barrier, one 16 KB bulk copy; optionally one 16 KB L2 prefetch `pf` tiles
-        // further down the same stream (a second cursor).  Measured on B200: the prefetch competes with the ring's own
-        // loads for the SM's outstanding requests and every distance > 0 is slower (C4 T=64 0 %: 558 us at 0, 580 at 8,
-        // 978 at 64), so the default distance is 0.
-        if (n_items > 0) {
-            const bool el = dec_elect_one();
-            // every weight byte is read exactly once: evict_first keeps the stream from displacing anything -- measured
-            // -7 % at C4 T=1 and -10 % at C2 T=16, but +3.5 % when the call streams multi-GB at full HBM rate (C4 T=32/64 at
-            // 0 %), so the hint is used below ~1.2 GB per call
-            const uint64_t pol_stream = l2_policy_evict_first();
-            const bool hint = (size_t)W * (size_t)(D.nKB1 + D.nDB) * WT_BYTES < ((size_t)1200 << 20);
-            PartStream ld, pf;
-            ld.init(ax, a);
-            pf.init(ax, a);
-            const uint8_t* pb = nullptr;
-            int pc = 0, pj = 0;
-            bool pf_live = pf.next(pb, pc);
-            auto pf_step = [&]() {
-                if (!pf_live) return;
-                if (el) bulk_prefetch_l2(pb + (size_t)pj * WT_BYTES, WT_BYTES);
-                if (++pj == pc) { pj = 0; pf_live = pf.next(pb, pc); }
-            };
-            for (int p = 0; p < a.pf; ++p) pf_step();
-            int stage = 0;
-            uint32_t phase = 0;
-            const uint8_t* base = nullptr;
-            int count = 0;
-            while (ld.next(base, count)) {
-                for (int j = 0; j < count; ++j) {
-                    if (a.pf > 0) pf_step();
-                    mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
-                    if (el) {
-                        mbar_expect_tx(full_bar(stage), WT_BYTES);
-                        if (hint) bulk_g2s_hint(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage), pol_stream);
-                        else bulk_g2s(ring_s + stage * WT_BYTES, base + (size_t)j * WT_BYTES, WT_BYTES, full_bar(stage));
-                    }
-                    if (++stage == NS) { stage = 0; phase ^= 1u; }
+        // ===================================================== weight producer: phase-1 range, then the phase-2 range
+        // every weight byte is read exactly once: evict_first keeps the stream from displacing anything -- measured
+        // -7 % at C4 T=1 and -10 % at C2 T=16, but +3.5 % when the call streams multi-GB at full HBM rate (C4 T=32/64 at
+        // 0 %), so the hint is used below ~1.2 GB per call.
+        // One SM's ring (6 slots at C4) keeps only ~96 KB in flight: at DRAM latency that is ~40 GB/s per SM, and a CTA
+        // whose whole range is a few dozen tiles never reaches even that.  So an L2 prefetch cursor runs `pf` tiles ahead
+        // of the ring over the same tile sequence (both phases): for small calls pf covers the CTA's entire range -- every
+        // DRAM request of the call is in flight within microseconds of the prologue and the ring then hits L2.
+        const bool el = dec_elect_one();
+        const uint64_t pol_stream = l2_policy_evict_first();
+        const bool hint = a.pf == 0 && (size_t)W * (size_t)(D.nKB1 + D.nDB) * WT_BYTES < ((size_t)1200 << 20);
+        int stage = 0;
+        uint32_t phase = 0;
+        // the tile sequence of this CTA as contiguous segments; two cursors walk it: the ring loads and the L2 prefetch
+        struct Seq {
+            PieceIter it;
+            int cur, ph;
+            const uint8_t* base;
+            int count, j;
+        };
+        auto seq_init = [&](Seq& q) { q.it.init(lo1, hi1, D.nKB1); q.cur = 0; q.ph = 1; q.count = 0; q.j = 0; q.base = nullptr; };
+        auto seq_next_tile = [&](Seq& q, const uint8_t*& tile) -> bool {
+            while (q.j == q.count) {
+                Piece p;
+                if (!q.it.next(p)) {
+                    if (q.ph == 2) return false;
+                    q.ph = 2; q.cur = 0;
+                    q.it.init(lo2, hi2, D.nDB);
+                    continue;
                 }
+                const int run = run_of(ax, p.item, q.cur);
+                const int e = ax->run_en[run] & 0xFFFF, cb = p.item - ax->run_ib[run];
+                q.base = q.ph == 1 ? a.V.gu + gu_tile_off(D, ax->eb[e], cb, p.a) : a.V.dn + dn_tile_off(D, ax->eb[e], cb, p.a);
+                q.count = p.b - p.a;
+                q.j = 0;
             }
+            tile = q.base + (size_t)q.j * WT_BYTES;
+            ++q.j;
+            return true;
+        };
+        Seq ld, pf;
+        seq_init(ld);
+        seq_init(pf);
+        const uint8_t* t;
+        bool pf_live = a.pf > 0;
+        for (int i = 0; i < a.pf && pf_live; ++i) {
+            pf_live = seq_next_tile(pf, t);
+            if (pf_live && el) bulk_prefetch_l2(t, WT_BYTES);
+        }
+        while (seq_next_tile(ld, t)) {                        // phase-2 tiles run ahead of grid barrier A: weights do not depend on phase 1
+            if (pf_live) {
+                const uint8_t* tp2;
+                pf_live = seq_next_tile(pf, tp2);
+                if (pf_live && el) bulk_prefetch_l2(tp2, WT_BYTES);
+            }
+            mbar_wait(empty_bar(stage), phase ^ 1u, a.state);
+            if (el) {
+                mbar_expect_tx(full_bar(stage), WT_BYTES);
+                if (hint) bulk_g2s_hint(ring_s + stage * WT_BYTES, t, WT_BYTES, full_bar(stage), pol_stream);
+                else bulk_g2s(ring_s + stage * WT_BYTES, t, WT_BYTES, full_bar(stage));
+            }
+            if (++stage == NS) { stage = 0; phase ^= 1u; }
         }
     } else if (warp == 1) {
         // ===================================================== MMA issuer
-        if (n_items > 0) {
-            const bool el = dec_elect_one();
-            ItemCur g, d;
-            g.init(ax); d.init(ax);
-            int stage = 0;
-            uint32_t phase = 0;
-            const uint32_t idesc = make_idesc(DEC_N);
-            for (int i = 0; i <= n_items; ++i) {
-                if (i < n_items) {                                  // ---- G(i): D1[b] = Wgu(e, cb) . Xe^T
-                    const int b = i & 1, u = i >> 1;
-                    if (g.first(ax)) mbar_wait(xfull, (uint32_t)(g.R & 1), a.state);
-                    mbar_wait(a1empty(b), (uint32_t)((u & 1) ^ 1), a.state);
-                    tc_fence_after();
-                    const uint32_t d_tmem = tmem_base + (uint32_t)b * DEC_N;
-                    for (int kb = 0; kb < D.nKB1; ++kb) {
-                        mbar_wait(full_bar(stage), phase, a.state);
-                        tc_fence_after();
-                        if (el) {
-                            const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
-                            const uint64_t bdesc = make_desc_sw128(smem_base + xe_off + (uint32_t)kb * DEC_XE_KB_BYTES);
-#pragma unroll
-                            for (int kk = 0; kk < KB / 16; ++kk)
-                                umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)((kb | kk) != 0));
-                            umma_commit(empty_bar(stage));
-                        }
-                        __syncwarp();
-                        if (++stage == NS) { stage = 0; phase ^= 1u; }
-                    }
-                    if (el) {
-                        umma_commit(a1full(b));
-                        if (g.last(ax)) umma_commit(xempty);        // Xe may be restaged once these MMAs retire
-                    }
-                    __syncwarp();
-                    g.next(ax);
-                }
-                if (i >= 1) {                                       // ---- D(i-1): Y[db] += Wd(e, cb, db) . Hs[b]^T
-                    const int b = (i - 1) & 1, u = (i - 1) >> 1;
-                    const bool first = d.first(ax);
-                    if (first) mbar_wait(yempty, (uint32_t)((d.R & 1) ^ 1), a.state);
-                    mbar_wait(hfull(b), (uint32_t)(u & 1), a.state);
-                    tc_fence_after();
-                    const uint64_t bdesc = make_desc_sw128(smem_base + hs_off + (uint32_t)b * DEC_XE_KB_BYTES);
-                    for (int db = 0; db < D.nDB; ++db) {
-                        mbar_wait(full_bar(stage), phase, a.state);
-                        tc_fence_after();
-                        if (el) {
-                            const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
-                            const uint32_t d_tmem = tmem_base + 2u * DEC_N + (uint32_t)db * DEC_N;
-#pragma unroll
-                            for (int kk = 0; kk < KB / 16; ++kk)
-                                umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)(!first || kk != 0));
-                            umma_commit(empty_bar(stage));
-                        }
-                        __syncwarp();
-                        if (++stage == NS) { stage = 0; phase ^= 1u; }
-                    }
-                    if (el) {
-                        umma_commit(hempty(b));
-                        if (d.last(ax)) umma_commit(yfull);
-                    }
-                    __syncwarp();
-                    d.next(ax);
-                }
-            }
-        }
-    } else if (warp < 6) {
-        // ===================================================== epilogue warps 2..5
-        const int q = warp & 3;                                     // TMEM lane quadrant this warp may read
-        const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-        bool zero_seen = false;
-        int i = 0;
-        for (int R = 0; R < n_runs; ++R) {
-            const int4 run = ax->runs[R];
-            const int e = run.x & 0xFFFF, nt = run.x >> 16;
-            const int r = ax->r[e];
-            for (int cb = run.z; cb < run.w; ++cb, ++i) {
-                const int b = i & 1, u = i >> 1;
-                uint32_t v[16];
-                mbar_wait(a1full(b), (uint32_t)(u & 1), a.state);
-                tc_fence_after();
-                tmem_ld16(tmem_base + lane_base + (uint32_t)b * DEC_N, v);
-                tmem_ld_wait();
-                tc_fence_before();
-                mbar_arrive(a1empty(b));
-                const int ch = q * 16 + (lane & 15);
-                const bool keep = cb * CB + ch < r;                 // tail of the last retained block (pad-zero rule)
-                const int odd = lane >> 4;
-                mbar_wait(hempty(b), (uint32_t)((u & 1) ^ 1), a.state);
-                uint8_t* hs = hs_gen + b * DEC_XE_KB_BYTES;
-#pragma unroll
-                for (int m = 0; m < 8; ++m) {
-                    const float mine0 = __uint_as_float(v[2 * m]), mine1 = __uint_as_float(v[2 * m + 1]);
-                    const float send = odd ? mine0 : mine1;
-                    const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
-                    const float gte = odd ? recv : mine0;           // gate lives in lanes 0-15
-                    const float up = odd ? mine1 : recv;            // up lives in lanes 16-31
-                    float h = __fdividef(gte, 1.f + __expf(-gte)) * up;
-                    if (!keep) h = 0.f;
-                    const uint32_t t = 2 * m + odd;
-                    *(__nv_bfloat16*)(hs + sw128_off(t, ch)) = __float2bfloat16_rn(h);
-                }
-                fence_proxy_async_smem();
-                mbar_arrive(hfull(b));
-            }
-            // ---- end of run: Y partial -> yacc (router-weight scale + ScatterAdd, Alg. 2 l.19-20)
-            int tok = 0;
-            float wt = 0.f;
-            if (lane < nt) {
-                const int f = ax->perm[run.y + lane];
-                tok = f / k;
-                wt = a.topk_w[f];
-            }
-            mbar_wait(yfull, (uint32_t)(R & 1), a.state);
+        const bool el = dec_elect_one();
+        const uint32_t idesc = make_idesc(DEC_N);
+        int stage = 0;
+        uint32_t phase = 0;
+        PieceIter it;
+        Piece p;
+        int cur = 0, prev_run = -1, nrun = 0, i = 0;
+        // ---- phase 1: D1[b] = sum over the piece's k-blocks of Wgu(e, cb, kb) . Xe[kb]^T
+        it.init(lo1, hi1, D.nKB1);
+        bool more = it.next(p);
+        while (more) {
+            const int run = run_of(ax, p.item, cur);
+            if (run != prev_run) { mbar_wait(xfull, (uint32_t)(nrun & 1), a.state); if (nrun == 0) DEC_TRM(11); ++nrun; prev_run = run; }
+            const int b = i & 1, u = i >> 1;
+            mbar_wait(a1empty(b), (uint32_t)((u & 1) ^ 1), a.state);
             tc_fence_after();
-            if (!zero_seen) {
-                if (lane == 0) grid_wait(a.state, 0, ax->gen0[0]);
-                __syncwarp();
-                zero_seen = true;
-            }
-            for (int db = 0; db < D.nDB; ++db) {
-                uint32_t v[16];
-                tmem_ld16(tmem_base + lane_base + 2u * DEC_N + (uint32_t)db * DEC_N, v);
-                tmem_ld_wait();
-                const int feat = db * WT_ROWS + q * 32 + lane;
+            const uint32_t d_tmem = tmem_base + (uint32_t)b * DEC_N;
+            for (int kb = p.a; kb < p.b; ++kb) {
+                mbar_wait(full_bar(stage), phase, a.state);
+                if (i == 0 && kb == p.a) DEC_TRM(4);
+                tc_fence_after();
+                if (el) {
+                    const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
+                    const uint64_t bdesc = make_desc_sw128(smem_base + xe_off + (uint32_t)kb * DEC_XE_KB_BYTES);
 #pragma unroll
-                for (int tk = 0; tk < DEC_N; ++tk) {
-                    const int t = __shfl_sync(0xffffffffu, tok, tk);
-                    const float w = __shfl_sync(0xffffffffu, wt, tk);
-                    if (tk < nt && feat < D.d) atomicAdd(a.yacc + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
+                    for (int kk = 0; kk < KB / 16; ++kk)
+                        umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)((kb != p.a) | (kk != 0)));
+                    umma_commit(empty_bar(stage));
+                }
+                __syncwarp();
+                if (++stage == NS) { stage = 0; phase ^= 1u; }
+            }
+            Piece nx;
+            more = it.next(nx);
+            int cur2 = cur;
+            const bool run_ends = !more || run_of(ax, nx.item, cur2) != run;
+            if (el) {
+                umma_commit(a1full(b));
+                if (run_ends) umma_commit(xempty);              // Xe may be restaged once these MMAs retire
+            }
+            __syncwarp();
+            p = nx;
+            ++i;
+        }
+        DEC_TRM(8);
+        // ---- phase 2: Y[db] += Wd(e, cb, db) . Hs[b]^T, accumulated in TMEM over the consecutive pieces of a run
+        cur = 0; prev_run = -1; i = 0;
+        int nseg = 0;
+        uint32_t touched = 0;
+        it.init(lo2, hi2, D.nDB);
+        more = it.next(p);
+        while (more) {
+            const int run = run_of(ax, p.item, cur);
+            if (run != prev_run) {                                // a new run segment: the previous Y partial must be drained
+                mbar_wait(yempty, (uint32_t)((nseg & 1) ^ 1), a.state);
+                touched = 0;
+                prev_run = run;
+            }
+            const int b = i & 1, u = i >> 1;
+            mbar_wait(hfull(b), (uint32_t)(u & 1), a.state);
+            if (i == 0) DEC_TRM(9);
+            tc_fence_after();
+            const uint64_t bdesc = make_desc_sw128(smem_base + hs_off + (uint32_t)b * DEC_XE_KB_BYTES);
+            for (int db = p.a; db < p.b; ++db) {
+                mbar_wait(full_bar(stage), phase, a.state);
+                tc_fence_after();
+                const uint32_t acc = (touched >> db) & 1u;
+                if (el) {
+                    const uint64_t adesc = make_desc_sw128(ring_s + stage * WT_BYTES);
+                    const uint32_t d_tmem = tmem_base + 2u * DEC_N + (uint32_t)db * DEC_N;
+#pragma unroll
+                    for (int kk = 0; kk < KB / 16; ++kk)
+                        umma_bf16(d_tmem, adesc + 2u * kk, bdesc + 2u * kk, idesc, (uint32_t)(acc | (kk != 0)));
+                    umma_commit(empty_bar(stage));
+                }
+                __syncwarp();
+                touched |= 1u << db;
+                if (++stage == NS) { stage = 0; phase ^= 1u; }
+            }
+            Piece nx;
+            more = it.next(nx);
+            int cur2 = cur;
+            const bool run_ends = !more || run_of(ax, nx.item, cur2) != run;
+            if (el) {
+                umma_commit(hempty(b));
+                if (run_ends) umma_commit(yfull);
+            }
+            __syncwarp();
+            if (run_ends) ++nseg;
+            p = nx;
+            ++i;
+        }
+        DEC_TRM(10);
+    } else if (warp < 6) {
+        // ===================================================== epilogue warps 2..5 (TMEM lane quadrant q = warp & 3)
+        const int q = warp & 3;
+        const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+        const int row = q * 32 + lane;                              // packed gate/up row (phase 1), output feature in a block (phase 2)
+        PieceIter it;
+        Piece p;
+        int i = 0;
+        // ---- phase 1: the piece's fp32 partial -> scratch slot (item + CTA): 64 contiguous bytes per thread
+        it.init(lo1, hi1, D.nKB1);
+        while (it.next(p)) {
+            const int b = i & 1, u = i >> 1;
+            uint32_t v[16];
+            mbar_wait(a1full(b), (uint32_t)(u & 1), a.state);
+            tc_fence_after();
+            tmem_ld16(tmem_base + lane_base + (uint32_t)b * DEC_N, v);
+            tmem_ld_wait();
+            tc_fence_before();
+            mbar_arrive(a1empty(b));
+            float4* dst = (float4*)(a.part + ((size_t)(p.item + (int)blockIdx.x) * WT_ROWS + row) * DEC_N);
+#pragma unroll
+            for (int m = 0; m < 4; ++m)
+                dst[m] = make_float4(__uint_as_float(v[4 * m]), __uint_as_float(v[4 * m + 1]), __uint_as_float(v[4 * m + 2]),
+                                     __uint_as_float(v[4 * m + 3]));
+            ++i;
+        }
+        // ---- grid barrier A: every partial is written (and yacc is zeroed) before anybody reads / reduces
+        __threadfence();
+        asm volatile("bar.sync 2, 128;" ::: "memory");
+        DEC_TRE(2);
+        if (tid == 64) {
+            grid_arrive(a.state, 0, G);
+            grid_wait(a.state, 0, ax->gen0[0]);
+        }
+        asm volatile("bar.sync 2, 128;" ::: "memory");
+        DEC_TRE(3);
+        // ---- phase 2
+        int cur = 0, prev_run = -1, nseg = 0;
+        uint32_t touched = 0;
+        i = 0;
+        it.init(lo2, hi2, D.nDB);
+        bool more = it.next(p);
+        while (more) {
+            const int run = run_of(ax, p.item, cur);
+            if (run != prev_run) { touched = 0; prev_run = run; }
+            const int en = ax->run_en[run];
+            const int e = en & 0xFFFF, nt = en >> 16;
+            const int cb = p.item - ax->run_ib[run];
+            const int b = i & 1, u = i >> 1;
+            // h of item (run, cb): sum of the partials of the CTAs that touched the item in phase 1
+            float acc[16];
+#pragma unroll
+            for (int m = 0; m < 16; ++m) acc[m] = 0.f;
+            {
+                const long long t0 = (long long)p.item * D.nKB1;
+                const int c0 = cta_of_tile(t0, T1, (int)G), c1 = cta_of_tile(t0 + D.nKB1 - 1, T1, (int)G);
+                for (int c = c0; c <= c1; ++c) {
+                    // a CTA between c0 and c1 holds a piece of this item unless its own range is empty (fewer tiles than CTAs)
+                    if (T1 * c / G == T1 * (c + 1) / G) continue;
+                    const float4* src = (const float4*)(a.part + ((size_t)(p.item + c) * WT_ROWS + row) * DEC_N);
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        const float4 f = __ldcg(src + m);
+                        acc[4 * m] += f.x; acc[4 * m + 1] += f.y; acc[4 * m + 2] += f.z; acc[4 * m + 3] += f.w;
+                    }
                 }
             }
-            tc_fence_before();
-            mbar_arrive(yempty);
+            const int ch = q * 16 + (lane & 15);
+            const bool keep = cb * CB + ch < ax->r[e];              // tail of the last retained block (pad-zero rule)
+            const int odd = lane >> 4;
+            mbar_wait(hempty(b), (uint32_t)((u & 1) ^ 1), a.state);
+            uint8_t* hs = hs_gen + b * DEC_XE_KB_BYTES;
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const float mine0 = acc[2 * m], mine1 = acc[2 * m + 1];
+                const float send = odd ? mine0 : mine1;
+                const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
+                const float gte = odd ? recv : mine0;               // gate lives in lanes 0-15
+                const float up = odd ? mine1 : recv;                // up lives in lanes 16-31
+                float h = __fdividef(gte, 1.f + __expf(-gte)) * up;
+                if (!keep) h = 0.f;
+                const uint32_t t = 2 * m + odd;
+                *(__nv_bfloat16*)(hs + sw128_off(t, ch)) = __float2bfloat16_rn(h);
+            }
+            fence_proxy_async_smem();
+            mbar_arrive(hfull(b));
+            touched |= ((p.b >= 32 ? 0xFFFFFFFFu : ((1u << p.b) - 1u)) & ~((1u << p.a) - 1u));
+            Piece nx;
+            more = it.next(nx);
+            int cur2 = cur;
+            const bool run_ends = !more || run_of(ax, nx.item, cur2) != run;
+            if (run_ends) {
+                // ---- end of the run segment: touched feature blocks of Y -> yacc (router-weight scale + ScatterAdd, Alg. 2 l.19-20)
+                int tok = 0;
+                float wt = 0.f;
+                if (lane < nt) {
+                    const int f = ax->perm[ax->run_pos[run] + lane];
+                    tok = f / k;
+                    wt = a.topk_w[f];
+                }
+                mbar_wait(yfull, (uint32_t)(nseg & 1), a.state);
+                tc_fence_after();
+                for (int db = 0; db < D.nDB; ++db) {
+                    if (!((touched >> db) & 1u)) continue;
+                    uint32_t v[16];
+                    tmem_ld16(tmem_base + lane_base + 2u * DEC_N + (uint32_t)db * DEC_N, v);
+                    tmem_ld_wait();
+                    const int feat = db * WT_ROWS + row;
+#pragma unroll
+                    for (int tk = 0; tk < DEC_N; ++tk) {
+                        const int t = __shfl_sync(0xffffffffu, tok, tk);
+                        const float w = __shfl_sync(0xffffffffu, wt, tk);
+                        if (tk < nt && feat < D.d) atomicAdd(a.yacc + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
+                    }
+                }
+                tc_fence_before();
+                mbar_arrive(yempty);
+                ++nseg;
+            }
+            p = nx;
+            ++i;
         }
     } else {
-        // ===================================================== stagers, warps 6..9: x rows of the run -> Xe
+        // ===================================================== stagers, warps 6..9: x rows of a run -> Xe (phase 1 only)
         const int st = tid - 192;                                   // 0..127
         const int cpr = D.d >> 3;                                   // 16-byte chunks per x row
-        for (int R = 0; R < n_runs; ++R) {
-            const int4 run = ax->runs[R];
-            const int nt = run.x >> 16;
-            mbar_wait(xempty, (uint32_t)((R & 1) ^ 1), a.state);
-            const int total = nt * cpr;
-            for (int i0 = st; i0 < total; i0 += 128 * 8) {
-                uint4 v[8];
+        PieceIter it;
+        Piece p;
+        int cur = 0, prev_run = -1, nrun = 0, staged = 0;           // staged = rows of Xe that may hold a previous run's tokens
+        it.init(lo1, hi1, D.nKB1);
+        while (it.next(p)) {
+            const int run = run_of(ax, p.item, cur);
+            if (run == prev_run) continue;
+            prev_run = run;
+            const int nt = ax->run_en[run] >> 16, pos = ax->run_pos[run];
+            mbar_wait(xempty, (uint32_t)((nrun & 1) ^ 1), a.state);
+            ++nrun;
+            // row-outer / chunk-inner: no divisions; 2 rows x up to 4 column steps = 8 loads in flight per thread
+            for (int pr0 = 0; pr0 < nt; pr0 += 2) {
+                const uint4* s0 = a.x + (size_t)((int)ax->perm[pos + pr0] / k) * cpr;
+                const uint4* s1 = pr0 + 1 < nt ? a.x + (size_t)((int)ax->perm[pos + pr0 + 1] / k) * cpr : nullptr;
+                for (int c0 = st; c0 < cpr; c0 += 512) {
+                    uint4 v0[4], v1[4];
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const int idx = i0 + u * 128;
-                    if (idx < total) {
-                        const int p = idx / cpr, c = idx - p * cpr;
-                        const int f = ax->perm[run.y + p];
-                        v[u] = __ldg(a.x + (size_t)(f / k) * cpr + c);
+                    for (int u = 0; u < 4; ++u) {
+                        const int c = c0 + 128 * u;
+                        v0[u] = c < cpr ? __ldg(s0 + c) : make_uint4(0, 0, 0, 0);
+                        v1[u] = (s1 && c < cpr) ? __ldg(s1 + c) : make_uint4(0, 0, 0, 0);
                     }
-                }
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const int idx = i0 + u * 128;
-                    if (idx < total) {
-                        const int p = idx / cpr, c = idx - p * cpr;
-                        *(uint4*)(xe_gen + (size_t)(c >> 3) * DEC_XE_KB_BYTES + sw128_chunk((uint32_t)p, (uint32_t)(c & 7))) = v[u];
+                    for (int u = 0; u < 4; ++u) {
+                        const int c = c0 + 128 * u;
+                        if (c < cpr) {
+                            uint8_t* dst = xe_gen + (size_t)(c >> 3) * DEC_XE_KB_BYTES;
+                            *(uint4*)(dst + sw128_chunk((uint32_t)pr0, (uint32_t)(c & 7))) = v0[u];
+                            if (s1) *(uint4*)(dst + sw128_chunk((uint32_t)(pr0 + 1), (uint32_t)(c & 7))) = v1[u];
+                        }
                     }
                 }
             }
+            // rows of a previous, larger run must not leak into this one: clear rows nt .. staged-1
+            for (int pr = nt; pr < staged; ++pr)
+                for (int c = st; c < cpr; c += 128)
+                    *(uint4*)(xe_gen + (size_t)(c >> 3) * DEC_XE_KB_BYTES + sw128_chunk((uint32_t)pr, (uint32_t)(c & 7))) = make_uint4(0, 0, 0, 0);
+            staged = nt;
             fence_proxy_async_smem();
             mbar_arrive(xfull);
         }
@@ -577,20 +661,18 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     __threadfence();                                               // this thread's reductions are performed
     tc_fence_before();
     __syncthreads();
-    DEC_TR(2);
+    DEC_TR(4);
     if (warp == 1) {
         tc_fence_after();
         tmem_dealloc(tmem_base, 512);
     }
     if (tid == 0) {
-        DEC_TR(5);
         grid_arrive(a.state, 1, G);
-        DEC_TR(6);
-        grid_wait(a.state, 1, ax->gen0[1]);
         DEC_TR(7);
+        grid_wait(a.state, 1, ax->gen0[1]);
     }
     __syncthreads();
-    DEC_TR(3);
+    DEC_TR(5);
     {
         const size_t n4 = (size_t)a.T * D.d / 4;
         const float4* src = (const float4*)a.yacc;
@@ -609,7 +691,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             dst[i] = o;
         }
     }
-    DEC_TR(4);
+    DEC_TR(6);
 }
 
 // ---------------------------------------------------------------------------------------------- host side
@@ -622,21 +704,29 @@ int decode_slots(const Dims& D) {
 
 bool decode_supported(const Dims& D) { return D.nDB * DEC_N + 2 * DEC_N <= 512 && decode_slots(D) >= 4; }
 
+// most phase-1 partial slots a call with T*k = A assignments can need: (items + CTAs); monotonic in A
+size_t decode_part_bytes(const Dims& D, long long A) {
+    const long long a = A < DEC_MAX_A ? A : DEC_MAX_A;
+    long long runs = a / DEC_N + D.E;
+    if (runs > a) runs = a;                                   // a run holds at least one assignment
+    return (size_t)(runs * D.nCB + DEC_MAX_CTAS + 1) * DEC_PART * sizeof(float);
+}
+
 cudaError_t init_decode_kernel() {
     return cudaFuncSetAttribute(k_decode, cudaFuncAttributeMaxDynamicSharedMemorySize, DEC_SMEM_MAX);
 }
 
 cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
-                          const int* ids, const float* topk_w, int T, int k, float* yacc, const __nv_bfloat16* y_add,
-                          __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st) {
+                          const int* ids, const float* topk_w, int T, int k, float* yacc, float* part,
+                          const __nv_bfloat16* y_add, __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st) {
     DecArgs a{};
     a.D = D; a.V = V; a.r_table = r_table; a.x = (const uint4*)x; a.ids = ids; a.topk_w = topk_w;
-    a.yacc = yacc; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.T = T; a.k = k; a.A = T * k;
+    a.yacc = yacc; a.part = part; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.T = T; a.k = k; a.A = T * k;
     a.slots = decode_slots(D);
     a.pf = pf;
     const int smem = dec_fixed_smem(D) + a.slots * WT_BYTES;
-    void* args[] = {(void*)&a};
-    return cudaLaunchCooperativeKernel((const void*)k_decode, dim3(num_sms), dim3(DEC_THREADS), args, (size_t)smem, st);
+    const int grid = num_sms < DEC_MAX_CTAS ? num_sms : DEC_MAX_CTAS;
+    return launch_pdl(k_decode, dim3(grid), dim3(DEC_THREADS), (size_t)smem, st, a);
 }
 
 }  // namespace fxm

@@ -97,6 +97,7 @@ struct Workspace {
     int4* tt;               // [NT + 1] token tiles: {expert, first padded row, valid rows, GEMM-1 work prefix}; tt[ntt] = sentinel
     uint8_t* H;             // [nCB][P][128 B]   SwiGLU activations, swizzled panels
     float* yacc;            // [T][d] fp32 accumulator of y: the scatter-add target of GEMM-2 / of the decode kernel
+    float* dec_part;        // decode kernel: fp32 partial gate/up sums, one 8 KB slot per (item, CTA) piece
     int RB;                 // route blocks
     int chunk;              // flat assignments per route block
     int P;                  // padded-row capacity (multiple of 16)
@@ -119,6 +120,8 @@ __host__ inline int route_tok_chunk(long long T, int E) {
     const long long c = (per + 31) / 32 * 32;
     return (int)(c > 0 ? c : 32);
 }
+
+size_t decode_part_bytes(const Dims& D, long long A);   // fxm_decode.cu; monotonic in A
 
 __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base) {
     Workspace w{};
@@ -145,6 +148,7 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.tt = (int4*)(b + take(sizeof(int4) * ((size_t)NT + 1)));
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
     w.yacc = (float*)(b + take((size_t)T * D.d * sizeof(float)));       // every T: the size is monotonic in T
+    w.dec_part = (float*)(b + take(decode_part_bytes(D, (long long)A)));
     w.RB = RB;
     w.chunk = chunk;
     w.P = P;
@@ -274,7 +278,7 @@ cudaError_t launch_action_cost(const float* alpha, int K, const int* num_host, i
 bool decode_supported(const Dims& D);
 cudaError_t init_decode_kernel();
 cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
-                          const int* ids, const float* topk_w, int T, int k, float* yacc, const __nv_bfloat16* y_add,
-                          __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st);
+                          const int* ids, const float* topk_w, int T, int k, float* yacc, float* part,
+                          const __nv_bfloat16* y_add, __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st);
 
 }  // namespace fxm
