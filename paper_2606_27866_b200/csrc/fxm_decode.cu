@@ -130,6 +130,10 @@ __device__ __forceinline__ void grid_wait(DevState* st, int i, uint32_t gen0) {
     }
 }
 
+__device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t& v0, uint32_t& v1) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(v0), "=r"(v1) : "r"(taddr) : "memory");
+}
+
 // ---- the two tile lists.  Phase p has tiles_per_item = nKB1 (p = 1) or nDB (p = 2); tile t belongs to item t / tpi.
 // A PIECE is the part of one item inside a CTA's range: item, local tile range [a, b).
 struct Piece { int item, a, b; };
@@ -589,6 +593,27 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                 }
                 mbar_wait(yfull, (uint32_t)(nseg & 1), a.state);
                 tc_fence_after();
+                if (nt <= 2) {
+                    // one or two tokens (single-token decode): two columns per feature block, eight blocks per TMEM wait
+                    const int t0 = __shfl_sync(0xffffffffu, tok, 0), t1 = __shfl_sync(0xffffffffu, tok, 1);
+                    const float w0 = __shfl_sync(0xffffffffu, wt, 0), w1 = __shfl_sync(0xffffffffu, wt, 1);
+                    for (int db0 = 0; db0 < D.nDB; db0 += 8) {
+                        uint32_t v0[8], v1[8];
+#pragma unroll
+                        for (int u = 0; u < 8; ++u)
+                            if (db0 + u < D.nDB && ((touched >> (db0 + u)) & 1u))
+                                tmem_ld2(tmem_base + lane_base + 2u * DEC_N + (uint32_t)(db0 + u) * DEC_N, v0[u], v1[u]);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const int feat = (db0 + u) * WT_ROWS + row;
+                            if (db0 + u < D.nDB && ((touched >> (db0 + u)) & 1u) && feat < D.d) {
+                                atomicAdd(a.yacc + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
+                                if (nt == 2) atomicAdd(a.yacc + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
+                            }
+                        }
+                    }
+                } else
                 for (int db = 0; db < D.nDB; ++db) {
                     if (!((touched >> db) & 1u)) continue;
                     uint32_t v[16];
@@ -622,9 +647,10 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             if (run == prev_run) continue;
             prev_run = run;
             const int nt = ax->run_en[run] >> 16, pos = ax->run_pos[run];
-            mbar_wait(xempty, (uint32_t)((nrun & 1) ^ 1), a.state);
-            ++nrun;
-            // row-outer / chunk-inner: no divisions; 2 rows x up to 4 column steps = 8 loads in flight per thread
+            // row-outer / chunk-inner: no divisions; 2 rows x up to 4 column steps = 8 loads in flight per thread.  The
+            // loads of the first batch are issued BEFORE the wait for the panel (only the stores need it free), so a run
+            // of one or two tokens is already in registers when the previous run's last MMA retires.
+            bool waited = false;
             for (int pr0 = 0; pr0 < nt; pr0 += 2) {
                 const uint4* s0 = a.x + (size_t)((int)ax->perm[pos + pr0] / k) * cpr;
                 const uint4* s1 = pr0 + 1 < nt ? a.x + (size_t)((int)ax->perm[pos + pr0 + 1] / k) * cpr : nullptr;
@@ -636,6 +662,11 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                         v0[u] = c < cpr ? __ldg(s0 + c) : make_uint4(0, 0, 0, 0);
                         v1[u] = (s1 && c < cpr) ? __ldg(s1 + c) : make_uint4(0, 0, 0, 0);
                     }
+                    if (!waited) {
+                        mbar_wait(xempty, (uint32_t)((nrun & 1) ^ 1), a.state);
+                        ++nrun;
+                        waited = true;
+                    }
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const int c = c0 + 128 * u;
@@ -646,6 +677,10 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                         }
                     }
                 }
+            }
+            if (!waited) {                                          // threads beyond the row width (d < 1024) issued nothing
+                mbar_wait(xempty, (uint32_t)((nrun & 1) ^ 1), a.state);
+                ++nrun;
             }
             // rows of a previous, larger run must not leak into this one: clear rows nt .. staged-1
             for (int pr = nt; pr < staged; ++pr)
