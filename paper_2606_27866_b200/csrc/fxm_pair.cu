@@ -290,8 +290,8 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
             mbar_init(full_bar(s), rank == 0 ? 2 : 1);            // leader: own producer + the peer's relay
             mbar_init(empty_bar(s), 1);
         }
-        // "columns drained": GEMM-1 one arrival per CTA (after its epilogue barrier), GEMM-2 one per epilogue warp
-        for (int q = 0; q < PAIR_TQ; ++q) { mbar_init(tfull_bar(q), 1); mbar_init(tempty_bar(q), MODE == 1 ? 2 : 2 * PAIR_EPI_WARPS); }
+        // "columns drained": one arrival per epilogue warp of both CTAs (a warp arrives as soon as its share is in registers)
+        for (int q = 0; q < PAIR_TQ; ++q) { mbar_init(tfull_bar(q), 1); mbar_init(tempty_bar(q), 2 * PAIR_EPI_WARPS); }
         fence_barrier_init();
     }
     if (warp == 1) tmem_alloc2(smem_u32((const void*)tmem_slot), 512);
@@ -319,6 +319,15 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
         return a.V.dn + dn_tile_off(D, it.eblk, 0, it.blk);
     };
 
+    // Register budget (GEMM-1, 768 threads): the epilogue warps hold a 64-value share of the accumulator, the producer /
+    // MMA / gather warps need few registers.  The pool is the CTA's OWN launch allocation (768 threads x 80 registers = 61440;
+    // the SM's remaining registers are not part of it -- an inc beyond it waits forever): 8 x 32 x 48 + 16 x 32 x 96 = 61440.  Every role adjusts its own budget at
+    // the top of its branch (that is where ptxas picks it up).  setmaxnreg is WARPGROUP-aligned: all four warps of a warpgroup must
+    // execute the same instruction, so one dec dominates every non-epilogue role (warps 0-7 = two whole warpgroups).
+#define FXM_REG_DEC() do { if constexpr (MODE == 1) asm volatile("setmaxnreg.dec.sync.aligned.u32 48;" ::: "memory"); } while (0)
+#define FXM_REG_INC() do { if constexpr (MODE == 1) asm volatile("setmaxnreg.inc.sync.aligned.u32 96;" ::: "memory"); } while (0)
+    if (warp < EPI0) {
+    FXM_REG_DEC();
     if (warp == 0) {
         // ===================================================== producer (both CTAs): weight tile + token half per k-block
         const bool leader_lane = elect_one();
@@ -470,7 +479,9 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
             }
             __syncwarp();
         }
-    } else if (warp >= EPI0) {
+    }
+    } else {
+        FXM_REG_INC();
         // ===================================================== epilogue warps (both CTAs, own TMEM lanes)
         const int q = warp & 3;                                // TMEM lane quadrant this warp may read
         constexpr int NWQ = PAIR_EPI_WARPS / 4;                // warps per lane quadrant
@@ -488,77 +499,79 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                 const size_t nthr = (size_t)gridDim.x * (32 * PAIR_EPI_WARPS);
                 for (size_t i = (size_t)blockIdx.x * (32 * PAIR_EPI_WARPS) + et; i < n4; i += nthr) z[i] = make_uint4(0, 0, 0, 0);
             }
-            // A sub-tile is drained in CHUNKS of 128 token columns: TMEM -> registers -> SwiGLU -> a 16 KB staging buffer
-            // in the FINAL global layout (swizzled H panel rows) -> one bulk store per chunk.  Two staging buffers alternate.
-            constexpr int CH = 128;
+            // A warp owns up to four 16-token groups of a sub-tile (its lane quadrant = 16 gate + 16 up channels): it pulls
+            // them into 64 registers and hands the TMEM columns back to the MMA warp AT ONCE -- the next tile's MMAs run
+            // while SwiGLU is computed from registers.  The bf16 results go to a 32 KB staging buffer in the FINAL global
+            // layout (swizzled H panel rows of this CTA's channel block), one bulk store per sub-tile.
             const uint64_t pol_keep = l2_policy_evict_last();         // H panels: read back by GEMM-2
-            uint32_t nchunk = 0;
+            const int chn = q * 16 + (lane & 15);
+            const int odd = lane >> 4;
+            uint32_t soff[8];                                         // staging offset of token row 2m + odd (rows repeat every 8)
+#pragma unroll
+            for (int m = 0; m < 8; ++m) soff[m] = sw128_off((uint32_t)(2 * m + odd), (uint32_t)chn);
+            bool store_pending = false;
             for (int wi = wi0; wi < W; wi += wstep, ++tj) {
                 const PairItem it = pair_item<MODE>(a, wi, rank, cur);
                 const int nsub = it.n1 ? 2 : 1;
                 uint32_t cc0, cc1, need_unused;
                 const uint32_t sq0 = ring.seq;
                 ring.alloc_item((uint32_t)it.n0, (uint32_t)it.n1, cc0, cc1, need_unused);
+                const bool keep = it.blk * CB + chn < it.r;           // tail mask of the last retained block (pad-zero rule)
                 for (int sidx = 0; sidx < nsub; ++sidx) {
                     const int n = sidx ? it.n1 : it.n0;
                     const uint32_t col0 = sidx ? cc1 : cc0;
                     const uint32_t sq = sq0 + sidx;
                     const int rowS = it.row0 + (sidx ? it.n0 : 0);
                     const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + col0;
+                    const int ngrp = n >> 4;                           // <= 16 groups in a sub-tile of <= 256 tokens
+                    const int gbeg = ngrp * wq / NWQ, gend = ngrp * (wq + 1) / NWQ;     // <= 4 of them are this warp's
                     mbar_wait(tfull_bar(sq), (sq / PAIR_TQ) & 1u, a.state);
                     if (et == 0 && rank == 0 && sidx == 0) FXM_TR(MODE, tj, 4, FXM_CLK());
                     tc_fence_after();
-                    for (int ch0 = 0; ch0 < n; ch0 += CH, ++nchunk) {
-                        const int rows = min(CH, n - ch0);
-                        uint8_t* stg = stg_gen + (nchunk & 1u) * 16384u;
-                        const int ngrp = rows >> 4;                          // 16-column groups in this chunk
-                        const int gbeg = ngrp * wq / NWQ, gend = ngrp * (wq + 1) / NWQ;
-                        if (it.valid && gbeg < gend) {
-                            uint32_t va[16], vb[16];
-                            const int chn = q * 16 + (lane & 15);
-                            const bool keep = it.blk * CB + chn < it.r;       // tail mask of the last retained block (pad-zero rule)
-                            const int odd = lane >> 4;
-                            auto swiglu16 = [&](const uint32_t (&v)[16], int t0) {
+                    uint32_t v[4][16];
+                    if (it.valid) {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+                            if (gbeg + u < gend) tmem_ld16(taddr + (uint32_t)(gbeg + u) * 16u, v[u]);
+                        tmem_ld_wait();
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) {                                   // this warp no longer needs the columns
+                        if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
+                    }
+                    if (store_pending) {                               // the previous sub-tile's bulk store has read the staging buffer
+                        if (et == 0) bulk_wait_read0();
+                        epi_bar_sync_all();
+                        store_pending = false;
+                    }
+                    if (it.valid) {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (gbeg + u < gend) {
+                                uint8_t* sg = stg_gen + (uint32_t)(gbeg + u) * (16u * ROW_BYTES);
 #pragma unroll
                                 for (int m = 0; m < 8; ++m) {
-                                    const float mine0 = __uint_as_float(v[2 * m]), mine1 = __uint_as_float(v[2 * m + 1]);
+                                    const float mine0 = __uint_as_float(v[u][2 * m]), mine1 = __uint_as_float(v[u][2 * m + 1]);
                                     const float send = odd ? mine0 : mine1;                    // what the twin lane needs
                                     const float recv = __shfl_xor_sync(0xffffffffu, send, 16);
                                     const float g = odd ? recv : mine0;                        // gate lives in lanes 0-15
-                                    const float u = odd ? mine1 : recv;                        // up lives in lanes 16-31
-                                    float hv = __fdividef(g, 1.f + __expf(-g)) * u;
+                                    const float up = odd ? mine1 : recv;                       // up lives in lanes 16-31
+                                    float hv = __fdividef(g, 1.f + __expf(-g)) * up;
                                     if (!keep) hv = 0.f;
-                                    const uint32_t t = t0 + 2 * m + odd;                       // token row inside the chunk
-                                    *(__nv_bfloat16*)(stg + sw128_off(t, chn)) = __float2bfloat16_rn(hv);
+                                    *(__nv_bfloat16*)(sg + soff[m]) = __float2bfloat16_rn(hv);
                                 }
-                            };
-                            tmem_ld16(taddr + ch0 + gbeg * 16, va);
-                            for (int g = gbeg; g < gend; g += 2) {
-                                tmem_ld_wait();
-                                if (g + 1 < gend) tmem_ld16(taddr + ch0 + (g + 1) * 16, vb);
-                                swiglu16(va, g * 16);
-                                tmem_ld_wait();
-                                if (g + 2 < gend) tmem_ld16(taddr + ch0 + (g + 2) * 16, va);
-                                if (g + 1 < gend) swiglu16(vb, (g + 1) * 16);
-                            }
-                        }
-                        const bool last = ch0 + CH >= n;
-                        fence_proxy_async_smem();                      // staging writes -> visible to the bulk-copy engine
-                        if (last) tc_fence_before();
-                        if (et == 0) bulk_wait_read0();                // the previous chunk's store has left the OTHER buffer
-                        epi_bar_sync_all();
-                        if (et == 0) {
-                            if (it.valid) {
-                                uint8_t* gdst = a.H + ((size_t)it.blk * a.P + rowS + ch0) * ROW_BYTES;
-                                bulk_s2g_hint(gdst, stg_base + (nchunk & 1u) * 16384u, (uint32_t)rows * ROW_BYTES, pol_keep);
-                                bulk_commit();
-                            }
-                            if (last) {                                // all epilogue warps have drained this sub-tile's columns
-                                if (rank == 0) mbar_arrive(tempty_bar(sq)); else mbar_arrive_remote(tempty_bar(sq), 0);
-                                if (rank == 0 && sidx == nsub - 1) FXM_TR(MODE, tj, 5, FXM_CLK());
                             }
                         }
                     }
+                    fence_proxy_async_smem();                          // staging writes -> visible to the bulk-copy engine
+                    epi_bar_sync_all();
+                    if (et == 0 && it.valid) {
+                        bulk_s2g_hint(a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES, stg_base, (uint32_t)n * ROW_BYTES, pol_keep);
+                        bulk_commit();
+                    }
+                    store_pending = it.valid;                          // warp-uniform across the CTA
+                    if (et == 0 && rank == 0 && sidx == nsub - 1) FXM_TR(MODE, tj, 5, FXM_CLK());
                 }
             }
             if (et == 0) bulk_wait0();
