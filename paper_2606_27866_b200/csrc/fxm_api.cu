@@ -16,6 +16,7 @@ struct fxm_layer {
     uint8_t* blob;           // caller's buffer
     int* tables;             // [MAX_TABLES][TABLE_STRIDE] int32
     DevState* state;
+    uint32_t* dec_cnt;       // decode kernel: per-item piece counters (blob tail, zero between calls)
     int* rank_dev;           // device copy of channel_rank (full layers packed with a ranking), else null
     int clipped;             // 1: offline-clipped layer: widths are bounded by r_clip
     std::vector<int> r_clip; // [E] exported widths of a clipped layer
@@ -63,14 +64,16 @@ static bool make_dims(int E, int d, int I, Dims* D) {
     return true;
 }
 
-// tail of a blob, after `wbytes` of weight tiles: [16 budget tables][state][eblk][channel_rank copy (full layers only)]
-struct Tail { size_t tables, state, eblk, rank, total; };
+// tail of a blob, after `wbytes` of weight tiles: [16 budget tables][state][eblk][decode item counters][channel_rank copy
+// (full layers only)]
+struct Tail { size_t tables, state, eblk, dcnt, rank, total; };
 static Tail tail_map(const Dims& D, size_t wbytes, bool with_rank) {
     Tail t;
     t.tables = align_up(wbytes, 1024);
     t.state = t.tables + sizeof(int) * MAX_TABLES * TABLE_STRIDE;
     t.eblk = align_up(t.state + sizeof(DevState), 1024);
-    t.rank = align_up(t.eblk + sizeof(uint32_t) * MAX_E, 1024);
+    t.dcnt = align_up(t.eblk + sizeof(uint32_t) * MAX_E, 1024);
+    t.rank = align_up(t.dcnt + decode_cnt_bytes(D), 1024);
     t.total = with_rank ? align_up(t.rank + sizeof(int) * (size_t)D.E * D.I, 1024) : t.rank;
     return t;
 }
@@ -111,6 +114,7 @@ static fxm_layer* new_layer(const Dims& D, uint8_t* blob, const Tail& tl, int sm
     L->tables = (int*)(blob + tl.tables);
     L->state = (DevState*)(blob + tl.state);
     L->V.eblk = (const uint32_t*)(blob + tl.eblk);
+    L->dec_cnt = (uint32_t*)(blob + tl.dcnt);
     L->rank_dev = nullptr; L->clipped = 0;
     L->n_registered = 0; L->current = -1; L->impl = FXM_IMPL_TCGEN05; L->num_sms = sms; L->tile_n_override = 0;
     L->host_tables.assign((size_t)MAX_TABLES * TABLE_STRIDE, 0);
@@ -128,6 +132,7 @@ static fxm_layer* new_layer(const Dims& D, uint8_t* blob, const Tail& tl, int sm
 static fxm_status init_tail(fxm_layer* L, cudaStream_t st) {
     if (cudaMemsetAsync(L->tables, 0, sizeof(int) * MAX_TABLES * TABLE_STRIDE + sizeof(DevState), st) != cudaSuccess)
         return FXM_ECUDA;
+    if (cudaMemsetAsync(L->dec_cnt, 0, decode_cnt_bytes(L->D), st) != cudaSuccess) return FXM_ECUDA;
     void* hp = nullptr;
     if (cudaHostAlloc(&hp, 64, cudaHostAllocMapped) == cudaSuccess && hp) {
         std::memset(hp, 0, 64);
@@ -408,7 +413,7 @@ static fxm_status ffn_impl(fxm_layer* L, const void* x, const int32_t* topk_ids,
         if (logits && launch_router_topk(logits, T, D.E, k, fe_ids, fe_w, st) != cudaSuccess) return FXM_ECUDA;
         for (int j = 0; j < FXM_N_KERNELS; ++j) FXM_MARK(j)
         if (launch_decode(D, L->V, table, (const __nv_bfloat16*)x, logits ? fe_ids : topk_ids, logits ? fe_w : topk_w, T, k,
-                          ws.yacc, ws.dec_part, (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->num_sms,
+                          ws.yacc, ws.dec_part, (const __nv_bfloat16*)y_add, (__nv_bfloat16*)y, L->state, L->dec_cnt, L->num_sms,
                           decode_prefetch(L, T, k), st) != cudaSuccess)
             return FXM_ECUDA;
         FXM_MARK(FXM_N_KERNELS)

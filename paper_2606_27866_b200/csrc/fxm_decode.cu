@@ -21,10 +21,13 @@
 // Roles (320 threads): warp 0 weight producer (16 KB cp.async.bulk per tile through a shared-memory ring; it starts
 // fetching phase-2 tiles while the grid barrier is still closing), warp 1 MMA issuer, warps 2-5 epilogue, warps 6-9
 // stage the <= 16 token rows x[t] of a run into swizzled K-major panels Xe (X[pi], Alg. 2 l.7).
-// Grid barriers (sense-reversing counters in DevState): A between the phases (it also orders the zeroing of yacc
-// before every reduction), B before yacc -> y (one rounding to bf16).  The launch is an ordinary one with the
-// programmatic-dependent-launch attribute, grid = #SMs, one CTA per SM: every CTA is resident before a dependent kernel
-// may start, and nothing the CTAs wait for depends on a later kernel, so the barriers cannot deadlock.
+// Synchronisation between CTAs (all resident: grid = #SMs, one CTA per SM; nothing a CTA waits for depends on a later
+// kernel, so none of this can deadlock):
+//   * phase 1 -> phase 2 is NOT a grid barrier: a phase-2 piece waits for the per-item counter of ITS item (the two or
+//     three CTAs that hold phase-1 pieces of it each add 1 after their partial is in global memory);
+//   * "yacc is zeroed" is a split barrier: every CTA arrives in its prologue and checks before its first reduction;
+//   * one grid barrier before yacc -> y (one rounding to bf16), a single ever-growing counter (see cnt_arrive).
+// The launch is an ordinary one with the programmatic-dependent-launch attribute.
 // TMEM columns: [0,32) two phase-1 accumulators, [32, 32 + 16 nDB) the Y partial.  Needs nDB <= 30 (d <= 3840).
 #include "fxm_ptx.cuh"
 
@@ -32,11 +35,14 @@ namespace fxm {
 
 constexpr int DEC_THREADS = 320;
 constexpr int DEC_N = 16;                         // tokens per run = UMMA N
-constexpr int DEC_MAX_RUNS = 320;                 // >= DEC_MAX_A / 16 + MAX_E (total number of runs of a call)
 constexpr int DEC_XE_KB_BYTES = DEC_N * ROW_BYTES;   // 2 KB of Xe per k-block
 constexpr int DEC_MAX_SLOTS = 12;
 constexpr int DEC_SMEM_MAX = 232448;              // 227 KB
 constexpr int DEC_PART = WT_ROWS * DEC_N;         // floats of one phase-1 partial: 128 packed rows x 16 tokens (8 KB)
+#ifndef FXM_DEC_BURST
+#define FXM_DEC_BURST 16
+#endif
+constexpr int DEC_BURST = FXM_DEC_BURST;          // phase-2 tiles pulled into L2 while the CTA waits for the phase-1 partials (0 = none)
 constexpr int DEC_MAX_CTAS = 160;                 // the partial-slot capacity is sized for at most this many CTAs
 
 struct DecArgs {
@@ -51,6 +57,7 @@ struct DecArgs {
     const uint2* y_add;        // [T][d] bf16 or null: shared-expert output added in fp32 before the rounding of y
     __nv_bfloat16* y;          // [T][d]
     DevState* state;
+    uint32_t* icnt;            // [items] phase-1 pieces written per item (blob tail; zero on entry, zeroed again on exit)
     int T, k, A;
     int slots;                 // ring depth
     int pf;                    // L2 prefetch distance in 16 KB tiles (0 = none)
@@ -67,7 +74,7 @@ struct DecAux {
     uint64_t bars[2 * DEC_MAX_SLOTS + 16];
     uint32_t tmem_slot;
     int n_runs, W;
-    uint32_t gen0[2];
+    unsigned long long ztarget;    // value of DevState::dec_zcnt at which every CTA of THIS launch has zeroed its slice of yacc
 };
 // prologue-only scratch, aliased on the weight ring (>= 4 slots = 64 KB)
 struct DecTmp {
@@ -97,37 +104,53 @@ __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-// Grid barrier, one thread per CTA (all CTAs are resident, see the header).  Two levels, because 148 atomics on ONE address
-// serialise in L2 (measured: 10-20 us per barrier): CTA b arrives on sub-counter b % 8, the last arriver of a
-// sub-counter arrives on the top counter, the last of those bumps the generation word that everyone polls (it lives in
-// another 128-byte line than the counters).  Every counter is reset by its last arriver before the generation moves.
-__device__ __forceinline__ void grid_arrive(DevState* st, int i, uint32_t G) {
-    __threadfence();
-    const uint32_t grp = blockIdx.x & 7u;
-    const uint32_t gsize = (G - grp + 7u) >> 3;                       // CTAs with this residue
-    if (atomicAdd(&st->bar_sub[i][grp], 1u) == gsize - 1u) {
-        st->bar_sub[i][grp] = 0u;
-        __threadfence();
-        const uint32_t ngrp = G < 8u ? G : 8u;
-        if (atomicAdd(&st->bar_count[i], 1u) == ngrp - 1u) {
-            st->bar_count[i] = 0u;
-            __threadfence();
-            atomicAdd(&st->bar_gen[i], 1u);
-        }
-    }
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
 }
-__device__ __forceinline__ void grid_wait(DevState* st, int i, uint32_t gen0) {
+// Grid-wide synchronisation without a reset and without a chain of dependent round trips (all CTAs are resident, see the
+// header).  A counter only grows; every launch on a layer has the same grid size G and adds exactly G, so the value a
+// CTA's own arrival returns names the target of ITS launch, (old / G + 1) * G.  The arrival is a release (it publishes
+// what the CTA wrote before the preceding block-level barrier), the poll is an acquire.  After the last arrival a
+// poller needs one L2 round trip -- the two-level counter + generation word this replaces needed four.
+__device__ __forceinline__ unsigned long long cnt_arrive(unsigned long long* c) {
+    unsigned long long old;
+    asm volatile("atom.acq_rel.gpu.global.add.u64 %0, [%1], 1;" : "=l"(old) : "l"(c) : "memory");
+    return old;
+}
+__device__ __forceinline__ unsigned long long cnt_target(unsigned long long old, uint32_t G) { return (old / G + 1ull) * G; }
+__device__ __forceinline__ void wait_timeout(DevState* st) {
+    atomicOr(&st->flags, 2u);
+    if (st->hflag) *(volatile uint32_t*)st->hflag = 2u;
+    __threadfence_system();
+    __trap();
+}
+__device__ __forceinline__ void cnt_wait(const unsigned long long* c, unsigned long long target, DevState* st) {
+    if (ld_acquire_u64(c) >= target) return;
     const long long t0 = clock64();
     uint32_t spins = 0;
-    while (ld_acquire_u32(&st->bar_gen[i]) == gen0) {
-        __nanosleep(200);                                          // 148 pollers: keep the L2 slice of the barrier words quiet
-        if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) {
-            atomicOr(&st->flags, 2u);
-            if (st->hflag) *(volatile uint32_t*)st->hflag = 2u;
-            __threadfence_system();
-            __trap();
-        }
+    while (ld_acquire_u64(c) < target) {
+        __nanosleep(64);
+        if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) wait_timeout(st);
     }
+}
+// item readiness: the phase-1 pieces of an item are written by a few CTAs; each adds 1 (release) after its partial is in
+// global memory, the phase-2 reader polls (acquire) until all of them have
+__device__ __forceinline__ void item_signal(uint32_t* c) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(c) : "memory");
+}
+__device__ __forceinline__ void item_wait(const uint32_t* c, uint32_t need, DevState* st) {
+    if (ld_acquire_u32(c) >= need) return;
+    const long long t0 = clock64();
+    uint32_t spins = 0;
+    while (ld_acquire_u32(c) < need) {
+        __nanosleep(32);
+        if ((++spins & 0x3FFu) == 0 && clock64() - t0 > 4000000000LL) wait_timeout(st);
+    }
+}
+__device__ __forceinline__ void red_add_f32(float* p, float v) {
+    asm volatile("red.relaxed.gpu.global.add.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
 }
 
 __device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t& v0, uint32_t& v1) {
@@ -216,10 +239,6 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     }
     if (warp == 1) tmem_alloc(smem_u32(&ax->tmem_slot), 512);
     pdl_wait();                                              // the previous kernel may still use the workspace / write x, ids
-    if (tid == 0) {
-        ax->gen0[0] = ld_acquire_u32(&a.state->bar_gen[0]);      // read before this CTA arrives anywhere
-        ax->gen0[1] = ld_acquire_u32(&a.state->bar_gen[1]);
-    }
     bool bad = false;
     for (int f = tid; f < A; f += DEC_THREADS) {
         int id = a.ids[f];
@@ -228,7 +247,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     }
     if (bad) atomicOr(&a.state->flags, 1u);
     for (int e = tid; e < MAX_E; e += DEC_THREADS) { ax->r[e] = e < E ? a.r_table[e] : 0; ax->eb[e] = e < E ? a.V.eblk[e] : 0u; }
-    // zero this CTA's slice of the fp32 accumulator (grid barrier A orders it before every reduction)
+    // zero this CTA's slice of the fp32 accumulator; the arrival below (after the next block barrier) publishes it, and every
+    // CTA checks that ALL slices are published before its first reduction (a split barrier: arrive here, wait ~20 us later)
     {
         float4* z = (float4*)a.yacc;
         const size_t n4 = (size_t)a.T * D.d / 4;
@@ -246,6 +266,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = ax->tmem_slot;
+    unsigned long long zold = 0;
+    if (tid == DEC_THREADS - 1) zold = cnt_arrive(&a.state->dec_zcnt);     // the result is not needed before the end of the prologue
     for (int base = wlo; base < whi; base += 32) {
         const int f = base + lane;
         const int id = f < whi ? (int)tp->ids[f] : -1;
@@ -324,6 +346,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     __syncthreads();
     // Xe / Hs start as zeros (rows beyond a run's token count are never staged)
     for (int i = tid; i < (int)((aux_off - xe_off) / 16); i += DEC_THREADS) ((uint4*)xe_gen)[i] = make_uint4(0, 0, 0, 0);
+    if (tid == DEC_THREADS - 1) ax->ztarget = cnt_target(zold, G);
     fence_proxy_async_smem();
     __syncthreads();
     const int W = ax->W;
@@ -377,6 +400,11 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         seq_init(ld);
         seq_init(pf);
         const uint8_t* t;
+        // Between the last phase-1 tile and the first H of phase 2 lie ~5 us (partials -> global memory -> item counter ->
+        // partials read back -> SwiGLU) in which the ring is full of phase-2 tiles and this SM requests nothing.  At that
+        // moment -- and only then, so that the requests do not compete with the ring's own loads -- the next DEC_BURST
+        // tiles of the phase-2 range are pulled into L2: HBM keeps streaming through the gap.
+        int p2_issued = 0;
         bool pf_live = a.pf > 0;
         for (int i = 0; i < a.pf && pf_live; ++i) {
             pf_live = seq_next_tile(pf, t);
@@ -393,6 +421,12 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                 mbar_expect_tx(full_bar(stage), WT_BYTES);
                 if (hint) bulk_g2s_hint(ring_s + stage * WT_BYTES, t, WT_BYTES, full_bar(stage), pol_stream);
                 else bulk_g2s(ring_s + stage * WT_BYTES, t, WT_BYTES, full_bar(stage));
+            }
+            if (DEC_BURST > 0 && a.pf == 0 && ld.ph == 2 && ++p2_issued == NS) {
+                Seq b = ld;
+                const uint8_t* tb;
+                for (int i = 0; i < DEC_BURST && seq_next_tile(b, tb); ++i)
+                    if (el) bulk_prefetch_l2(tb, WT_BYTES);
             }
             if (++stage == NS) { stage = 0; phase ^= 1u; }
         }
@@ -515,18 +549,13 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             for (int m = 0; m < 4; ++m)
                 dst[m] = make_float4(__uint_as_float(v[4 * m]), __uint_as_float(v[4 * m + 1]), __uint_as_float(v[4 * m + 2]),
                                      __uint_as_float(v[4 * m + 3]));
+            // the piece is written: tell the readers of this item (no grid barrier between the phases -- a phase-2 piece
+            // waits only for the few CTAs that hold pieces of ITS item)
+            asm volatile("bar.sync 2, 128;" ::: "memory");
+            if (tid == 64) item_signal(a.icnt + p.item);
             ++i;
         }
-        // ---- grid barrier A: every partial is written (and yacc is zeroed) before anybody reads / reduces
-        __threadfence();
-        asm volatile("bar.sync 2, 128;" ::: "memory");
         DEC_TRE(2);
-        if (tid == 64) {
-            grid_arrive(a.state, 0, G);
-            grid_wait(a.state, 0, ax->gen0[0]);
-        }
-        asm volatile("bar.sync 2, 128;" ::: "memory");
-        DEC_TRE(3);
         // ---- phase 2
         int cur = 0, prev_run = -1, nseg = 0;
         uint32_t touched = 0;
@@ -547,14 +576,30 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             {
                 const long long t0 = (long long)p.item * D.nKB1;
                 const int c0 = cta_of_tile(t0, T1, (int)G), c1 = cta_of_tile(t0 + D.nKB1 - 1, T1, (int)G);
-                for (int c = c0; c <= c1; ++c) {
-                    // a CTA between c0 and c1 holds a piece of this item unless its own range is empty (fewer tiles than CTAs)
-                    if (T1 * c / G == T1 * (c + 1) / G) continue;
-                    const float4* src = (const float4*)(a.part + ((size_t)(p.item + c) * WT_ROWS + row) * DEC_N);
+                // a CTA between c0 and c1 holds a piece of this item unless its own range is empty (fewer tiles than CTAs)
+                auto holds = [&](int c) { return T1 * c / G != T1 * (c + 1) / G; };
+                if (lane == 0) {
+                    uint32_t need = 0;
+                    for (int c = c0; c <= c1; ++c) need += holds(c) ? 1u : 0u;
+                    item_wait(a.icnt + p.item, need, a.state);
+                }
+                __syncwarp();
+                if (i == 0) DEC_TRE(3);
+                // two pieces per step: eight independent 16-byte loads in flight per thread
+                for (int c = c0; c <= c1; c += 2) {
+                    const bool h0 = holds(c), h1 = c + 1 <= c1 && holds(c + 1);
+                    const float4* s0 = (const float4*)(a.part + ((size_t)(p.item + c) * WT_ROWS + row) * DEC_N);
+                    const float4* s1 = s0 + (size_t)WT_ROWS * DEC_N / 4;
+                    float4 f0[4], f1[4];
 #pragma unroll
                     for (int m = 0; m < 4; ++m) {
-                        const float4 f = __ldcg(src + m);
-                        acc[4 * m] += f.x; acc[4 * m + 1] += f.y; acc[4 * m + 2] += f.z; acc[4 * m + 3] += f.w;
+                        f0[m] = h0 ? __ldcg(s0 + m) : make_float4(0.f, 0.f, 0.f, 0.f);
+                        f1[m] = h1 ? __ldcg(s1 + m) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+#pragma unroll
+                    for (int m = 0; m < 4; ++m) {
+                        acc[4 * m] += f0[m].x + f1[m].x; acc[4 * m + 1] += f0[m].y + f1[m].y;
+                        acc[4 * m + 2] += f0[m].z + f1[m].z; acc[4 * m + 3] += f0[m].w + f1[m].w;
                     }
                 }
             }
@@ -593,6 +638,10 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                 }
                 mbar_wait(yfull, (uint32_t)(nseg & 1), a.state);
                 tc_fence_after();
+                if (nseg == 0) {                                    // every CTA's slice of yacc is zeroed (arrived in the prologues)
+                    if (lane == 0) cnt_wait(&a.state->dec_zcnt, ax->ztarget, a.state);
+                    __syncwarp();
+                }
                 if (nt <= 2) {
                     // one or two tokens (single-token decode): two columns per feature block, eight blocks per TMEM wait
                     const int t0 = __shfl_sync(0xffffffffu, tok, 0), t1 = __shfl_sync(0xffffffffu, tok, 1);
@@ -608,8 +657,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                         for (int u = 0; u < 8; ++u) {
                             const int feat = (db0 + u) * WT_ROWS + row;
                             if (db0 + u < D.nDB && ((touched >> (db0 + u)) & 1u) && feat < D.d) {
-                                atomicAdd(a.yacc + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
-                                if (nt == 2) atomicAdd(a.yacc + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
+                                red_add_f32(a.yacc + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
+                                if (nt == 2) red_add_f32(a.yacc + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
                             }
                         }
                     }
@@ -624,7 +673,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     for (int tk = 0; tk < DEC_N; ++tk) {
                         const int t = __shfl_sync(0xffffffffu, tok, tk);
                         const float w = __shfl_sync(0xffffffffu, wt, tk);
-                        if (tk < nt && feat < D.d) atomicAdd(a.yacc + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
+                        if (tk < nt && feat < D.d) red_add_f32(a.yacc + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
                     }
                 }
                 tc_fence_before();
@@ -693,7 +742,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     }
 
     // ------------------------------------------------------------------------------------------ yacc -> y
-    __threadfence();                                               // this thread's reductions are performed
+    // final grid barrier: every reduction into yacc is performed before anybody rounds it.  The arrival of thread 0 is a
+    // release that follows the block barrier, so it covers the reductions of all 320 threads.
     tc_fence_before();
     __syncthreads();
     DEC_TR(4);
@@ -702,12 +752,14 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         tmem_dealloc(tmem_base, 512);
     }
     if (tid == 0) {
-        grid_arrive(a.state, 1, G);
+        const unsigned long long target = cnt_target(cnt_arrive(&a.state->dec_bcnt), G);
         DEC_TR(7);
-        grid_wait(a.state, 1, ax->gen0[1]);
+        cnt_wait(&a.state->dec_bcnt, target, a.state);
     }
     __syncthreads();
     DEC_TR(5);
+    // the item counters go back to zero for the next call (nobody reads them after the barrier above)
+    for (int i = (int)((long long)W * blockIdx.x / G) + tid; i < (int)((long long)W * (blockIdx.x + 1) / G); i += DEC_THREADS) a.icnt[i] = 0u;
     {
         const size_t n4 = (size_t)a.T * D.d / 4;
         const float4* src = (const float4*)a.yacc;
@@ -753,10 +805,11 @@ cudaError_t init_decode_kernel() {
 
 cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
                           const int* ids, const float* topk_w, int T, int k, float* yacc, float* part,
-                          const __nv_bfloat16* y_add, __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st) {
+                          const __nv_bfloat16* y_add, __nv_bfloat16* y, DevState* state, uint32_t* item_cnt, int num_sms, int pf,
+                          cudaStream_t st) {
     DecArgs a{};
     a.D = D; a.V = V; a.r_table = r_table; a.x = (const uint4*)x; a.ids = ids; a.topk_w = topk_w;
-    a.yacc = yacc; a.part = part; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.T = T; a.k = k; a.A = T * k;
+    a.yacc = yacc; a.part = part; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.icnt = item_cnt; a.T = T; a.k = k; a.A = T * k;
     a.slots = decode_slots(D);
     a.pf = pf;
     const int smem = dec_fixed_smem(D) + a.slots * WT_BYTES;

@@ -25,6 +25,7 @@ constexpr int MAX_K = 16;
 constexpr int TABLE_STRIDE = 256;      // int32 per resident budget table
 constexpr int MAX_TABLES = 16;         // FXM_MAX_BUDGETS registered + 1 "set_budget" slot
 constexpr int DEC_MAX_A = 1024;        // most assignments T*k the fused decode kernel takes (int16 indices, smem routing)
+constexpr int DEC_MAX_RUNS = 320;      // >= DEC_MAX_A / 16 + MAX_E: most runs (expert, <= 16 tokens) of one decode call
 
 // byte offset of element (row, col) inside a swizzled tile whose rows are 128 B; row is the row index
 // relative to a base that is a multiple of 8 rows.
@@ -54,14 +55,16 @@ __host__ __device__ inline size_t dn_bytes(const Dims& D) { return (size_t)D.E *
 struct DevState {           // lives at the tail of the packed blob (zeroed by pack)
     uint32_t flags;         // bit0: expert id out of range; bit1: pipeline wait timed out
     uint32_t ticket;        // route: blocks that have published their histogram (reset by the last one)
-    uint32_t bar_count[2];  // decode kernel: top-level arrivals at grid barrier 0 / 1 (reset by the last arriver)
-    uint32_t bar_sub[2][8]; // decode kernel: first-level arrivals, CTA b uses counter b % 8 (reset by their last arrivers)
-    uint32_t pad0[10];
+    uint32_t pad0[2];
+    unsigned long long dec_zcnt;  // decode kernel: arrivals "my slice of yacc is zeroed" -- a counter that only grows: every launch adds
+                            //   exactly its grid size G (the same for every launch on this layer), so the value a CTA's own
+                            //   arrival returns tells it the target of ITS launch: (old / G + 1) * G.  64 bits: never wraps.
+    uint32_t pad1[24];
     uint32_t* hflag;        // host-mapped (pinned) word that also receives bit1: readable after a trap has killed the context
-                            // -> 128 bytes: the polled words below live in their own line
-    uint32_t bar_gen[2];    // decode kernel: generation of grid barrier 0 / 1 (sense reversal; never reset)
+                            // -> 128 bytes: the words below live in their own line
+    unsigned long long dec_bcnt;  // decode kernel: arrivals at the final grid barrier (same scheme as dec_zcnt)
     uint32_t route_gen;     // route kernel: bumped by the last block to publish its histogram (sense reversal; never reset)
-    uint32_t pad1[29];
+    uint32_t pad2[29];
 };
 static_assert(sizeof(DevState) == 256, "DevState layout");
 
@@ -279,6 +282,9 @@ bool decode_supported(const Dims& D);
 cudaError_t init_decode_kernel();
 cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table, const __nv_bfloat16* x,
                           const int* ids, const float* topk_w, int T, int k, float* yacc, float* part,
-                          const __nv_bfloat16* y_add, __nv_bfloat16* y, DevState* state, int num_sms, int pf, cudaStream_t st);
+                          const __nv_bfloat16* y_add, __nv_bfloat16* y, DevState* state, uint32_t* item_cnt, int num_sms, int pf,
+                          cudaStream_t st);
+// per-item "phase-1 pieces written" counters of the decode kernel (library-owned, in the blob's tail; zero between calls)
+__host__ __device__ inline size_t decode_cnt_bytes(const Dims& D) { return sizeof(uint32_t) * (size_t)DEC_MAX_RUNS * D.nCB; }
 
 }  // namespace fxm

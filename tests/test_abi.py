@@ -73,7 +73,7 @@ def test_clipped_bytes_follow_the_linear_law():
         assert L.fxm_clipped_bytes(E, d, I, rr.ctypes.data, ctypes.byref(n)) == 0
         sizes.append(n.value)
     const = sizes[-1]
-    assert const < 64 * 1024
+    assert const < 128 * 1024                                      # header + 16 tables + state + decode item counters
     for r, n in zip((2560, 1920, 1536, 1280, 640), sizes):
         assert n - const == 6 * d * E * r                          # widths are multiples of 64 here: exact
     bad = np.full(E, I + 1, np.int32)
