@@ -359,6 +359,15 @@ def run_ours(args):
                       lay.channel_rank)
     L.set_budget(r)
     torch.cuda.synchronize()
+    if args.switch_only:
+        # nothing but the C5 switching loop (for a profiler's launch list: which kernels and copies a budget switch costs)
+        sampler = ClockSampler(local)
+        sampler.start()
+        out = {"switch": run_switch(torch, fx, gen, L, sh, args.switch_steps, sampler)}
+        sampler.stop()
+        assert L.device_flags() == 0
+        print(json.dumps(out), flush=True)
+        return
     dev = to_device(fx, torch, hb)
     y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
     stream = torch.cuda.current_stream()
@@ -598,6 +607,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-sweep", action="store_true", help="skip the budget_sweep and switch legs")
     ap.add_argument("--switch-steps", type=int, default=200)
+    ap.add_argument("--switch-only", action="store_true", help="run only the C5 switching loop (N=1) and print its record")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from an ncu --set full capture of this config (else null)")
     args = ap.parse_args()

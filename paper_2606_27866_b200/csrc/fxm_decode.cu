@@ -39,10 +39,6 @@ constexpr int DEC_XE_KB_BYTES = DEC_N * ROW_BYTES;   // 2 KB of Xe per k-block
 constexpr int DEC_MAX_SLOTS = 12;
 constexpr int DEC_SMEM_MAX = 232448;              // 227 KB
 constexpr int DEC_PART = WT_ROWS * DEC_N;         // floats of one phase-1 partial: 128 packed rows x 16 tokens (8 KB)
-#ifndef FXM_DEC_BURST
-#define FXM_DEC_BURST 16
-#endif
-constexpr int DEC_BURST = FXM_DEC_BURST;          // phase-2 tiles pulled into L2 while the CTA waits for the phase-1 partials (0 = none)
 constexpr int DEC_MAX_CTAS = 160;                 // the partial-slot capacity is sized for at most this many CTAs
 
 struct DecArgs {
@@ -52,7 +48,10 @@ struct DecArgs {
     const uint4* x;            // [T][d] bf16
     const int* ids;            // [T][k]
     const float* topk_w;       // [T][k]
-    float* yacc;               // [T][d] fp32 scratch (workspace)
+    float* yacc;               // [R][T][d] fp32 scratch (workspace): R copies of the accumulator, CTA b adds into copy b % R
+    int R;                     // copies (1 .. 16, R * T <= 64): with a handful of tokens every CTA's reductions land on the same
+                               //   few lines and serialise in L2 (~100 cycles per 128-byte reduction and line; measured 5-10 us
+                               //   at T = 1); spreading them over R copies divides that by R, the final pass sums the copies
     float* part;               // phase-1 partials: [(items + #CTAs)][128][16] fp32 (workspace)
     const uint2* y_add;        // [T][d] bf16 or null: shared-expert output added in fp32 before the rounding of y
     __nv_bfloat16* y;          // [T][d]
@@ -251,7 +250,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     // CTA checks that ALL slices are published before its first reduction (a split barrier: arrive here, wait ~20 us later)
     {
         float4* z = (float4*)a.yacc;
-        const size_t n4 = (size_t)a.T * D.d / 4;
+        const size_t n4 = (size_t)a.R * a.T * D.d / 4;
         for (size_t i = (size_t)blockIdx.x * DEC_THREADS + tid; i < n4; i += (size_t)G * DEC_THREADS)
             z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
@@ -400,11 +399,6 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         seq_init(ld);
         seq_init(pf);
         const uint8_t* t;
-        // Between the last phase-1 tile and the first H of phase 2 lie ~5 us (partials -> global memory -> item counter ->
-        // partials read back -> SwiGLU) in which the ring is full of phase-2 tiles and this SM requests nothing.  At that
-        // moment -- and only then, so that the requests do not compete with the ring's own loads -- the next DEC_BURST
-        // tiles of the phase-2 range are pulled into L2: HBM keeps streaming through the gap.
-        int p2_issued = 0;
         bool pf_live = a.pf > 0;
         for (int i = 0; i < a.pf && pf_live; ++i) {
             pf_live = seq_next_tile(pf, t);
@@ -421,12 +415,6 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                 mbar_expect_tx(full_bar(stage), WT_BYTES);
                 if (hint) bulk_g2s_hint(ring_s + stage * WT_BYTES, t, WT_BYTES, full_bar(stage), pol_stream);
                 else bulk_g2s(ring_s + stage * WT_BYTES, t, WT_BYTES, full_bar(stage));
-            }
-            if (DEC_BURST > 0 && a.pf == 0 && ld.ph == 2 && ++p2_issued == NS) {
-                Seq b = ld;
-                const uint8_t* tb;
-                for (int i = 0; i < DEC_BURST && seq_next_tile(b, tb); ++i)
-                    if (el) bulk_prefetch_l2(tb, WT_BYTES);
             }
             if (++stage == NS) { stage = 0; phase ^= 1u; }
         }
@@ -530,6 +518,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         const int q = warp & 3;
         const uint32_t lane_base = (uint32_t)(q * 32) << 16;
         const int row = q * 32 + lane;                              // packed gate/up row (phase 1), output feature in a block (phase 2)
+        float* const ycopy = a.yacc + (size_t)(blockIdx.x % (uint32_t)a.R) * a.T * D.d;     // this CTA's copy of the accumulator
         PieceIter it;
         Piece p;
         int i = 0;
@@ -657,8 +646,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                         for (int u = 0; u < 8; ++u) {
                             const int feat = (db0 + u) * WT_ROWS + row;
                             if (db0 + u < D.nDB && ((touched >> (db0 + u)) & 1u) && feat < D.d) {
-                                red_add_f32(a.yacc + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
-                                if (nt == 2) red_add_f32(a.yacc + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
+                                red_add_f32(ycopy + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
+                                if (nt == 2) red_add_f32(ycopy + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
                             }
                         }
                     }
@@ -673,7 +662,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     for (int tk = 0; tk < DEC_N; ++tk) {
                         const int t = __shfl_sync(0xffffffffu, tok, tk);
                         const float w = __shfl_sync(0xffffffffu, wt, tk);
-                        if (tk < nt && feat < D.d) red_add_f32(a.yacc + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
+                        if (tk < nt && feat < D.d) red_add_f32(ycopy + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
                     }
                 }
                 tc_fence_before();
@@ -766,6 +755,10 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         uint2* dst = (uint2*)a.y;
         for (size_t i = (size_t)blockIdx.x * DEC_THREADS + tid; i < n4; i += (size_t)G * DEC_THREADS) {
             float4 f = __ldcg(src + i);
+            for (int r = 1; r < a.R; ++r) {                          // the other copies of the accumulator
+                const float4 g = __ldcg(src + (size_t)r * n4 + i);
+                f.x += g.x; f.y += g.y; f.z += g.z; f.w += g.w;
+            }
             if (a.y_add) {
                 const uint2 sa = __ldg(a.y_add + i);
                 f.x += __uint_as_float(sa.x << 16); f.y += __uint_as_float(sa.x & 0xFFFF0000u);
@@ -810,6 +803,7 @@ cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table,
     DecArgs a{};
     a.D = D; a.V = V; a.r_table = r_table; a.x = (const uint4*)x; a.ids = ids; a.topk_w = topk_w;
     a.yacc = yacc; a.part = part; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.icnt = item_cnt; a.T = T; a.k = k; a.A = T * k;
+    a.R = (T >= DEC_YACC_ROWS || T < 1) ? 1 : (DEC_YACC_ROWS / T < 16 ? DEC_YACC_ROWS / T : 16);     // map_workspace sizes yacc for >= DEC_YACC_ROWS rows
     a.slots = decode_slots(D);
     a.pf = pf;
     const int smem = dec_fixed_smem(D) + a.slots * WT_BYTES;

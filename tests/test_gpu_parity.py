@@ -231,8 +231,9 @@ def test_decode_groups_runs_and_skew(T, k, E, bias):
 
 
 def test_decode_repeated_calls_and_interleaving_with_general_path():
-    """The grid barriers of the decode kernel are sense-reversing counters that live across calls: many calls in a
-    row (no host sync), alternating with general-path calls and with budget switches, must all be right."""
+    """The decode kernel's grid-wide synchronisation lives across calls (ever-growing arrival counters in the layer's state,
+    per-item readiness counters that every call hands back zeroed): many calls in a row (no host sync), alternating with
+    general-path calls and with budget switches, must all be right."""
     import torch
     import gpu_util as gu
     fx = _fx()
