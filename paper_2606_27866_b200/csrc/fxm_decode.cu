@@ -17,7 +17,8 @@
 //            channels >= r_e, round once to bf16 -> Hs; Y[db] += Wd_tile(e, cb, db) . Hs^T accumulates in
 //            TMEM over the consecutive pieces of a run; at the end of the run segment the touched feature blocks are
 //            scaled by the router weight (Alg. 2 l.19) and added to yacc[t][:] with fp32 reductions (l.20 ScatterAdd).
-//   Both phases are balanced to +-1 tile whatever the routing and the budget.
+//   Both phases are balanced to +-1 tile whatever the routing and the budget.  With no more runs than CTAs (a handful of
+//   tokens) the CTAs are first dealt out to the runs, so that no range crosses a run boundary (struct Split).
 // Roles (320 threads): warp 0 weight producer (16 KB cp.async.bulk per tile through a shared-memory ring; it starts
 // fetching phase-2 tiles while the grid barrier is still closing), warp 1 MMA issuer, warps 2-5 epilogue, warps 6-9
 // stage the <= 16 token rows x[t] of a run into swizzled K-major panels Xe (X[pi], Alg. 2 l.7).
@@ -48,10 +49,7 @@ struct DecArgs {
     const uint4* x;            // [T][d] bf16
     const int* ids;            // [T][k]
     const float* topk_w;       // [T][k]
-    float* yacc;               // [R][T][d] fp32 scratch (workspace): R copies of the accumulator, CTA b adds into copy b % R
-    int R;                     // copies (1 .. 16, R * T <= 64): with a handful of tokens every CTA's reductions land on the same
-                               //   few lines and serialise in L2 (~100 cycles per 128-byte reduction and line; measured 5-10 us
-                               //   at T = 1); spreading them over R copies divides that by R, the final pass sums the copies
+    float* yacc;               // [T][d] fp32 scratch (workspace)
     float* part;               // phase-1 partials: [(items + #CTAs)][128][16] fp32 (workspace)
     const uint2* y_add;        // [T][d] bf16 or null: shared-expert output added in fp32 before the rounding of y
     __nv_bfloat16* y;          // [T][d]
@@ -68,11 +66,14 @@ struct DecAux {
     int run_pos[DEC_MAX_RUNS];     // first sorted position of the run
     int run_ib[DEC_MAX_RUNS + 1];  // first item of the run; [n_runs] = W
     int16_t perm[DEC_MAX_A];       // sorted position -> flat assignment index
+    float wts[DEC_MAX_A];          // topk_w by flat assignment index (read once in the prologue)
     int r[MAX_E];
     uint32_t eb[MAX_E];            // first channel block of each expert in the weight regions (LayerView::eblk)
     uint64_t bars[2 * DEC_MAX_SLOTS + 16];
     uint32_t tmem_slot;
     int n_runs, W;
+    int aligned;                   // 1: the CTAs are dealt out to the runs first (crun), no CTA's range crosses a run boundary
+    int16_t crun[DEC_MAX_CTAS + 2];    // aligned: first CTA of run r (r <= n_runs <= G); crun[n_runs] = G
     unsigned long long ztarget;    // value of DevState::dec_zcnt at which every CTA of THIS launch has zeroed its slice of yacc
 };
 // prologue-only scratch, aliased on the weight ring (>= 4 slots = 64 KB)
@@ -181,6 +182,42 @@ __device__ __forceinline__ int run_of(const DecAux* ax, int item, int& cur) {
 // CTA that owns tile t of a list of Tn tiles split over G CTAs as [c Tn / G, (c + 1) Tn / G)
 __device__ __forceinline__ int cta_of_tile(long long t, long long Tn, int G) { return (int)(((t + 1) * G - 1) / Tn); }
 
+// How the tile list of a phase (tpi tiles per item) is cut into one contiguous range per CTA.
+//   flat:    CTA c owns [c Tn / G, (c + 1) Tn / G) of the whole list (balanced to +-1 tile; ranges cross run boundaries).
+//   aligned: when the call has no more runs than CTAs (a handful of tokens), the CTAs are dealt out to the runs in
+//            proportion to their items (run r gets the CTAs [crun[r], crun[r+1])) and each run's tiles are cut evenly
+//            among ITS CTAs.  No range crosses a run boundary, so no CTA restages x in phase 1 or drains and refills its
+//            Y partial in phase 2 -- measured at C4 T=1: the four CTAs with a run boundary finished phase 2 ~3 us after
+//            the rest and the whole grid waited for them.  Costs an imbalance of at most one part in ~18.
+struct Split {
+    const DecAux* ax;
+    long long W;
+    int G, aligned;
+    __device__ __forceinline__ void range(int c, int tpi, long long& lo, long long& hi) const {
+        if (!aligned) { const long long Tn = W * tpi; lo = Tn * c / G; hi = Tn * (c + 1) / G; return; }
+        int r = 0;
+        while ((int)ax->crun[r + 1] <= c) ++r;
+        const int c0 = ax->crun[r], nc = ax->crun[r + 1] - c0;
+        const long long tb = (long long)ax->run_ib[r] * tpi, n = (long long)(ax->run_ib[r + 1] - ax->run_ib[r]) * tpi;
+        lo = tb + n * (c - c0) / nc;
+        hi = tb + n * (c - c0 + 1) / nc;
+    }
+    // owner of tile t, which belongs to run `run`
+    __device__ __forceinline__ int owner(long long t, int run, int tpi) const {
+        if (!aligned) return cta_of_tile(t, W * tpi, G);
+        const int c0 = ax->crun[run], nc = ax->crun[run + 1] - c0;
+        const long long tb = (long long)ax->run_ib[run] * tpi, n = (long long)(ax->run_ib[run + 1] - ax->run_ib[run]) * tpi;
+        return c0 + (int)(((t - tb + 1) * nc - 1) / n);
+    }
+    // does CTA c (a CTA of run `run` when aligned) own any tile of the phase?
+    __device__ __forceinline__ bool holds(int c, int run, int tpi) const {
+        if (!aligned) { const long long Tn = W * tpi; return Tn * c / G != Tn * (c + 1) / G; }
+        const int c0 = ax->crun[run], nc = ax->crun[run + 1] - c0;
+        const long long n = (long long)(ax->run_ib[run + 1] - ax->run_ib[run]) * tpi;
+        return n * (c - c0) / nc != n * (c - c0 + 1) / nc;
+    }
+};
+
 #ifdef FXM_TRACE
 __device__ unsigned long long g_dtrace[148][16];
 __device__ __forceinline__ unsigned long long dec_now() {
@@ -238,19 +275,27 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     }
     if (warp == 1) tmem_alloc(smem_u32(&ax->tmem_slot), 512);
     pdl_wait();                                              // the previous kernel may still use the workspace / write x, ids
-    bool bad = false;
-    for (int f = tid; f < A; f += DEC_THREADS) {
-        int id = a.ids[f];
-        if (id < 0 || id >= E) { bad = true; id = -1; }
-        tp->ids[f] = (int16_t)id;
+    // Every global load of the prologue is issued at once (ids, router weights, the width table, the block index: one
+    // DRAM round trip when the lines are cold), the zeroing below runs while they are in flight, then they are consumed.
+    constexpr int PER = (DEC_MAX_A + DEC_THREADS - 1) / DEC_THREADS;
+    static_assert(MAX_E <= DEC_THREADS, "one width per thread");
+    int idv[PER];
+    float wv[PER];
+#pragma unroll
+    for (int u = 0; u < PER; ++u) {
+        const int f = tid + u * DEC_THREADS;
+        idv[u] = f < A ? __ldg(a.ids + f) : 0;
+        wv[u] = f < A ? __ldg(a.topk_w + f) : 0.f;
     }
-    if (bad) atomicOr(&a.state->flags, 1u);
-    for (int e = tid; e < MAX_E; e += DEC_THREADS) { ax->r[e] = e < E ? a.r_table[e] : 0; ax->eb[e] = e < E ? a.V.eblk[e] : 0u; }
+    const int rv = tid < E ? __ldg(a.r_table + tid) : 0;
+    const uint32_t ebv = tid < E ? __ldg(a.V.eblk + tid) : 0u;
+    // a handful of tokens: pull x into L2 now, the stagers ask for their rows only after the grouping
+    if (tid == 0 && (size_t)a.T * D.d * 2 <= 65536) bulk_prefetch_l2(a.x, (uint32_t)((size_t)a.T * D.d * 2));
     // zero this CTA's slice of the fp32 accumulator; the arrival below (after the next block barrier) publishes it, and every
     // CTA checks that ALL slices are published before its first reduction (a split barrier: arrive here, wait ~20 us later)
     {
         float4* z = (float4*)a.yacc;
-        const size_t n4 = (size_t)a.R * a.T * D.d / 4;
+        const size_t n4 = (size_t)a.T * D.d / 4;
         for (size_t i = (size_t)blockIdx.x * DEC_THREADS + tid; i < n4; i += (size_t)G * DEC_THREADS)
             z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
@@ -261,6 +306,23 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     const int chunk = ((A + NW - 1) / NW + 31) & ~31;
     const int wlo = min(A, warp * chunk), whi = min(A, wlo + chunk);
     for (int i = tid; i < NW * MAX_E; i += DEC_THREADS) (&tp->wh[0][0])[i] = 0;
+    // Xe / Hs start as zeros (rows beyond a run's token count are never staged)
+    for (int i = tid; i < (int)((aux_off - xe_off) / 16); i += DEC_THREADS) ((uint4*)xe_gen)[i] = make_uint4(0, 0, 0, 0);
+    {
+        bool bad = false;
+#pragma unroll
+        for (int u = 0; u < PER; ++u) {
+            const int f = tid + u * DEC_THREADS;
+            if (f < A) {
+                int id = idv[u];
+                if (id < 0 || id >= E) { bad = true; id = -1; }
+                tp->ids[f] = (int16_t)id;
+                ax->wts[f] = wv[u];
+            }
+        }
+        if (bad) atomicOr(&a.state->flags, 1u);
+        if (tid < MAX_E) { ax->r[tid] = rv; ax->eb[tid] = ebv; }
+    }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -342,16 +404,28 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             ax->run_ib[slot] = tp->ibase[tid] + g * nb;
         }
     }
-    __syncthreads();
-    // Xe / Hs start as zeros (rows beyond a run's token count are never staged)
-    for (int i = tid; i < (int)((aux_off - xe_off) / 16); i += DEC_THREADS) ((uint4*)xe_gen)[i] = make_uint4(0, 0, 0, 0);
     if (tid == DEC_THREADS - 1) ax->ztarget = cnt_target(zold, G);
-    fence_proxy_async_smem();
+    fence_proxy_async_smem();                                // the zeros of Xe / Hs -> visible to the tensor core's reads
     __syncthreads();
     const int W = ax->W;
-    const long long T1 = (long long)W * D.nKB1, T2 = (long long)W * D.nDB;
-    const long long lo1 = T1 * blockIdx.x / G, hi1 = T1 * (blockIdx.x + 1) / G;
-    const long long lo2 = T2 * blockIdx.x / G, hi2 = T2 * (blockIdx.x + 1) / G;
+    // deal the CTAs out to the runs (see Split): possible when every run gets at least one CTA
+    if (warp == 0) {
+        const int nr = ax->n_runs;
+        bool ok = nr >= 1 && nr <= (int)G && W > 0;
+        if (ok) {
+            for (int r = lane; r <= nr; r += 32) ax->crun[r] = (int16_t)((long long)G * ax->run_ib[r] / W);
+            __syncwarp();
+            for (int r = lane; r < nr; r += 32) ok = ok && ax->crun[r + 1] > ax->crun[r];
+        }
+        ok = __all_sync(0xffffffffu, ok);
+        if (lane == 0) ax->aligned = ok ? 1 : 0;
+    }
+    __syncthreads();
+    Split sp;
+    sp.ax = ax; sp.W = W; sp.G = (int)G; sp.aligned = ax->aligned;
+    long long lo1, hi1, lo2, hi2;
+    sp.range((int)blockIdx.x, D.nKB1, lo1, hi1);
+    sp.range((int)blockIdx.x, D.nDB, lo2, hi2);
     DEC_TR(1);
 
     if (warp == 0) {
@@ -518,7 +592,6 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         const int q = warp & 3;
         const uint32_t lane_base = (uint32_t)(q * 32) << 16;
         const int row = q * 32 + lane;                              // packed gate/up row (phase 1), output feature in a block (phase 2)
-        float* const ycopy = a.yacc + (size_t)(blockIdx.x % (uint32_t)a.R) * a.T * D.d;     // this CTA's copy of the accumulator
         PieceIter it;
         Piece p;
         int i = 0;
@@ -550,6 +623,41 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         uint32_t touched = 0;
         i = 0;
         it.init(lo2, hi2, D.nDB);
+        // the CTAs c0 .. c1 hold the phase-1 pieces of an item (except those whose own range is empty)
+        auto item_ctas = [&](int item, int run, int& c0, int& c1) {
+            const long long t0 = (long long)item * D.nKB1;
+            c0 = sp.owner(t0, run, D.nKB1);
+            c1 = sp.owner(t0 + D.nKB1 - 1, run, D.nKB1);
+        };
+        auto item_need = [&](int item, int run) -> uint32_t {
+            int c0, c1;
+            item_ctas(item, run, c0, c1);
+            uint32_t need = 0;
+            for (int c = c0; c <= c1; ++c) need += sp.holds(c, run, D.nKB1) ? 1u : 0u;
+            return need;
+        };
+        auto load_partials = [&](int item, int run, float (&out)[16]) {
+            int c0, c1;
+            item_ctas(item, run, c0, c1);
+#pragma unroll
+            for (int m = 0; m < 16; ++m) out[m] = 0.f;
+            for (int c = c0; c <= c1; c += 2) {          // two pieces per step: eight independent 16-byte loads in flight per thread
+                const bool h0 = sp.holds(c, run, D.nKB1), h1 = c + 1 <= c1 && sp.holds(c + 1, run, D.nKB1);
+                const float4* s0 = (const float4*)(a.part + ((size_t)(item + c) * WT_ROWS + row) * DEC_N);
+                const float4* s1 = s0 + (size_t)WT_ROWS * DEC_N / 4;
+                float4 f0[4], f1[4];
+#pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    f0[m] = h0 ? __ldcg(s0 + m) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    f1[m] = h1 ? __ldcg(s1 + m) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    out[4 * m] += f0[m].x + f1[m].x; out[4 * m + 1] += f0[m].y + f1[m].y;
+                    out[4 * m + 2] += f0[m].z + f1[m].z; out[4 * m + 3] += f0[m].w + f1[m].w;
+                }
+            }
+        };
         bool more = it.next(p);
         while (more) {
             const int run = run_of(ax, p.item, cur);
@@ -560,38 +668,14 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             const int b = i & 1, u = i >> 1;
             // h of item (run, cb): sum of the partials of the CTAs that touched the item in phase 1
             float acc[16];
-#pragma unroll
-            for (int m = 0; m < 16; ++m) acc[m] = 0.f;
-            {
-                const long long t0 = (long long)p.item * D.nKB1;
-                const int c0 = cta_of_tile(t0, T1, (int)G), c1 = cta_of_tile(t0 + D.nKB1 - 1, T1, (int)G);
-                // a CTA between c0 and c1 holds a piece of this item unless its own range is empty (fewer tiles than CTAs)
-                auto holds = [&](int c) { return T1 * c / G != T1 * (c + 1) / G; };
-                if (lane == 0) {
-                    uint32_t need = 0;
-                    for (int c = c0; c <= c1; ++c) need += holds(c) ? 1u : 0u;
-                    item_wait(a.icnt + p.item, need, a.state);
-                }
-                __syncwarp();
-                if (i == 0) DEC_TRE(3);
-                // two pieces per step: eight independent 16-byte loads in flight per thread
-                for (int c = c0; c <= c1; c += 2) {
-                    const bool h0 = holds(c), h1 = c + 1 <= c1 && holds(c + 1);
-                    const float4* s0 = (const float4*)(a.part + ((size_t)(p.item + c) * WT_ROWS + row) * DEC_N);
-                    const float4* s1 = s0 + (size_t)WT_ROWS * DEC_N / 4;
-                    float4 f0[4], f1[4];
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) {
-                        f0[m] = h0 ? __ldcg(s0 + m) : make_float4(0.f, 0.f, 0.f, 0.f);
-                        f1[m] = h1 ? __ldcg(s1 + m) : make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
-#pragma unroll
-                    for (int m = 0; m < 4; ++m) {
-                        acc[4 * m] += f0[m].x + f1[m].x; acc[4 * m + 1] += f0[m].y + f1[m].y;
-                        acc[4 * m + 2] += f0[m].z + f1[m].z; acc[4 * m + 3] += f0[m].w + f1[m].w;
-                    }
-                }
-            }
+            if (lane == 0) item_wait(a.icnt + p.item, item_need(p.item, run), a.state);
+            __syncwarp();
+            if (i == 0) DEC_TRE(3);
+            load_partials(p.item, run, acc);
+            Piece nx;
+            more = it.next(nx);
+            int cur2 = cur;
+            const int run_nx = more ? run_of(ax, nx.item, cur2) : -1;
             const int ch = q * 16 + (lane & 15);
             const bool keep = cb * CB + ch < ax->r[e];              // tail of the last retained block (pad-zero rule)
             const int odd = lane >> 4;
@@ -612,10 +696,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             fence_proxy_async_smem();
             mbar_arrive(hfull(b));
             touched |= ((p.b >= 32 ? 0xFFFFFFFFu : ((1u << p.b) - 1u)) & ~((1u << p.a) - 1u));
-            Piece nx;
-            more = it.next(nx);
-            int cur2 = cur;
-            const bool run_ends = !more || run_of(ax, nx.item, cur2) != run;
+            const bool run_ends = !more || run_nx != run;
             if (run_ends) {
                 // ---- end of the run segment: touched feature blocks of Y -> yacc (router-weight scale + ScatterAdd, Alg. 2 l.19-20)
                 int tok = 0;
@@ -623,7 +704,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                 if (lane < nt) {
                     const int f = ax->perm[ax->run_pos[run] + lane];
                     tok = f / k;
-                    wt = a.topk_w[f];
+                    wt = ax->wts[f];
                 }
                 mbar_wait(yfull, (uint32_t)(nseg & 1), a.state);
                 tc_fence_after();
@@ -646,8 +727,8 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                         for (int u = 0; u < 8; ++u) {
                             const int feat = (db0 + u) * WT_ROWS + row;
                             if (db0 + u < D.nDB && ((touched >> (db0 + u)) & 1u) && feat < D.d) {
-                                red_add_f32(ycopy + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
-                                if (nt == 2) red_add_f32(ycopy + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
+                                red_add_f32(a.yacc + (size_t)t0 * D.d + feat, w0 * __uint_as_float(v0[u]));
+                                if (nt == 2) red_add_f32(a.yacc + (size_t)t1 * D.d + feat, w1 * __uint_as_float(v1[u]));
                             }
                         }
                     }
@@ -662,11 +743,12 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                     for (int tk = 0; tk < DEC_N; ++tk) {
                         const int t = __shfl_sync(0xffffffffu, tok, tk);
                         const float w = __shfl_sync(0xffffffffu, wt, tk);
-                        if (tk < nt && feat < D.d) red_add_f32(ycopy + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
+                        if (tk < nt && feat < D.d) red_add_f32(a.yacc + (size_t)t * D.d + feat, w * __uint_as_float(v[tk]));
                     }
                 }
                 tc_fence_before();
                 mbar_arrive(yempty);
+                DEC_TRE(12);
                 ++nseg;
             }
             p = nx;
@@ -741,6 +823,10 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         tmem_dealloc(tmem_base, 512);
     }
     if (tid == 0) {
+#ifdef FXM_TRACE
+        asm volatile("fence.acq_rel.gpu;" ::: "memory");
+        DEC_TR(13);
+#endif
         const unsigned long long target = cnt_target(cnt_arrive(&a.state->dec_bcnt), G);
         DEC_TR(7);
         cnt_wait(&a.state->dec_bcnt, target, a.state);
@@ -755,10 +841,6 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         uint2* dst = (uint2*)a.y;
         for (size_t i = (size_t)blockIdx.x * DEC_THREADS + tid; i < n4; i += (size_t)G * DEC_THREADS) {
             float4 f = __ldcg(src + i);
-            for (int r = 1; r < a.R; ++r) {                          // the other copies of the accumulator
-                const float4 g = __ldcg(src + (size_t)r * n4 + i);
-                f.x += g.x; f.y += g.y; f.z += g.z; f.w += g.w;
-            }
             if (a.y_add) {
                 const uint2 sa = __ldg(a.y_add + i);
                 f.x += __uint_as_float(sa.x << 16); f.y += __uint_as_float(sa.x & 0xFFFF0000u);
@@ -803,7 +885,6 @@ cudaError_t launch_decode(const Dims& D, const LayerView& V, const int* r_table,
     DecArgs a{};
     a.D = D; a.V = V; a.r_table = r_table; a.x = (const uint4*)x; a.ids = ids; a.topk_w = topk_w;
     a.yacc = yacc; a.part = part; a.y_add = (const uint2*)y_add; a.y = y; a.state = state; a.icnt = item_cnt; a.T = T; a.k = k; a.A = T * k;
-    a.R = (T >= DEC_YACC_ROWS || T < 1) ? 1 : (DEC_YACC_ROWS / T < 16 ? DEC_YACC_ROWS / T : 16);     // map_workspace sizes yacc for >= DEC_YACC_ROWS rows
     a.slots = decode_slots(D);
     a.pf = pf;
     const int smem = dec_fixed_smem(D) + a.slots * WT_BYTES;

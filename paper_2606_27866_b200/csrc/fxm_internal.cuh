@@ -25,7 +25,6 @@ constexpr int MAX_K = 16;
 constexpr int TABLE_STRIDE = 256;      // int32 per resident budget table
 constexpr int MAX_TABLES = 16;         // FXM_MAX_BUDGETS registered + 1 "set_budget" slot
 constexpr int DEC_MAX_A = 1024;        // most assignments T*k the fused decode kernel takes (int16 indices, smem routing)
-constexpr int DEC_YACC_ROWS = 64;      // the decode kernel keeps R copies of its fp32 accumulator, R * T <= DEC_YACC_ROWS
 constexpr int DEC_MAX_RUNS = 320;      // >= DEC_MAX_A / 16 + MAX_E: most runs (expert, <= 16 tokens) of one decode call
 
 // byte offset of element (row, col) inside a swizzled tile whose rows are 128 B; row is the row index
@@ -151,8 +150,7 @@ __host__ inline Workspace map_workspace(const Dims& D, int T, int k, void* base)
     w.bhist = (int*)(b + take(sizeof(int) * (size_t)RT_MAX_BLOCKS * D.E));   // capacity, not RB: the size stays monotonic in T
     w.tt = (int4*)(b + take(sizeof(int4) * ((size_t)NT + 1)));
     w.H = b + take((size_t)D.nCB * P * ROW_BYTES);
-    // every T (the size is monotonic in T); at least DEC_YACC_ROWS rows: the decode kernel spreads its reductions over copies
-    w.yacc = (float*)(b + take((size_t)(T > DEC_YACC_ROWS ? T : DEC_YACC_ROWS) * D.d * sizeof(float)));
+    w.yacc = (float*)(b + take((size_t)T * D.d * sizeof(float)));       // every T: the size is monotonic in T
     w.dec_part = (float*)(b + take(decode_part_bytes(D, (long long)A)));
     w.RB = RB;
     w.chunk = chunk;

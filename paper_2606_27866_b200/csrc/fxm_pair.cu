@@ -69,20 +69,7 @@ constexpr int PAIR_TQ = 8;                      // TMEM sub-tile barrier ring
 #ifndef FXM_PAIR_PF
 #define FXM_PAIR_PF 0
 #endif
-constexpr int PAIR_PF = FXM_PAIR_PF;
-// tuning knobs (A/B builds only; the defaults are the product)
-#ifndef FXM_PAIR_WPOL
-#define FXM_PAIR_WPOL 1      // 1: weight tiles are loaded evict_first
-#endif
-#ifndef FXM_PAIR_HPOL
-#define FXM_PAIR_HPOL 1      // 1: H panels are stored evict_last
-#endif
-#ifndef FXM_G2_ORDER
-#define FXM_G2_ORDER 0       // 0: GEMM-2 items in (token tile, feature pair) order; 1: (feature pair, token tile)
-#endif
-#ifndef FXM_G2_EPI
-#define FXM_G2_EPI 0         // 0: red.global.add.f32; 1: plain stores and 2: nothing (both WRONG results, timing experiments)
-#endif                     // weight tiles the L2 prefetch cursor runs ahead (measured: 0 is fastest, 12 costs 2-5 %)
+constexpr int PAIR_PF = FXM_PAIR_PF;                     // weight tiles the L2 prefetch cursor runs ahead (measured: 0 is fastest, 12 costs 2-5 %)
 
 struct PairArgs {
     Dims D;
@@ -215,14 +202,8 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
         pairblk = wi - q.w;
     } else {
         const int nDBp = (D.nDB + 1) >> 1;
-        if (FXM_G2_ORDER == 0) {
-            q = a.items[wi / nDBp];
-            pairblk = wi % nDBp;
-        } else {
-            const int ntt = a.sched->ntt;
-            q = a.items[wi % ntt];
-            pairblk = wi / ntt;
-        }
+        q = a.items[wi / nDBp];
+        pairblk = wi % nDBp;
     }
     it.e = q.x;
     it.row0 = q.y;
@@ -396,8 +377,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                 if (leader_lane) {
                     const uint32_t sb = smem_base + s * stage_bytes;
                     mbar_expect_tx(full_bar(s), tx);
-                    if (FXM_PAIR_WPOL) bulk_g2s_hint(sb, asrc + kb * astride, WT_BYTES, full_bar(s), pol_stream);
-                    else bulk_g2s(sb, asrc + kb * astride, WT_BYTES, full_bar(s));
+                    bulk_g2s_hint(sb, asrc + kb * astride, WT_BYTES, full_bar(s), pol_stream);
                     if (!gather) {                                     // else: the gather warps bring the same bytes
                         bulk_g2s(sb + WT_BYTES, b0 + kb * bstride, h0 * ROW_BYTES, full_bar(s));
                         if (h1) bulk_g2s(sb + WT_BYTES + h0 * ROW_BYTES, b1 + kb * bstride, h1 * ROW_BYTES, full_bar(s));
@@ -593,8 +573,7 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                     fence_proxy_async_smem();                          // staging writes -> visible to the bulk-copy engine
                     epi_bar_sync_all();
                     if (et == 0 && it.valid) {
-                        if (FXM_PAIR_HPOL) bulk_s2g_hint(a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES, stg_base, (uint32_t)n * ROW_BYTES, pol_keep);
-                        else bulk_s2g(a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES, stg_base, (uint32_t)n * ROW_BYTES);
+                        bulk_s2g_hint(a.H + ((size_t)it.blk * a.P + rowS) * ROW_BYTES, stg_base, (uint32_t)n * ROW_BYTES, pol_keep);
                         bulk_commit();
                     }
                     store_pending = it.valid;                          // warp-uniform across the CTA
@@ -652,13 +631,9 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
 #pragma unroll
                                 for (int jj = 0; jj < 16; ++jj) {
                                     const int2 tw = r16[jj];           // same address in every lane: a broadcast
-                                    if (tw.x >= 0) {
-                                        if (FXM_G2_EPI == 0)
-                                            asm volatile("red.relaxed.gpu.global.add.f32 [%0], %1;" ::"l"(ycol + (size_t)tw.x * D.d),
-                                                         "f"(__int_as_float(tw.y) * __uint_as_float(v[u][jj])) : "memory");
-                                        else if (FXM_G2_EPI == 1)
-                                            ycol[(size_t)tw.x * D.d] = __int_as_float(tw.y) * __uint_as_float(v[u][jj]);
-                                    }
+                                    if (tw.x >= 0)
+                                        asm volatile("red.relaxed.gpu.global.add.f32 [%0], %1;" ::"l"(ycol + (size_t)tw.x * D.d),
+                                                     "f"(__int_as_float(tw.y) * __uint_as_float(v[u][jj])) : "memory");
                                 }
                             }
                         }

@@ -29,6 +29,7 @@ __global__ void __launch_bounds__(256) k_saliency_gu(int d, size_t rows, size_t 
     const size_t per4 = per >> 3;                                // chunks per gradient set
     for (size_t row = blockIdx.x * 8ull + (threadIdx.x >> 5); row < rows; row += (size_t)gridDim.x * 8) {
         float acc = 0.f;
+#pragma unroll 2
         for (int c = lane; c < cpr; c += 32) {
             const size_t o = row * cpr + c;
             const uint4 wg = __ldcs(Wg + o), wu = __ldcs(Wu + o);
@@ -84,7 +85,7 @@ __global__ void k_saliency_sum(const float* __restrict__ part, int slots, size_t
 }
 
 int saliency_row_chunks(const Dims& D) {
-    int R = (148 * 2 + D.E - 1) / D.E;                           // about two blocks per SM
+    int R = (148 * 8 + D.E - 1) / D.E;                           // about eight blocks per SM: a thread keeps only 12 loads in flight
     if (R > 16) R = 16;
     if (R > D.d) R = D.d;
     return R < 1 ? 1 : R;
