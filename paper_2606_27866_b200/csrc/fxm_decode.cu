@@ -40,6 +40,7 @@ constexpr int DEC_XE_KB_BYTES = DEC_N * ROW_BYTES;   // 2 KB of Xe per k-block
 constexpr int DEC_MAX_SLOTS = 12;
 constexpr int DEC_SMEM_MAX = 232448;              // 227 KB
 constexpr int DEC_PART = WT_ROWS * DEC_N;         // floats of one phase-1 partial: 128 packed rows x 16 tokens (8 KB)
+constexpr int DEC_ALIGN_MIN_CTAS = 12;            // the run-aligned split is used when every run gets at least this many CTAs
 constexpr int DEC_MAX_CTAS = 160;                 // the partial-slot capacity is sized for at most this many CTAs
 
 struct DecArgs {
@@ -188,7 +189,9 @@ __device__ __forceinline__ int cta_of_tile(long long t, long long Tn, int G) { r
 //            proportion to their items (run r gets the CTAs [crun[r], crun[r+1])) and each run's tiles are cut evenly
 //            among ITS CTAs.  No range crosses a run boundary, so no CTA restages x in phase 1 or drains and refills its
 //            Y partial in phase 2 -- measured at C4 T=1: the four CTAs with a run boundary finished phase 2 ~3 us after
-//            the rest and the whole grid waited for them.  Costs an imbalance of at most one part in ~18.
+//            the rest and the whole grid waited for them.  Costs an imbalance of one part in (CTAs per run), so it is used
+//            only when every run gets >= DEC_ALIGN_MIN_CTAS CTAs (with 2-3 CTAs per run -- T=64 and a heterogeneous table --
+//            it cost 35 %).
 struct Split {
     const DecAux* ax;
     long long W;
@@ -408,14 +411,14 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     fence_proxy_async_smem();                                // the zeros of Xe / Hs -> visible to the tensor core's reads
     __syncthreads();
     const int W = ax->W;
-    // deal the CTAs out to the runs (see Split): possible when every run gets at least one CTA
+    // deal the CTAs out to the runs (see Split) when every run gets enough of them
     if (warp == 0) {
         const int nr = ax->n_runs;
         bool ok = nr >= 1 && nr <= (int)G && W > 0;
         if (ok) {
             for (int r = lane; r <= nr; r += 32) ax->crun[r] = (int16_t)((long long)G * ax->run_ib[r] / W);
             __syncwarp();
-            for (int r = lane; r < nr; r += 32) ok = ok && ax->crun[r + 1] > ax->crun[r];
+            for (int r = lane; r < nr; r += 32) ok = ok && ax->crun[r + 1] - ax->crun[r] >= DEC_ALIGN_MIN_CTAS;
         }
         ok = __all_sync(0xffffffffu, ok);
         if (lane == 0) ax->aligned = ok ? 1 : 0;
