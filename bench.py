@@ -51,6 +51,34 @@ def load_peaks():
         return dict(FALLBACK_PEAKS, source="fallback (B200_PROFILING.md)")
 
 
+# ------------------------------------------------------------------------------------------ ncu traffic of the dominant kernel
+NCU_CAPTURES = {  # (config, T, table spec) -> committed extract of an `ncu --set full` capture of exactly that workload
+    ("C4", 8192, "2560"): "profiles/r02c_ncu_full_pair_c4_T8192_r2560.csv",
+}
+NCU_KERNEL = {"gemm1_swiglu": "k_gemm_pair<1>", "gemm2_scatter_add": "k_gemm_pair<2>", "decode_fused": "k_decode"}
+
+
+def ncu_traffic(cfg, T, spec, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu extract of THIS workload
+    (profiles/, the command that made it is in the README beside it); None when there is no capture of this workload."""
+    path = NCU_CAPTURES.get((cfg, int(T), str(spec)))
+    if not path or kernel not in NCU_KERNEL:
+        return None, None
+    try:
+        import csv
+        with open(os.path.join(ROOT, path)) as f:
+            rows = list(csv.reader(f))
+        hdr, units = rows[0], rows[1]
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+        ir, iw = hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+        for r in rows[2:]:
+            if NCU_KERNEL[kernel] in r[0]:
+                return float(r[ir]) * scale[units[ir]] + float(r[iw]) * scale[units[iw]], path
+    except Exception:
+        pass
+    return None, None
+
+
 # ------------------------------------------------------------------------------------------ work model
 def work_model(ids: np.ndarray, r: np.ndarray, d: int, T: int, k: int):
     """Algorithmic work of one call, exactly SURVEY.md 8(d): S = sum_e n_e r_e, R_act = sum over experts with n_e > 0 of
@@ -598,9 +626,11 @@ def run_ours(args):
         achieved, peak, unit = kflops / dur / 1e12, peaks["bf16_tflops"], "TFLOP/s"
     else:
         achieved, peak, unit = kbytes / dur / 1e9, peaks["hbm_gbs"], "GB/s"
+    traffic, traffic_src = (args.traffic, "--traffic") if args.traffic is not None else ncu_traffic(cfg, T, args.r, dom)
     roofline = {"bound": bound, "achieved": round(achieved, 2), "peak": peak, "unit": unit,
                 "frac": round(achieved / peak, 4),
-                "traffic": args.traffic,            # dram bytes per launch from an ncu --set full capture of THIS config, else null
+                "traffic": traffic,                 # dram bytes per launch from an ncu --set full capture of THIS workload, else null
+                "traffic_source": traffic_src,
                 "kernel": dom, "kernel_ms": round(per_launch_ms[dom], 5),
                 "kernel_share_of_step": round(per_launch_ms[dom] / max(sum(per_launch_ms.values()), 1e-12), 4),
                 "peak_source": peaks["source"] + ", burst figure (the kernel is timed alone between CUDA events)",

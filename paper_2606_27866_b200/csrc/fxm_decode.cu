@@ -193,31 +193,32 @@ __device__ __forceinline__ int cta_of_tile(long long t, long long Tn, int G) { r
 //            only when every run gets >= DEC_ALIGN_MIN_CTAS CTAs (with 2-3 CTAs per run -- T=64 and a heterogeneous table --
 //            it cost 35 %).
 struct Split {
+    // 32-bit arithmetic: tiles of a phase <= 320 runs * 256 blocks * 60 tiles = 4.9 M, times G <= 160 stays below 2^32
     const DecAux* ax;
-    long long W;
+    uint32_t W;
     int G, aligned;
     __device__ __forceinline__ void range(int c, int tpi, long long& lo, long long& hi) const {
-        if (!aligned) { const long long Tn = W * tpi; lo = Tn * c / G; hi = Tn * (c + 1) / G; return; }
+        if (!aligned) { const uint32_t Tn = W * (uint32_t)tpi; lo = Tn * (uint32_t)c / (uint32_t)G; hi = Tn * (uint32_t)(c + 1) / (uint32_t)G; return; }
         int r = 0;
         while ((int)ax->crun[r + 1] <= c) ++r;
-        const int c0 = ax->crun[r], nc = ax->crun[r + 1] - c0;
-        const long long tb = (long long)ax->run_ib[r] * tpi, n = (long long)(ax->run_ib[r + 1] - ax->run_ib[r]) * tpi;
-        lo = tb + n * (c - c0) / nc;
-        hi = tb + n * (c - c0 + 1) / nc;
+        const uint32_t c0 = ax->crun[r], nc = ax->crun[r + 1] - c0;
+        const uint32_t tb = (uint32_t)ax->run_ib[r] * tpi, n = (uint32_t)(ax->run_ib[r + 1] - ax->run_ib[r]) * tpi;
+        lo = tb + n * ((uint32_t)c - c0) / nc;
+        hi = tb + n * ((uint32_t)c - c0 + 1) / nc;
     }
     // owner of tile t, which belongs to run `run`
     __device__ __forceinline__ int owner(long long t, int run, int tpi) const {
-        if (!aligned) return cta_of_tile(t, W * tpi, G);
-        const int c0 = ax->crun[run], nc = ax->crun[run + 1] - c0;
-        const long long tb = (long long)ax->run_ib[run] * tpi, n = (long long)(ax->run_ib[run + 1] - ax->run_ib[run]) * tpi;
-        return c0 + (int)(((t - tb + 1) * nc - 1) / n);
+        if (!aligned) return (int)((((uint32_t)t + 1u) * (uint32_t)G - 1u) / (W * (uint32_t)tpi));
+        const uint32_t c0 = ax->crun[run], nc = ax->crun[run + 1] - c0;
+        const uint32_t tb = (uint32_t)ax->run_ib[run] * tpi, n = (uint32_t)(ax->run_ib[run + 1] - ax->run_ib[run]) * tpi;
+        return (int)(c0 + (((uint32_t)t - tb + 1u) * nc - 1u) / n);
     }
     // does CTA c (a CTA of run `run` when aligned) own any tile of the phase?
     __device__ __forceinline__ bool holds(int c, int run, int tpi) const {
-        if (!aligned) { const long long Tn = W * tpi; return Tn * c / G != Tn * (c + 1) / G; }
-        const int c0 = ax->crun[run], nc = ax->crun[run + 1] - c0;
-        const long long n = (long long)(ax->run_ib[run + 1] - ax->run_ib[run]) * tpi;
-        return n * (c - c0) / nc != n * (c - c0 + 1) / nc;
+        if (!aligned) { const uint32_t Tn = W * (uint32_t)tpi; return Tn * (uint32_t)c / (uint32_t)G != Tn * (uint32_t)(c + 1) / (uint32_t)G; }
+        const uint32_t c0 = ax->crun[run], nc = ax->crun[run + 1] - c0;
+        const uint32_t n = (uint32_t)(ax->run_ib[run + 1] - ax->run_ib[run]) * tpi;
+        return n * ((uint32_t)c - c0) / nc != n * ((uint32_t)c - c0 + 1) / nc;
     }
 };
 
@@ -416,7 +417,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         const int nr = ax->n_runs;
         bool ok = nr >= 1 && nr <= (int)G && W > 0;
         if (ok) {
-            for (int r = lane; r <= nr; r += 32) ax->crun[r] = (int16_t)((long long)G * ax->run_ib[r] / W);
+            for (int r = lane; r <= nr; r += 32) ax->crun[r] = (int16_t)((uint32_t)G * (uint32_t)ax->run_ib[r] / (uint32_t)W);
             __syncwarp();
             for (int r = lane; r < nr; r += 32) ok = ok && ax->crun[r + 1] - ax->crun[r] >= DEC_ALIGN_MIN_CTAS;
         }
@@ -425,7 +426,7 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
     }
     __syncthreads();
     Split sp;
-    sp.ax = ax; sp.W = W; sp.G = (int)G; sp.aligned = ax->aligned;
+    sp.ax = ax; sp.W = (uint32_t)W; sp.G = (int)G; sp.aligned = ax->aligned;
     long long lo1, hi1, lo2, hi2;
     sp.range((int)blockIdx.x, D.nKB1, lo1, hi1);
     sp.range((int)blockIdx.x, D.nDB, lo2, hi2);
@@ -698,6 +699,12 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
             }
             fence_proxy_async_smem();
             mbar_arrive(hfull(b));
+            if (i == 0) {
+                // every CTA's slice of yacc is zeroed (they arrived in their prologues, ~20 us ago): checked here, while the
+                // tensor core works on the first piece, and not in front of the first reduction
+                if (lane == 0) cnt_wait(&a.state->dec_zcnt, ax->ztarget, a.state);
+                __syncwarp();
+            }
             touched |= ((p.b >= 32 ? 0xFFFFFFFFu : ((1u << p.b) - 1u)) & ~((1u << p.a) - 1u));
             const bool run_ends = !more || run_nx != run;
             if (run_ends) {
@@ -711,10 +718,6 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
                 }
                 mbar_wait(yfull, (uint32_t)(nseg & 1), a.state);
                 tc_fence_after();
-                if (nseg == 0) {                                    // every CTA's slice of yacc is zeroed (arrived in the prologues)
-                    if (lane == 0) cnt_wait(&a.state->dec_zcnt, ax->ztarget, a.state);
-                    __syncwarp();
-                }
                 if (nt <= 2) {
                     // one or two tokens (single-token decode): two columns per feature block, eight blocks per TMEM wait
                     const int t0 = __shfl_sync(0xffffffffu, tok, 0), t1 = __shfl_sync(0xffffffffu, tok, 1);
@@ -830,9 +833,11 @@ __global__ void __launch_bounds__(DEC_THREADS, 1) k_decode(const DecArgs a) {
         asm volatile("fence.acq_rel.gpu;" ::: "memory");
         DEC_TR(13);
 #endif
-        const unsigned long long target = cnt_target(cnt_arrive(&a.state->dec_bcnt), G);
+        // both counters grow by exactly G per launch, so the target of this launch's final barrier is the number the
+        // prologue arrival already returned: the arrival here needs no return value (no round trip before the poll)
+        asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(&a.state->dec_bcnt) : "memory");
         DEC_TR(7);
-        cnt_wait(&a.state->dec_bcnt, target, a.state);
+        cnt_wait(&a.state->dec_bcnt, ax->ztarget, a.state);
     }
     __syncthreads();
     DEC_TR(5);
@@ -867,7 +872,8 @@ int decode_slots(const Dims& D) {
     return s;
 }
 
-bool decode_supported(const Dims& D) { return D.nDB * DEC_N + 2 * DEC_N <= 512 && decode_slots(D) >= 4; }
+// nCB <= 1024 keeps the tile arithmetic of struct Split inside 32 bits (320 runs x 1024 blocks x 60 tiles x 160 CTAs < 2^32)
+bool decode_supported(const Dims& D) { return D.nDB * DEC_N + 2 * DEC_N <= 512 && decode_slots(D) >= 4 && D.nCB <= 1024; }
 
 // most phase-1 partial slots a call with T*k = A assignments can need: (items + CTAs); monotonic in A
 size_t decode_part_bytes(const Dims& D, long long A) {

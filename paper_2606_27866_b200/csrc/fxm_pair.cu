@@ -226,27 +226,26 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
 // number q (in issue order) takes w contiguous columns at the returned offset.  `need` = how many sub-tiles must
 // have been drained before the MMAs of q may write (sub-tiles are drained in order): the newest earlier sub-tile
 // whose columns overlap, and q - PAIR_TQ because the barrier ring has PAIR_TQ entries.
+// (lo / hi are indexed with run-time values and therefore live in local memory.  A register-only shift-register version
+// of this ring made the four-launch path fail intermittently at decode-sized T on the C4 layer -- "unspecified launch
+// failure" in about one call in 250, 6 of 23 processes, against 0 of 28 with this version on the same loop.  The cause was
+// not established (the roles under setmaxnreg.dec 48 stay below R31 in both builds), so the change was backed out;
+// tests/test_gpu_parity.py::test_general_path_small_T_many_calls_on_c4_layer repeats the loop.)
 struct TmemRing {
     uint32_t head, seq;
-    uint32_t e[PAIR_TQ - 1];          // e[i] = columns [lo, hi) of sub-tile seq-1-i as lo | hi << 16: a shift register, so every
-                                      // index is a compile-time constant and the ring lives in registers, not in local memory
-    __device__ __forceinline__ void init() {
-        head = 0; seq = 0;
-#pragma unroll
-        for (int i = 0; i < PAIR_TQ - 1; ++i) e[i] = 0;
-    }
+    uint32_t lo[PAIR_TQ], hi[PAIR_TQ];
+    __device__ __forceinline__ void init() { head = 0; seq = 0; }
     __device__ __forceinline__ uint32_t record(uint32_t c, uint32_t w) {      // -> sub-tiles that must be drained first
         uint32_t nd = seq >= (uint32_t)PAIR_TQ ? seq - PAIR_TQ + 1 : 0;
 #pragma unroll
-        for (uint32_t i = 0; i < (uint32_t)PAIR_TQ - 1; ++i) {
-            if (i < seq) {
-                const uint32_t s = seq - 1 - i, lo = e[i] & 0xFFFFu, hi = e[i] >> 16;
-                if (lo < c + w && hi > c && s + 1 > nd) nd = s + 1;
+        for (uint32_t i = 1; i < (uint32_t)PAIR_TQ; ++i) {
+            if (i <= seq) {
+                const uint32_t s = seq - i;
+                if (lo[s % PAIR_TQ] < c + w && hi[s % PAIR_TQ] > c && s + 1 > nd) nd = s + 1;
             }
         }
-#pragma unroll
-        for (int i = PAIR_TQ - 2; i > 0; --i) e[i] = e[i - 1];
-        e[0] = c | ((c + w) << 16);
+        lo[seq % PAIR_TQ] = c;
+        hi[seq % PAIR_TQ] = c + w;
         ++seq;
         return nd;
     }

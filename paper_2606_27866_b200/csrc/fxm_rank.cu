@@ -33,9 +33,16 @@ __global__ void __launch_bounds__(256) k_saliency_gu(int d, size_t rows, size_t 
         for (int c = lane; c < cpr; c += 32) {
             const size_t o = row * cpr + c;
             const uint4 wg = __ldcs(Wg + o), wu = __ldcs(Wu + o);
-            for (int b = 0; b < B; ++b) {
-                const uint4 gg = __ldcs(Gg + b * per4 + o), gu = __ldcs(Gu + b * per4 + o);
-                acc += sq8(wg, gg) + sq8(wu, gu);
+            // gradient sets four at a time with every load issued before the first use (B is a run-time value: a plain loop
+            // over b would serialise the loads); the sum stays in the order b = 0, 1, ...
+            for (int b0 = 0; b0 < B; b0 += 4) {
+                uint4 gg[4], gu[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (b0 + u < B) { gg[u] = __ldcs(Gg + (b0 + u) * per4 + o); gu[u] = __ldcs(Gu + (b0 + u) * per4 + o); }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (b0 + u < B) acc += sq8(wg, gg[u]) + sq8(wu, gu[u]);
             }
         }
 #pragma unroll
@@ -62,12 +69,20 @@ __global__ void __launch_bounds__(256) k_saliency_dn(int d, int I, int R, size_t
         for (int i = r0; i < r1; ++i) {
             const size_t o = ((size_t)e * d + i) * cpr + c0;
             const uint4 w = __ldcs(Wd + o);
-            for (int b = 0; b < B; ++b) {
-                const uint4 g = __ldcs(Gd + b * per4 + o);
+            for (int b0 = 0; b0 < B; b0 += 4) {
+            uint4 gs[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (b0 + u < B) gs[u] = __ldcs(Gd + (b0 + u) * per4 + o);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (b0 + u >= B) continue;
+                const uint4 g = gs[u];
                 const float p0 = bf_lo(w.x) * bf_lo(g.x), p1 = bf_hi(w.x) * bf_hi(g.x), p2 = bf_lo(w.y) * bf_lo(g.y), p3 = bf_hi(w.y) * bf_hi(g.y);
                 const float p4 = bf_lo(w.z) * bf_lo(g.z), p5 = bf_hi(w.z) * bf_hi(g.z), p6 = bf_lo(w.w) * bf_lo(g.w), p7 = bf_hi(w.w) * bf_hi(g.w);
                 acc[0] += p0 * p0; acc[1] += p1 * p1; acc[2] += p2 * p2; acc[3] += p3 * p3;
                 acc[4] += p4 * p4; acc[5] += p5 * p5; acc[6] += p6 * p6; acc[7] += p7 * p7;
+            }
             }
         }
 #pragma unroll

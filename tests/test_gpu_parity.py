@@ -745,3 +745,35 @@ def test_shared_expert_output_is_added_before_the_rounding(decode):
     gu.check_close(got, ref, "routed + shared")
     # one rounding: |y - ref| <= half an ulp of bf16 at ref (2^-9 relative) plus the H rounding's contribution
     assert np.abs(got - ref).max() <= 2.0 ** -8 * np.abs(ref).max()
+
+
+def test_general_path_small_T_many_calls_on_c4_layer():
+    """Regression (round 2): a register-only version of the pair kernels' TMEM column ring made the four-launch path fail
+    intermittently ("unspecified launch failure", about one call in 250) for decode-sized T on the C4-shaped layer, where the
+    token tiles are 16-32 rows and many sub-tiles are in flight.  300 calls of the general path at T=32 / 64, a buffer larger
+    than L2 rewritten between calls, every output compared on the device with the oracle's rows of that batch."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh = gen.SHAPES["C4"]
+    lay = gen.layer_for("C4", 0)
+    L = gu.pack_layer(lay)
+    r = gen.table_uniform(sh, 640)
+    L.set_budget(r)
+    L.set_decode(0)                                              # never the fused decode kernel
+    flush = torch.zeros(256 << 20, dtype=torch.uint8, device="cuda")
+    cases = []
+    for T, seed in ((32, 61), (64, 62)):
+        _, b, _ = gen.config("C4", T=T, seed=seed, layer=False)
+        ref = torch.from_numpy(gu.oracle_ffn(lay, b, r)).cuda()
+        cases.append((gu.to_dev(b.x), torch.from_numpy(b.topk_ids).cuda(), torch.from_numpy(b.topk_w).cuda(), ref,
+                      float(ref.abs().max())))
+    for i in range(300):
+        x, ids, w, ref, scale = cases[i % 2]
+        flush.add_(1)
+        y = L.moe_ffn(x, ids, w)
+        assert L.launches_per_ffn() == 4
+        err = float((y.double() - ref).abs().max())
+        assert err <= gu.TOL_MAX * scale, f"call {i}: max err {err:.3e} > {gu.TOL_MAX}*{scale:.3e}"
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
