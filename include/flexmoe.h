@@ -233,8 +233,9 @@ fxm_status fxm_set_tile_n(fxm_layer* L, int tile_n);
  * weight-streaming decode kernel instead of the four launches above.  prefetch_tiles = how many 16 KB weight tiles
  * each CTA's L2 prefetch cursor runs ahead of its shared-memory ring (0..4096; default 0 = none: every distance
  * tried was measured slower on B200, see profiles/).  Tuning knob only: results agree within the stated tolerance
- * either way.  Needs d <= 3840, else the general path is used. */
-#define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 768
+ * either way.  Needs d <= 3840, else the general path is used.  Default 640: measured on the C4-shaped layer the
+ * four-launch path wins from T*k = 768 on (an expert with more than 16 tokens streams its weights twice here). */
+#define FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS 640
 #define FXM_DECODE_DEFAULT_PREFETCH 0
 fxm_status fxm_set_decode(fxm_layer* L, int max_assignments, int prefetch_tiles);
 /* Synchronises `stream`, then returns the sticky device flag word (bit0: expert id out of range,

@@ -132,7 +132,7 @@ def workspace_bytes_host(E: int, d: int, I: int, T_max: int, k: int) -> int:
 
 N_KERNELS = 5
 KERNEL_NAMES = ("route", "gemm1_swiglu", "gemm2_scatter_add", "finalize", "decode_fused")
-DECODE_DEFAULT_MAX_ASSIGNMENTS = 768
+DECODE_DEFAULT_MAX_ASSIGNMENTS = 640
 DECODE_DEFAULT_PREFETCH = 0
 
 
