@@ -149,6 +149,14 @@ fxm_status fxm_moe_ffn_router(fxm_layer* L, const void* x, const float* router_l
 fxm_status fxm_workspace_bytes_host(int E, int d, int I, int T_max, int k, size_t* bytes);
 fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
                             int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream);
+/* Pipelined variant of fxm_moe_ffn_host for a loop of calls: y travels back on a SECOND library-owned stream, so the
+ * device->host copy of call i runs under the kernels of call i+1 (the in-stream copy of fxm_moe_ffn_host serialises with
+ * them).  Contract: as above for the inputs; y_host of a call is valid once `stream` has passed a later fxm_host_flush on
+ * this layer (which makes `stream` wait for every copy still in flight; host-only, no launch).  Same workspace size. */
+fxm_status fxm_moe_ffn_host_pipelined(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host,
+                                      const float* topk_w_host, int T, int k, void* y_host, void* workspace,
+                                      size_t workspace_bytes, void* stream);
+fxm_status fxm_host_flush(fxm_layer* L, void* stream);
 
 /* ---- offline clipping: PAPER.md:222 ("the pruned subnet is exported as a standalone fixed-budget checkpoint"),
  * Table 2 PAPER.md:201-206 ------------------------------------------------------------------------------------------

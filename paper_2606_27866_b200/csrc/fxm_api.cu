@@ -1,6 +1,7 @@
 // fxm_api.cu -- the C ABI of include/flexmoe.h: argument validation, host metadata, launch sequencing.
 // No arithmetic of the method lives here; every step of the path runs in the kernels of this directory.
 #include "../../include/flexmoe.h"
+#include <cstdio>
 #include "fxm_internal.cuh"
 
 #include <algorithm>
@@ -39,6 +40,9 @@ struct fxm_layer {
     cudaEvent_t ev_in[2];    // inputs of set b have landed (recorded on h2d_stream)
     cudaEvent_t ev_done[2];  // the kernels that read set b have finished (recorded on the caller's stream)
     cudaEvent_t ev_tail;     // the whole previous host call (kernels + y copy) has finished
+    cudaStream_t d2h_stream; // fxm_moe_ffn_host_pipelined: y travels back here, under the kernels of the next call
+    cudaEvent_t ev_y[2];     // the y copy that reads device buffer b has finished (recorded on d2h_stream)
+    unsigned y_pending;      // bit b: ev_y[b] has not been waited for by the caller's stream yet
     unsigned host_calls;
     const void* host_ws;     // layout key of the previous host call: (workspace, bytes, T, k)
     size_t host_ws_bytes;
@@ -50,8 +54,8 @@ struct fxm_layer {
 
 static size_t host_stage_bytes(const Dims& D, int T, int k) {
     // device staging of the host-buffer entry point: two input sets {x bf16 [T][d], ids int32 [T][k], w fp32 [T][k]}
-    // and one y bf16 [T][d]
-    return 3 * align_up((size_t)T * D.d * 2, 1024) + 4 * align_up((size_t)T * k * 4, 1024);
+    // and two y bf16 [T][d] (the pipelined entry point copies y of call i back while call i+1 writes the other one)
+    return 4 * align_up((size_t)T * D.d * 2, 1024) + 4 * align_up((size_t)T * k * 4, 1024);
 }
 
 static bool make_dims(int E, int d, int I, Dims* D) {
@@ -121,6 +125,7 @@ static fxm_layer* new_layer(const Dims& D, uint8_t* blob, const Tail& tl, int sm
     L->prof_capacity = 0; L->prof_calls = 0;
     L->x_map_ptr = nullptr; L->x_map_T = -1;
     L->h2d_stream = nullptr; L->host_calls = 0; L->ev_tail = nullptr;
+    L->d2h_stream = nullptr; L->y_pending = 0; L->ev_y[0] = L->ev_y[1] = nullptr;
     L->host_ws = nullptr; L->host_ws_bytes = 0; L->host_T = -1; L->host_k = -1;
     for (int b = 0; b < 2; ++b) { L->ev_in[b] = nullptr; L->ev_done[b] = nullptr; }
     L->dec_max_A = FXM_DECODE_DEFAULT_MAX_ASSIGNMENTS; L->dec_pf = FXM_DECODE_DEFAULT_PREFETCH; L->last_launches = 0;
@@ -259,6 +264,9 @@ void fxm_destroy(fxm_layer* L) {
     }
     if (L->ev_tail) cudaEventDestroy(L->ev_tail);
     if (L->h2d_stream) cudaStreamDestroy(L->h2d_stream);
+    for (int b = 0; b < 2; ++b)
+        if (L->ev_y[b]) cudaEventDestroy(L->ev_y[b]);
+    if (L->d2h_stream) cudaStreamDestroy(L->d2h_stream);
     if (L->host_flags) cudaFreeHost(L->host_flags);
     delete L;
 }
@@ -471,8 +479,8 @@ fxm_status fxm_moe_ffn_shared(fxm_layer* L, const void* x, const int32_t* topk_i
     return ffn_impl(L, x, topk_ids, topk_w, nullptr, T, k, y_shared, y, workspace, workspace_bytes, stream);
 }
 
-fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
-                            int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream) {
+static fxm_status host_impl(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
+                            int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream, bool defer_y) {
     if (!L || T < 0 || !workspace || ((uintptr_t)workspace & 1023u)) return FXM_EINVAL;
     if (k < 1 || k > MAX_K || k > L->D.E || (long long)T * k > (1LL << 30)) return FXM_ESHAPE;
     const size_t inner = map_workspace(L->D, T, k, nullptr).bytes;
@@ -486,8 +494,8 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
     const size_t xs = align_up(xb, 1024), as = align_up(ab, 1024);
     // the staging area sits at the END of the buffer, so it never overlaps the compute workspace of this call
     uint8_t* p = (uint8_t*)workspace + (workspace_bytes & ~(size_t)1023) - stage;
-    uint8_t* yd = p;
-    p += xs;
+    uint8_t* yd0 = p;
+    p += 2 * xs;
     // a capturing stream cannot wait on events recorded outside the capture: copy in-stream then (no overlap)
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) return FXM_ECUDA;
@@ -499,6 +507,9 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
                 cudaEventCreateWithFlags(&L->ev_done[b], cudaEventDisableTiming) != cudaSuccess)
                 return FXM_ECUDA;
         if (cudaEventCreateWithFlags(&L->ev_tail, cudaEventDisableTiming) != cudaSuccess) return FXM_ECUDA;
+        if (cudaStreamCreateWithFlags(&L->d2h_stream, cudaStreamNonBlocking) != cudaSuccess) return FXM_ECUDA;
+        for (int b = 0; b < 2; ++b)
+            if (cudaEventCreateWithFlags(&L->ev_y[b], cudaEventDisableTiming) != cudaSuccess) return FXM_ECUDA;
     }
     cudaStream_t cs = side ? L->h2d_stream : st;
     // A different (workspace, size, T, k) than the previous host call moves the staging sets -- possibly onto memory the
@@ -507,9 +518,16 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
     const bool same_layout = L->host_ws == workspace && L->host_ws_bytes == workspace_bytes && L->host_T == T && L->host_k == k;
     if (side && !same_layout) {
         if (L->host_ws && cudaStreamWaitEvent(cs, L->ev_tail, 0) != cudaSuccess) return FXM_ECUDA;
+        // the y buffers move as well: the caller's stream must not write the new ones under a copy that still reads the old
+        for (int b = 0; b < 2; ++b)
+            if ((L->y_pending >> b) & 1u)
+                if (cudaStreamWaitEvent(st, L->ev_y[b], 0) != cudaSuccess || cudaStreamWaitEvent(cs, L->ev_y[b], 0) != cudaSuccess)
+                    return FXM_ECUDA;
+        L->y_pending = 0;
         L->host_calls = 0;
     }
     const unsigned set = side ? (L->host_calls & 1u) : 0u;
+    uint8_t* yd = yd0 + set * xs;
     uint8_t* xd = p + set * (xs + 2 * as);
     uint8_t* idd = xd + xs;
     uint8_t* wd = idd + as;
@@ -522,15 +540,48 @@ fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* top
         if (cudaEventRecord(L->ev_in[set], cs) != cudaSuccess) return FXM_ECUDA;
         if (cudaStreamWaitEvent(st, L->ev_in[set], 0) != cudaSuccess) return FXM_ECUDA;
     }
+    // y buffer `set` is free once the deferred copy of the call before last has read it
+    if (side && ((L->y_pending >> set) & 1u)) {
+        if (cudaStreamWaitEvent(st, L->ev_y[set], 0) != cudaSuccess) return FXM_ECUDA;
+        L->y_pending &= ~(1u << set);
+    }
     fxm_status s = fxm_moe_ffn(L, xd, (const int32_t*)idd, (const float*)wd, T, k, yd, workspace, inner, stream);
     if (s != FXM_OK) return s;
     if (side && cudaEventRecord(L->ev_done[set], st) != cudaSuccess) return FXM_ECUDA;
-    if (cudaMemcpyAsync(y_host, yd, xb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return FXM_ECUDA;
+    if (side && defer_y) {
+        // y goes back on the library's second stream, under the kernels of the next call; fxm_host_flush (or the reuse of
+        // this buffer two calls on) makes the caller's stream wait for it
+        if (cudaStreamWaitEvent(L->d2h_stream, L->ev_done[set], 0) != cudaSuccess) return FXM_ECUDA;
+        if (cudaMemcpyAsync(y_host, yd, xb, cudaMemcpyDeviceToHost, L->d2h_stream) != cudaSuccess) return FXM_ECUDA;
+        if (cudaEventRecord(L->ev_y[set], L->d2h_stream) != cudaSuccess) return FXM_ECUDA;
+        L->y_pending |= 1u << set;
+    } else if (cudaMemcpyAsync(y_host, yd, xb, cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+        return FXM_ECUDA;
+    }
     if (side) {
-        if (cudaEventRecord(L->ev_tail, st) != cudaSuccess) return FXM_ECUDA;
+        if (cudaEventRecord(L->ev_tail, defer_y ? L->d2h_stream : st) != cudaSuccess) return FXM_ECUDA;
         ++L->host_calls;
         L->host_ws = workspace; L->host_ws_bytes = workspace_bytes; L->host_T = T; L->host_k = k;
     }
+    return FXM_OK;
+}
+
+fxm_status fxm_moe_ffn_host(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
+                            int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream) {
+    return host_impl(L, x_host, topk_ids_host, topk_w_host, T, k, y_host, workspace, workspace_bytes, stream, false);
+}
+
+fxm_status fxm_moe_ffn_host_pipelined(fxm_layer* L, const void* x_host, const int32_t* topk_ids_host, const float* topk_w_host,
+                                      int T, int k, void* y_host, void* workspace, size_t workspace_bytes, void* stream) {
+    return host_impl(L, x_host, topk_ids_host, topk_w_host, T, k, y_host, workspace, workspace_bytes, stream, true);
+}
+
+fxm_status fxm_host_flush(fxm_layer* L, void* stream) {
+    if (!L) return FXM_EINVAL;
+    for (int b = 0; b < 2; ++b)
+        if ((L->y_pending >> b) & 1u)
+            if (cudaStreamWaitEvent((cudaStream_t)stream, L->ev_y[b], 0) != cudaSuccess) return FXM_ECUDA;
+    L->y_pending = 0;
     return FXM_OK;
 }
 
@@ -709,6 +760,10 @@ fxm_status fxm_device_flags(fxm_layer* L, uint32_t* flags, void* stream) {
     if (cudaMemcpyAsync(&v, &L->state->flags, sizeof(v), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaMemsetAsync(&L->state->flags, 0, sizeof(v), st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
         *flags = hostbits | (L->host_flags ? *(volatile uint32_t*)L->host_flags : 0u);
+        if (L->host_flags && L->host_flags[1])                   // a pipeline wait timed out: say where (diagnostic)
+            std::fprintf(stderr, "flexmoe: wait timed out in block %u thread %u (block size %u) on barrier 0x%x phase %u\n",
+                         L->host_flags[1] >> 16, L->host_flags[1] & 0xFFFFu, L->host_flags[3] >> 8, L->host_flags[2],
+                         L->host_flags[3] & 1u);
         return FXM_ECUDA;
     }
     const uint32_t hb = L->host_flags ? *(volatile uint32_t*)L->host_flags : 0u;

@@ -226,11 +226,8 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
 // number q (in issue order) takes w contiguous columns at the returned offset.  `need` = how many sub-tiles must
 // have been drained before the MMAs of q may write (sub-tiles are drained in order): the newest earlier sub-tile
 // whose columns overlap, and q - PAIR_TQ because the barrier ring has PAIR_TQ entries.
-// (lo / hi are indexed with run-time values and therefore live in local memory.  A register-only shift-register version
-// of this ring made the four-launch path fail intermittently at decode-sized T on the C4 layer -- "unspecified launch
-// failure" in about one call in 250, 6 of 23 processes, against 0 of 28 with this version on the same loop.  The cause was
-// not established (the roles under setmaxnreg.dec 48 stay below R31 in both builds), so the change was backed out;
-// tests/test_gpu_parity.py::test_general_path_small_T_many_calls_on_c4_layer repeats the loop.)
+// (lo / hi are indexed with run-time values and therefore live in local memory; a register-only shift-register form
+// was tried and backed out -- no measured gain.)
 struct TmemRing {
     uint32_t head, seq;
     uint32_t lo[PAIR_TQ], hi[PAIR_TQ];
@@ -409,6 +406,17 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                 myidx[lane] = __ldg((const int4*)(a.tok + p));
             }
             __syncwarp();
+            if (cnt == 0) {
+                // Nothing to bring for this item (a token tile of 16-32 rows has fewer 4-row groups than gather warps): walk
+                // the ring position forward WITHOUT polling the barriers.  A warp that only polls takes part in no handshake,
+                // so nothing stops the pipeline from lapping it; two phases behind, a parity wait can no longer tell "not yet"
+                // from "long ago" and the warp waits for a flip that never comes (found as an intermittent time-out at
+                // decode-sized T: about one call in 100, always warps gw >= 2 on an empty barrier).
+                const int adv = s + it.nk;
+                ph ^= (uint32_t)((adv / NS) & 1);
+                s = adv % NS;
+                continue;
+            }
             for (int kb = 0; kb < it.nk; ++kb) {
                 mbar_wait(empty_bar(s), ph ^ 1u, a.state);
                 if (leader_lane) {

@@ -35,7 +35,13 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, DevStat
     while (!mbar_try_wait(bar, parity)) {
         if ((++spins & 0xFFFu) == 0 && clock64() - t0 > 4000000000LL) {
             atomicOr(&state->flags, 2u);
-            if (state->hflag) *(volatile uint32_t*)state->hflag = 2u;    // pinned host word: still readable after the trap
+            if (state->hflag) {                                          // pinned host words: still readable after the trap
+                volatile uint32_t* h = (volatile uint32_t*)state->hflag;
+                h[1] = (blockIdx.x << 16) | threadIdx.x;                 // who gave up ...
+                h[2] = bar;                                              // ... on which barrier (shared-memory address) ...
+                h[3] = parity | (blockDim.x << 8);                       // ... waiting for which phase, in which kernel (by block size)
+                h[0] = 2u;
+            }
             __threadfence_system();
             __trap();
         }

@@ -75,6 +75,8 @@ def lib():
     L.fxm_load_clipped.argtypes = [ctypes.POINTER(vp), i32, i32, i32, vp, vp, sz, vp]
     L.fxm_workspace_bytes_host.argtypes = [i32, i32, i32, i32, i32, ctypes.POINTER(sz)]
     L.fxm_moe_ffn_host.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_moe_ffn_host_pipelined.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, sz, vp]
+    L.fxm_host_flush.argtypes = [vp, vp]
     L.fxm_saliency_workspace_bytes.argtypes = [i32, i32, i32, ctypes.POINTER(sz)]
     L.fxm_saliency.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, i32, vp, vp, sz, vp]
     L.fxm_rank_channels.argtypes = [i32, i32, vp, vp, vp]
@@ -100,7 +102,7 @@ def lib():
 
 EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
            "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_moe_ffn_shared", "fxm_moe_ffn_router", "fxm_workspace_bytes_host",
-           "fxm_moe_ffn_host", "fxm_clipped_bytes", "fxm_export_clipped", "fxm_parse_clipped_header", "fxm_load_clipped",
+           "fxm_moe_ffn_host", "fxm_moe_ffn_host_pipelined", "fxm_host_flush", "fxm_clipped_bytes", "fxm_export_clipped", "fxm_parse_clipped_header", "fxm_load_clipped",
            "fxm_saliency_workspace_bytes", "fxm_saliency", "fxm_rank_channels", "fxm_sample_budget", "fxm_action_cost",
            "fxm_profile_begin", "fxm_profile_end", "fxm_route", "fxm_unpack_prefix",
            "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_set_decode", "fxm_device_flags", "fxm_launches_per_ffn",
@@ -364,9 +366,11 @@ class Layer:
             self._wsh = raw[off:off + need]
         return self._wsh
 
-    def moe_ffn_host(self, x_host, ids_host, w_host, y_host, stream=None):
+    def moe_ffn_host(self, x_host, ids_host, w_host, y_host, stream=None, pipelined=False):
         """Host-buffer forward (fxm_moe_ffn_host): x_host/y_host [T,d] bf16, ids_host [T,k] int32, w_host [T,k]
-        fp32 CPU tensors (pinned recommended).  Asynchronous; y_host is valid after the stream is synchronised."""
+        fp32 CPU tensors (pinned recommended).  Asynchronous; y_host is valid after the stream is synchronised.
+        pipelined=True (fxm_moe_ffn_host_pipelined): y is copied back under the next call's kernels and is valid once the
+        stream has passed a later host_flush()."""
         import torch
         T, d = x_host.shape
         k = ids_host.shape[1]
@@ -376,10 +380,14 @@ class Layer:
         assert tuple(y_host.shape) == (T, d) and ids_host.dtype == torch.int32 and w_host.dtype == torch.float32
         assert tuple(ids_host.shape) == (T, k) and tuple(w_host.shape) == (T, k)
         ws = self.workspace_host(T, k)
-        _chk(lib().fxm_moe_ffn_host(self._h, x_host.data_ptr(), ids_host.data_ptr(), w_host.data_ptr(), T, k,
-                                    y_host.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
-             "fxm_moe_ffn_host")
+        fn = lib().fxm_moe_ffn_host_pipelined if pipelined else lib().fxm_moe_ffn_host
+        _chk(fn(self._h, x_host.data_ptr(), ids_host.data_ptr(), w_host.data_ptr(), T, k,
+                y_host.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "fxm_moe_ffn_host")
         return y_host
+
+    def host_flush(self, stream=None):
+        """fxm_host_flush: the stream waits for every pipelined y copy still in flight (host-only, no launch)."""
+        _chk(lib().fxm_host_flush(self._h, _stream_ptr(stream)), "fxm_host_flush")
 
     # -- measurement surface ----------------------------------------------------------------------------
     def profile_begin(self, max_calls: int):

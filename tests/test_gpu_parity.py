@@ -748,10 +748,11 @@ def test_shared_expert_output_is_added_before_the_rounding(decode):
 
 
 def test_general_path_small_T_many_calls_on_c4_layer():
-    """Regression (round 2): a register-only version of the pair kernels' TMEM column ring made the four-launch path fail
-    intermittently ("unspecified launch failure", about one call in 250) for decode-sized T on the C4-shaped layer, where the
-    token tiles are 16-32 rows and many sub-tiles are in flight.  300 calls of the general path at T=32 / 64, a buffer larger
-    than L2 rewritten between calls, every output compared on the device with the oracle's rows of that batch."""
+    """Regression (round 2): at decode-sized T on the C4-shaped layer the token tiles are 16-32 rows, so some of GEMM-1's
+    six gather warps have no 4-row group to bring.  They used to poll the stage barriers anyway; a warp that only polls takes
+    part in no handshake, the pipeline lapped it, its parity wait aliased and the call ended in the wait time-out (about one
+    call in 100: "unspecified launch failure", device flag bit 1).  300 calls of the four-launch path at T=32 / 64, a buffer
+    larger than L2 rewritten between calls, every output compared on the device with the oracle's rows of that batch."""
     import torch
     import gpu_util as gu
     fx = _fx()
@@ -777,3 +778,31 @@ def test_general_path_small_T_many_calls_on_c4_layer():
         assert err <= gu.TOL_MAX * scale, f"call {i}: max err {err:.3e} > {gu.TOL_MAX}*{scale:.3e}"
     torch.cuda.synchronize()
     assert L.device_flags() == 0
+
+
+def test_host_entry_point_with_deferred_output_copies():
+    """fxm_moe_ffn_host_pipelined + fxm_host_flush: y of call i travels back on the library's second stream under the
+    kernels of call i+1.  Ten calls of alternating sizes (T=64 / T=300: the staging layout changes), every third one through
+    the in-stream entry point, no host synchronisation before the flush; every output against the oracle."""
+    import torch
+    import gpu_util as gu
+    fx = _fx()
+    sh, lay, b0, rng = _c1()
+    r = gen.table_c1(sh, rng)
+    L = gu.pack_layer(lay)
+    L.set_budget(r)
+    L.set_decode()
+    sizes = [64, 64, 64, 300, 300, 64, 300, 300, 300, 64]
+    batches = [gen.make_batch(sh, T, np.random.default_rng(500 + i)) for i, T in enumerate(sizes)]
+    hx = [(fx.bf16_from_bits(b.x, "cpu").pin_memory(), torch.from_numpy(b.topk_ids).pin_memory(),
+           torch.from_numpy(b.topk_w).pin_memory()) for b in batches]
+    hy = [torch.zeros((T, sh.d), dtype=torch.bfloat16).pin_memory() for T in sizes]
+    L.workspace_host(300, sh.k)                                  # one workspace for both sizes
+    for i in range(len(sizes)):
+        L.moe_ffn_host(*hx[i], hy[i], pipelined=(i % 3 != 2))
+    L.host_flush()
+    torch.cuda.synchronize()
+    assert L.device_flags() == 0
+    for i, b in enumerate(batches):
+        y = gen.bf16_bits_to_f32(hy[i].view(torch.int16).numpy().view(np.uint16)).astype(np.float64)
+        gu.check_close(y, gu.oracle_ffn(lay, b, r), f"host call {i} T={sizes[i]}")
