@@ -289,7 +289,8 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < PAIR_MAX_STAGES; ++s) {
-            mbar_init(full_bar(s), rank == 0 ? 2 : 1);            // leader: own producer + the peer's relay
+            // leader: own producer + the peer's relay; GEMM-1: + one arrival per gather warp
+            mbar_init(full_bar(s), (rank == 0 ? 2 : 1) + (MODE == 1 ? PAIR_GW : 0));
             mbar_init(empty_bar(s), 1);
         }
         // "columns drained": one arrival per epilogue warp of both CTAs (a warp arrives as soon as its share is in registers)
@@ -406,23 +407,19 @@ k_gemm_pair(const PairArgs a, const __grid_constant__ CUtensorMap xmap) {
                 myidx[lane] = __ldg((const int4*)(a.tok + p));
             }
             __syncwarp();
-            if (cnt == 0) {
-                // Nothing to bring for this item (a token tile of 16-32 rows has fewer 4-row groups than gather warps): walk
-                // the ring position forward WITHOUT polling the barriers.  A warp that only polls takes part in no handshake,
-                // so nothing stops the pipeline from lapping it; two phases behind, a parity wait can no longer tell "not yet"
-                // from "long ago" and the warp waits for a flip that never comes (found as an intermittent time-out at
-                // decode-sized T: about one call in 100, always warps gw >= 2 on an empty barrier).
-                const int adv = s + it.nk;
-                ph ^= (uint32_t)((adv / NS) & 1);
-                s = adv % NS;
-                continue;
-            }
             for (int kb = 0; kb < it.nk; ++kb) {
                 mbar_wait(empty_bar(s), ph ^ 1u, a.state);
                 if (leader_lane) {
                     const uint32_t dst = smem_base + s * stage_bytes + WT_BYTES + (uint32_t)gw * (4u * ROW_BYTES);
                     for (int j = 0; j < cnt; ++j)
                         tma_gather4(dst + (uint32_t)j * (PAIR_GW * 4u * ROW_BYTES), &xmap, kb * KB, myidx[j], full_bar(s));
+                    // Every gather warp ARRIVES on the stage's full barrier, also when it had no group to bring (a token tile of
+                    // 16-32 rows has fewer 4-row groups than gather warps).  A warp that only polls the empty barriers takes part
+                    // in no handshake: the pipeline can lap it, and two phases behind a parity wait can no longer tell "not yet"
+                    // from "long ago" -- found as an intermittent time-out at decode-sized T (about one call in 100, always
+                    // warps gw >= 2 on an empty barrier).  Skipping the waits instead lets the warp run AHEAD, which aliases
+                    // the same way once it has rows to bring again.  With the arrival it can do neither.
+                    mbar_arrive(full_bar(s));
                 }
                 __syncwarp();
                 if (++s == NS) { s = 0; ph ^= 1u; }
