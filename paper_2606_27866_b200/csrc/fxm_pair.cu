@@ -196,18 +196,33 @@ __device__ __forceinline__ PairItem pair_item(const PairArgs& a, int wi, uint32_
     PairItem it;
     int4 q;
     int pairblk;
+    // Items of one expert are walked BLOCK-major: (block pair, token tile) instead of (token tile, block pair).  The tiles of
+    // an expert read the same weight tiles; with a static stride over the item list they now run on neighbouring clusters in
+    // the same round, so the second reader finds the tile in L2 (or merges with the miss in flight) instead of fetching it
+    // from HBM again 40 us later.  The tile list stays tile-major (tt[j].w = work prefix of tile j); .z carries the number
+    // of tiles of the expert (nt) and the tile's index among them (t0).
     if (MODE == 1) {
         while (__ldg(&a.items[cur + 1].w) <= wi) ++cur;
         q = __ldg(a.items + cur);
-        pairblk = wi - q.w;
+        const int nt = (q.z >> 16) & 0xFF, t0 = (q.z >> 24) & 0xFF;
+        const int nbp = __ldg(&a.items[cur + 1].w) - q.w;          // block pairs per tile (the same for every tile of the expert)
+        const int L = wi - (q.w - t0 * nbp);                        // position inside the expert's nt * nbp items
+        pairblk = L / nt;
+        const int t = L - pairblk * nt;
+        if (t != t0) q = __ldg(a.items + (cur - t0 + t));
     } else {
         const int nDBp = (D.nDB + 1) >> 1;
-        q = a.items[wi / nDBp];
-        pairblk = wi % nDBp;
+        const int jt = wi / nDBp;
+        q = a.items[jt];
+        const int nt = (q.z >> 16) & 0xFF, t0 = (q.z >> 24) & 0xFF;
+        const int L = wi - (jt - t0) * nDBp;
+        pairblk = L / nt;
+        const int t = L - pairblk * nt;
+        if (t != t0) q = a.items[jt - t0 + t];
     }
     it.e = q.x;
     it.row0 = q.y;
-    const int n = (q.z + 15) & ~15;
+    const int n = ((q.z & 0xFFFF) + 15) & ~15;
     // one sub-tile up to 256 tokens, else two balanced ones (both multiples of 16)
     it.n0 = n <= PAIR_NSUB ? n : (((n >> 4) + 1) >> 1) << 4;
     it.n1 = n - it.n0;

@@ -268,8 +268,13 @@ k_route(const RouteArgs a, const RouteWs w, DevState* __restrict__ state) {
                     const int p0 = s_poff[e];
                     // balanced split of the padded segment into nt tiles of <= tile_n rows, each a multiple of 16 rows
                     const int per = per_rows(np, nt);
-                    for (int row = 0; row < np; row += per, ++j, wk += nb)
-                        w.tt[j] = make_int4(e, p0 + row, min(per, n - row), wk);   // .z = valid rows of the tile (>= 1)
+                    // .z = valid rows of the tile (>= 1) | tiles of this expert << 16 | index of the tile among them << 24: the
+                    // GEMM kernels walk an expert's items block-major ((block, tile) order), so that the tiles of one expert,
+                    // which read the same weight tiles, run on neighbouring clusters at the same time (fxm_pair.cu pair_item)
+                    const int ntz = nt <= 15 ? nt : 1;
+                    int ti = 0;
+                    for (int row = 0; row < np; row += per, ++j, wk += nb, ++ti)
+                        w.tt[j] = make_int4(e, p0 + row, min(per, n - row) | (ntz << 16) | ((nt <= 15 ? ti : 0) << 24), wk);
                 }
                 {
                     int mx = nt > 0 ? min(per_rows(np, nt), np) : 0;               // rows of this expert's widest tile

@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(128) k_gemm1_simt(Dims D, LayerView V,
     const int ntt = sched->ntt;
     for (int wi = blockIdx.x; wi < ntt * D.nCB; wi += gridDim.x) {
         const int4 t = tt[wi / D.nCB];
-        const int e = t.x, row0 = t.y, nvalid = t.z, cb = wi % D.nCB;
+        const int e = t.x, row0 = t.y, nvalid = t.z & 0xFFFF, cb = wi % D.nCB;
         const int r = r_table[e];
         if (cb * CB >= r) continue;                                   // pruned block: never issued
         const uint32_t eb = V.eblk[e];
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(128) k_gemm2_simt(Dims D, LayerView V,
     for (int wi = blockIdx.x; wi < ntt * D.nDB; wi += gridDim.x) {
         const int j = wi / D.nDB, db = wi % D.nDB;
         const int4 t = tt[j];
-        const int e = t.x, row0 = t.y, nvalid = t.z;
+        const int e = t.x, row0 = t.y, nvalid = t.z & 0xFFFF;
         const int r = r_table[e];
         const uint32_t eb = V.eblk[e];
         const int nkb = (r + KB - 1) / KB;
