@@ -46,7 +46,8 @@ typedef enum {
     FXM_EWORKSPACE = 6, /* workspace_bytes smaller than fxm_workspace_bytes(E,d,I,T,k)                     */
     FXM_ESTATE = 7,     /* moe_ffn before any budget was installed                                         */
     FXM_ECUDA = 8,      /* a CUDA runtime call failed (no device, launch failure, earlier async fault)     */
-    FXM_ENOMEM = 9      /* a host allocation of the library failed                                         */
+    FXM_ENOMEM = 9,     /* a host allocation of the library failed                                         */
+    FXM_ELIMIT = 10     /* a no-allocation entry point was given a problem larger than its fixed scratch   */
 } fxm_status;
 
 #define FXM_MAX_BUDGETS 15 /* tables that fxm_register_budgets can keep resident */
@@ -187,6 +188,18 @@ fxm_status fxm_saliency_workspace_bytes(int E, int d, int I, size_t* bytes);
 fxm_status fxm_saliency(int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down, const void* G_gate,
                         const void* G_up, const void* G_down, int B, float* s_out, void* workspace, size_t workspace_bytes,
                         void* stream);
+/* The same computation for callers that cannot allocate device memory or pass scratch (CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the partial sums live in a device array inside the library image, FXM_SALIENCY_STATIC_BYTES
+ * (8 MB) on every GPU that loads the library, held until the process exits.  The call allocates nothing (no cudaMalloc /
+ * cudaFree / allocating library routine); inputs and s_out are the caller's, as above.  Shapes whose scratch need
+ * (fxm_saliency_workspace_bytes) exceeds FXM_SALIENCY_STATIC_BYTES are rejected with FXM_ELIMIT -- use fxm_saliency then
+ * (the C2-shaped weight set, E=60 I=1408, needs 5.8 MB and fits; the C4-shaped one, E=64 I=2560, needs 11.1 MB and does not).
+ * All calls on a device SHARE the array: calls that overlap on the GPU (streams with no ordering between them) race;
+ * calls on one stream, or ordered by events, are safe.  Nothing in the array needs clearing between calls (every slot
+ * that is read is written first by the same call).  Same results as fxm_saliency, bit for bit. */
+#define FXM_SALIENCY_STATIC_BYTES ((size_t)8 << 20)
+fxm_status fxm_saliency_static(int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down,
+                               const void* G_gate, const void* G_up, const void* G_down, int B, float* s_out, void* stream);
 /* channel_rank_out[e][p] (device int32 [E][I]) = ORIGINAL index of the p-th most important channel of expert e: s sorted
  * in descending order, equal saliencies keep ascending original index (readings R3, R4) -- exactly the
  * channel_rank fxm_pack takes (copy it to the host first: pack validates it there).  I <= 16384. */

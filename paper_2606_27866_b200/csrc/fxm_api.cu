@@ -169,6 +169,7 @@ const char* fxm_status_string(fxm_status s) {
         case FXM_ESTATE: return "FXM_ESTATE: no budget installed";
         case FXM_ECUDA: return "FXM_ECUDA: CUDA runtime failure";
         case FXM_ENOMEM: return "FXM_ENOMEM: host allocation failed";
+        case FXM_ELIMIT: return "FXM_ELIMIT: problem larger than the fixed scratch of a no-allocation entry point";
     }
     return "FXM_?";
 }
@@ -698,6 +699,22 @@ fxm_status fxm_saliency(int E, int d, int I, const void* W_gate, const void* W_u
     if (launch_saliency(D, (const __nv_bfloat16*)W_gate, (const __nv_bfloat16*)W_up, (const __nv_bfloat16*)W_down,
                         (const __nv_bfloat16*)G_gate, (const __nv_bfloat16*)G_up, (const __nv_bfloat16*)G_down, B, s_out,
                         (float*)workspace, (cudaStream_t)stream) != cudaSuccess)
+        return FXM_ECUDA;
+    return FXM_OK;
+}
+
+fxm_status fxm_saliency_static(int E, int d, int I, const void* W_gate, const void* W_up, const void* W_down, const void* G_gate,
+                               const void* G_up, const void* G_down, int B, float* s_out, void* stream) {
+    Dims D;
+    if (!W_gate || !W_up || !W_down || !G_gate || !G_up || !G_down || !s_out || B < 1) return FXM_EINVAL;
+    const uintptr_t al = (uintptr_t)W_gate | (uintptr_t)W_up | (uintptr_t)W_down | (uintptr_t)G_gate | (uintptr_t)G_up |
+                         (uintptr_t)G_down;
+    if (al & 15u) return FXM_EINVAL;
+    if (!make_dims(E, d, I, &D)) return FXM_ESHAPE;
+    if (saliency_workspace_bytes(D) > SALIENCY_STATIC_BYTES) return FXM_ELIMIT;      // beyond the fixed scratch: use fxm_saliency
+    if (launch_saliency_static(D, (const __nv_bfloat16*)W_gate, (const __nv_bfloat16*)W_up, (const __nv_bfloat16*)W_down,
+                               (const __nv_bfloat16*)G_gate, (const __nv_bfloat16*)G_up, (const __nv_bfloat16*)G_down, B, s_out,
+                               (cudaStream_t)stream) != cudaSuccess)
         return FXM_ECUDA;
     return FXM_OK;
 }

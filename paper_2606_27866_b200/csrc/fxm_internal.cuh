@@ -269,6 +269,11 @@ size_t saliency_workspace_bytes(const Dims& D);
 cudaError_t launch_saliency(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
                             const __nv_bfloat16* Gg, const __nv_bfloat16* Gu, const __nv_bfloat16* Gd, int B, float* s,
                             float* part, cudaStream_t st);
+// no-allocation variant: the partial sums live in a file-scope device array of fxm_rank.cu (8 MB per GPU that loads the library)
+constexpr size_t SALIENCY_STATIC_BYTES = (size_t)8 << 20;
+cudaError_t launch_saliency_static(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
+                                   const __nv_bfloat16* Gg, const __nv_bfloat16* Gu, const __nv_bfloat16* Gd, int B, float* s,
+                                   cudaStream_t st);
 cudaError_t init_rank_kernel();
 bool rank_supported(int I);
 cudaError_t launch_rank(int E, int I, const float* s, int* rank, cudaStream_t st);

@@ -10,6 +10,8 @@
 // All sums are fixed-order (no floating-point atomics): results are reproducible run to run.
 #include "fxm_internal.cuh"
 
+#include <mutex>
+
 namespace fxm {
 
 __device__ __forceinline__ float bf_lo(uint32_t u) { return __uint_as_float(u << 16); }
@@ -121,6 +123,49 @@ cudaError_t launch_saliency(const Dims& D, const __nv_bfloat16* Wg, const __nv_b
     if (b3 > 148 * 8) b3 = 148 * 8;
     k_saliency_sum<<<(unsigned)b3, 256, 0, st>>>(part, 1 + R, rows, 1.0f / (float)B, s);
     return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ no-allocation variant
+// fxm_saliency_static: the same three kernels with their partial-sum scratch in a file-scope device array instead of a
+// caller buffer, for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).
+// The array is part of the library image: every GPU that loads the library holds SALIENCY_STATIC_BYTES until exit.
+// In HOST code `g_saliency_scratch` is only a stand-in for the symbol, not a device address (a kernel handed it would
+// fault, or silently use host memory where the GPU can reach it); the device address comes from cudaGetSymbolAddress,
+// looked up once per device with that device current.  Nothing in the array has to start at zero: every slot the
+// summing kernel reads (slot 0: gate/up rows, slots 1..R: down-column chunks) is written in full by the two kernels
+// before it in the same call, so stale contents of an earlier call are never read.  All calls on a device share the
+// array: calls that overlap on the GPU (different streams without an ordering between them) race.
+static __device__ __align__(256) float g_saliency_scratch[SALIENCY_STATIC_BYTES / sizeof(float)];
+
+constexpr int SALIENCY_MAX_DEVICES = 64;
+static float* g_saliency_scratch_addr[SALIENCY_MAX_DEVICES];   // device address of the array on device i (nullptr: not looked up yet)
+static std::mutex g_saliency_scratch_mutex;
+
+static cudaError_t saliency_static_scratch(float** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= SALIENCY_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_saliency_scratch_mutex);
+    if (!g_saliency_scratch_addr[dev]) {
+        float* ptr = nullptr;
+        e = cudaGetSymbolAddress((void**)&ptr, g_saliency_scratch);      // the current device's copy of the array
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        g_saliency_scratch_addr[dev] = ptr;
+    }
+    *out = g_saliency_scratch_addr[dev];
+    return cudaSuccess;
+}
+
+cudaError_t launch_saliency_static(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloat16* Wu, const __nv_bfloat16* Wd,
+                                   const __nv_bfloat16* Gg, const __nv_bfloat16* Gu, const __nv_bfloat16* Gd, int B, float* s,
+                                   cudaStream_t st) {
+    if (saliency_workspace_bytes(D) > SALIENCY_STATIC_BYTES) return cudaErrorInvalidValue;   // the caller checks first
+    float* part = nullptr;
+    const cudaError_t e = saliency_static_scratch(&part);
+    if (e != cudaSuccess) return e;
+    return launch_saliency(D, Wg, Wu, Wd, Gg, Gu, Gd, B, s, part, st);
 }
 
 // ------------------------------------------------------------------------------------------------ rank

@@ -21,7 +21,7 @@ IMPL_SIMT_DEBUG = 1
 MAX_BUDGETS = 15
 
 _STATUS = ["FXM_OK", "FXM_EINVAL", "FXM_ESHAPE", "FXM_EPERM", "FXM_EBUDGET", "FXM_ENOTNESTED",
-           "FXM_EWORKSPACE", "FXM_ESTATE", "FXM_ECUDA", "FXM_ENOMEM"]
+           "FXM_EWORKSPACE", "FXM_ESTATE", "FXM_ECUDA", "FXM_ENOMEM", "FXM_ELIMIT"]
 
 
 class FxmError(RuntimeError):
@@ -79,6 +79,7 @@ def lib():
     L.fxm_host_flush.argtypes = [vp, vp]
     L.fxm_saliency_workspace_bytes.argtypes = [i32, i32, i32, ctypes.POINTER(sz)]
     L.fxm_saliency.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, i32, vp, vp, sz, vp]
+    L.fxm_saliency_static.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp, vp, i32, vp, vp]
     L.fxm_rank_channels.argtypes = [i32, i32, vp, vp, vp]
     L.fxm_sample_budget.argtypes = [vp, vp, vp, i32, vp, i32, vp, vp]
     L.fxm_action_cost.argtypes = [vp, vp, i32, vp, i32, vp, vp, vp]
@@ -103,7 +104,7 @@ def lib():
 EXPORTS = ["fxm_packed_bytes", "fxm_workspace_bytes", "fxm_pack", "fxm_set_budget", "fxm_register_budgets",
            "fxm_select_budget", "fxm_ratio_to_width", "fxm_moe_ffn", "fxm_moe_ffn_shared", "fxm_moe_ffn_router", "fxm_workspace_bytes_host",
            "fxm_moe_ffn_host", "fxm_moe_ffn_host_pipelined", "fxm_host_flush", "fxm_clipped_bytes", "fxm_export_clipped", "fxm_parse_clipped_header", "fxm_load_clipped",
-           "fxm_saliency_workspace_bytes", "fxm_saliency", "fxm_rank_channels", "fxm_sample_budget", "fxm_action_cost",
+           "fxm_saliency_workspace_bytes", "fxm_saliency", "fxm_saliency_static", "fxm_rank_channels", "fxm_sample_budget", "fxm_action_cost",
            "fxm_profile_begin", "fxm_profile_end", "fxm_route", "fxm_unpack_prefix",
            "fxm_debug_read_h", "fxm_set_impl", "fxm_set_tile_n", "fxm_set_decode", "fxm_device_flags", "fxm_launches_per_ffn",
            "fxm_status_string", "fxm_destroy"]
@@ -155,6 +156,25 @@ def saliency(W_gate, W_up, W_down, G_gate, G_up, G_down, stream=None):
                             G_up.data_ptr(), G_down.data_ptr(), B, s.data_ptr(), ws.data_ptr(), ws.numel(),
                             _stream_ptr(stream)), "fxm_saliency")
     return s
+
+
+SALIENCY_STATIC_BYTES = 8 << 20
+
+
+def saliency_static(W_gate, W_up, W_down, G_gate, G_up, G_down, out, stream=None):
+    """Eq. 2 through fxm_saliency_static: no workspace argument, nothing allocated (the scratch is a fixed 8 MB device array
+    inside the library).  `out`: a preallocated CUDA fp32 [E,I] tensor.  Raises FXM_ELIMIT for shapes beyond the scratch."""
+    import torch
+    E, I, d = W_gate.shape
+    B = G_gate.shape[0]
+    for t in (W_gate, W_up, W_down, G_gate, G_up, G_down):
+        assert t.is_cuda and t.dtype == torch.bfloat16 and t.is_contiguous()
+    assert tuple(W_down.shape) == (E, d, I) and tuple(G_gate.shape) == (B, E, I, d) and tuple(G_down.shape) == (B, E, d, I)
+    assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous() and tuple(out.shape) == (E, I)
+    _chk(lib().fxm_saliency_static(E, d, I, W_gate.data_ptr(), W_up.data_ptr(), W_down.data_ptr(), G_gate.data_ptr(),
+                                   G_up.data_ptr(), G_down.data_ptr(), B, out.data_ptr(), _stream_ptr(stream)),
+         "fxm_saliency_static")
+    return out
 
 
 def rank_channels(s, stream=None):

@@ -110,8 +110,9 @@ def test_ratio_to_width_is_integer_ceil_and_matches_oracle():
 
 def test_status_strings():
     L = fx.lib()
-    for i in range(10):
+    for i in range(11):
         assert L.fxm_status_string(i).decode().startswith("FXM_")
+    assert L.fxm_status_string(10).decode().startswith("FXM_ELIMIT")
 
 
 def test_null_arguments_do_not_crash():
