@@ -53,7 +53,7 @@ def load_peaks():
 
 # ------------------------------------------------------------------------------------------ ncu traffic of the dominant kernel
 NCU_CAPTURES = {  # (config, T, table spec) -> committed extract of an `ncu --set full` capture of exactly that workload
-    ("C4", 8192, "2560"): "profiles/r02c_ncu_full_pair_c4_T8192_r2560.csv",
+    ("C4", 8192, "2560"): "profiles/r02d_ncu_full_pair_c4_T8192_r2560.csv",
 }
 NCU_KERNEL = {"gemm1_swiglu": "k_gemm_pair<1>", "gemm2_scatter_add": "k_gemm_pair<2>", "decode_fused": "k_decode"}
 

@@ -46,9 +46,9 @@ def test_roofline_takes_the_larger_floor():
 
 def test_ncu_traffic_reads_the_committed_extract_of_the_headline_workload_only():
     v, src = bench.ncu_traffic("C4", 8192, "2560", "gemm1_swiglu")
-    path = os.path.join(ROOT, "profiles", "r02c_ncu_full_pair_c4_T8192_r2560.csv")
+    path = os.path.join(ROOT, "profiles", "r02d_ncu_full_pair_c4_T8192_r2560.csv")
     if os.path.exists(path):
-        assert src == "profiles/r02c_ncu_full_pair_c4_T8192_r2560.csv"
+        assert src == "profiles/r02d_ncu_full_pair_c4_T8192_r2560.csv"
         assert 2.4e9 < v < 8e9                                  # gate/up weights once is 2.35 GB; the capture has ~4.7 GB
     else:
         assert v is None
