@@ -16,20 +16,29 @@ namespace fxm {
 
 __device__ __forceinline__ float bf_lo(uint32_t u) { return __uint_as_float(u << 16); }
 __device__ __forceinline__ float bf_hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
+constexpr int SAL_GU_ROWS = 4;                  // gate / up rows per warp of a row block (a block covers 32 rows)
 __device__ __forceinline__ float sq8(const uint4& w, const uint4& g) {
     const float p0 = bf_lo(w.x) * bf_lo(g.x), p1 = bf_hi(w.x) * bf_hi(g.x), p2 = bf_lo(w.y) * bf_lo(g.y), p3 = bf_hi(w.y) * bf_hi(g.y);
     const float p4 = bf_lo(w.z) * bf_lo(g.z), p5 = bf_hi(w.z) * bf_hi(g.z), p6 = bf_lo(w.w) * bf_lo(g.w), p7 = bf_hi(w.w) * bf_hi(g.w);
     return ((p0 * p0 + p1 * p1) + (p2 * p2 + p3 * p3)) + ((p4 * p4 + p5 * p5) + (p6 * p6 + p7 * p7));
 }
 
-// gate and up rows: one warp per (e, j); the row of d bf16 is read with 16-byte loads, weights once, gradients B times
-__global__ void __launch_bounds__(256) k_saliency_gu(int d, size_t rows, size_t per, const uint4* __restrict__ Wg,
-                                                     const uint4* __restrict__ Wu, const uint4* __restrict__ Gg,
-                                                     const uint4* __restrict__ Gu, int B, float* __restrict__ part0) {
+// One launch streams all three weight tensors and their gradients.  Blocks [0, dn_blocks) sum W_down columns, the rest sum
+// gate / up rows; the column blocks are the long ones and come first, so the short row blocks fill the tail of the grid.
+// Both roles issue every load of a step (12 x 16 bytes per thread at B = 2) before the first use: the kernel is bound
+// by HBM only while enough requests are in flight, so a thread must never wait on one load at a time.
+//
+// gate and up rows: one warp per (e, j), four rows per warp and block; the row of d bf16 is read with 16-byte loads,
+// weights once, gradients B times.
+__device__ __forceinline__ void saliency_gu_rows(size_t blk, int d, size_t rows, size_t per, const uint4* __restrict__ Wg,
+                                                 const uint4* __restrict__ Wu, const uint4* __restrict__ Gg,
+                                                 const uint4* __restrict__ Gu, int B, float* __restrict__ part0) {
     const int lane = threadIdx.x & 31;
     const int cpr = d >> 3;                                      // 16-byte chunks per row
     const size_t per4 = per >> 3;                                // chunks per gradient set
-    for (size_t row = blockIdx.x * 8ull + (threadIdx.x >> 5); row < rows; row += (size_t)gridDim.x * 8) {
+    for (int j = 0; j < SAL_GU_ROWS; ++j) {
+        const size_t row = (blk * SAL_GU_ROWS + j) * 8ull + (threadIdx.x >> 5);
+        if (row >= rows) return;
         float acc = 0.f;
 #pragma unroll 2
         for (int c = lane; c < cpr; c += 32) {
@@ -53,47 +62,74 @@ __global__ void __launch_bounds__(256) k_saliency_gu(int d, size_t rows, size_t 
     }
 }
 
-// down columns: block (e, r) owns the rows [r0, r1) of W_down[e] [d][I]; a thread owns 8 consecutive columns of a 2048-wide
-// column tile, so a row segment is read as 256 consecutive 16-byte chunks.  Partial column sums go to slot 1 + r.
-__global__ void __launch_bounds__(256) k_saliency_dn(int d, int I, int R, size_t per, const uint4* __restrict__ Wd,
-                                                     const uint4* __restrict__ Gd, int B, float* __restrict__ part) {
-    const int e = blockIdx.x / R, r = blockIdx.x % R;
-    const int E = gridDim.x / R;
-    const int r0 = (int)((long long)d * r / R), r1 = (int)((long long)d * (r + 1) / R);
-    const int cpr = I >> 3;                                      // chunks per row (I % 16 == 0)
-    const size_t per4 = per >> 3;
-    float* out = part + ((size_t)(1 + r) * E + e) * I;
-    for (int c0 = threadIdx.x; c0 < cpr; c0 += 256) {
-        float acc[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) acc[q] = 0.f;
-#pragma unroll 4
-        for (int i = r0; i < r1; ++i) {
-            const size_t o = ((size_t)e * d + i) * cpr + c0;
-            const uint4 w = __ldcs(Wd + o);
-            for (int b0 = 0; b0 < B; b0 += 4) {
-            uint4 gs[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-                if (b0 + u < B) gs[u] = __ldcs(Gd + (b0 + u) * per4 + o);
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                if (b0 + u >= B) continue;
-                const uint4 g = gs[u];
-                const float p0 = bf_lo(w.x) * bf_lo(g.x), p1 = bf_hi(w.x) * bf_hi(g.x), p2 = bf_lo(w.y) * bf_lo(g.y), p3 = bf_hi(w.y) * bf_hi(g.y);
-                const float p4 = bf_lo(w.z) * bf_lo(g.z), p5 = bf_hi(w.z) * bf_hi(g.z), p6 = bf_lo(w.w) * bf_lo(g.w), p7 = bf_hi(w.w) * bf_hi(g.w);
-                acc[0] += p0 * p0; acc[1] += p1 * p1; acc[2] += p2 * p2; acc[3] += p3 * p3;
-                acc[4] += p4 * p4; acc[5] += p5 * p5; acc[6] += p6 * p6; acc[7] += p7 * p7;
-            }
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < 8; ++q) out[(size_t)c0 * 8 + q] = acc[q];
-    }
+__device__ __forceinline__ void sq8_acc(float (&acc)[8], const uint4& w, const uint4& g) {
+    const float p0 = bf_lo(w.x) * bf_lo(g.x), p1 = bf_hi(w.x) * bf_hi(g.x), p2 = bf_lo(w.y) * bf_lo(g.y), p3 = bf_hi(w.y) * bf_hi(g.y);
+    const float p4 = bf_lo(w.z) * bf_lo(g.z), p5 = bf_hi(w.z) * bf_hi(g.z), p6 = bf_lo(w.w) * bf_lo(g.w), p7 = bf_hi(w.w) * bf_hi(g.w);
+    acc[0] += p0 * p0; acc[1] += p1 * p1; acc[2] += p2 * p2; acc[3] += p3 * p3;
+    acc[4] += p4 * p4; acc[5] += p5 * p5; acc[6] += p6 * p6; acc[7] += p7 * p7;
 }
 
-// s = (slot 0 + slot 1 + ... + slot R) / B, slots summed in index order
+// down columns: a WARP owns (e, r, cg): rows [r0, r1) of W_down[e] [d][I], 32 consecutive 16-byte chunks of each row (a
+// lane owns 8 consecutive columns); the eight warps of a block take neighbouring items, so a block reads contiguous row
+// segments whatever I is.  Rows go four at a time: the weight chunks of the four rows and two gradient sets of each are
+// loaded before the first multiply.  Per column the sum runs over the rows in order (inside a group of four rows: b in
+// order for B <= 2, pairs of gradient sets in order beyond).  Partial column sums go to slot 1 + r.
+__device__ __forceinline__ void saliency_dn_cols(size_t blk, int E, int d, int I, int R, size_t per,
+                                                 const uint4* __restrict__ Wd, const uint4* __restrict__ Gd, int B,
+                                                 float* __restrict__ part) {
+    const int lane = threadIdx.x & 31;
+    const int cpr = I >> 3;                                      // chunks per row (I % 16 == 0)
+    const int CG = (cpr + 31) >> 5;
+    const size_t item = blk * 8ull + (threadIdx.x >> 5);
+    if (item >= (size_t)E * R * CG) return;
+    const int cg = (int)(item % CG), r = (int)(item / CG % R), e = (int)(item / CG / R);
+    const int c0 = cg * 32 + lane;
+    if (c0 >= cpr) return;
+    const int r0 = (int)((long long)d * r / R), r1 = (int)((long long)d * (r + 1) / R);
+    const size_t per4 = per >> 3;
+    float acc[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = 0.f;
+    const uint4* w_ptr = Wd + ((size_t)e * d + r0) * cpr + c0;
+    const uint4* g_ptr = Gd + ((size_t)e * d + r0) * cpr + c0;
+    for (int i = r0; i < r1; i += 4, w_ptr += 4 * (size_t)cpr, g_ptr += 4 * (size_t)cpr) {
+        const int nr = r1 - i;                                   // rows left (>= 1); rows beyond are neither read nor summed
+        uint4 w[4];
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+            if (v < nr) w[v] = __ldcs(w_ptr + (size_t)v * cpr);
+        for (int b0 = 0; b0 < B; b0 += 2) {
+            uint4 g[4][2];
+#pragma unroll
+            for (int v = 0; v < 4; ++v)
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (v < nr && b0 + u < B) g[v][u] = __ldcs(g_ptr + (b0 + u) * per4 + (size_t)v * cpr);
+#pragma unroll
+            for (int v = 0; v < 4; ++v)
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (v < nr && b0 + u < B) sq8_acc(acc, w[v], g[v][u]);
+        }
+    }
+    float4* out = (float4*)(part + ((size_t)(1 + r) * E + e) * I + (size_t)c0 * 8);
+    out[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+    out[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+}
+
+__global__ void __launch_bounds__(256, 3) k_saliency(int E, int d, int I, int R, size_t rows, size_t per, unsigned dn_blocks,
+                                                     const uint4* __restrict__ Wg, const uint4* __restrict__ Wu,
+                                                     const uint4* __restrict__ Wd, const uint4* __restrict__ Gg,
+                                                     const uint4* __restrict__ Gu, const uint4* __restrict__ Gd, int B,
+                                                     float* __restrict__ part) {
+    if (blockIdx.x < dn_blocks) saliency_dn_cols(blockIdx.x, E, d, I, R, per, Wd, Gd, B, part);
+    else saliency_gu_rows(blockIdx.x - dn_blocks, d, rows, per, Wg, Wu, Gg, Gu, B, part);
+}
+
+// s = (slot 0 + slot 1 + ... + slot R) / B, slots summed in index order.  Launched as a programmatic dependent of
+// k_saliency (its launch latency runs under that kernel's tail); the wait returns once k_saliency has completed.
 __global__ void k_saliency_sum(const float* __restrict__ part, int slots, size_t n, float inv_b, float* __restrict__ s) {
+    pdl_wait();
     for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         float acc = 0.f;
         for (int q = 0; q < slots; ++q) acc += part[(size_t)q * n + i];
@@ -102,7 +138,7 @@ __global__ void k_saliency_sum(const float* __restrict__ part, int slots, size_t
 }
 
 int saliency_row_chunks(const Dims& D) {
-    int R = (148 * 8 + D.E - 1) / D.E;                           // about eight blocks per SM: a thread keeps only 12 loads in flight
+    int R = (148 * 8 + D.E - 1) / D.E;                           // row chunks per expert (= partial-sum slots): enough warp items for every SM
     if (R > 16) R = 16;
     if (R > D.d) R = D.d;
     return R < 1 ? 1 : R;
@@ -114,25 +150,27 @@ cudaError_t launch_saliency(const Dims& D, const __nv_bfloat16* Wg, const __nv_b
                             float* part, cudaStream_t st) {
     const size_t rows = (size_t)D.E * D.I, per = rows * D.d;
     const int R = saliency_row_chunks(D);
-    size_t b1 = (rows + 7) / 8;
-    if (b1 > 148 * 16) b1 = 148 * 16;
-    k_saliency_gu<<<(unsigned)b1, 256, 0, st>>>(D.d, rows, per, (const uint4*)Wg, (const uint4*)Wu, (const uint4*)Gg,
-                                                 (const uint4*)Gu, B, part);
-    k_saliency_dn<<<D.E * R, 256, 0, st>>>(D.d, D.I, R, per, (const uint4*)Wd, (const uint4*)Gd, B, part);
+    const size_t CG = ((size_t)(D.I >> 3) + 31) / 32;
+    const size_t dn_blocks = ((size_t)D.E * R * CG + 7) / 8, gu_blocks = (rows + 8 * SAL_GU_ROWS - 1) / (8 * SAL_GU_ROWS);
+    if (dn_blocks + gu_blocks > 0x7FFFFFFFull) return cudaErrorInvalidConfiguration;
+    k_saliency<<<(unsigned)(dn_blocks + gu_blocks), 256, 0, st>>>(D.E, D.d, D.I, R, rows, per, (unsigned)dn_blocks, (const uint4*)Wg,
+                                                                  (const uint4*)Wu, (const uint4*)Wd, (const uint4*)Gg,
+                                                                  (const uint4*)Gu, (const uint4*)Gd, B, part);
     size_t b3 = (rows + 255) / 256;
     if (b3 > 148 * 8) b3 = 148 * 8;
-    k_saliency_sum<<<(unsigned)b3, 256, 0, st>>>(part, 1 + R, rows, 1.0f / (float)B, s);
-    return cudaGetLastError();
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return launch_pdl(k_saliency_sum, dim3((unsigned)b3), dim3(256), 0, st, (const float*)part, 1 + R, rows, 1.0f / (float)B, s);
 }
 
 // ------------------------------------------------------------------------------------------------ no-allocation variant
-// fxm_saliency_static: the same three kernels with their partial-sum scratch in a file-scope device array instead of a
+// fxm_saliency_static: the same two kernels with their partial-sum scratch in a file-scope device array instead of a
 // caller buffer, for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).
 // The array is part of the library image: every GPU that loads the library holds SALIENCY_STATIC_BYTES until exit.
 // In HOST code `g_saliency_scratch` is only a stand-in for the symbol, not a device address (a kernel handed it would
 // fault, or silently use host memory where the GPU can reach it); the device address comes from cudaGetSymbolAddress,
 // looked up once per device with that device current.  Nothing in the array has to start at zero: every slot the
-// summing kernel reads (slot 0: gate/up rows, slots 1..R: down-column chunks) is written in full by the two kernels
+// summing kernel reads (slot 0: gate/up rows, slots 1..R: down-column chunks) is written in full by the kernel
 // before it in the same call, so stale contents of an earlier call are never read.  All calls on a device share the
 // array: calls that overlap on the GPU (different streams without an ordering between them) race.
 static __device__ __align__(256) float g_saliency_scratch[SALIENCY_STATIC_BYTES / sizeof(float)];
