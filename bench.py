@@ -534,6 +534,12 @@ def run_ours(args):
         assert L.device_flags() == 0
         print(json.dumps(out), flush=True)
         return
+    if args.next_only:
+        # nothing but the SURVEY.md 8(f) legs (for a profiler: the saliency / export / router kernels at bench size)
+        out = {"next": run_next(torch, fx, gen, L, lay, cfg, sh, peaks)}
+        assert L.device_flags() == 0
+        print(json.dumps(out), flush=True)
+        return
     dev = to_device(fx, torch, hb)
     y = torch.empty((T, sh.d), dtype=torch.bfloat16, device="cuda")
     stream = torch.cuda.current_stream()
@@ -780,6 +786,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the budget_sweep and switch legs")
     ap.add_argument("--switch-steps", type=int, default=200)
     ap.add_argument("--switch-only", action="store_true", help="run only the C5 switching loop (N=1) and print its record")
+    ap.add_argument("--next-only", action="store_true", help="run only the SURVEY.md 8(f) legs (N=1) and print their record")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from an ncu --set full capture of this config (else null)")
     args = ap.parse_args()

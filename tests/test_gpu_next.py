@@ -21,9 +21,13 @@ def _bf16(rng, shape, std):
 
 
 # ------------------------------------------------------------------------------ NEXT-2: saliency + ranking
-@pytest.mark.parametrize("E,d,I,B", [(3, 64, 16, 1), (5, 192, 80, 3), (8, 256, 512, 2), (60, 512, 1408, 2), (2, 128, 4112, 1)])
+@pytest.mark.parametrize("E,d,I,B", [(3, 64, 16, 1), (5, 192, 80, 3), (8, 256, 512, 2), (60, 512, 1408, 2), (2, 128, 4112, 1),
+                                     (100, 64, 48, 3), (7, 192, 272, 5), (200, 64, 16, 2)])
 def test_saliency_matches_oracle_and_rank_is_exact_on_the_same_keys(E, d, I, B):
-    """Eq. 2 in fp32 (fixed summation order) vs the fp64 oracle: every s within 1e-5 relative.  The ranking is index
+    """The last three shapes: row chunks of W_down that are not a multiple of the kernel's four-row step (E=100, d=64:
+    12 chunks of 5 or 6 rows; E=200: 6 chunks of 10 or 11), column groups with idle lanes (I=272: 34 chunks = one full
+    group + 2 lanes) and an odd number of gradient sets beyond the two loaded at a time.
+    Eq. 2 in fp32 (fixed summation order) vs the fp64 oracle: every s within 1e-5 relative.  The ranking is index
     work: on the SAME keys (the kernel's own fp32 s) it must equal the oracle's rank bit for bit (ties -> lower index),
     and where the oracle's own saliencies are separated by more than the fp32 error the two ranks agree."""
     import torch
