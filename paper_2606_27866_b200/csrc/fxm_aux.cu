@@ -27,8 +27,9 @@ __global__ void k_pack_gu(Dims D, const uint4* __restrict__ Wg, const uint4* __r
     }
 }
 
-// one thread per 16-byte chunk of the packed down region (8 gathered channels of one output feature)
-__global__ void k_pack_dn(Dims D, const uint16_t* __restrict__ Wd, const int* __restrict__ rank,
+// Fallback of k_pack_dn_rows (W_down not 16-byte aligned, or one row larger than the shared-memory budget):
+// one thread per 16-byte chunk of the packed down region (8 gathered channels of one output feature), 2-byte global gathers
+__global__ void k_pack_dn_gather(Dims D, const uint16_t* __restrict__ Wd, const int* __restrict__ rank,
                           uint4* __restrict__ out, size_t n_chunks) {
     for (size_t g = blockIdx.x * (size_t)blockDim.x + threadIdx.x; g < n_chunks; g += (size_t)gridDim.x * blockDim.x) {
         const uint32_t ch = g & 7, pr = (g >> 3) & 127;
@@ -57,6 +58,61 @@ __global__ void k_pack_dn(Dims D, const uint16_t* __restrict__ Wd, const int* __
     }
 }
 
+// The packed down region the fast way.  W~down = W_down P^T permutes COLUMNS, so gathering from global memory pulls a
+// 32-byte sector per 2-byte element.  Instead block (e, group of `rpb` output features) stages its rows of W_down[e] in
+// shared memory with coalesced 16-byte loads (each byte of W_down is read from HBM exactly once), gathers the ranked
+// columns from there, and writes its 128-byte rows of every k-block tile: consecutive threads write consecutive 16-byte
+// chunks (the SW128 permutation stays inside a 128-byte row), rpb x 128 contiguous bytes per tile.  rpb divides the
+// 128-row tile; rows >= d (padded feature block) and channels >= I (padded channel block) are zeros, as in the gather version.
+constexpr int PACK_DN_SMEM = 160 * 1024;
+__global__ void __launch_bounds__(256) k_pack_dn_rows(Dims D, const uint16_t* __restrict__ Wd, const int* __restrict__ rank,
+                                                      uint4* __restrict__ out, int rpb) {
+    extern __shared__ __align__(16) uint8_t pack_smem[];
+    uint16_t* srow = (uint16_t*)pack_smem;                        // [rpb][I]
+    const int groups = D.nDB * WT_ROWS / rpb;
+    const int e = blockIdx.x / groups, i0 = (blockIdx.x % groups) * rpb;   // first (padded) output feature of the block
+    const int cpr = D.I >> 3;                                    // 16-byte chunks per row (I % 16 == 0)
+    const int n_stage = rpb * cpr;
+    for (int q0 = threadIdx.x; q0 < n_stage; q0 += 256 * 4) {    // four loads in flight per thread
+        uint4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int q = q0 + u * 256, i = i0 + q / cpr;
+            v[u] = make_uint4(0, 0, 0, 0);
+            if (q < n_stage && i < D.d) v[u] = __ldcs((const uint4*)(Wd + ((size_t)e * D.d + i) * D.I) + q % cpr);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (q0 + u * 256 < n_stage) ((uint4*)srow)[q0 + u * 256] = v[u];
+    }
+    __syncthreads();
+    const int db = i0 / WT_ROWS, pr0 = i0 % WT_ROWS;
+    const int per_kb = rpb * 8;                                  // chunks of one k-block tile that belong to this block
+    const int* rk = rank ? rank + (size_t)e * D.I : nullptr;
+    for (int q = threadIdx.x; q < D.nCB * per_kb; q += 256) {
+        const int kb2 = q / per_kb, rl = (q % per_kb) >> 3, ch = q & 7;
+        const int p0 = kb2 * KB + ch * 8;                        // first ranked channel position of the chunk
+        uint4 v4 = make_uint4(0, 0, 0, 0);
+        if (p0 < D.I) {                                          // I % 16 == 0: the chunk is inside or outside as a whole
+            int c[8];
+            if (rk) {
+                const int4 a = __ldg((const int4*)(rk + p0)), b = __ldg((const int4*)(rk + p0) + 1);
+                c[0] = a.x; c[1] = a.y; c[2] = a.z; c[3] = a.w; c[4] = b.x; c[5] = b.y; c[6] = b.z; c[7] = b.w;
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) c[j] = p0 + j;
+            }
+            const uint16_t* row = srow + (size_t)rl * D.I;
+            v4.x = row[c[0]] | ((uint32_t)row[c[1]] << 16);
+            v4.y = row[c[2]] | ((uint32_t)row[c[3]] << 16);
+            v4.z = row[c[4]] | ((uint32_t)row[c[5]] << 16);
+            v4.w = row[c[6]] | ((uint32_t)row[c[7]] << 16);
+        }
+        const size_t tile = ((size_t)e * D.nCB + kb2) * D.nDB + db;
+        __stcs(out + ((tile * WT_BYTES + sw128_chunk(pr0 + rl, ch)) >> 4), v4);
+    }
+}
+
 __global__ void k_eblk_full(uint32_t* __restrict__ eblk, int E, int nCB) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e < E) eblk[e] = (uint32_t)e * (uint32_t)nCB;
@@ -69,7 +125,20 @@ cudaError_t launch_pack(const Dims& D, const __nv_bfloat16* Wg, const __nv_bfloa
     const int b_gu = (int)((n_gu + threads - 1) / threads < 148 * 64 ? (n_gu + threads - 1) / threads : 148 * 64);
     const int b_dn = (int)((n_dn + threads - 1) / threads < 148 * 64 ? (n_dn + threads - 1) / threads : 148 * 64);
     k_pack_gu<<<b_gu, threads, 0, st>>>(D, (const uint4*)Wg, (const uint4*)Wu, rank_dev, (uint4*)packed, n_gu);
-    k_pack_dn<<<b_dn, threads, 0, st>>>(D, (const uint16_t*)Wd, rank_dev, (uint4*)(packed + gu_bytes(D)), n_dn);
+    // output features per block of k_pack_dn_rows (divides 128): 16 while that leaves five blocks per SM (<= 40 KB of rows),
+    // 8 if that does; fewer only when a row is so long that 8 of them exceed the shared-memory budget
+    int rpb = 16;
+    if ((size_t)rpb * D.I * 2 > 40 * 1024) rpb = 8;
+    while (rpb && (size_t)rpb * D.I * 2 > (size_t)PACK_DN_SMEM) rpb >>= 1;
+    if (rpb && ((uintptr_t)Wd & 15u) == 0) {
+        const size_t smem = (size_t)rpb * D.I * 2;
+        cudaError_t e = cudaFuncSetAttribute(k_pack_dn_rows, cudaFuncAttributeMaxDynamicSharedMemorySize, PACK_DN_SMEM);
+        if (e != cudaSuccess) return e;
+        k_pack_dn_rows<<<D.E * (D.nDB * WT_ROWS / rpb), threads, smem, st>>>(D, (const uint16_t*)Wd, rank_dev,
+                                                                           (uint4*)(packed + gu_bytes(D)), rpb);
+    } else {
+        k_pack_dn_gather<<<b_dn, threads, 0, st>>>(D, (const uint16_t*)Wd, rank_dev, (uint4*)(packed + gu_bytes(D)), n_dn);
+    }
     k_eblk_full<<<1, MAX_E, 0, st>>>(eblk_dev, D.E, D.nCB);
     return cudaGetLastError();
 }

@@ -41,6 +41,28 @@ def test_pack_unpack_roundtrip_bitexact(d, E, I):
             assert np.array_equal(fx.bf16_to_bits(Wd), Dt[e, :, :r]) if r else True
 
 
+@pytest.mark.parametrize("d,E,I", [(192, 3, 80), (128, 2, 1408)])
+def test_pack_with_w_down_two_byte_aligned_only(d, E, I):
+    """fxm_pack asks only 2-byte alignment of W_down (include/flexmoe.h).  A 16-byte aligned W_down is packed by the
+    kernel that stages whole rows in shared memory, any other one by the gather kernel: both must give the oracle's
+    W~down bit for bit (Eq. 3)."""
+    import torch
+    fx = _fx()
+    sh, lay, rng = _small_layer(3, d, E, min(2, E), I)
+    buf = torch.zeros(E * d * I + 8, dtype=torch.bfloat16, device="cuda")
+    Wd = buf[1:1 + E * d * I].view(E, d, I)                       # data_ptr 2 bytes past a 16-byte boundary
+    Wd.copy_(fx.bf16_from_bits(lay.W_down, "cuda"))
+    assert Wd.data_ptr() % 16 == 2 and Wd.is_contiguous()
+    L = fx.Layer.pack(fx.bf16_from_bits(lay.W_gate, "cuda"), fx.bf16_from_bits(lay.W_up, "cuda"), Wd, lay.channel_rank)
+    torch.cuda.synchronize()
+    Gt, Ut, Dt = oracle.pack(lay.W_gate, lay.W_up, lay.W_down, lay.channel_rank)
+    for e in range(E):
+        Wg_, Wu_, Wd_ = L.unpack_prefix(e, I)
+        torch.cuda.synchronize()
+        assert np.array_equal(fx.bf16_to_bits(Wd_), Dt[e])
+        assert np.array_equal(fx.bf16_to_bits(Wg_), Gt[e])
+
+
 def test_pack_rejects_non_permutation():
     import gpu_util as gu
     fx = _fx()
