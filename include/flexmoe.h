@@ -71,7 +71,9 @@ fxm_status fxm_workspace_bytes(int E, int d, int I, int T_max, int k, size_t* by
 
 /* ---- (1) pack: Eq. 3; layout prior art App. C.2, PAPER.md:526-540 ---------------------
  * W_gate, W_up : device, bf16 [E][I][d]   (row c of expert e = channel c)
- * W_down       : device, bf16 [E][d][I]   (column c = channel c)
+ * W_down       : device, bf16 [E][d][I]   (column c = channel c).  W_gate / W_up must be 16-byte aligned; W_down needs only
+ *                2-byte alignment, but a 16-byte aligned W_down packs ~8x faster (whole rows staged in shared memory
+ *                instead of 2-byte gathers).  Misalignment beyond that -> FXM_EINVAL.
  * channel_rank : HOST int32 [E][I] or NULL (= identity).  channel_rank[e][p] is the ORIGINAL index of the
  *                p-th most important channel of expert e (argsort-descending output; gather semantics).
  *                Validated on the host before anything is enqueued (FXM_EPERM).
