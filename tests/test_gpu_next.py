@@ -65,6 +65,32 @@ def test_saliency_matches_oracle_and_rank_is_exact_on_the_same_keys(E, d, I, B):
         assert np.array_equal(rk_gpu[e][gap_ok], rk_ref[e][gap_ok])
 
 
+def test_saliency_at_bench_size_sampled_experts():
+    """The launch configuration bench.py times (C2-sized weights, E=60, I=1408, d=2048, B=2: 3.1 GB, 720 column blocks +
+    2640 row blocks in one grid, generated on the device as bench.py does) against the oracle on sampled experts:
+    every channel of experts 0, 17, 31 and 59, both through fxm_saliency and through fxm_saliency_static."""
+    import torch
+    fx = _fx()
+    E, I, d, B = 60, 1408, 2048, 2
+    g = torch.Generator(device="cuda")
+    g.manual_seed(11)
+    mk = lambda *shape: (torch.randn(*shape, device="cuda", dtype=torch.float32, generator=g) * 0.02).to(torch.bfloat16)
+    Wg, Wu, Wd = mk(E, I, d), mk(E, I, d), mk(E, d, I)
+    Gg, Gu, Gd = mk(B, E, I, d), mk(B, E, I, d), mk(B, E, d, I)
+    s = fx.saliency(Wg, Wu, Wd, Gg, Gu, Gd)
+    s2 = torch.empty_like(s)
+    fx.saliency_static(Wg, Wu, Wd, Gg, Gu, Gd, s2)
+    torch.cuda.synchronize()
+    assert torch.equal(s, s2)
+    s_gpu = s.cpu().numpy()
+    assert np.isfinite(s_gpu).all() and (s_gpu > 0).all()
+    bits = fx.bf16_to_bits
+    for e in (0, 17, 31, 59):
+        ref = oracle.saliency(bits(Wg[e:e + 1]), bits(Wu[e:e + 1]), bits(Wd[e:e + 1]),
+                              bits(Gg[:, e:e + 1]), bits(Gu[:, e:e + 1]), bits(Gd[:, e:e + 1]))[0]
+        assert np.abs(s_gpu[e] / ref - 1).max() <= 2e-5, (e, np.abs(s_gpu[e] / ref - 1).max())
+
+
 def test_ranked_pack_orders_channels_by_importance_and_keeps_the_function():
     """The whole offline front: saliency -> rank -> pack.  With the device ranking, (1) the packed prefix holds the
     channels in descending saliency, (2) at full width the FFN equals the unranked dense layer (permutation invariance,
