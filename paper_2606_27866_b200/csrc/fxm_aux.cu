@@ -6,24 +6,39 @@
 namespace fxm {
 
 // ---------------------------------------------------------------------------------------------- pack
-// one thread per 16-byte chunk of the packed gate/up region (full layer: expert e starts at channel block e * nCB)
+// one thread per 16-byte chunk of the packed gate/up region (full layer: expert e starts at channel block e * nCB), four
+// chunks per step: rank entry -> weight chunk is a dependent chain, so the four chains are issued side by side
 __global__ void k_pack_gu(Dims D, const uint4* __restrict__ Wg, const uint4* __restrict__ Wu,
                           const int* __restrict__ rank, uint4* __restrict__ out, size_t n_chunks) {
-    for (size_t g = blockIdx.x * (size_t)blockDim.x + threadIdx.x; g < n_chunks; g += (size_t)gridDim.x * blockDim.x) {
-        const uint32_t ch = g & 7, pr = (g >> 3) & 127;
-        const size_t tile = g >> 10;
-        const int kb = (int)(tile % D.nKB1);
-        const int cb = (int)((tile / D.nKB1) % D.nCB);
-        const int e = (int)(tile / ((size_t)D.nKB1 * D.nCB));
-        const int p = cb * CB + (pr >> 5) * 16 + (pr & 15);     // ranked channel position
-        const bool is_up = (pr & 31) >= 16;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (p < D.I) {
-            const int c = rank ? rank[(size_t)e * D.I + p] : p;  // ORIGINAL channel index (gather semantics)
-            const size_t src = (((size_t)e * D.I + c) * D.d + (size_t)kb * KB + ch * 8) >> 3;
-            v = is_up ? Wu[src] : Wg[src];
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t g0 = blockIdx.x * (size_t)blockDim.x + threadIdx.x; g0 < n_chunks; g0 += 4 * stride) {
+        const uint4* src[4];
+        size_t dst[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t g = g0 + u * stride;
+            src[u] = nullptr;
+            dst[u] = 0;
+            if (g >= n_chunks) continue;
+            const uint32_t ch = g & 7, pr = (g >> 3) & 127;
+            const size_t tile = g >> 10;
+            const int kb = (int)(tile % D.nKB1);
+            const int cb = (int)((tile / D.nKB1) % D.nCB);
+            const int e = (int)(tile / ((size_t)D.nKB1 * D.nCB));
+            const int p = cb * CB + (pr >> 5) * 16 + (pr & 15);     // ranked channel position
+            const bool is_up = (pr & 31) >= 16;
+            dst[u] = (tile * WT_BYTES + sw128_chunk(pr, ch)) >> 4;
+            if (p < D.I) {
+                const int c = rank ? __ldg(rank + (size_t)e * D.I + p) : p;  // ORIGINAL channel index (gather semantics)
+                src[u] = (is_up ? Wu : Wg) + ((((size_t)e * D.I + c) * D.d + (size_t)kb * KB + ch * 8) >> 3);
+            }
         }
-        out[(tile * WT_BYTES + sw128_chunk(pr, ch)) >> 4] = v;
+        uint4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = src[u] ? __ldcs(src[u]) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            if (g0 + u * stride < n_chunks) __stcs(out + dst[u], v[u]);
     }
 }
 
